@@ -1,0 +1,141 @@
+/*
+ * gint.h -- C ABI of libgint.so: real-space grid integration for numerical-atomic-orbital (LCAO)
+ * Kohn-Sham DFT on one NVIDIA B200 (sm_100a), fp64.
+ *
+ * What the library computes (PAPER.md = arXiv 2409.09399 text, /root/reference/PAPER.md):
+ *   gint_vlocal  Eq. 2:  H_{mu nu} = sum_r phi_mu(r - R_mu) V(r) phi_nu(r - R_nu) dV
+ *   gint_rho     Eq. 3:  rho(r)    = sum_{mu nu} rho_{mu nu} phi_mu(r - R_mu) phi_nu(r - R_nu)
+ *   on a uniform periodic mesh, processed in grid batches whose "neighbouring atoms" are the atoms with a
+ *   batch point closer than their cutoff radius (section 2.3.2); orbitals are
+ *   zero at and beyond the cutoff (Fig. 6).
+ * Conventions the paper leaves open are fixed in DESIGN.md "Readings" (R1..R9) and repeated at each call.
+ *
+ * General rules
+ *   - every function returns GINT_OK (0) or a negative gint_status; none throws or exits;
+ *     gint_last_error() returns a thread-local, NUL-terminated message for the last failure.
+ *   - units: bohr.  All host arrays are BORROWED for the duration of the call and copied inside.
+ *   - device pointers are BORROWED, must be 8-byte aligned and belong to the device given to gint_init.
+ *   - gint_vlocal / gint_rho only ENQUEUE work on the given CUDA stream (a cudaStream_t passed as void*,
+ *     e.g. torch.cuda.current_stream().cuda_stream); they do not synchronise.  A context owns its
+ *     neighbour tables and scratch buffers: do not use one context from two streams at the same time.
+ *   - there is no CPU fallback: without a usable CUDA device gint_init fails with GINT_ERR_CUDA.
+ */
+#ifndef GINT_H
+#define GINT_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gint_ctx gint_ctx;
+
+typedef enum gint_status {
+    GINT_OK = 0,
+    GINT_ERR_INVALID_ARG = -1,   /* NULL pointer, negative size, non-finite value, det(cell) <= 0, ...        */
+    GINT_ERR_UNSUPPORTED = -2,   /* l > 2, more than GINT_MAX_ORB orbitals per atom, batch too large for smem */
+    GINT_ERR_CUDA = -3,          /* a CUDA runtime call failed (message holds cudaGetErrorString)             */
+    GINT_ERR_OUT_OF_MEMORY = -4, /* host or device allocation failed                                          */
+    GINT_ERR_BAD_STATE = -5      /* NULL / freed context                                                      */
+} gint_status;
+
+#define GINT_MAX_L 2
+#define GINT_MAX_ORB 32          /* orbitals per atom (sum over shells of 2l+1) */
+
+/* flags of gint_init: three 8-bit fields override the grid-batch edge lengths (mesh points) along a1,a2,a3;
+ * 0 = choose automatically so that one batch's orbital values fit in shared memory (PAPER.md:165 uses
+ * batches of 27..1000 points; Table 3 sweeps 125..512). */
+#define GINT_FLAG_BATCH(bx, by, bz) ((unsigned long long)(bx) | ((unsigned long long)(by) << 8) | ((unsigned long long)(bz) << 16))
+
+/*
+ * gint_init -- "gint_init(basis tables, atoms, cell, mesh)" of BASELINE.json north_star.
+ * Builds, on the device: the radial interpolation tables, the sparse pair list (all ordered keys
+ * (A, B, n) with |tau_B + n.cell - tau_A| < rc_A + rc_B, strict; reading R7), the grid batches and, per
+ * batch, the list of atom images with at least one batch point closer than rc.
+ *
+ *   n_species, n_shell[n_species], shell_l[sum n_shell] (0..2), rcut[n_species] (bohr)
+ *   dr                    radial table spacing; knot i of every shell sits at r = i*dr
+ *   n_knot[n_species]     knots per shell of that species; (n_knot-1)*dr must be >= rcut
+ *   tab_y, tab_y2         concatenated [species][shell][knot] radial values R(i*dr) and cubic-spline second
+ *                         derivatives (input DATA; reading R5: R(r) = a y_i + b y_{i+1} + ((a^3-a) y2_i +
+ *                         (b^3-b) y2_{i+1}) dr^2/6 with i = min(floor(r/dr), n_knot-2), b = r/dr - i, a = 1-b)
+ *   n_atoms, atom_species[n_atoms], atom_pos[n_atoms*3]   Cartesian, need not be wrapped into the cell
+ *   cell[9]               rows a1, a2, a3; det > 0
+ *   mesh[3]               N1, N2, N3 >= 1; mesh point (i,j,k) sits at (i/N1) a1 + (j/N2) a2 + (k/N3) a3,
+ *                         flat index g = (i*N2 + j)*N3 + k, dV = det(cell)/(N1 N2 N3)            (reading R1)
+ *   device                CUDA device ordinal
+ * Orbital of shell s, m = -l..l:  phi = R_s(|d|) Y_lm(d/|d|), d = r - tau_A - n.cell, zero for |d| >= rc;
+ * real spherical harmonics without Condon-Shortley phase, order l=1: (y,z,x), l=2: (xy,yz,3z^2-1,xz,x^2-y^2)
+ * (reading R4).  Orbitals of one atom are ordered by shell, then m.
+ * On success *out owns device memory until gint_free.
+ */
+int gint_init(gint_ctx** out,
+              int n_species, const int* n_shell, const int* shell_l, const double* rcut,
+              double dr, const int* n_knot, const double* tab_y, const double* tab_y2,
+              int n_atoms, const int* atom_species, const double* atom_pos,
+              const double cell[9], const int mesh[3],
+              int device, unsigned long long flags);
+
+/* total orbitals = sum over atoms of norb(species). */
+int gint_n_orb(const gint_ctx* ctx, long long* n_orb_total);
+
+/* number of ordered pair keys and total doubles of an H (or D) value array. */
+int gint_n_pairs(const gint_ctx* ctx, long long* n_pairs, long long* n_values);
+
+/* pair list in lexicographic order of (A, B, n1, n2, n3): A[n_pairs], B[n_pairs], R3[n_pairs*3],
+ * offset[n_pairs+1] (host arrays supplied by the caller; any may be NULL to skip).  Block p is row-major
+ * norb(A) x norb(B) doubles at offset[p].  Both (A,B,n) and (B,A,-n) are listed. */
+int gint_get_pairs(const gint_ctx* ctx, int* A, int* B, int* R3, long long* offset);
+
+/*
+ * gint_vlocal -- Eq. 2 made periodic (reading R8):
+ *   H_p[mu,nu] = dV * sum_g V_g * sum_{t in Z^3} phi_{A mu}(r_g; t) phi_{B nu}(r_g; t + n),   p = (A,B,n).
+ *   V_dev  device, N1*N2*N3 doubles, index g (N3 fastest)           -- read
+ *   H_dev  device, n_values doubles in pair-list layout               -- OVERWRITTEN (every block, both
+ *          (A,B,n) and its mirror (B,A,-n) = transpose)
+ */
+int gint_vlocal(gint_ctx* ctx, const double* V_dev, double* H_dev, void* cuda_stream);
+
+/*
+ * gint_rho -- Eq. 3, reading R9:
+ *   rho_g = sum over ordered pairs of atom images ((A,t),(B,t')) non-zero at r_g of
+ *           phi_A(r_g;t)^T  D_(A,B,t'-t)  phi_B(r_g;t').      No symmetry of D is assumed.
+ *   D_dev    device, n_values doubles in pair-list layout             -- read
+ *   rho_dev  device, N1*N2*N3 doubles                                 -- OVERWRITTEN
+ */
+int gint_rho(gint_ctx* ctx, const double* D_dev, double* rho_dev, void* cuda_stream);
+
+/* Host-buffer convenience forms (the end-to-end path timed by bench.py's "e2e"): copy the input from host
+ * memory (pinned or pageable) to context-owned device buffers, run the device path, copy the result back to
+ * host memory and synchronise the stream before returning. */
+int gint_vlocal_host(gint_ctx* ctx, const double* V_host, double* H_host, void* cuda_stream);
+int gint_rho_host(gint_ctx* ctx, const double* D_host, double* rho_host, void* cuda_stream);
+
+/* statistics, out[GINT_N_STATS] (long long).  Filled at init except the GINT_STAT_ALG_* entries, which are
+ * counted on the device on the first call that asks for them (the context is not const for that reason). */
+enum {
+    GINT_STAT_N_BATCH = 0,        /* non-empty grid batches                                                 */
+    GINT_STAT_N_BATCH_EMPTY = 1,  /* batches without any neighbouring atom                                  */
+    GINT_STAT_BATCH_BX = 2, GINT_STAT_BATCH_BY = 3, GINT_STAT_BATCH_BZ = 4,
+    GINT_STAT_NEIGH_ENTRIES = 5,  /* sum over batches of neighbouring atom images                          */
+    GINT_STAT_MAX_NB = 6,         /* max neighbouring atom images of one batch                              */
+    GINT_STAT_MAX_COLS = 7,       /* max orbitals of one batch                                              */
+    GINT_STAT_PADDED_MACS = 8,    /* sum_b k_b * cols_b^2 (what a dense, non-symmetric batch product costs) */
+    GINT_STAT_N_CANON = 9,        /* canonical pair keys (one of each mirror pair)                          */
+    GINT_STAT_ALG_INCIDENCE = 10, /* sum_g #atoms with |d| < rc at g                                        */
+    GINT_STAT_ALG_SUM_N = 11,     /* sum_g n_g,   n_g = orbitals non-zero at g                              */
+    GINT_STAT_ALG_SUM_N2 = 12,    /* sum_g n_g^2                                                            */
+    GINT_STAT_NONEMPTY_POINTS = 13,
+    GINT_STAT_SMEM_BYTES = 14,    /* dynamic shared memory of the contraction kernels                       */
+    GINT_STAT_DEVICE_BYTES = 15,  /* device memory owned by the context                                     */
+    GINT_N_STATS = 16
+};
+int gint_stats(gint_ctx* ctx, long long* out);
+
+int gint_free(gint_ctx* ctx);
+
+const char* gint_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GINT_H */

@@ -1,0 +1,126 @@
+// gint_internal.h -- context layout and helpers shared by the translation units of libgint.so.
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "../../include/gint.h"
+
+#define GINT_MAX_SHELL 12          // radial shells per species
+#define GINT_MAX_NB 96             // neighbouring atom images per grid batch
+#define GINT_MAX_K 128             // mesh points per grid batch
+#define GINT_THREADS 512           // threads per CTA of the contraction kernels (16 warps)
+
+// ---- error plumbing -------------------------------------------------------------------------------
+void gint_set_error(const char* fmt, ...);
+#define GINT_FAIL(code, ...) do { gint_set_error(__VA_ARGS__); return (code); } while (0)
+#define GINT_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { \
+    gint_set_error("%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    return e_ == cudaErrorMemoryAllocation ? GINT_ERR_OUT_OF_MEMORY : GINT_ERR_CUDA; } } while (0)
+
+// ---- device-side descriptions ---------------------------------------------------------------------
+struct SpeciesDev {
+    double rc;                      // cutoff radius
+    int n_shell;
+    int norb;
+    int n_int;                      // spline intervals per shell (n_knot - 1)
+    int tab_off;                    // first row (interval) of this species in the coefficient table
+    int row_len;                    // doubles per table row = 4 * n_shell
+    int l[GINT_MAX_SHELL];
+};
+
+// Geometry and batching constants, passed by value to every kernel.
+struct Geom {
+    double a[9];                    // cell rows a1,a2,a3
+    double inv[9];                  // frac = pos * inv (row vector convention)
+    double hgt[3];                  // distance between lattice planes along each axis
+    double dV;
+    double inv_dr;
+    int N[3];                       // mesh
+    int bs[3];                      // batch edge lengths (points)
+    int nb[3];                      // batches along each axis
+    int K;                          // bs[0]*bs[1]*bs[2]
+    int LD;                         // leading dimension (doubles) of the orbital tile in shared memory
+    int key_m;                      // pair keys: |n_i| <= key_m, key_M = 2*key_m+1
+    int key_M;
+    int max_cols;                   // max orbitals of one batch
+    int max_nb;                     // max neighbour entries of one batch
+};
+
+// One neighbouring atom image of a grid batch.
+struct NeighEntry {
+    int atom;
+    int shift;                      // (t1+64) | (t2+64)<<8 | (t3+64)<<16
+};
+
+__host__ __device__ inline int pack_shift(int t1, int t2, int t3) { return (t1 + 64) | ((t2 + 64) << 8) | ((t3 + 64) << 16); }
+__host__ __device__ inline void unpack_shift(int s, int& t1, int& t2, int& t3) {
+    t1 = (s & 255) - 64; t2 = ((s >> 8) & 255) - 64; t3 = ((s >> 16) & 255) - 64;
+}
+
+// Mesh point (i,j,k) -> Cartesian position (reading R1).  Used by the neighbour pass AND the orbital
+// evaluation so that both take the |d| < rc decision on bit-identical numbers.
+__host__ __device__ inline void mesh_point(const Geom& g, int i, int j, int k, double& x, double& y, double& z) {
+    double u = (double)i / (double)g.N[0], v = (double)j / (double)g.N[1], w = (double)k / (double)g.N[2];
+    x = u * g.a[0] + v * g.a[3] + w * g.a[6];
+    y = u * g.a[1] + v * g.a[4] + w * g.a[7];
+    z = u * g.a[2] + v * g.a[5] + w * g.a[8];
+}
+
+struct gint_ctx {
+    int device = 0;
+    Geom geom{};
+    // basis
+    int n_species = 0;
+    std::vector<SpeciesDev> h_species;
+    SpeciesDev* d_species = nullptr;
+    double* d_tab = nullptr;         // [rows][row_len]: per interval, per shell c0..c3 (R = ((c3 b + c2) b + c1) b + c0)
+    // atoms
+    int n_atoms = 0;
+    std::vector<int> h_atom_species;
+    std::vector<double> h_atom_pos;
+    double* d_atom_pos = nullptr;    // [n_atoms*3]
+    int* d_atom_species = nullptr;
+    long long n_orb_total = 0;
+    // public pair list (lexicographic), host copies for gint_get_pairs
+    long long n_pairs = 0, n_values = 0;
+    std::vector<int> h_pA, h_pB, h_pR;
+    std::vector<long long> h_poff;
+    long long* d_poff = nullptr;     // [n_pairs+1] offsets of the public blocks
+    int* d_pcanon = nullptr;         // [n_pairs] canonical index of the key itself or of its mirror
+    unsigned char* d_pflag = nullptr;// [n_pairs] 1 = key is canonical, 0 = key is the mirror of a canonical key
+    int* d_pnA = nullptr;            // [n_pairs] norb(A) | norb(B) << 16
+    // canonical (one per mirror pair) keys: the internal accumulation layout
+    long long n_canon = 0, n_cvalues = 0;
+    int* d_crow = nullptr;           // [n_atoms+1] first canonical key of row A
+    unsigned long long* d_ckey = nullptr; // [n_canon] packed (B, n) ascending inside a row
+    unsigned int* d_coff = nullptr;  // [n_canon+1] offsets (doubles) into the canonical value array
+    int* d_cpub = nullptr;           // [n_canon] public index of the canonical key
+    int* d_cmir = nullptr;           // [n_canon] public index of its mirror (== d_cpub for (A,A,0))
+    double* d_cval = nullptr;        // [n_cvalues] canonical-half scratch: H accumulation / symmetrised D
+    // batches
+    long long n_batch_total = 0, n_batch = 0, n_batch_empty = 0, n_entries = 0;
+    int* d_bstart = nullptr;         // [n_batch_total+1] CSR into d_bent
+    NeighEntry* d_bent = nullptr;    // neighbour entries sorted by (atom, shift lexicographic)
+    int* d_order = nullptr;          // [n_batch_total] batch ids: non-empty heavy-first, then empty ones
+    long long padded_macs = 0;
+    size_t smem_bytes = 0;
+    size_t device_bytes = 0;
+    // lazily computed statistics
+    bool have_alg = false;
+    long long alg[4] = {0, 0, 0, 0};
+    // host-path staging
+    double* d_stage_in = nullptr; size_t stage_in_n = 0;
+    double* d_stage_out = nullptr; size_t stage_out_n = 0;
+};
+
+// implemented in gint_kernels.cu
+int gint_launch_vlocal(gint_ctx* c, const double* V, double* H, cudaStream_t st);
+int gint_launch_rho(gint_ctx* c, const double* D, double* rho, cudaStream_t st);
+int gint_launch_alg_stats(gint_ctx* c);
+int gint_configure_kernels(gint_ctx* c);
+size_t gint_smem_needed(const Geom& g);

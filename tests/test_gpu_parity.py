@@ -1,0 +1,143 @@
+"""GPU parity: libgint.so (through the C ABI, via the ctypes binding) against the CPU oracle, element by element,
+on the same seeded inputs.  Bar (BASELINE.json north_star): max|dH|/max|H| <= 1e-10, max|drho|/max|rho| <= 1e-10.
+The pair list is integer work: bit-exact.
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2409_09399_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+def _gint(w, flags=0):
+    from paper_2409_09399_b200.gint import Gint
+    return Gint.from_workload(w, flags=flags)
+
+
+def _rel(a, b):
+    return float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
+
+
+def _check_pairs(g, plist):
+    A, B, R, off = g.pairs()
+    oA, oB, oR, ooff = plist
+    assert np.array_equal(A, oA) and np.array_equal(B, oB) and np.array_equal(R, oR) and np.array_equal(off, ooff)
+
+
+def _full_parity(torch, w, flags=0, seed_extra=None):
+    plist = O.pairs(w)
+    g = _gint(w, flags)
+    _check_pairs(g, plist)
+    V = W.make_potential(w)
+    D = W.make_density_blocks(w, *plist)
+    if seed_extra is not None:       # break the symmetry of D: the library must honour all ordered blocks
+        D = D + 0.3 * np.random.default_rng(seed_extra).standard_normal(D.size)
+    H_or = O.vlocal(w, V, plist)
+    rho_or = O.rho(w, D, plist)
+    H = g.vlocal(torch.from_numpy(V).cuda()).cpu().numpy()
+    rho = g.rho(torch.from_numpy(D).cuda()).cpu().numpy()
+    eH, er = _rel(H, H_or), _rel(rho, rho_or)
+    st = g.stats()
+    g.close()
+    assert eH <= TOL, f"H parity {eH:.3e}"
+    assert er <= TOL, f"rho parity {er:.3e}"
+    return st
+
+
+def test_cfg0_full(torch_cuda):
+    st = _full_parity(torch_cuda, W.make_workload(0))
+    assert st["n_batch_empty"] == 0
+
+
+def test_cfg0_nonsymmetric_D(torch_cuda):
+    _full_parity(torch_cuda, W.make_workload(0), seed_extra=7)
+
+
+@pytest.mark.parametrize("shape", [(2, 2, 2), (3, 3, 5), (5, 2, 3), (1, 1, 1), (4, 2, 7)])
+def test_cfg0_batch_shapes(torch_cuda, shape):
+    """Ragged edge batches (24 is not a multiple of 5 or 7) and other batch shapes give the same result."""
+    from paper_2409_09399_b200.gint import batch_flag
+    st = _full_parity(torch_cuda, W.make_workload(0), flags=batch_flag(*shape))
+    assert (st["batch_bx"], st["batch_by"], st["batch_bz"]) == shape
+
+
+def test_cfg1_full(torch_cuda):
+    st = _full_parity(torch_cuda, W.make_workload(1))
+    assert st["n_batch_empty"] > 0          # vacuum
+
+
+def test_skew_cell_two_species(torch_cuda):
+    """Non-orthogonal cell, two species with different rc / shell sets, atoms outside the home cell, self images."""
+    torch = torch_cuda
+    b1 = W.make_basis(4.0, shells=((0, 0.7), (1, 0.5), (2, 0.45)))
+    b2 = W.make_basis(3.0, shells=((0, 0.9), (0, 0.3), (1, 0.6)))
+    basis = W.Basis(2, np.array([3, 3], np.int32), np.concatenate([b1.shell_l, b2.shell_l]),
+                    np.array([4.0, 3.0]), W.DR, np.concatenate([b1.n_knot, b2.n_knot]),
+                    np.concatenate([b1.tab_y, b2.tab_y]), np.concatenate([b1.tab_y2, b2.tab_y2]))
+    cell = np.array([[5.0, 0.3, 0.0], [1.7, 4.6, 0.2], [0.4, -0.5, 5.5]])
+    pos = np.array([[0.1, 0.2, 0.3], [2.5, 2.0, 1.0], [7.9, -1.0, 6.0], [3.3, 3.9, 4.4]])
+    w = W.Workload("skew", 90, cell, np.array([17, 19, 23], np.int32), np.array([0, 1, 1, 0], np.int32), pos, basis)
+    plist = O.pairs(w)
+    g = _gint(w)
+    _check_pairs(g, plist)
+    rng = np.random.default_rng(11)
+    V = rng.standard_normal(w.n_points)
+    D = rng.standard_normal(int(plist[3][-1]))
+    H = g.vlocal(torch.from_numpy(V).cuda()).cpu().numpy()
+    rho = g.rho(torch.from_numpy(D).cuda()).cpu().numpy()
+    g.close()
+    assert _rel(H, O.vlocal(w, V, plist)) <= TOL
+    assert _rel(rho, O.rho(w, D, plist)) <= TOL
+
+
+def test_host_entry_points(torch_cuda):
+    torch = torch_cuda
+    w = W.make_workload(0)
+    plist = O.pairs(w)
+    g = _gint(w)
+    V = W.make_potential(w)
+    D = W.make_density_blocks(w, *plist)
+    H = np.empty(g.n_values)
+    rho = torch.empty(g.n_points, dtype=torch.float64).pin_memory()
+    g.vlocal_host(V, H)
+    g.rho_host(torch.from_numpy(D).pin_memory(), rho)
+    g.close()
+    assert _rel(H, O.vlocal(w, V, plist)) <= TOL
+    assert _rel(rho.numpy(), O.rho(w, D, plist)) <= TOL
+
+
+def test_empty_and_single_atom(torch_cuda):
+    torch = torch_cuda
+    basis = W.make_basis(5.0)
+    cell = np.eye(3) * 30.0
+    # no atoms at all: H is empty, rho is zero
+    w0 = W.Workload("empty", 91, cell, np.array([12, 12, 12], np.int32), np.zeros(0, np.int32), np.zeros((0, 3)), basis)
+    g = _gint(w0)
+    assert g.n_pairs == 0 and g.n_values == 0
+    rho = g.rho(torch.zeros(0, dtype=torch.float64, device="cuda")).cpu().numpy()
+    assert np.all(rho == 0)
+    g.close()
+    # one atom in a big box: one on-site block
+    w1 = W.Workload("single", 92, cell, np.array([40, 40, 40], np.int32), np.zeros(1, np.int32), np.array([[3.0, 29.0, 15.0]]), basis)
+    plist = O.pairs(w1)
+    g = _gint(w1)
+    _check_pairs(g, plist)
+    assert g.n_pairs == 1
+    V = np.random.default_rng(3).standard_normal(w1.n_points)
+    D = np.random.default_rng(4).standard_normal(169)
+    H = g.vlocal(torch.from_numpy(V).cuda()).cpu().numpy()
+    rho = g.rho(torch.from_numpy(D).cuda()).cpu().numpy()
+    g.close()
+    assert _rel(H, O.vlocal(w1, V, plist)) <= TOL
+    assert _rel(rho, O.rho(w1, D, plist)) <= TOL
