@@ -127,9 +127,17 @@ enum {
     GINT_STAT_NONEMPTY_POINTS = 13,
     GINT_STAT_SMEM_BYTES = 14,    /* dynamic shared memory of the contraction kernels                       */
     GINT_STAT_DEVICE_BYTES = 15,  /* device memory owned by the context                                     */
-    GINT_N_STATS = 16
+    GINT_STAT_LAUNCHES_VLOCAL = 16, /* kernels one gint_vlocal call launches (memsets not counted)          */
+    GINT_STAT_LAUNCHES_RHO = 17,  /* kernels one gint_rho call launches                                     */
+    GINT_N_STATS = 18
 };
 int gint_stats(gint_ctx* ctx, long long* out);
+
+/* Device durations (seconds) of the dominant kernels in the LAST gint_vlocal / gint_rho call on this context,
+ * measured with CUDA events recorded on the caller's stream immediately before and after the kernel.
+ * Synchronises on those events.  out[0] = vlocal contraction kernel, out[1] = rho contraction kernel; an entry
+ * is -1 when that call has not been made yet. */
+int gint_kernel_times(gint_ctx* ctx, double out[2]);
 
 int gint_free(gint_ctx* ctx);
 

@@ -253,6 +253,7 @@ static void free_ctx(gint_ctx* c) {
     cudaFree(c->d_crow); cudaFree(c->d_ckey); cudaFree(c->d_coff); cudaFree(c->d_cpub); cudaFree(c->d_cmir); cudaFree(c->d_cval);
     cudaFree(c->d_bstart); cudaFree(c->d_bent); cudaFree(c->d_order);
     cudaFree(c->d_stage_in); cudaFree(c->d_stage_out);
+    for (auto& e : c->ev) if (e) cudaEventDestroy(e);
     delete c;
 }
 
@@ -308,8 +309,8 @@ static int build_basis(gint_ctx* c, int n_species, const int* n_shell, const int
 static int build_pairs(gint_ctx* c) {
     const int n = c->n_atoms;
     Geom& g = c->geom;
-    int* d_cnt; GINT_CUDA(cudaMalloc(&d_cnt, sizeof(int) * n));
-    k_pairs<false><<<n, 256>>>(g, n, c->d_atom_pos, c->d_atom_species, c->d_species, d_cnt, nullptr, nullptr, nullptr);
+    int* d_cnt; GINT_CUDA(cudaMalloc(&d_cnt, sizeof(int) * (n ? n : 1)));
+    if (n > 0) k_pairs<false><<<n, 256>>>(g, n, c->d_atom_pos, c->d_atom_species, c->d_species, d_cnt, nullptr, nullptr, nullptr);
     GINT_CUDA(cudaGetLastError());
     std::vector<int> cnt(n);
     GINT_CUDA(cudaMemcpy(cnt.data(), d_cnt, sizeof(int) * n, cudaMemcpyDeviceToHost));
@@ -322,12 +323,14 @@ static int build_pairs(gint_ctx* c) {
     GINT_CUDA(cudaMalloc(&d_pB, sizeof(int) * (np ? np : 1)));
     GINT_CUDA(cudaMalloc(&d_pR, sizeof(int) * 3 * (np ? np : 1)));
     GINT_CUDA(cudaMemcpy(d_rs, rs.data(), sizeof(long long) * (n + 1), cudaMemcpyHostToDevice));
-    k_pairs<true><<<n, 256>>>(g, n, c->d_atom_pos, c->d_atom_species, c->d_species, d_cnt, d_rs, d_pB, d_pR);
+    if (n > 0) k_pairs<true><<<n, 256>>>(g, n, c->d_atom_pos, c->d_atom_species, c->d_species, d_cnt, d_rs, d_pB, d_pR);
     GINT_CUDA(cudaGetLastError());
     c->n_pairs = np;
     c->h_pA.resize(np); c->h_pB.resize(np); c->h_pR.resize(3 * np); c->h_poff.resize(np + 1);
-    GINT_CUDA(cudaMemcpy(c->h_pB.data(), d_pB, sizeof(int) * np, cudaMemcpyDeviceToHost));
-    GINT_CUDA(cudaMemcpy(c->h_pR.data(), d_pR, sizeof(int) * 3 * np, cudaMemcpyDeviceToHost));
+    if (np > 0) {
+        GINT_CUDA(cudaMemcpy(c->h_pB.data(), d_pB, sizeof(int) * np, cudaMemcpyDeviceToHost));
+        GINT_CUDA(cudaMemcpy(c->h_pR.data(), d_pR, sizeof(int) * 3 * np, cudaMemcpyDeviceToHost));
+    }
     cudaFree(d_cnt); cudaFree(d_rs); cudaFree(d_pB); cudaFree(d_pR);
 
     // host bookkeeping: offsets, canonical half, mirror map (integer work on ~1e6 keys)
@@ -579,6 +582,7 @@ extern "C" int gint_init(gint_ctx** out, int n_species, const int* n_shell, cons
     }
     c->smem_bytes = gint_smem_needed(g);
     if ((rc = gint_configure_kernels(c))) { free_ctx(c); return rc; }
+    for (auto& e : c->ev) GINT_CUDA(cudaEventCreate(&e));
     GINT_CUDA(cudaDeviceSynchronize());
     *out = c;
     return GINT_OK;
@@ -625,6 +629,22 @@ extern "C" int gint_stats(gint_ctx* ctx, long long* out) {
     out[GINT_STAT_ALG_INCIDENCE] = ctx->alg[0]; out[GINT_STAT_ALG_SUM_N] = ctx->alg[1]; out[GINT_STAT_ALG_SUM_N2] = ctx->alg[2];
     out[GINT_STAT_NONEMPTY_POINTS] = ctx->alg[3];
     out[GINT_STAT_SMEM_BYTES] = (long long)ctx->smem_bytes; out[GINT_STAT_DEVICE_BYTES] = (long long)ctx->device_bytes;
+    out[GINT_STAT_LAUNCHES_VLOCAL] = 2; out[GINT_STAT_LAUNCHES_RHO] = 2;
+    return GINT_OK;
+}
+
+extern "C" int gint_kernel_times(gint_ctx* ctx, double out[2]) {
+    if (!ctx) GINT_FAIL(GINT_ERR_BAD_STATE, "NULL context");
+    if (!out) GINT_FAIL(GINT_ERR_INVALID_ARG, "NULL output");
+    GINT_CUDA(cudaSetDevice(ctx->device));
+    for (int k = 0; k < 2; k++) {
+        out[k] = -1.0;
+        if (!ctx->timed[k]) continue;
+        float ms = 0.f;
+        GINT_CUDA(cudaEventSynchronize(ctx->ev[2 * k + 1]));
+        GINT_CUDA(cudaEventElapsedTime(&ms, ctx->ev[2 * k], ctx->ev[2 * k + 1]));
+        out[k] = 1e-3 * (double)ms;
+    }
     return GINT_OK;
 }
 

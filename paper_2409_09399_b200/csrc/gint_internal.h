@@ -113,6 +113,9 @@ struct gint_ctx {
     // lazily computed statistics
     bool have_alg = false;
     long long alg[4] = {0, 0, 0, 0};
+    // CUDA events around the two main kernels (gint_kernel_times)
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    bool timed[2] = {false, false};
     // host-path staging
     double* d_stage_in = nullptr; size_t stage_in_n = 0;
     double* d_stage_out = nullptr; size_t stage_out_n = 0;

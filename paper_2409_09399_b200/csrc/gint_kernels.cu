@@ -494,9 +494,12 @@ int gint_launch_vlocal(gint_ctx* c, const double* V, double* H, cudaStream_t st)
     if (c->n_values == 0) return GINT_OK;
     GINT_CUDA(cudaMemsetAsync(c->d_cval, 0, sizeof(double) * (size_t)c->n_cvalues, st));
     if (c->n_batch > 0) {
+        GINT_CUDA(cudaEventRecord(c->ev[0], st));
         k_vlocal<<<(unsigned)c->n_batch, GINT_THREADS, c->smem_bytes, st>>>(c->geom, c->d_order, c->d_bstart, c->d_bent, c->d_atom_pos,
             c->d_atom_species, c->d_species, c->d_tab, c->d_crow, c->d_ckey, c->d_coff, V, c->d_cval);
         GINT_CUDA(cudaGetLastError());
+        GINT_CUDA(cudaEventRecord(c->ev[1], st));
+        c->timed[0] = true;
     }
     k_expand_H<<<(unsigned)((c->n_pairs + 7) / 8), 256, 0, st>>>(c->n_pairs, c->d_poff, c->d_pcanon, c->d_pflag, c->d_pnA, c->d_coff, c->d_cval, H);
     GINT_CUDA(cudaGetLastError());
@@ -510,9 +513,12 @@ int gint_launch_rho(gint_ctx* c, const double* D, double* rho, cudaStream_t st) 
     if (c->n_batch == 0) return GINT_OK;
     k_sym_D<<<(unsigned)((c->n_canon + 7) / 8), 256, 0, st>>>(c->n_canon, c->d_poff, c->d_cpub, c->d_cmir, c->d_pnA, c->d_coff, D, c->d_cval);
     GINT_CUDA(cudaGetLastError());
+    GINT_CUDA(cudaEventRecord(c->ev[2], st));
     k_rho<<<(unsigned)c->n_batch, GINT_THREADS, c->smem_bytes, st>>>(c->geom, c->d_order, c->d_bstart, c->d_bent, c->d_atom_pos,
         c->d_atom_species, c->d_species, c->d_tab, c->d_crow, c->d_ckey, c->d_coff, c->d_cval, rho);
     GINT_CUDA(cudaGetLastError());
+    GINT_CUDA(cudaEventRecord(c->ev[3], st));
+    c->timed[1] = true;
     return GINT_OK;
 }
 

@@ -17,10 +17,10 @@ _lib = None
 
 STAT_NAMES = ("n_batch", "n_batch_empty", "batch_bx", "batch_by", "batch_bz", "neigh_entries", "max_nb", "max_cols",
               "padded_macs", "n_canon", "alg_incidence", "alg_sum_n", "alg_sum_n2", "nonempty_points", "smem_bytes",
-              "device_bytes")
+              "device_bytes", "launches_vlocal", "launches_rho")
 
 EXPORTS = ("gint_init", "gint_n_orb", "gint_n_pairs", "gint_get_pairs", "gint_vlocal", "gint_rho", "gint_vlocal_host",
-           "gint_rho_host", "gint_stats", "gint_free", "gint_last_error")
+           "gint_rho_host", "gint_stats", "gint_kernel_times", "gint_free", "gint_last_error")
 
 
 class GintError(RuntimeError):
@@ -102,6 +102,12 @@ class Gint:
         out = np.zeros(len(STAT_NAMES), np.int64)
         _check(lib().gint_stats(self._ctx, out.ctypes.data_as(C.POINTER(C.c_longlong))))
         return dict(zip(STAT_NAMES, (int(x) for x in out)))
+
+    def kernel_times(self) -> dict:
+        """Device seconds of the main contraction kernels in the last vlocal / rho call (CUDA events in the library)."""
+        out = (C.c_double * 2)()
+        _check(lib().gint_kernel_times(self._ctx, out))
+        return {"vlocal_main": float(out[0]), "rho_main": float(out[1])}
 
     # ------------------------------------------------------------------ device path
     @staticmethod
