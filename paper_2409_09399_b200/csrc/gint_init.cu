@@ -133,14 +133,23 @@ __global__ void __launch_bounds__(256) k_coarse_candidates(Geom g, int cbx, int 
 
 // Stage B: one warp per batch.  An image is a neighbour of the batch iff at least one batch point is closer
 // than rc, decided on the same numbers the orbital evaluation uses (mesh_point()).
+// COUNT pass: number of neighbours and of their orbitals.  FILL pass: the entries, sorted by falling activity
+// (number of batch points inside the sphere; ties keep the (atom, shift) order) so that the atoms that are non-zero
+// on every point of the batch come first and atoms with similar zero patterns share fragments of 8 orbitals;
+// then the number G of atom groups the contraction kernels tile this batch with (<= GINT_TILE_ATOMS atoms and
+// <= GINT_TILE_ORB orbitals per group).
 template <bool FILL>
 __global__ void __launch_bounds__(256) k_batch_neighbours(Geom g, int cbx, int cby, int cbz, int ncy, int ncz,
                                                           const ImageDev* __restrict__ img, int cap, const int* __restrict__ cand,
                                                           const int* __restrict__ cand_count, long long n_batch_total,
                                                           int* __restrict__ count, int* __restrict__ cols,
                                                           const SpeciesDev* __restrict__ sp, const int* __restrict__ spec,
-                                                          const int* __restrict__ bstart, NeighEntry* __restrict__ bent) {
-    const long long b = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
+                                                          const int* __restrict__ bstart, NeighEntry* __restrict__ bent,
+                                                          int* __restrict__ bgroups) {
+    __shared__ int s_act[FILL ? 8 : 1][FILL ? GINT_MAX_NB : 1];
+    __shared__ int s_img[FILL ? 8 : 1][FILL ? GINT_MAX_NB : 1];
+    const int w = threadIdx.x >> 5;
+    const long long b = (long long)blockIdx.x * 8 + w;
     const int lane = threadIdx.x & 31;
     if (b >= n_batch_total) return;
     const int bz = (int)(b % g.nb[2]), by = (int)((b / g.nb[2]) % g.nb[1]), bx = (int)(b / ((long long)g.nb[2] * g.nb[1]));
@@ -148,31 +157,68 @@ __global__ void __launch_bounds__(256) k_batch_neighbours(Geom g, int cbx, int c
     const int ex = min(g.bs[0], g.N[0] - i0), ey = min(g.bs[1], g.N[1] - j0), ez = min(g.bs[2], g.N[2] - k0);
     const int Kb = ex * ey * ez;
     const int cell = ((bx / cbx) * ncy + (by / cby)) * ncz + (bz / cbz);
-    // this lane's points (up to GINT_MAX_K/32 = 4)
-    double px[4], py[4], pz[4];
-    int np = 0;
-    for (int q = lane; q < Kb; q += 32) {
-        int qk = q % ez, qj = (q / ez) % ey, qi = q / (ez * ey);
-        mesh_point(g, i0 + qi, j0 + qj, k0 + qk, px[np], py[np], pz[np]);
-        np++;
-    }
     int n = 0, ncol = 0;
     const int nc = min(cand_count[cell], cap);
-    const int base = FILL ? bstart[b] : 0;
     for (int c = 0; c < nc; c++) {
-        const ImageDev im = img[cand[(size_t)cell * cap + c]];
-        bool hit = false;
-        for (int t = 0; t < np; t++) {
-            double dx = px[t] - im.x, dy = py[t] - im.y, dz = pz[t] - im.z;
-            hit |= sqrt(dx * dx + dy * dy + dz * dz) < im.rc;
+        const int qi = cand[(size_t)cell * cap + c];
+        const ImageDev im = img[qi];
+        int hits = 0;
+        for (int q = lane; q < Kb; q += 32) {
+            const int qk = q % ez, qj = (q / ez) % ey, qx = q / (ez * ey);
+            double px, py, pz;
+            mesh_point(g, i0 + qx, j0 + qj, k0 + qk, px, py, pz);
+            const double dx = px - im.x, dy = py - im.y, dz = pz - im.z;
+            hits += sqrt(dx * dx + dy * dy + dz * dz) < im.rc;
         }
-        if (__any_sync(0xffffffffu, hit)) {
-            if (FILL && lane == 0) { bent[base + n].atom = im.atom; bent[base + n].shift = im.shift; }
+#pragma unroll
+        for (int d = 16; d; d >>= 1) hits += __shfl_xor_sync(0xffffffffu, hits, d);
+        if (hits > 0) {
+            if (FILL && lane == 0 && n < GINT_MAX_NB) { s_act[w][n] = hits; s_img[w][n] = qi; }
             n++;
             ncol += sp[spec[im.atom]].norb;
         }
     }
-    if (!FILL && lane == 0) { count[b] = n; cols[b] = ncol; }
+    if (!FILL) {
+        if (lane == 0) { count[b] = n; cols[b] = ncol; }
+        return;
+    }
+    __syncwarp();
+    const int base = bstart[b];
+    for (int e = lane; e < n; e += 32) {                   // rank sort by (activity desc, position asc)
+        const int a = s_act[w][e];
+        int rank = 0;
+        for (int j = 0; j < n; j++) { const int aj = s_act[w][j]; rank += (aj > a) || (aj == a && j < e); }
+        const ImageDev im = img[s_img[w][e]];
+        bent[base + rank].atom = im.atom; bent[base + rank].shift = im.shift;
+    }
+    __syncwarp();
+    if (lane == 0) {
+        int G = (n + GINT_TILE_ATOMS - 1) / GINT_TILE_ATOMS;
+        for (; G < n; G++) {
+            bool ok = true;
+            for (int k = 0; k < G && ok; k++) {
+                int o = 0;
+                for (int e = group_begin(k, n, G); e < group_begin(k + 1, n, G); e++) o += sp[spec[bent[base + e].atom]].norb;
+                ok = o <= GINT_TILE_ORB;
+            }
+            if (ok) break;
+        }
+        bgroups[b] = G;
+    }
+}
+
+// tile descriptors: all group pairs I <= J of every batch, batches in mesh order
+__global__ void __launch_bounds__(256) k_tiles_fill(long long n_batch_total, const int* __restrict__ bgroups,
+                                                    const int* __restrict__ tstart, int2* __restrict__ tile) {
+    const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= n_batch_total) return;
+    const int G = bgroups[b];
+    int o = tstart[b];
+    for (int I = 0; I < G; I++) for (int J = I; J < G; J++) tile[o++] = make_int2((int)b, I | (J << 8) | (G << 16));
+}
+__global__ void __launch_bounds__(256) k_tiles_count(long long n, const int* __restrict__ bgroups, int* __restrict__ tcount) {
+    const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < n) { const int G = bgroups[b]; tcount[b] = G * (G + 1) / 2; }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -251,7 +297,7 @@ static void free_ctx(gint_ctx* c) {
     cudaFree(c->d_species); cudaFree(c->d_tab); cudaFree(c->d_atom_pos); cudaFree(c->d_atom_species);
     cudaFree(c->d_poff); cudaFree(c->d_pcanon); cudaFree(c->d_pflag); cudaFree(c->d_pnA);
     cudaFree(c->d_crow); cudaFree(c->d_ckey); cudaFree(c->d_coff); cudaFree(c->d_cpub); cudaFree(c->d_cmir); cudaFree(c->d_cval);
-    cudaFree(c->d_bstart); cudaFree(c->d_bent); cudaFree(c->d_order);
+    cudaFree(c->d_bstart); cudaFree(c->d_bent); cudaFree(c->d_tile);
     cudaFree(c->d_stage_in); cudaFree(c->d_stage_out);
     for (auto& e : c->ev) if (e) cudaEventDestroy(e);
     delete c;
@@ -410,7 +456,6 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, bool* 
     for (int i = 0; i < 3; i++) { g.bs[i] = std::min(bs[i], g.N[i]); g.nb[i] = (g.N[i] + g.bs[i] - 1) / g.bs[i]; }
     g.K = g.bs[0] * g.bs[1] * g.bs[2];
     if (g.K > GINT_MAX_K) GINT_FAIL(GINT_ERR_UNSUPPORTED, "batch of %d points (max %d)", g.K, GINT_MAX_K);
-    g.LD = ((g.K + 15) / 16) * 16 + 4;
     const long long nbt = (long long)g.nb[0] * g.nb[1] * g.nb[2];
     if (nbt > 2000000000LL) GINT_FAIL(GINT_ERR_UNSUPPORTED, "%lld batches", nbt);
     c->n_batch_total = nbt;
@@ -471,7 +516,7 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, bool* 
     GINT_CUDA(cudaMalloc(&d_cols, sizeof(int) * nbt));
     const unsigned gridB = (unsigned)((nbt + 7) / 8);
     k_batch_neighbours<false><<<gridB, 256>>>(g, cb[0], cb[1], cb[2], nc[1], nc[2], d_img, cap, d_cand, d_ccount, nbt, d_count, d_cols,
-                                              c->d_species, c->d_atom_species, nullptr, nullptr);
+                                              c->d_species, c->d_atom_species, nullptr, nullptr, nullptr);
     GINT_CUDA(cudaGetLastError());
     std::vector<int> count(nbt), cols(nbt);
     GINT_CUDA(cudaMemcpy(count.data(), d_count, sizeof(int) * nbt, cudaMemcpyDeviceToHost));
@@ -479,7 +524,7 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, bool* 
     int max_nb = 0, max_cols = 0;
     for (long long b = 0; b < nbt; b++) { max_nb = std::max(max_nb, count[b]); max_cols = std::max(max_cols, cols[b]); }
     g.max_nb = std::max(max_nb, 1); g.max_cols = std::max(max_cols, 1);
-    const bool ok = max_nb <= GINT_MAX_NB && gint_smem_needed(g) <= smem_limit;
+    const bool ok = max_nb <= GINT_MAX_NB && gint_smem_needed(g) <= smem_limit;     // else: try a smaller batch shape
     if (!ok) { cudaFree(d_img); cudaFree(d_cand); cudaFree(d_ccount); cudaFree(d_count); cudaFree(d_cols); return GINT_OK; }
     *fits = true;
 
@@ -489,22 +534,28 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, bool* 
     if ((rc = device_excl_scan(d_count, nbt, c->d_bstart, &n_ent))) return rc;
     c->n_entries = n_ent;
     if ((rc = dev_alloc(c, &c->d_bent, (size_t)n_ent))) return rc;
+    int *d_bgroups = nullptr, *d_tcount = nullptr, *d_tstart = nullptr;
+    GINT_CUDA(cudaMalloc(&d_bgroups, sizeof(int) * nbt));
+    GINT_CUDA(cudaMalloc(&d_tcount, sizeof(int) * nbt));
+    GINT_CUDA(cudaMalloc(&d_tstart, sizeof(int) * (nbt + 1)));
     k_batch_neighbours<true><<<gridB, 256>>>(g, cb[0], cb[1], cb[2], nc[1], nc[2], d_img, cap, d_cand, d_ccount, nbt, d_count, d_cols,
-                                             c->d_species, c->d_atom_species, c->d_bstart, c->d_bent);
+                                             c->d_species, c->d_atom_species, c->d_bstart, c->d_bent, d_bgroups);
+    GINT_CUDA(cudaGetLastError());
+    const unsigned gridT = (unsigned)((nbt + 255) / 256);
+    k_tiles_count<<<gridT, 256>>>(nbt, d_bgroups, d_tcount);
+    GINT_CUDA(cudaGetLastError());
+    long long n_tiles = 0;
+    if ((rc = device_excl_scan(d_tcount, nbt, d_tstart, &n_tiles))) return rc;
+    c->n_tiles = n_tiles;
+    if ((rc = dev_alloc(c, &c->d_tile, (size_t)n_tiles))) return rc;
+    k_tiles_fill<<<gridT, 256>>>(nbt, d_bgroups, d_tstart, c->d_tile);
     GINT_CUDA(cudaGetLastError());
     GINT_CUDA(cudaDeviceSynchronize());
     cudaFree(d_img); cudaFree(d_cand); cudaFree(d_ccount); cudaFree(d_count); cudaFree(d_cols);
+    cudaFree(d_bgroups); cudaFree(d_tcount); cudaFree(d_tstart);
 
-    // schedule: non-empty batches heavy-first (stable counting sort on the orbital count, so batches of equal
-    // weight keep their spatial order and concurrently running CTAs touch neighbouring H / D blocks), empty last.
-    std::vector<long long> hist(max_cols + 2, 0);
-    for (long long b = 0; b < nbt; b++) hist[max_cols - cols[b]]++;
-    long long acc = 0;
-    for (int k = 0; k <= max_cols; k++) { long long t = hist[k]; hist[k] = acc; acc += t; }
-    std::vector<int> order(nbt);
     c->padded_macs = 0; c->n_batch = 0;
     for (long long b = 0; b < nbt; b++) {
-        order[hist[max_cols - cols[b]]++] = (int)b;
         if (cols[b] > 0) {
             c->n_batch++;
             int bz = (int)(b % g.nb[2]), by = (int)((b / g.nb[2]) % g.nb[1]), bx = (int)(b / ((long long)g.nb[2] * g.nb[1]));
@@ -513,7 +564,6 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, bool* 
         }
     }
     c->n_batch_empty = nbt - c->n_batch;
-    if ((rc = dev_upload(c, &c->d_order, order))) return rc;
     return GINT_OK;
 }
 
@@ -554,6 +604,7 @@ extern "C" int gint_init(gint_ctx** out, int n_species, const int* n_shell, cons
     for (int i = 0; i < 3; i++) g.N[i] = mesh[i];
     g.dV = det3(cell) / ((double)mesh[0] * mesh[1] * mesh[2]);
     g.inv_dr = 1.0 / dr;
+    for (int i = 0; i < 3; i++) for (int k = 0; k < 3; k++) g.step[3 * i + k] = cell[3 * i + k] / (double)mesh[i];
     c->n_atoms = n_atoms;
     c->h_atom_species.assign(atom_species, atom_species + n_atoms);
     c->h_atom_pos.assign(atom_pos, atom_pos + 3 * (size_t)n_atoms);
@@ -569,11 +620,11 @@ extern "C" int gint_init(gint_ctx** out, int n_species, const int* n_shell, cons
     const int fx = (int)(flags & 255), fy = (int)((flags >> 8) & 255), fz = (int)((flags >> 16) & 255);
     bool fits = false;
     if (fx || fy || fz) {
-        const int bs[3] = {fx ? fx : 4, fy ? fy : 4, fz ? fz : 4};
+        const int bs[3] = {fx ? fx : 8, fy ? fy : 8, fz ? fz : 8};
         if ((rc = build_batches(c, bs, smem_limit, &fits))) { free_ctx(c); return rc; }
         if (!fits) { free_ctx(c); GINT_FAIL(GINT_ERR_UNSUPPORTED, "requested batch %dx%dx%d needs more shared memory than %zu bytes (or > %d neighbours)", bs[0], bs[1], bs[2], smem_limit, GINT_MAX_NB); }
     } else {
-        static const int shapes[][3] = {{4, 4, 4}, {4, 4, 2}, {4, 2, 2}, {2, 2, 2}, {2, 2, 1}, {1, 1, 1}};
+        static const int shapes[][3] = {{8, 8, 8}, {4, 4, 8}, {4, 4, 4}, {2, 2, 4}, {1, 1, 4}, {1, 1, 1}};
         for (auto& s : shapes) {
             if ((rc = build_batches(c, s, smem_limit, &fits))) { free_ctx(c); return rc; }
             if (fits) break;

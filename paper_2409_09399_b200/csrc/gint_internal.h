@@ -12,8 +12,14 @@
 
 #define GINT_MAX_SHELL 12          // radial shells per species
 #define GINT_MAX_NB 96             // neighbouring atom images per grid batch
-#define GINT_MAX_K 128             // mesh points per grid batch
+#define GINT_MAX_K 4096            // mesh points per grid batch
 #define GINT_THREADS 512           // threads per CTA of the contraction kernels (16 warps)
+// tile geometry of the contraction kernels: one CTA owns the block of H (or D) between two groups of atoms
+#define GINT_TILE_ATOMS 8          // atom images per group
+#define GINT_TILE_ORB 104          // orbitals per group = 13 fragments of 8 (8 atoms x 13 orbitals exactly)
+#define GINT_TILE_FRAG 13
+#define GINT_CHUNK 32              // mesh points evaluated per pipeline stage (8 k-steps of 4 points)
+#define GINT_LD 36                 // row stride (doubles) of the orbital tiles in shared memory: = 4 mod 16, conflict-free
 
 // ---- error plumbing -------------------------------------------------------------------------------
 void gint_set_error(const char* fmt, ...);
@@ -38,13 +44,13 @@ struct Geom {
     double a[9];                    // cell rows a1,a2,a3
     double inv[9];                  // frac = pos * inv (row vector convention)
     double hgt[3];                  // distance between lattice planes along each axis
+    double step[9];                 // mesh steps: rows a1/N1, a2/N2, a3/N3
     double dV;
     double inv_dr;
     int N[3];                       // mesh
     int bs[3];                      // batch edge lengths (points)
     int nb[3];                      // batches along each axis
     int K;                          // bs[0]*bs[1]*bs[2]
-    int LD;                         // leading dimension (doubles) of the orbital tile in shared memory
     int key_m;                      // pair keys: |n_i| <= key_m, key_M = 2*key_m+1
     int key_M;
     int max_cols;                   // max orbitals of one batch
@@ -65,10 +71,10 @@ __host__ __device__ inline void unpack_shift(int s, int& t1, int& t2, int& t3) {
 // Mesh point (i,j,k) -> Cartesian position (reading R1).  Used by the neighbour pass AND the orbital
 // evaluation so that both take the |d| < rc decision on bit-identical numbers.
 __host__ __device__ inline void mesh_point(const Geom& g, int i, int j, int k, double& x, double& y, double& z) {
-    double u = (double)i / (double)g.N[0], v = (double)j / (double)g.N[1], w = (double)k / (double)g.N[2];
-    x = u * g.a[0] + v * g.a[3] + w * g.a[6];
-    y = u * g.a[1] + v * g.a[4] + w * g.a[7];
-    z = u * g.a[2] + v * g.a[5] + w * g.a[8];
+    const double u = (double)i, v = (double)j, w = (double)k;
+    x = fma(w, g.step[6], fma(v, g.step[3], u * g.step[0]));
+    y = fma(w, g.step[7], fma(v, g.step[4], u * g.step[1]));
+    z = fma(w, g.step[8], fma(v, g.step[5], u * g.step[2]));
 }
 
 struct gint_ctx {
@@ -106,7 +112,9 @@ struct gint_ctx {
     long long n_batch_total = 0, n_batch = 0, n_batch_empty = 0, n_entries = 0;
     int* d_bstart = nullptr;         // [n_batch_total+1] CSR into d_bent
     NeighEntry* d_bent = nullptr;    // neighbour entries sorted by (atom, shift lexicographic)
-    int* d_order = nullptr;          // [n_batch_total] batch ids: non-empty heavy-first, then empty ones
+    int* d_order = nullptr;          // [n_batch_total] batch ids: non-empty first (mesh order), then empty ones
+    long long n_tiles = 0;
+    int2* d_tile = nullptr;          // [n_tiles] {batch id, I | J<<8 | G<<16}: group pair (I <= J) of G groups of the batch
     long long padded_macs = 0;
     size_t smem_bytes = 0;
     size_t device_bytes = 0;
@@ -127,3 +135,6 @@ int gint_launch_rho(gint_ctx* c, const double* D, double* rho, cudaStream_t st);
 int gint_launch_alg_stats(gint_ctx* c);
 int gint_configure_kernels(gint_ctx* c);
 size_t gint_smem_needed(const Geom& g);
+
+// Split of the n neighbour entries of a batch into G groups of consecutive entries: group k = [k*n/G, (k+1)*n/G).
+__host__ __device__ inline int group_begin(int k, int n, int G) { return (int)(((long long)k * n) / G); }
