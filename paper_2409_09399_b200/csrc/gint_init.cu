@@ -148,6 +148,7 @@ __global__ void __launch_bounds__(256) k_batch_neighbours(Geom g, int cbx, int c
                                                           int* __restrict__ bgroups) {
     __shared__ int s_act[FILL ? 8 : 1][FILL ? GINT_MAX_NB : 1];
     __shared__ int s_img[FILL ? 8 : 1][FILL ? GINT_MAX_NB : 1];
+    __shared__ unsigned s_mlo[FILL ? 8 : 1][FILL ? GINT_MAX_NB : 1], s_mhi[FILL ? 8 : 1][FILL ? GINT_MAX_NB : 1];
     const int w = threadIdx.x >> 5;
     const long long b = (long long)blockIdx.x * 8 + w;
     const int lane = threadIdx.x & 31;
@@ -163,17 +164,21 @@ __global__ void __launch_bounds__(256) k_batch_neighbours(Geom g, int cbx, int c
         const int qi = cand[(size_t)cell * cap + c];
         const ImageDev im = img[qi];
         int hits = 0;
+        unsigned mlo = 0, mhi = 0;
         for (int q = lane; q < Kb; q += 32) {
             const int qk = q % ez, qj = (q / ez) % ey, qx = q / (ez * ey);
             double px, py, pz;
             mesh_point(g, i0 + qx, j0 + qj, k0 + qk, px, py, pz);
             const double dx = px - im.x, dy = py - im.y, dz = pz - im.z;
-            hits += sqrt(dx * dx + dy * dy + dz * dz) < im.rc;
+            const bool in = fma(dx, dx, fma(dy, dy, dz * dz)) < im.rc * im.rc;    // same expression as the orbital evaluation
+            hits += in;
+            if (FILL && in) { const int cl = (qx >> 1) * 16 + (qj >> 1) * 4 + (qk >> 1); if (cl < 32) mlo |= 1u << cl; else mhi |= 1u << (cl - 32); }
         }
 #pragma unroll
         for (int d = 16; d; d >>= 1) hits += __shfl_xor_sync(0xffffffffu, hits, d);
+        if (FILL) { mlo = __reduce_or_sync(0xffffffffu, mlo); mhi = __reduce_or_sync(0xffffffffu, mhi); }
         if (hits > 0) {
-            if (FILL && lane == 0 && n < GINT_MAX_NB) { s_act[w][n] = hits; s_img[w][n] = qi; }
+            if (FILL && lane == 0 && n < GINT_MAX_NB) { s_act[w][n] = hits; s_img[w][n] = qi; s_mlo[w][n] = mlo; s_mhi[w][n] = mhi; }
             n++;
             ncol += sp[spec[im.atom]].norb;
         }
@@ -190,6 +195,7 @@ __global__ void __launch_bounds__(256) k_batch_neighbours(Geom g, int cbx, int c
         for (int j = 0; j < n; j++) { const int aj = s_act[w][j]; rank += (aj > a) || (aj == a && j < e); }
         const ImageDev im = img[s_img[w][e]];
         bent[base + rank].atom = im.atom; bent[base + rank].shift = im.shift;
+        bent[base + rank].mask = (unsigned long long)s_mlo[w][e] | ((unsigned long long)s_mhi[w][e] << 32);
     }
     __syncwarp();
     if (lane == 0) {
@@ -455,7 +461,7 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, bool* 
     *fits = false;
     for (int i = 0; i < 3; i++) { g.bs[i] = std::min(bs[i], g.N[i]); g.nb[i] = (g.N[i] + g.bs[i] - 1) / g.bs[i]; }
     g.K = g.bs[0] * g.bs[1] * g.bs[2];
-    if (g.K > GINT_MAX_K) GINT_FAIL(GINT_ERR_UNSUPPORTED, "batch of %d points (max %d)", g.K, GINT_MAX_K);
+    for (int i = 0; i < 3; i++) if (bs[i] < 1 || bs[i] > GINT_MAX_BS) GINT_FAIL(GINT_ERR_UNSUPPORTED, "batch edge %d (1..%d supported)", bs[i], GINT_MAX_BS);
     const long long nbt = (long long)g.nb[0] * g.nb[1] * g.nb[2];
     if (nbt > 2000000000LL) GINT_FAIL(GINT_ERR_UNSUPPORTED, "%lld batches", nbt);
     c->n_batch_total = nbt;
@@ -580,7 +586,7 @@ extern "C" int gint_init(gint_ctx** out, int n_species, const int* n_shell, cons
     for (int i = 0; i < 9; i++) if (!std::isfinite(cell[i])) GINT_FAIL(GINT_ERR_INVALID_ARG, "cell has a non-finite entry");
     if (!(det3(cell) > 0)) GINT_FAIL(GINT_ERR_INVALID_ARG, "det(cell) = %g must be positive", det3(cell));
     for (int i = 0; i < 3; i++) if (mesh[i] < 1) GINT_FAIL(GINT_ERR_INVALID_ARG, "mesh[%d] = %d", i, mesh[i]);
-    if ((double)mesh[0] * mesh[1] * mesh[2] > 2.0e9 * GINT_MAX_K) GINT_FAIL(GINT_ERR_UNSUPPORTED, "mesh too large");
+    if ((double)mesh[0] * mesh[1] * mesh[2] > 2.0e9 * 512) GINT_FAIL(GINT_ERR_UNSUPPORTED, "mesh too large");
     for (int a = 0; a < n_atoms; a++) {
         if (atom_species[a] < 0 || atom_species[a] >= n_species) GINT_FAIL(GINT_ERR_INVALID_ARG, "atom %d: species %d out of range", a, atom_species[a]);
         for (int k = 0; k < 3; k++) if (!std::isfinite(atom_pos[3 * a + k])) GINT_FAIL(GINT_ERR_INVALID_ARG, "atom %d: non-finite position", a);

@@ -12,14 +12,17 @@
 
 #define GINT_MAX_SHELL 12          // radial shells per species
 #define GINT_MAX_NB 96             // neighbouring atom images per grid batch
-#define GINT_MAX_K 4096            // mesh points per grid batch
-#define GINT_THREADS 512           // threads per CTA of the contraction kernels (16 warps)
+#define GINT_MAX_BS 8              // largest grid-batch edge (points): 4 x 4 x 4 cubelets of 2 x 2 x 2 points = one 64-bit mask
+#define GINT_WARPS 16              // warps per CTA of the contraction kernels
+#define GINT_THREADS (32 * GINT_WARPS)
 // tile geometry of the contraction kernels: one CTA owns the block of H (or D) between two groups of atoms
 #define GINT_TILE_ATOMS 8          // atom images per group
 #define GINT_TILE_ORB 104          // orbitals per group = 13 fragments of 8 (8 atoms x 13 orbitals exactly)
 #define GINT_TILE_FRAG 13
-#define GINT_CHUNK 32              // mesh points evaluated per pipeline stage (8 k-steps of 4 points)
-#define GINT_LD 36                 // row stride (doubles) of the orbital tiles in shared memory: = 4 mod 16, conflict-free
+#define GINT_SEG_COLS 7            // column fragments of one segment (a warp owns two segments: row fragment x <= 7 column fragments)
+#define GINT_MAX_SEG (2 * GINT_WARPS)
+#define GINT_CHUNK 32              // mesh points per pipeline stage = 4 cubelets of 8 points
+#define GINT_LD 40                 // row stride (doubles) of the orbital tiles in shared memory: = 8 mod 16, LDS.128 conflict-free
 
 // ---- error plumbing -------------------------------------------------------------------------------
 void gint_set_error(const char* fmt, ...);
@@ -61,6 +64,7 @@ struct Geom {
 struct NeighEntry {
     int atom;
     int shift;                      // (t1+64) | (t2+64)<<8 | (t3+64)<<16
+    unsigned long long mask;        // bit (cx*16 + cy*4 + cz): cubelet (2x2x2 points) of the batch with a point inside the sphere
 };
 
 __host__ __device__ inline int pack_shift(int t1, int t2, int t3) { return (t1 + 64) | ((t2 + 64) << 8) | ((t3 + 64) << 16); }

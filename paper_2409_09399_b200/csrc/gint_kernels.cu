@@ -1,102 +1,91 @@
 // gint_kernels.cu -- the per-call hot path (north_star steps 2 and 3), fp64, sm_100a.
 //
 // Work decomposition.  The mesh is cut into grid batches (default 8x8x8 points) whose neighbouring
-// atom images were listed by gint_init, most active first, and split into G groups of at most
-// 8 atoms / 104 orbitals.  One CTA owns one TILE = (batch, group I, group J), I <= J: the 104 x 104 block of
-// Phi_I^T diag(V dV) Phi_J (gint_vlocal, Eq. 2) or of the density blocks D_IJ (gint_rho, Eq. 3
-// PAPER.md:73).  That block stays in REGISTERS (DMMA accumulators, resp. DMMA B fragments) while the CTA streams
-// over the batch in chunks of 32 mesh points: all 16 warps first evaluate the orbitals of the <= 16 atoms of the
-// tile at the chunk's points into shared memory (the paper's orbital-value kernel, never written to
-// global memory), then contract them on the FP64 tensor pipe (mma.sync m8n8k4 f64 = DMMA.8x8x4).  Fragments
-// (8 orbitals x 4 points) on which every atom is outside its cutoff sphere (Fig. 6: zero padding)
-// are skipped with per-chunk bit masks, so zero padding costs (almost) no arithmetic.
+// atom images were listed by gint_init, most active first, each with a 64-bit ACTIVITY MASK over the
+// batch's 4x4x4 "cubelets" of 2x2x2 mesh points (bit set = some point of the cubelet lies inside the atom's cutoff
+// sphere; Fig. 6: everything else is zero padding).  The neighbours of a batch are split into G
+// groups of at most 8 atoms / 104 orbitals.  One CTA owns one TILE = (batch, group I, group J), I <= J: the
+// 104 x 104 block of Phi_I^T diag(V dV) Phi_J (gint_vlocal, Eq. 2) or of the density blocks D_IJ
+// (gint_rho, Eq. 3).  That block stays in REGISTERS (DMMA accumulators, resp. stationary DMMA
+// operands): the 13 x 13 fragments (8 x 8 orbitals) of the block are cut into SEGMENTS of one row fragment x up to
+// 7 column fragments, two segments per warp, dealt to the 14 warps so that the four SM sub-partitions carry equal
+// numbers of DMMAs; in a diagonal tile (I == J) only the fragments on or above the atom diagonal are segments.
+// The CTA walks over the cubelets on which both groups are active, 4 cubelets (32 points) per pipeline stage: the
+// orbital values of the needed (atom, cubelet) items are evaluated into shared memory (the paper's orbital-value
+// kernel, never written to global memory; items compacted so that a quarter warp = one atom on one
+// cubelet), then every warp runs the DMMA chains (mma.sync m8n8k4 f64 = DMMA.8x8x4) of its segments on the cubelets
+// where the segment is active -- straight-line code specialised on the segment length, one bit test per cubelet.
 // Only one of each mirror pair of blocks, (A,B,n) / (B,A,-n), is accumulated ("canonical half"); small
 // streaming kernels convert between the public pair-list layout and the canonical layout.
 #include "gint_internal.h"
 
+typedef unsigned long long u64;
+#define GINT_EVAL_GROUP 3          // radial shells whose spline coefficients are loaded together (registers vs memory-level parallelism)
+
 // ---------------------------------------------------------------------------------------------------
 // shared memory of the tile kernels
+struct PairEnt { unsigned off; unsigned short sr, sc; };   // element (oa, ob) of the atom pair at off + oa*sr + ob*sc; off = ~0u: none
+struct SlotInfo { double rc2; int n_int, nsh, tab_off, lpack; };   // lpack: 2 bits of l per shell
+
 struct TileSmem {
-    // phi[stage][side][orbital row][GINT_LD]: side 0 = group I, side 1 = group J (scaled by V dV in vlocal)
+    // phi[stage][side][orbital row][GINT_LD]: side 0 = group I, side 1 = group J (scaled by V dV in vlocal);
+    // column 8q + p = point p of the stage's q-th cubelet
     double phi[2][2][GINT_TILE_ORB][GINT_LD];
-    double pos[16][3];                  // slot s < 8: atom s of group I; slot 8 + s: atom s of group J
-    double4 pts[2][GINT_CHUNK];         // [stage][point of the chunk]: x, y, z, weight (V dV in vlocal)
-    double pvalid[2][GINT_CHUNK];       // 1 = the lane's point exists (inside the batch and the mesh), 0 = padding
-    double red[GINT_CHUNK];             // rho: per-point partial sums of the chunk
-    int spec[16];
-    int atom[16];
-    int shift[16];
+    double4 pts[2][GINT_CHUNK];         // [stage][point]: x, y, z, weight (V dV in vlocal, 1 in rho)
+    double red[2][GINT_WARPS][GINT_CHUNK];   // rho: per-warp partial sums of the stage's points
+    double pos[16][4];                  // slot s < 8: atom s of group I; slot 8 + s: atom s of group J
+    SlotInfo sinfo[16];
+    u64 amask[16];                      // cubelets on which the slot's atom is non-zero
+    u64 need[16];                       // cubelets on which the slot's orbital rows are read by some segment
+    u64 fmask[2][16];                   // [side][fragment]: OR of amask over the atoms with orbitals in the fragment
+    u64 hmask[2];                       // side J: OR of fmask over the column fragments 0..6 / 7..12
+    u64 U;                              // cubelets the tile walks over: (any I fragment) & (any J fragment)
+    PairEnt pair[GINT_TILE_ATOMS][GINT_TILE_ATOMS];   // canonical block of (I atom a, J atom b)
+    int atom[16], shift[16], spec[16];
     int cstart[2][GINT_TILE_ATOMS + 1]; // first orbital row of each atom inside its group
-    unsigned int pair_off[GINT_TILE_ATOMS][GINT_TILE_ATOMS];   // canonical block offset of (I atom a, J atom b); ~0u = none
-    unsigned char pair_tr[GINT_TILE_ATOMS][GINT_TILE_ATOMS];   // 1 = the canonical key is (b, a): transposed
-    unsigned char row_atom[2][GINT_TILE_ORB];                  // orbital row -> atom slot inside the group (255 = padding)
-    unsigned char row_orb[2][GINT_TILE_ORB];                   // orbital row -> orbital index inside the atom
-    unsigned char frag_atoms[2][16];                           // fragment -> bit mask of the atoms it holds orbitals of
-    unsigned char slot_mask[2][16];                            // [stage][slot]: bit k = atom active on k-step k of the chunk
+    int seg[GINT_MAX_SEG];              // slot warp + 14 k: row fragment | first column fragment << 8 | n columns << 16
+    int nitem[2], neval[2];             // [stage]: items of the stage, of which the first neval need a real evaluation
+    int ncub;
+    unsigned char valid[2][GINT_CHUNK]; // the stage's point exists (inside the batch and the mesh)
+    unsigned char item[2][64];          // [stage][k]: slot << 2 | cubelet of the stage
+    unsigned char cub[64 + 4];          // the tile's cubelets (bit numbers of U, ascending)
+    unsigned char row_atom[2][GINT_TILE_ORB];   // orbital row -> atom slot inside the group (255 = padding)
+    unsigned char row_orb[2][GINT_TILE_ORB];    // orbital row -> orbital index inside the atom
+    unsigned char frag_atoms[2][16];            // fragment -> bit mask of the atoms it holds orbitals of
 };
 size_t gint_smem_needed(const Geom&) { return sizeof(TileSmem); }
 
-__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
-
-
-// A predicated-off DMMA still occupies the FP64 tensor pipe for its full duration (measured), and ptxas turns
-// `if (bit) dmma`, the arms of a C switch and short loops around a DMMA all into predicated DMMAs.  So the choice
-// of which of a row's four column fragments to multiply is made by an indexed branch (brx.idx) written in PTX:
-// sixteen entry points into chains of mma instructions, one per value of the 4-bit column mask.
-#define GINT_MMA(c0, c1, a, b) "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {" c0 "," c1 "},{" a "},{" b "},{" c0 "," c1 "};\n\t"
-// DMMA A x B_j into accumulator j for every set bit j of m (0..15); `A` and `B` are PTX operand names
-#define GINT_MMA_CHAINS(D0, D1, D2, D3)                                                                       \
-    "{\n\t"                                                                                                   \
-    "ts: .branchtargets C0, C1, C2, C3, C4, C5, C6, C7, C8, C9, C10, C11, C12, C13, C14, C15;\n\t"              \
-    "brx.idx %13, ts;\n\t"                                                                                    \
-    "C15: " D0 "C14: " D1 "bra C12;\n\t"                                                                        \
-    "C13: " D0 "C12: " D2 "C8: " D3 "bra C0;\n\t"                                                                \
-    "C11: " D0 "C10: " D1 "bra C8;\n\t"                                                                         \
-    "C9: " D0 "bra C8;\n\t"                                                                                    \
-    "C7: " D0 "C6: " D1 "C4: " D2 "bra C0;\n\t"                                                                  \
-    "C5: " D0 "bra C4;\n\t"                                                                                    \
-    "C3: " D0 "C2: " D1 "bra C0;\n\t"                                                                           \
-    "C1: " D0 "C0:\n\t"                                                                                        \
-    "}"
-// one k-step of one fragment row: acc[j] += a x b[j] for the set bits j of m
-__device__ __forceinline__ void dmma_row(double (&acc)[4][2], double a, const double (&b)[4], unsigned m) {
-    asm volatile(GINT_MMA_CHAINS(GINT_MMA("%0", "%1", "%8", "%9"), GINT_MMA("%2", "%3", "%8", "%10"),
-                                 GINT_MMA("%4", "%5", "%8", "%11"), GINT_MMA("%6", "%7", "%8", "%12"))
-                 : "+d"(acc[0][0]), "+d"(acc[0][1]), "+d"(acc[1][0]), "+d"(acc[1][1]), "+d"(acc[2][0]), "+d"(acc[2][1]),
-                   "+d"(acc[3][0]), "+d"(acc[3][1])
-                 : "d"(a), "d"(b[0]), "d"(b[1]), "d"(b[2]), "d"(b[3]), "r"(m));
-}
-// two k-steps (a0 x b0[j], a1 x b1[j]) into the same accumulators: the rho kernel's 8-orbital fragment row
-__device__ __forceinline__ void dmma_row2(double (&acc)[4][2], double a0, double a1, const double (&b0)[4], const double (&b1)[4], unsigned m) {
-    asm volatile(GINT_MMA_CHAINS(GINT_MMA("%0", "%1", "%8", "%9") GINT_MMA("%0", "%1", "%14", "%15"),
-                                 GINT_MMA("%2", "%3", "%8", "%10") GINT_MMA("%2", "%3", "%14", "%16"),
-                                 GINT_MMA("%4", "%5", "%8", "%11") GINT_MMA("%4", "%5", "%14", "%17"),
-                                 GINT_MMA("%6", "%7", "%8", "%12") GINT_MMA("%6", "%7", "%14", "%18"))
-                 : "+d"(acc[0][0]), "+d"(acc[0][1]), "+d"(acc[1][0]), "+d"(acc[1][1]), "+d"(acc[2][0]), "+d"(acc[2][1]),
-                   "+d"(acc[3][0]), "+d"(acc[3][1])
-                 : "d"(a0), "d"(b0[0]), "d"(b0[1]), "d"(b0[2]), "d"(b0[3]), "r"(m),
-                   "d"(a1), "d"(b1[0]), "d"(b1[1]), "d"(b1[2]), "d"(b1[3]));
+__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};" : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
 }
 
 struct TileView {
     int b, I, J, G;                  // batch, groups
     int i0, j0, k0, ex, ey, ez;      // batch origin and extents (mesh points)
-    int nkz, nks, nchunk;            // k-steps along z per column, k-steps of the batch, chunks of 8 k-steps
+    int nchunk;                      // stages of 4 cubelets
     int nI, nJ;                      // atoms in the two groups
     int nfI, nfJ;                    // fragments (8 orbitals) in the two groups
     bool diag;
 };
 
+__device__ __forceinline__ u64 warp_or64(u64 v) {
+    const unsigned lo = __reduce_or_sync(0xffffffffu, (unsigned)v), hi = __reduce_or_sync(0xffffffffu, (unsigned)(v >> 32));
+    return (u64)lo | ((u64)hi << 32);
+}
+__device__ __forceinline__ u64 shfl64(u64 v, int src) {
+    const unsigned lo = __shfl_sync(0xffffffffu, (unsigned)v, src), hi = __shfl_sync(0xffffffffu, (unsigned)(v >> 32), src);
+    return (u64)lo | ((u64)hi << 32);
+}
+
 // ---------------------------------------------------------------------------------------------------
-// Tile set-up: atom slots, orbital-row maps, canonical block of every atom pair of the tile.
+// Tile set-up: atom slots, orbital-row maps, canonical block of every atom pair of the tile, activity masks,
+// cubelet list, segments.
 __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView& tv, const int2* __restrict__ tile,
                                            const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
                                            const double* __restrict__ atom_pos, const int* __restrict__ atom_spec,
                                            const SpeciesDev* __restrict__ sp, const int* __restrict__ crow,
-                                           const unsigned long long* __restrict__ ckey, const unsigned int* __restrict__ coff) {
-    const int tid = threadIdx.x;
+                                           const u64* __restrict__ ckey, const unsigned int* __restrict__ coff) {
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int2 td = tile[blockIdx.x];
     tv.b = td.x; tv.I = td.y & 255; tv.J = (td.y >> 8) & 255; tv.G = (td.y >> 16) & 255;
     tv.diag = tv.I == tv.J;
@@ -104,9 +93,6 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
     const int bz = b % g.nb[2], by = (b / g.nb[2]) % g.nb[1], bx = b / (g.nb[2] * g.nb[1]);
     tv.i0 = bx * g.bs[0]; tv.j0 = by * g.bs[1]; tv.k0 = bz * g.bs[2];
     tv.ex = min(g.bs[0], g.N[0] - tv.i0); tv.ey = min(g.bs[1], g.N[1] - tv.j0); tv.ez = min(g.bs[2], g.N[2] - tv.k0);
-    tv.nkz = (tv.ez + 3) >> 2;
-    tv.nks = tv.ex * tv.ey * tv.nkz;
-    tv.nchunk = (tv.nks + 7) >> 3;
     const int e0 = bstart[b], n = bstart[b + 1] - e0;
     const int eI = group_begin(tv.I, n, tv.G), eJ = group_begin(tv.J, n, tv.G);
     tv.nI = group_begin(tv.I + 1, n, tv.G) - eI;
@@ -117,17 +103,23 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
         const bool valid = a < (side ? tv.nJ : tv.nI);
         int atom = 0, shift = pack_shift(0, 0, 0), spec = 0;
         double x = 0, y = 0, z = 0;
+        u64 m = 0;
         if (valid) {
             const NeighEntry e = bent[e0 + (side ? eJ : eI) + a];
             int t1, t2, t3; unpack_shift(e.shift, t1, t2, t3);
-            atom = e.atom; shift = e.shift; spec = atom_spec[atom];
+            atom = e.atom; shift = e.shift; spec = atom_spec[atom]; m = e.mask;
             x = atom_pos[3 * atom + 0] + t1 * g.a[0] + t2 * g.a[3] + t3 * g.a[6];
             y = atom_pos[3 * atom + 1] + t1 * g.a[1] + t2 * g.a[4] + t3 * g.a[7];
             z = atom_pos[3 * atom + 2] + t1 * g.a[2] + t2 * g.a[5] + t3 * g.a[8];
         }
-        S.pos[tid][0] = x; S.pos[tid][1] = y; S.pos[tid][2] = z;
-        S.spec[tid] = spec; S.atom[tid] = atom; S.shift[tid] = shift;
-        S.slot_mask[0][tid] = 0; S.slot_mask[1][tid] = 0;
+        S.pos[tid][0] = x; S.pos[tid][1] = y; S.pos[tid][2] = z; S.pos[tid][3] = 0.0;
+        S.spec[tid] = spec; S.atom[tid] = atom; S.shift[tid] = shift; S.amask[tid] = m;
+        const SpeciesDev* Sp = sp + spec;
+        SlotInfo si; si.rc2 = Sp->rc * Sp->rc; si.n_int = Sp->n_int; si.nsh = valid ? Sp->n_shell : 0; si.tab_off = Sp->tab_off;
+        int lp = 0;
+        for (int k = 0; k < Sp->n_shell; k++) lp |= Sp->l[k] << (2 * k);
+        si.lpack = lp;
+        S.sinfo[tid] = si;
     }
     __syncthreads();
     if (tid < 2) {
@@ -148,34 +140,40 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
     } else if (tid < 2 * GINT_TILE_ORB + 32) {
         const int q = tid - 2 * GINT_TILE_ORB, side = q >> 4, f = q & 15;
         unsigned m = 0;
+        u64 fm = 0;
         for (int k = 0; k < GINT_TILE_ATOMS; k++)
-            if (S.cstart[side][k] < 8 * f + 8 && S.cstart[side][k + 1] > 8 * f) m |= 1u << k;
+            if (S.cstart[side][k] < 8 * f + 8 && S.cstart[side][k + 1] > 8 * f) { m |= 1u << k; fm |= S.amask[8 * side + k]; }
         S.frag_atoms[side][f] = (unsigned char)m;
-    } else if (tid >= 320 && tid < 320 + 64) {
-        const int q = tid - 320, a = q >> 3, bb = q & 7;
-        unsigned int off = 0xffffffffu; unsigned char tr = 0;
+        S.fmask[side][f] = fm;
+    } else if (tid >= 256 && tid < 256 + 64) {
+        const int q = tid - 256, a = q >> 3, bb = q & 7;
+        PairEnt pe; pe.off = 0xffffffffu; pe.sr = 0; pe.sc = 0;
         // diagonal tile: only pairs a <= b are accumulated (a == b is the full on-site block)
         if (a < tv.nI && bb < tv.nJ && !(tv.diag && a > bb)) {
             int A = S.atom[a], B = S.atom[8 + bb];
+            const int nA = S.cstart[0][a + 1] - S.cstart[0][a], nB = S.cstart[1][bb + 1] - S.cstart[1][bb];
             int ta1, ta2, ta3, tb1, tb2, tb3;
             unpack_shift(S.shift[a], ta1, ta2, ta3); unpack_shift(S.shift[8 + bb], tb1, tb2, tb3);
             int n1 = tb1 - ta1, n2 = tb2 - ta2, n3 = tb3 - ta3;
             const bool ge0 = n1 > 0 || (n1 == 0 && (n2 > 0 || (n2 == 0 && n3 >= 0)));
-            if (!(A < B || (A == B && ge0))) { const int t = A; A = B; B = t; n1 = -n1; n2 = -n2; n3 = -n3; tr = 1; }
+            bool tr = false;
+            if (!(A < B || (A == B && ge0))) { const int t = A; A = B; B = t; n1 = -n1; n2 = -n2; n3 = -n3; tr = true; }
             const int m = g.key_m;
             if (abs(n1) <= m && abs(n2) <= m && abs(n3) <= m) {
-                const unsigned long long M = (unsigned long long)g.key_M;
-                const unsigned long long want = (((unsigned long long)B * M + (unsigned long long)(n1 + m)) * M + (unsigned long long)(n2 + m)) * M + (unsigned long long)(n3 + m);
+                const u64 M = (u64)g.key_M;
+                const u64 want = (((u64)B * M + (u64)(n1 + m)) * M + (u64)(n2 + m)) * M + (u64)(n3 + m);
                 int lo = crow[A], hi = crow[A + 1] - 1;
                 while (lo <= hi) {
                     const int mid = (lo + hi) >> 1;
-                    const unsigned long long k = ckey[mid];
-                    if (k == want) { off = coff[mid]; break; }
+                    const u64 k = ckey[mid];
+                    if (k == want) { pe.off = coff[mid]; break; }
                     if (k < want) lo = mid + 1; else hi = mid - 1;
                 }
             }
+            // canonical key (b, a): the stored block is nB x nA and holds the transpose
+            pe.sr = (unsigned short)(tr ? 1 : nB); pe.sc = (unsigned short)(tr ? nA : 1);
         }
-        S.pair_off[a][bb] = off; S.pair_tr[a][bb] = tr;
+        S.pair[a][bb] = pe;
     }
     // padding rows (orbital rows between the group's last orbital and the end of its last fragment) must hold zeros
     for (int idx = tid; idx < 2 * 2 * 8 * GINT_LD; idx += blockDim.x) {
@@ -184,177 +182,233 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
         if (row < GINT_TILE_ORB) S.phi[st][side][row][col] = 0.0;
     }
     __syncthreads();
+    if (warp == 0) {
+        // union masks, cubelet list, per-slot read sets
+        const u64 vI = lane < tv.nfI ? S.fmask[0][lane] : 0ull;
+        const u64 vJ = lane < tv.nfJ ? S.fmask[1][lane] : 0ull;
+        const u64 anyI = warp_or64(vI);
+        const u64 h0 = warp_or64(lane < GINT_SEG_COLS ? vJ : 0ull) & anyI, h1 = warp_or64(lane >= GINT_SEG_COLS ? vJ : 0ull) & anyI;
+        const u64 U = h0 | h1;
+        const unsigned Ulo = (unsigned)U, Uhi = (unsigned)(U >> 32), lt = (1u << lane) - 1u;
+        if ((Ulo >> lane) & 1u) S.cub[__popc(Ulo & lt)] = (unsigned char)lane;
+        if ((Uhi >> lane) & 1u) S.cub[__popc(Ulo) + __popc(Uhi & lt)] = (unsigned char)(32 + lane);
+        const int ncub = __popc(Ulo) + __popc(Uhi);
+        if (lane < 4) S.cub[ncub + lane] = 0;
+        u64 m = 0;
+        if (lane < 16) {
+            const int side = lane >> 3, a = lane & 7;
+            const int nf = side ? tv.nfJ : tv.nfI;
+            for (int f = 0; f < nf; f++)
+                if ((S.frag_atoms[side][f] >> a) & 1) m |= side ? (f < GINT_SEG_COLS ? h0 : h1) : (S.fmask[0][f] & U);
+        }
+        const u64 mj = shfl64(m, (lane + 8) & 31);
+        if (tv.diag) m = lane < 8 ? (m | mj) : 0ull;      // the atoms are evaluated once, for both sides
+        if (lane < 16) S.need[lane] = m;
+        if (lane == 0) { S.U = U; S.hmask[0] = h0; S.hmask[1] = h1; S.ncub = ncub; }
+    } else if (warp == 1) {
+        // segments: piece (row fragment r, half h) = columns [cb, cb + n); sorted by falling n and dealt to the
+        // sub-partitions 0,1,2,3,3,2,1,0,... (warp w runs on sub-partition w % 4)
+        if (lane < GINT_MAX_SEG) S.seg[lane] = 0;
+        __syncwarp();
+        int pn = 0, pcb = 0;
+        const int r = lane >> 1, h = lane & 1;
+        if (lane < 2 * GINT_TILE_FRAG && r < tv.nfI) {
+            const int cf = tv.diag ? (S.cstart[1][S.row_atom[0][8 * r]] >> 3) : 0;
+            if (h == 0) { pcb = cf; pn = min(GINT_SEG_COLS, tv.nfJ) - cf; }
+            else { pcb = max(GINT_SEG_COLS, cf); pn = tv.nfJ - pcb; }
+            pn = max(pn, 0);
+        }
+        int rank = 0;
+        for (int j = 0; j < 2 * GINT_TILE_FRAG; j++) {
+            const int nj = __shfl_sync(0xffffffffu, pn, j);
+            rank += (nj > pn) || (nj == pn && j < lane);
+        }
+        if (pn > 0) {
+            const int k7 = rank & 7, s = k7 < 4 ? k7 : 7 - k7, j = 2 * (rank >> 3) + (k7 >= 4);
+            const int W = s < (GINT_WARPS & 3) ? (GINT_WARPS >> 2) + 1 : (GINT_WARPS >> 2);
+            S.seg[s + 4 * (j % W) + GINT_WARPS * (j / W)] = r | (pcb << 8) | (pn << 16);
+        }
+    }
+    __syncthreads();
+    tv.nchunk = (S.ncub + 3) >> 2;
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Orbital values of one atom at the 32 points of a chunk (north_star step 2): lane = point, the atom is
-// warp-uniform.  phi = R_s(|d|) Y_lm(d/|d|), zero for |d| >= rc (Fig. 6); radial part:
-// per-interval cubic in b = r/dr - i (reading R5).
-//   mode 0: out0 <- phi            mode 1: out0 <- w phi
-//   mode 2: out0 <- phi, out1 <- w phi          mode 3: out0 <- phi, out1 <- phi
-// Returns the 8-bit k-step activity mask of the atom on this chunk (bit k: some point of k-step k is inside).
-__device__ __forceinline__ unsigned eval_atom_chunk(const Geom& g, const SpeciesDev* __restrict__ S, const double* __restrict__ tab,
-                                                   bool valid, double dx, double dy, double dz, int mode, double w,
-                                                   double* __restrict__ out0, double* __restrict__ out1) {
-    const int lane = threadIdx.x & 31;
-    const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-    const double rc = S->rc;
-    const bool inside = valid && r2 < rc * rc;
-    const unsigned bal = __ballot_sync(0xffffffffu, inside);
-    unsigned km = (bal | (bal >> 1) | (bal >> 2) | (bal >> 3)) & 0x11111111u;   // bit 4k = any of the 4 points of k-step k
-    km = (km | (km >> 3)) & 0x03030303u; km = (km | (km >> 6)) & 0x000f000fu; km = (km | (km >> 12)) & 0xffu;
-    const int norb = S->norb;
-    double* o0 = out0 + lane;
-    double* o1 = out1 + lane;
-    if (bal == 0u) {
-        for (int o = 0; o < norb; o++) { o0[o * GINT_LD] = 0.0; if (mode >= 2) o1[o * GINT_LD] = 0.0; }
-        return 0u;
-    }
-    // lanes outside the sphere run the same instructions on a clamped radius and store zeros
-    const double w0 = inside ? (mode == 1 ? w : 1.0) : 0.0;
-    const double w1 = inside ? (mode == 2 ? w : 1.0) : 0.0;
-    // 1/r by two Newton steps from the single-precision reciprocal square root (relative error ~1e-7 -> 1e-14 -> 1e-28)
-    const double q = fmin(fmax(r2, 1e-30), rc * rc);
-    double ir = (double)rsqrtf((float)q);
-    ir = ir * fma(-0.5 * q, ir * ir, 1.5);
-    ir = ir * fma(-0.5 * q, ir * ir, 1.5);
-    const double r = q * ir;
-    const int nsh = S->n_shell;
-    const double x = r * g.inv_dr;
-    int i = (int)x;
-    i = min(i, S->n_int - 1);
-    const double bq = x - (double)i;
-    const double2* row = reinterpret_cast<const double2*>(tab) + ((size_t)S->tab_off + (size_t)i * nsh) * 2;
-    const bool tiny = r < 1e-12;
-    if (tiny) ir = 0.0;
-    const double ux = dx * ir, uy = dy * ir, uz = dz * ir;
-    const double lz = tiny ? 0.0 : 1.0;          // l > 0 orbitals vanish at the nucleus
-    int o = 0;
-#define GINT_PUT(v) do { const double v_ = (v); o0[o * GINT_LD] = w0 * v_; if (mode >= 2) o1[o * GINT_LD] = w1 * v_; o++; } while (0)
-#pragma unroll 1
-    for (int k = 0; k < nsh; k++) {
-        const double2 c01 = __ldg(row + 2 * k), c23 = __ldg(row + 2 * k + 1);
-        const double R = fma(fma(fma(c23.y, bq, c23.x), bq, c01.y), bq, c01.x);
-        const int l = S->l[k];
-        if (l == 0) {
-            GINT_PUT(R * 0.28209479177387814);
-        } else if (l == 1) {
-            const double R1 = R * 0.4886025119029199;
-            GINT_PUT(R1 * uy); GINT_PUT(R1 * uz); GINT_PUT(R1 * ux);
-        } else {
-            const double R2 = R * lz;
-            const double c2 = R2 * 1.0925484305920792;
-            GINT_PUT(c2 * ux * uy);
-            GINT_PUT(c2 * uy * uz);
-            GINT_PUT(R2 * 0.31539156525252005 * (3.0 * uz * uz - 1.0));
-            GINT_PUT(c2 * ux * uz);
-            GINT_PUT(R2 * 0.5462742152960396 * (ux * ux - uy * uy));
-        }
-    }
-#undef GINT_PUT
-    return km;
-}
-
-// mesh point of lane `lane` in chunk c of the batch: k-step ks = 8c + lane/4 = ((ix*ey)+iy)*nkz + kz, z = 4kz + lane%4
-__device__ __forceinline__ bool chunk_point(const TileView& tv, int c, int lane, int& gi, int& gj, int& gk) {
-    const int ks = 8 * c + (lane >> 2);
-    const int kz = ks % tv.nkz, t = ks / tv.nkz;
-    const int iy = t % tv.ey, ix = t / tv.ey;
-    const int iz = 4 * kz + (lane & 3);
+// Stage c of a tile = its cubelets 4c .. 4c+3; lane = 8 q + p: point p = (px, py, pz) bits of the q-th cubelet.
+__device__ __forceinline__ bool stage_point(const TileSmem& S, const TileView& tv, int c, int lane, int& gi, int& gj, int& gk) {
+    const int ci = 4 * c + (lane >> 3), p = lane & 7;
+    if (ci >= S.ncub) return false;
+    const int cl = S.cub[ci];
+    const int ix = 2 * (cl >> 4) + (p >> 2), iy = 2 * ((cl >> 2) & 3) + ((p >> 1) & 1), iz = 2 * (cl & 3) + (p & 1);
     gi = tv.i0 + ix; gj = tv.j0 + iy; gk = tv.k0 + iz;
-    return ks < tv.nks && iz < tv.ez;
+    return ix < tv.ex && iy < tv.ey && iz < tv.ez;
 }
 
-// Mesh points of chunk c (coordinates and the vlocal weight V dV) into pts[c & 1]; run by one warp, two chunks ahead
-// of the evaluation that consumes them, so that the global load of V is off the critical path.
+// Run by one warp, two stages ahead of the evaluation that consumes them (so that the global load of V is off the
+// critical path): the stage's mesh points (coordinates, vlocal weight V dV) and its compacted item list.  An item
+// is (atom slot, cubelet of the stage) whose orbital rows some segment reads on that cubelet: first the items on
+// which the atom is really non-zero (evaluated), then those that only need zeros.
 template <bool VLOCAL>
-__device__ __forceinline__ void make_points(const Geom& g, TileSmem& S, const TileView& tv, int c, const double* __restrict__ V) {
-    const int lane = threadIdx.x & 31;
+__device__ __forceinline__ void make_stage(const Geom& g, TileSmem& S, const TileView& tv, int c, const double* __restrict__ V) {
+    const int lane = threadIdx.x & 31, par = c & 1;
     int gi, gj, gk;
     double4 p = make_double4(0.0, 0.0, 0.0, 0.0);
-    double valid = 0.0;
-    if (c < tv.nchunk && chunk_point(tv, c, lane, gi, gj, gk)) {
+    const bool valid = stage_point(S, tv, c, lane, gi, gj, gk);
+    if (valid) {
         mesh_point(g, gi, gj, gk, p.x, p.y, p.z);
         p.w = VLOCAL ? __ldg(V + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk) * g.dV : 1.0;
-        valid = 1.0;
     }
-    S.pts[c & 1][lane] = p;
-    S.pvalid[c & 1][lane] = valid;
+    S.pts[par][lane] = p;
+    S.valid[par][lane] = valid ? 1 : 0;
+    // candidates: lane -> (slot lane >> 2, cubelet lane & 3) and (slot 8 + (lane >> 2), same cubelet)
+    const int ci = 4 * c + (lane & 3);
+    const bool inb = ci < S.ncub;
+    const int cl = inb ? S.cub[ci] : 0;
+    const int s0 = lane >> 2, s1 = 8 + s0;
+    const bool n0 = inb && ((S.need[s0] >> cl) & 1ull), n1 = inb && ((S.need[s1] >> cl) & 1ull);
+    const bool a0 = n0 && ((S.amask[s0] >> cl) & 1ull), a1 = n1 && ((S.amask[s1] >> cl) & 1ull);
+    const unsigned e0 = __ballot_sync(0xffffffffu, a0), e1 = __ballot_sync(0xffffffffu, a1);
+    const unsigned z0 = __ballot_sync(0xffffffffu, n0 && !a0), z1 = __ballot_sync(0xffffffffu, n1 && !a1);
+    const unsigned lt = (1u << lane) - 1u;
+    const int ne = __popc(e0) + __popc(e1);
+    if (a0) S.item[par][__popc(e0 & lt)] = (unsigned char)lane;
+    else if (n0) S.item[par][ne + __popc(z0 & lt)] = (unsigned char)lane;
+    if (a1) S.item[par][__popc(e0) + __popc(e1 & lt)] = (unsigned char)(32 + lane);
+    else if (n1) S.item[par][ne + __popc(z0) + __popc(z1 & lt)] = (unsigned char)(32 + lane);
+    if (lane == 0) { S.neval[par] = ne; S.nitem[par] = ne + __popc(z0) + __popc(z1); }
 }
 
-// Evaluation phase of chunk c into pipeline stage st: warp w evaluates slot w (slot < 8: group I, else group J).
-// vlocal: side I unscaled, side J scaled by V dV.  rho: both unscaled.  Diagonal tiles evaluate each atom once
-// and write both sides.
+// ---------------------------------------------------------------------------------------------------
+// Orbital evaluation of one stage (north_star step 2): a quarter warp = one item, lane p = point p of the cubelet.
+// phi = R_s(|d|) Y_lm(d/|d|), zero for |d| >= rc (Fig. 6); radial part: per-interval
+// cubic in b = r/dr - i (reading R5), coefficients read with 128-bit loads.  vlocal scales side J by V dV.
+// A diagonal tile evaluates each atom once and writes both sides.
 template <bool VLOCAL>
-__device__ __forceinline__ void eval_chunk(const Geom& g, TileSmem& S, const TileView& tv, int c, int st,
-                                           const SpeciesDev* __restrict__ sp, const double* __restrict__ tab) {
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int side = warp >> 3, a = warp & 7;
-    if (tv.diag ? (side == 1 || a >= tv.nI) : (a >= (side ? tv.nJ : tv.nI))) return;
-    const double4 p = S.pts[st][lane];
-    const bool valid = S.pvalid[st][lane] != 0.0;
-    const SpeciesDev* Sp = sp + S.spec[warp];
-    const double dx = p.x - S.pos[warp][0], dy = p.y - S.pos[warp][1], dz = p.z - S.pos[warp][2];
-    double* out0 = &S.phi[st][side][S.cstart[side][a]][0];
-    if (tv.diag) {
-        double* out1 = &S.phi[st][1][S.cstart[0][a]][0];
-        const unsigned km = eval_atom_chunk(g, Sp, tab, valid, dx, dy, dz, VLOCAL ? 2 : 3, p.w, out0, out1);
-        if (lane == 0) { S.slot_mask[st][a] = (unsigned char)km; S.slot_mask[st][8 + a] = (unsigned char)km; }
-    } else {
-        const unsigned km = eval_atom_chunk(g, Sp, tab, valid, dx, dy, dz, (VLOCAL && side == 1) ? 1 : 0, p.w, out0, out0);
-        if (lane == 0) S.slot_mask[st][warp] = (unsigned char)km;
+__device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, const TileView& tv, int st, int rank,
+                                           const double* __restrict__ tab) {
+    const int lane = threadIdx.x & 31;
+    const int nitem = S.nitem[st], neval = S.neval[st];
+    const bool two = tv.diag;
+    for (int base = 4 * rank; base < nitem; base += 4 * GINT_WARPS) {
+        const int idx = base + (lane >> 3);
+        const bool on = idx < nitem;
+        const int it = on ? S.item[st][idx] : 0;
+        const int slot = it >> 2, col = 8 * (it & 3) + (lane & 7);
+        const int side = slot >> 3, a = slot & 7;
+        double* o0 = &S.phi[st][side][S.cstart[side][a]][col];
+        double* o1 = &S.phi[st][1][S.cstart[side][a]][col];
+        if (base >= neval) {                        // the four items only need zeros
+            const int norb = on ? S.cstart[side][a + 1] - S.cstart[side][a] : 0;
+            for (int o = 0; o < norb; o++) { o0[o * GINT_LD] = 0.0; if (two) o1[o * GINT_LD] = 0.0; }
+            continue;
+        }
+        const SlotInfo si = S.sinfo[slot];
+        const double4 P = S.pts[st][col];
+        const double dx = P.x - S.pos[slot][0], dy = P.y - S.pos[slot][1], dz = P.z - S.pos[slot][2];
+        const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+        const bool inside = on && idx < neval && S.valid[st][col] && r2 < si.rc2;
+        // lanes outside the sphere run the same instructions on a clamped radius and store zeros
+        const double w0 = inside ? ((VLOCAL && side) ? P.w : 1.0) : 0.0;
+        const double w1 = inside ? (VLOCAL ? P.w : 1.0) : 0.0;
+        // 1/r by two Newton steps from the single-precision reciprocal square root (relative error ~1e-7 -> 1e-14 -> 1e-28)
+        const double q = fmin(fmax(r2, 1e-30), si.rc2);
+        double ir = (double)rsqrtf((float)q);
+        ir = ir * fma(-0.5 * q, ir * ir, 1.5);
+        ir = ir * fma(-0.5 * q, ir * ir, 1.5);
+        const double r = q * ir;
+        const int nsh = on ? si.nsh : 0;
+        const double x = r * g.inv_dr;
+        int i = (int)x;
+        i = min(i, si.n_int - 1);
+        const double bq = x - (double)i;
+        const double2* row = reinterpret_cast<const double2*>(tab) + ((size_t)si.tab_off + (size_t)i * si.nsh) * 2;
+        const bool tiny = r < 1e-12;
+        if (tiny) ir = 0.0;
+        const double ux = dx * ir, uy = dy * ir, uz = dz * ir;
+        const double lz = tiny ? 0.0 : 1.0;          // l > 0 orbitals vanish at the nucleus
+#define GINT_PUT(v) do { const double v_ = (v); *o0 = w0 * v_; o0 += GINT_LD; if (two) { *o1 = w1 * v_; o1 += GINT_LD; } } while (0)
+        for (int k0 = 0; k0 < nsh; k0 += GINT_EVAL_GROUP) {
+            double2 c01[GINT_EVAL_GROUP], c23[GINT_EVAL_GROUP];
+#pragma unroll
+            for (int u = 0; u < GINT_EVAL_GROUP; u++)
+                if (k0 + u < nsh) { c01[u] = __ldg(row + 2 * (k0 + u)); c23[u] = __ldg(row + 2 * (k0 + u) + 1); }
+#pragma unroll
+            for (int u = 0; u < GINT_EVAL_GROUP; u++) {
+                if (k0 + u >= nsh) break;
+                const double R = fma(fma(fma(c23[u].y, bq, c23[u].x), bq, c01[u].y), bq, c01[u].x);
+                const int l = (si.lpack >> (2 * (k0 + u))) & 3;
+                if (l == 0) {
+                    GINT_PUT(R * 0.28209479177387814);
+                } else if (l == 1) {
+                    const double R1 = R * 0.4886025119029199;
+                    GINT_PUT(R1 * uy); GINT_PUT(R1 * uz); GINT_PUT(R1 * ux);
+                } else {
+                    const double R2 = R * lz;
+                    const double c2 = R2 * 1.0925484305920792;
+                    GINT_PUT(c2 * ux * uy);
+                    GINT_PUT(c2 * uy * uz);
+                    GINT_PUT(R2 * 0.31539156525252005 * (3.0 * uz * uz - 1.0));
+                    GINT_PUT(c2 * ux * uz);
+                    GINT_PUT(R2 * 0.5462742152960396 * (ux * ux - uy * uy));
+                }
+            }
+        }
+#undef GINT_PUT
     }
 }
 
-// rows / columns of the 4 x 4 warp grid: n fragments are dealt to 4 warps, the first (n % 4) get one more
-__device__ __forceinline__ void warp_range(int n, int i, int& f0, int& nf) {
-    const int base = n >> 2, rem = n & 3;
-    f0 = i * base + min(i, rem); nf = base + (i < rem);
+// ---------------------------------------------------------------------------------------------------
+// Segments of a warp.
+struct Seg {
+    int row, cb, n;                  // row fragment, first column fragment, column fragments (0 = unused)
+    u64 act;                         // cubelets on which the row fragment and some column fragment are both active
+};
+__device__ __forceinline__ Seg load_seg(const TileSmem& S, int slot) {
+    const int w = S.seg[slot];
+    Seg s; s.row = w & 255; s.cb = (w >> 8) & 255; s.n = w >> 16;
+    u64 cm = 0;
+    for (int j = 0; j < s.n; j++) cm |= S.fmask[1][s.cb + j];
+    s.act = s.n ? (S.fmask[0][s.row] & cm) : 0ull;
+    return s;
 }
-// 8-bit k-step mask of a fragment = OR of the masks of the atoms it holds orbitals of
-__device__ __forceinline__ unsigned frag_kmask(const unsigned char* __restrict__ slot_mask8, unsigned atoms) {
-    unsigned m = 0;
-    while (atoms) { const int a = __ffs(atoms) - 1; atoms &= atoms - 1; m |= slot_mask8[a]; }
-    return m;
+// 4-bit activity of a segment on the cubelets of stage c
+__device__ __forceinline__ unsigned stage_bits(const TileSmem& S, int c, u64 act) {
+    const unsigned cw = *reinterpret_cast<const unsigned*>(&S.cub[4 * c]);
+    const int nq = min(4, S.ncub - 4 * c);
+    unsigned bits = 0;
+#pragma unroll
+    for (int q = 0; q < 4; q++) bits |= (unsigned)((act >> ((cw >> (8 * q)) & 63u)) & 1ull) << q;
+    return bits & ((1u << nq) - 1u);
 }
-// bit k of x -> bit 4k
-__device__ __forceinline__ unsigned spread8(unsigned x) {
-    x &= 0xffu; x = (x | (x << 12)) & 0x000f000fu; x = (x | (x << 6)) & 0x03030303u; x = (x | (x << 3)) & 0x11111111u;
-    return x;
-}
-// Activity words of this warp's fragments on the chunk in stage st: nibble k of RW (CW) holds, for k-step k (FOLD:
-// for the pair of k-steps 2k, 2k+1 = 8 points), one bit per fragment row (column) of the warp tile.
-template <bool FOLD>
-__device__ __forceinline__ void chunk_masks(const TileSmem& S, int st, int R0, int nr, int C0, int nc, unsigned& RW, unsigned& CW) {
-    const int lane = threadIdx.x & 31;
-    unsigned fm = 0;
-    if (lane < 8) {
-        const int side = lane >> 2, q = lane & 3;
-        if (q < (side ? nc : nr)) {
-            unsigned atoms = S.frag_atoms[side][(side ? C0 : R0) + q];
-            while (atoms) { const int a = __ffs(atoms) - 1; atoms &= atoms - 1; fm |= S.slot_mask[st][8 * side + a]; }
-        }
-        if (FOLD) { fm = (fm | (fm >> 1)) & 0x55u; fm = (fm | (fm >> 1)) & 0x33u; fm = (fm | (fm >> 2)) & 0x0fu; }
-        fm = spread8(fm) << q;
+
+// vlocal: acc[j] += Phi_I[row fragment]^T-slice x (V dV Phi_J)[column fragment cb + j] over the 8 points of every
+// active cubelet of the stage: one 128-bit shared load per operand fragment (points 2 lc, 2 lc + 1 of the lane's
+// orbital row) feeds two DMMA k-steps (k index lc <-> point 2 lc, then point 2 lc + 1).
+template <int N>
+__device__ __forceinline__ void vl_seg(double (&acc)[GINT_SEG_COLS][2], const double* __restrict__ pa, const double* __restrict__ pb, unsigned bits) {
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+        if (!((bits >> q) & 1u)) continue;
+        const double2 a = *reinterpret_cast<const double2*>(pa + 8 * q);
+        double2 bv[N];
+#pragma unroll
+        for (int j = 0; j < N; j++) bv[j] = *reinterpret_cast<const double2*>(pb + j * 8 * GINT_LD + 8 * q);
+#pragma unroll
+        for (int j = 0; j < N; j++) dmma884(acc[j], a.x, bv[j].x);
+#pragma unroll
+        for (int j = 0; j < N; j++) dmma884(acc[j], a.y, bv[j].y);
     }
-    RW = __reduce_or_sync(0xffffffffu, lane < 4 ? fm : 0u);
-    CW = __reduce_or_sync(0xffffffffu, lane >= 4 ? fm : 0u);
 }
-// fragment pairs this warp must compute: all of them, except, in a diagonal tile, those that hold no element with
-// atom(row) <= atom(col)
-__device__ __forceinline__ void warp_need(const TileSmem& S, const TileView& tv, int R0, int nr, int C0, int nc,
-                                          unsigned ratoms[4], unsigned catoms[4], unsigned need[4]) {
-#pragma unroll
-    for (int i = 0; i < 4; i++) { ratoms[i] = i < nr ? S.frag_atoms[0][R0 + i] : 0u; catoms[i] = i < nc ? S.frag_atoms[1][C0 + i] : 0u; }
-#pragma unroll
-    for (int i = 0; i < 4; i++) {
-        unsigned m = 0;
-#pragma unroll
-        for (int j = 0; j < 4; j++) {
-            const bool nd = ratoms[i] && catoms[j] && (!tv.diag || (31 - __clz(catoms[j])) >= (__ffs(ratoms[i]) - 1));
-            m |= nd ? 1u << j : 0u;
-        }
-        need[i] = m;
+__device__ __forceinline__ void vl_seg_dispatch(int n, double (&acc)[GINT_SEG_COLS][2], const double* pa, const double* pb, unsigned bits) {
+    switch (n) {
+        case 7: vl_seg<7>(acc, pa, pb, bits); break;
+        case 6: vl_seg<6>(acc, pa, pb, bits); break;
+        case 5: vl_seg<5>(acc, pa, pb, bits); break;
+        case 4: vl_seg<4>(acc, pa, pb, bits); break;
+        case 3: vl_seg<3>(acc, pa, pb, bits); break;
+        case 2: vl_seg<2>(acc, pa, pb, bits); break;
+        case 1: vl_seg<1>(acc, pa, pb, bits); break;
+        default: break;
     }
 }
 
@@ -365,178 +419,185 @@ __device__ __forceinline__ void warp_need(const TileSmem& S, const TileView& tv,
 __global__ void __launch_bounds__(GINT_THREADS, 1)
 k_vlocal_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
               const double* __restrict__ atom_pos, const int* __restrict__ atom_spec, const SpeciesDev* __restrict__ sp,
-              const double* __restrict__ tab, const int* __restrict__ crow, const unsigned long long* __restrict__ ckey,
+              const double* __restrict__ tab, const int* __restrict__ crow, const u64* __restrict__ ckey,
               const unsigned int* __restrict__ coff, const double* __restrict__ V, double* __restrict__ Hc) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TileSmem& S = *reinterpret_cast<TileSmem*>(smem_raw);
     TileView tv;
     tile_setup(g, S, tv, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff);
+    if (tv.nchunk == 0) return;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
-    // warp (wr, wc) of the 4 x 4 grid; the warps of one scheduler (warp % 4) sit on a diagonal so that the
-    // schedulers get equal numbers of fragments although 13 = 4 + 3 + 3 + 3
-    const int wr = warp >> 2, wc = ((warp & 3) + wr) & 3;
-    int R0, nr, C0, nc;
-    warp_range(tv.nfI, wr, R0, nr);
-    warp_range(tv.nfJ, wc, C0, nc);
-    unsigned ratoms[4], catoms[4], need[4];
-    warp_need(S, tv, R0, nr, C0, nc, ratoms, catoms, need);
-    double acc[4][4][2];
+    const Seg sA = load_seg(S, warp), sB = load_seg(S, warp + GINT_WARPS);
+    double accA[GINT_SEG_COLS][2], accB[GINT_SEG_COLS][2];
 #pragma unroll
-    for (int i = 0; i < 4; i++)
-#pragma unroll
-        for (int j = 0; j < 4; j++) { acc[i][j][0] = 0.0; acc[i][j][1] = 0.0; }
+    for (int j = 0; j < GINT_SEG_COLS; j++) { accA[j][0] = accA[j][1] = 0.0; accB[j][0] = accB[j][1] = 0.0; }
 
-    if (warp < 2) make_points<true>(g, S, tv, warp, V);
+    if (warp < 2) make_stage<true>(g, S, tv, warp, V);
     __syncthreads();
-    eval_chunk<true>(g, S, tv, 0, 0, sp, tab);
+    eval_stage<true>(g, S, tv, 0, warp, tab);
     for (int c = 0; c < tv.nchunk; c++) {
         const int st = c & 1;
-        __syncthreads();                       // stage st is complete; every warp has finished the MMAs of chunk c-1
-        if (warp == ((c + 2) & 15)) make_points<true>(g, S, tv, c + 2, V);
-        if (c + 1 < tv.nchunk) eval_chunk<true>(g, S, tv, c + 1, st ^ 1, sp, tab);
-        unsigned RW, CW;
-        chunk_masks<false>(S, st, R0, nr, C0, nc, RW, CW);
-        unsigned act = (RW | (RW >> 1) | (RW >> 2) | (RW >> 3)) & (CW | (CW >> 1) | (CW >> 2) | (CW >> 3)) & 0x11111111u;
-        const double* pa = &S.phi[st][0][R0 * 8 + lr][lc];
-        const double* pb = &S.phi[st][1][C0 * 8 + lr][lc];
-        while (act) {
-            const int p4 = __ffs(act) - 1; act &= act - 1;           // p4 = 4 * k-step
-            const unsigned r4 = RW >> p4, c4 = (CW >> p4) & 15u;
-            double bf[4];
-#pragma unroll
-            for (int j = 0; j < 4; j++) bf[j] = pb[j * 8 * GINT_LD + p4];      // inactive fragments: loaded, never used
-#pragma unroll
-            for (int i = 0; i < 4; i++) {
-                if (!((r4 >> i) & 1u)) continue;
-                const double a = pa[i * 8 * GINT_LD + p4];
-                dmma_row(acc[i], a, bf, c4 & need[i]);
-            }
-        }
+        __syncthreads();                       // stage st is complete; every warp has finished the MMAs of stage c-1
+        if (warp == (c + 2) % GINT_WARPS) make_stage<true>(g, S, tv, c + 2, V);
+        // half of the warps evaluate first, the other half multiply first, so that the FP64 tensor pipe has work
+        // while instructions of the evaluation issue
+        if (warp & 1) eval_stage<true>(g, S, tv, st ^ 1, warp, tab);
+        const unsigned bA = stage_bits(S, c, sA.act), bB = stage_bits(S, c, sB.act);
+        if (bA) vl_seg_dispatch(sA.n, accA, &S.phi[st][0][8 * sA.row + lr][2 * lc], &S.phi[st][1][8 * sA.cb + lr][2 * lc], bA);
+        if (bB) vl_seg_dispatch(sB.n, accB, &S.phi[st][0][8 * sB.row + lr][2 * lc], &S.phi[st][1][8 * sB.cb + lr][2 * lc], bB);
+        if (!(warp & 1)) eval_stage<true>(g, S, tv, st ^ 1, warp, tab);
     }
-    // flush: element (row, col) -> atom pair (a, b), orbitals (oa, ob) -> canonical block, transposed if the canonical
-    // key is (b, a).  Exact zeros (fragments never touched, atoms that do not overlap inside this batch) are skipped.
+    // flush: element (row, col) -> atom pair (a, b), orbitals (oa, ob) -> canonical block (transposed if the canonical
+    // key is (b, a)).  Exact zeros (fragments never touched, atoms that do not overlap inside this batch) are skipped.
 #pragma unroll
-    for (int i = 0; i < 4; i++) {
+    for (int s = 0; s < 2; s++) {
+        const Seg& sg = s ? sB : sA;
+        if (sg.n == 0 || sg.act == 0ull) continue;
+        const int row = 8 * sg.row + lr;
+        const int a = S.row_atom[0][row], oa = S.row_orb[0][row];
+        if (a == 255) continue;
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
-            if (!((need[i] >> j) & 1u)) continue;
-            const int row = (R0 + i) * 8 + lr;
-            const int a = S.row_atom[0][row], oa = S.row_orb[0][row];
-            if (a == 255) continue;
+        for (int j = 0; j < GINT_SEG_COLS; j++) {
+            if (j >= sg.n) break;
 #pragma unroll
             for (int e = 0; e < 2; e++) {
-                const double v = acc[i][j][e];
-                const int col = (C0 + j) * 8 + 2 * lc + e;
+                const double v = s ? accB[j][e] : accA[j][e];
+                const int col = 8 * (sg.cb + j) + 2 * lc + e;
                 const int bb = S.row_atom[1][col], ob = S.row_orb[1][col];
                 if (bb == 255 || v == 0.0) continue;
-                const unsigned off = S.pair_off[a][bb];
-                if (off == 0xffffffffu) continue;
-                const int nA = S.cstart[0][a + 1] - S.cstart[0][a], nB = S.cstart[1][bb + 1] - S.cstart[1][bb];
-                atomicAdd(Hc + off + (S.pair_tr[a][bb] ? ob * nA + oa : oa * nB + ob), v);
+                const PairEnt pe = S.pair[a][bb];
+                if (pe.off == 0xffffffffu) continue;
+                atomicAdd(Hc + pe.off + oa * pe.sr + ob * pe.sc, v);
             }
         }
     }
 }
 
 // ---------------------------------------------------------------------------------------------------
-// gint_rho main kernel (north_star step 3b): the density blocks Dh_IJ of the tile are the stationary DMMA B
-// fragments (registers); per chunk X = Phi_I Dh_IJ (32 points x 104) and rho_g += sum_j X_gj Phi_J,gj.
-// Dh = canonical-half, symmetrised density blocks (k_sym_D).  Warp (wr, wc): rows (k) and columns (n) of Dh.
-__device__ __forceinline__ unsigned fold_pairs(unsigned m) {     // 8 k-step bits -> 4 bits, one per 8 points
-    m = (m | (m >> 1)) & 0x55u; m = (m | (m >> 1)) & 0x33u; m = (m | (m >> 2)) & 0x0fu;
-    return m;
+// gint_rho main kernel (north_star step 3b).  The density blocks Dh_IJ of the tile are stationary DMMA A operands
+// (registers): per cubelet X^T = Dh_seg^T Phi_I (8 orbitals of J x 8 points per column fragment) and
+// rho_g += sum_j X_jg Phi_J,jg.  Dh = canonical-half, symmetrised density blocks (k_sym_D).
+template <int N>
+__device__ __forceinline__ void rho_seg(const double (&d)[GINT_SEG_COLS][2], const double* __restrict__ pi, const double* __restrict__ pj,
+                                        unsigned bits, double (&part)[4][2]) {
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+        if (!((bits >> q) & 1u)) continue;
+        const double b0 = pi[8 * q], b1 = pi[4 * GINT_LD + 8 * q];       // Phi_I[8 row + lc (+4)][point 8q + lr]
+        double2 f[N];
+#pragma unroll
+        for (int j = 0; j < N; j++) f[j] = *reinterpret_cast<const double2*>(pj + j * 8 * GINT_LD + 8 * q);
+        double x[N][2];
+#pragma unroll
+        for (int j = 0; j < N; j++) { x[j][0] = 0.0; x[j][1] = 0.0; dmma884(x[j], d[j][0], b0); }
+#pragma unroll
+        for (int j = 0; j < N; j++) dmma884(x[j], d[j][1], b1);
+#pragma unroll
+        for (int j = 0; j < N; j++) { part[q][0] = fma(x[j][0], f[j].x, part[q][0]); part[q][1] = fma(x[j][1], f[j].y, part[q][1]); }
+    }
 }
+__device__ __forceinline__ void rho_seg_dispatch(int n, const double (&d)[GINT_SEG_COLS][2], const double* pi, const double* pj,
+                                                 unsigned bits, double (&part)[4][2]) {
+    switch (n) {
+        case 7: rho_seg<7>(d, pi, pj, bits, part); break;
+        case 6: rho_seg<6>(d, pi, pj, bits, part); break;
+        case 5: rho_seg<5>(d, pi, pj, bits, part); break;
+        case 4: rho_seg<4>(d, pi, pj, bits, part); break;
+        case 3: rho_seg<3>(d, pi, pj, bits, part); break;
+        case 2: rho_seg<2>(d, pi, pj, bits, part); break;
+        case 1: rho_seg<1>(d, pi, pj, bits, part); break;
+        default: break;
+    }
+}
+// stationary operand of a segment: d[j][h] = Dh[orbital row 8 row + 4h + lc of I][orbital column 8 (cb + j) + lr of J]
+__device__ __forceinline__ void load_dseg(const TileSmem& S, const Seg& sg, const double* __restrict__ Dh, double (&d)[GINT_SEG_COLS][2]) {
+    const int lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
+#pragma unroll
+    for (int j = 0; j < GINT_SEG_COLS; j++)
+#pragma unroll
+        for (int h = 0; h < 2; h++) {
+            double v = 0.0;
+            if (j < sg.n) {
+                const int row = 8 * sg.row + 4 * h + lc, col = 8 * (sg.cb + j) + lr;
+                const int a = S.row_atom[0][row], bb = S.row_atom[1][col];
+                if (a != 255 && bb != 255) {
+                    const PairEnt pe = S.pair[a][bb];
+                    if (pe.off != 0xffffffffu) v = __ldg(Dh + pe.off + S.row_orb[0][row] * pe.sr + S.row_orb[1][col] * pe.sc);
+                }
+            }
+            d[j][h] = v;
+        }
+}
+// sum over the 14 warps of the partial densities of stage c and add them to rho (one warp)
+__device__ __forceinline__ void rho_store(const Geom& g, const TileSmem& S, const TileView& tv, int c, double* __restrict__ rho) {
+    const int lane = threadIdx.x & 31;
+    double v = 0.0;
+#pragma unroll
+    for (int w = 0; w < GINT_WARPS; w++) v += S.red[c & 1][w][lane];
+    int gi, gj, gk;
+    if (v != 0.0 && stage_point(S, tv, c, lane, gi, gj, gk)) atomicAdd(rho + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk, v);
+}
+
 __global__ void __launch_bounds__(GINT_THREADS, 1)
 k_rho_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
            const double* __restrict__ atom_pos, const int* __restrict__ atom_spec, const SpeciesDev* __restrict__ sp,
-           const double* __restrict__ tab, const int* __restrict__ crow, const unsigned long long* __restrict__ ckey,
+           const double* __restrict__ tab, const int* __restrict__ crow, const u64* __restrict__ ckey,
            const unsigned int* __restrict__ coff, const double* __restrict__ Dh, double* __restrict__ rho) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TileSmem& S = *reinterpret_cast<TileSmem*>(smem_raw);
     TileView tv;
     tile_setup(g, S, tv, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff);
+    if (tv.nchunk == 0) return;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
-    const int wr = warp >> 2, wc = ((warp & 3) + wr) & 3;
-    int R0, nr, C0, nc;
-    warp_range(tv.nfI, wr, R0, nr);       // rows of Dh (orbitals of group I), 8 per fragment = 2 DMMA k-steps
-    warp_range(tv.nfJ, wc, C0, nc);       // columns of Dh (orbitals of group J)
-    unsigned ratoms[4], catoms[4], need[4];
-    warp_need(S, tv, R0, nr, C0, nc, ratoms, catoms, need);
-    // stationary B fragments: dreg[i][h][j] = Dh[row (R0+i)*8 + 4h + lc][col (C0+j)*8 + lr]
-    double dreg[4][2][4];
-#pragma unroll
-    for (int i = 0; i < 4; i++)
-#pragma unroll
-        for (int h = 0; h < 2; h++)
-#pragma unroll
-            for (int j = 0; j < 4; j++) {
-                double v = 0.0;
-                if ((need[i] >> j) & 1u) {
-                    const int row = (R0 + i) * 8 + 4 * h + lc, col = (C0 + j) * 8 + lr;
-                    const int a = S.row_atom[0][row], bb = S.row_atom[1][col];
-                    if (a != 255 && bb != 255) {
-                        const unsigned off = S.pair_off[a][bb];
-                        if (off != 0xffffffffu) {
-                            const int oa = S.row_orb[0][row], ob = S.row_orb[1][col];
-                            const int nA = S.cstart[0][a + 1] - S.cstart[0][a], nB = S.cstart[1][bb + 1] - S.cstart[1][bb];
-                            v = __ldg(Dh + off + (S.pair_tr[a][bb] ? ob * nA + oa : oa * nB + ob));
-                        }
-                    }
-                }
-                dreg[i][h][j] = v;
-            }
+    const Seg sA = load_seg(S, warp), sB = load_seg(S, warp + GINT_WARPS);
+    double dA[GINT_SEG_COLS][2], dB[GINT_SEG_COLS][2];
+    load_dseg(S, sA, Dh, dA);
+    load_dseg(S, sB, Dh, dB);
+    // lane -> point of the stage after the butterfly reduction below
+    const int pt = 8 * (lr >> 1) + 2 * lc + (lr & 1);
 
-    if (warp < 2) make_points<false>(g, S, tv, warp, nullptr);
+    if (warp < 2) make_stage<false>(g, S, tv, warp, nullptr);
     __syncthreads();
-    eval_chunk<false>(g, S, tv, 0, 0, sp, tab);
+    eval_stage<false>(g, S, tv, 0, warp, tab);
     for (int c = 0; c < tv.nchunk; c++) {
         const int st = c & 1;
-        if (threadIdx.x < GINT_CHUNK) S.red[threadIdx.x] = 0.0;
         __syncthreads();
-        if (warp == ((c + 2) & 15)) make_points<false>(g, S, tv, c + 2, nullptr);
-        if (c + 1 < tv.nchunk) eval_chunk<false>(g, S, tv, c + 1, st ^ 1, sp, tab);
-        unsigned RW, CW;                        // nibble pf: fragments active on the 8 points 8pf .. 8pf+7
-        chunk_masks<true>(S, st, R0, nr, C0, nc, RW, CW);
-        unsigned act = (RW | (RW >> 1) | (RW >> 2) | (RW >> 3)) & (CW | (CW >> 1) | (CW >> 2) | (CW >> 3)) & 0x1111u;
-        while (act) {
-            const int p4 = __ffs(act) - 1; act &= act - 1;
-            const int pf = p4 >> 2;
-            const unsigned r4 = (RW >> p4) & 15u, c4 = (CW >> p4) & 15u;
-            double x[4][2];
+        if (warp == (c + 2) % GINT_WARPS) make_stage<false>(g, S, tv, c + 2, nullptr);
+        if (c > 0 && warp == (c + 3) % GINT_WARPS) rho_store(g, S, tv, c - 1, rho);
+        if (warp & 1) eval_stage<false>(g, S, tv, st ^ 1, warp, tab);
+        double part[4][2];
 #pragma unroll
-            for (int j = 0; j < 4; j++) { x[j][0] = 0.0; x[j][1] = 0.0; }
-            // A fragment: Phi_I[point 8pf + lr][orbital row (R0+i)*8 + 4h + lc]
-            const double* pa = &S.phi[st][0][R0 * 8 + lc][8 * pf + lr];
+        for (int q = 0; q < 4; q++) { part[q][0] = 0.0; part[q][1] = 0.0; }
+        const unsigned bA = stage_bits(S, c, sA.act), bB = stage_bits(S, c, sB.act);
+        if (bA) rho_seg_dispatch(sA.n, dA, &S.phi[st][0][8 * sA.row + lc][lr], &S.phi[st][1][8 * sA.cb + lr][2 * lc], bA, part);
+        if (bB) rho_seg_dispatch(sB.n, dB, &S.phi[st][0][8 * sB.row + lc][lr], &S.phi[st][1][8 * sB.cb + lr][2 * lc], bB, part);
+        // part[q][e]: points 8q + 2lc + e, partial over the lane's orbital row lr -> reduce-scatter over lr (lane bits 2..4)
+        double r4[4], r2[2], r1;
+        {
+            const bool hi = lane & 16;
 #pragma unroll
-            for (int i = 0; i < 4; i++) {
-                const unsigned m = ((r4 >> i) & 1u) ? (c4 & need[i]) : 0u;
-                if (!m) continue;
-                const double a0 = pa[(i * 8) * GINT_LD], a1 = pa[(i * 8 + 4) * GINT_LD];
-                dmma_row2(x, a0, a1, dreg[i][0], dreg[i][1], m);
+            for (int i = 0; i < 4; i++) {     // value index t = 2q + e; keep t < 4 on lanes with bit 4 clear
+                const double keep = hi ? part[2 + (i >> 1)][i & 1] : part[i >> 1][i & 1];
+                const double send = hi ? part[i >> 1][i & 1] : part[2 + (i >> 1)][i & 1];
+                r4[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
             }
-            // rho partial of point 8pf + lr: sum over this warp's columns of X * Phi_J
-            double part = 0.0;
-            const double* pj = &S.phi[st][1][C0 * 8 + 2 * lc][8 * pf + lr];
+            const bool mid = lane & 8;
 #pragma unroll
-            for (int j = 0; j < 4; j++) {
-                if (!((c4 >> j) & 1u)) continue;
-                part = fma(x[j][0], pj[(j * 8) * GINT_LD], part);
-                part = fma(x[j][1], pj[(j * 8 + 1) * GINT_LD], part);
+            for (int i = 0; i < 2; i++) {
+                const double keep = mid ? r4[2 + i] : r4[i], send = mid ? r4[i] : r4[2 + i];
+                r2[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
             }
-            part += __shfl_xor_sync(0xffffffffu, part, 1);
-            part += __shfl_xor_sync(0xffffffffu, part, 2);
-            if (lc == 0 && part != 0.0) atomicAdd(&S.red[8 * pf + lr], part);
+            const bool low = lane & 4;
+            const double keep = low ? r2[1] : r2[0], send = low ? r2[0] : r2[1];
+            r1 = keep + __shfl_xor_sync(0xffffffffu, send, 4);
         }
-        __syncthreads();
-        if (threadIdx.x < GINT_CHUNK) {
-            const double v = S.red[threadIdx.x];
-            int gi, gj, gk;
-            if (v != 0.0 && chunk_point(tv, c, threadIdx.x, gi, gj, gk))
-                atomicAdd(rho + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk, v);
-        }
+        S.red[st][warp][pt] = r1;
+        if (!(warp & 1)) eval_stage<false>(g, S, tv, st ^ 1, warp, tab);
     }
+    __syncthreads();
+    if (warp == 0) rho_store(g, S, tv, tv.nchunk - 1, rho);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -606,7 +667,7 @@ __global__ void __launch_bounds__(128) k_alg_stats(Geom g, const int* __restrict
                 const double dy = y - (atom_pos[3 * en.atom + 1] + t1 * g.a[1] + t2 * g.a[4] + t3 * g.a[7]);
                 const double dz = z - (atom_pos[3 * en.atom + 2] + t1 * g.a[2] + t2 * g.a[5] + t3 * g.a[8]);
                 const SpeciesDev* Sp = sp + atom_spec[en.atom];
-                if (sqrt(dx * dx + dy * dy + dz * dz) < Sp->rc) { na++; no += Sp->norb; }
+                if (fma(dx, dx, fma(dy, dy, dz * dz)) < Sp->rc * Sp->rc) { na++; no += Sp->norb; }
             }
             inc += na; sn += no; sn2 += (unsigned long long)no * no; ne += na > 0;
         }
