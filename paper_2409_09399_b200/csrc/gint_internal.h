@@ -13,14 +13,20 @@
 #define GINT_MAX_SHELL 12          // radial shells per species
 #define GINT_MAX_NB 96             // neighbouring atom images per grid batch
 #define GINT_MAX_BS 8              // largest grid-batch edge (points): 4 x 4 x 4 cubelets of 2 x 2 x 2 points = one 64-bit mask
-#define GINT_WARPS 16              // warps per CTA of the contraction kernels
+#define GINT_WARPS 16              // warps per CTA of the contraction kernels: 4 warp groups
 #define GINT_THREADS (32 * GINT_WARPS)
+#define GINT_MMA_WARPS 8           // warp groups 0,1: DMMA consumers (setmaxnreg.inc); warp groups 2,3: orbital-evaluation producers
+#define GINT_EVAL_WARPS (GINT_WARPS - GINT_MMA_WARPS)
+#define GINT_REGS_MMA 176          // registers per thread after setmaxnreg: 256 * 176 + 256 * 80 = 65536
+#define GINT_REGS_EVAL 80
+#define GINT_STAGES 3              // shared-memory ring of orbital-value stages between producers and consumers
 // tile geometry of the contraction kernels: one CTA owns the block of H (or D) between two groups of atoms
 #define GINT_TILE_ATOMS 8          // atom images per group
 #define GINT_TILE_ORB 104          // orbitals per group = 13 fragments of 8 (8 atoms x 13 orbitals exactly)
 #define GINT_TILE_FRAG 13
-#define GINT_SEG_COLS 7            // column fragments of one segment (a warp owns two segments: row fragment x <= 7 column fragments)
-#define GINT_MAX_SEG (2 * GINT_WARPS)
+#define GINT_SEG_COLS 7            // column fragments of one segment (row fragment x <= 7 column fragments)
+#define GINT_WARP_SEGS 4           // segments per consumer warp
+#define GINT_MAX_SEG (GINT_WARP_SEGS * GINT_MMA_WARPS)
 #define GINT_CHUNK 32              // mesh points per pipeline stage = 4 cubelets of 8 points
 #define GINT_LD 40                 // row stride (doubles) of the orbital tiles in shared memory: = 8 mod 16, LDS.128 conflict-free
 

@@ -8,7 +8,7 @@
 // 104 x 104 block of Phi_I^T diag(V dV) Phi_J (gint_vlocal, Eq. 2) or of the density blocks D_IJ
 // (gint_rho, Eq. 3).  That block stays in REGISTERS (DMMA accumulators, resp. stationary DMMA
 // operands): the 13 x 13 fragments (8 x 8 orbitals) of the block are cut into SEGMENTS of one row fragment x up to
-// 7 column fragments, two segments per warp, dealt to the 14 warps so that the four SM sub-partitions carry equal
+// 7 column fragments, four segments per consumer warp, dealt to the 8 consumer warps so that the four SM sub-partitions carry equal
 // numbers of DMMAs; in a diagonal tile (I == J) only the fragments on or above the atom diagonal are segments.
 // The CTA walks over the cubelets on which both groups are active, 4 cubelets (32 points) per pipeline stage: the
 // orbital values of the needed (atom, cubelet) items are evaluated into shared memory (the paper's orbital-value
@@ -27,12 +27,21 @@ typedef unsigned long long u64;
 struct PairEnt { unsigned off; unsigned short sr, sc; };   // element (oa, ob) of the atom pair at off + oa*sr + ob*sc; off = ~0u: none
 struct SlotInfo { double rc2; int n_int, nsh, tab_off, lpack; };   // lpack: 2 bits of l per shell
 
+struct TileView {
+    int b, I, J, G;                  // batch, groups
+    int i0, j0, k0, ex, ey, ez;      // batch origin and extents (mesh points)
+    int nchunk;                      // stages of 4 cubelets
+    int nI, nJ;                      // atoms in the two groups
+    int nfI, nfJ;                    // fragments (8 orbitals) in the two groups
+    bool diag;
+};
+
 struct TileSmem {
     // phi[stage][side][orbital row][GINT_LD]: side 0 = group I, side 1 = group J (scaled by V dV in vlocal);
     // column 8q + p = point p of the stage's q-th cubelet
-    double phi[2][2][GINT_TILE_ORB][GINT_LD];
+    double phi[GINT_STAGES][2][GINT_TILE_ORB][GINT_LD];
     double4 pts[2][GINT_CHUNK];         // [stage][point]: x, y, z, weight (V dV in vlocal, 1 in rho)
-    double red[2][GINT_WARPS][GINT_CHUNK];   // rho: per-warp partial sums of the stage's points
+    u64 full[GINT_STAGES], empty[GINT_STAGES];   // mbarriers: stage written by all producer warps / read by all consumer warps
     double pos[16][4];                  // slot s < 8: atom s of group I; slot 8 + s: atom s of group J
     SlotInfo sinfo[16];
     u64 amask[16];                      // cubelets on which the slot's atom is non-zero
@@ -43,9 +52,10 @@ struct TileSmem {
     PairEnt pair[GINT_TILE_ATOMS][GINT_TILE_ATOMS];   // canonical block of (I atom a, J atom b)
     int atom[16], shift[16], spec[16];
     int cstart[2][GINT_TILE_ATOMS + 1]; // first orbital row of each atom inside its group
-    int seg[GINT_MAX_SEG];              // slot warp + 14 k: row fragment | first column fragment << 8 | n columns << 16
+    int seg[GINT_MAX_SEG];              // slot (consumer warp) + 8 k: row fragment | first column fragment << 8 | n columns << 16
     int nitem[2], neval[2];             // [stage]: items of the stage, of which the first neval need a real evaluation
     int ncub;
+    TileView tv;                        // written by tile_setup; read from here afterwards to keep registers free
     unsigned char valid[2][GINT_CHUNK]; // the stage's point exists (inside the batch and the mesh)
     unsigned char item[2][64];          // [stage][k]: slot << 2 | cubelet of the stage
     unsigned char cub[64 + 4];          // the tile's cubelets (bit numbers of U, ascending)
@@ -55,19 +65,28 @@ struct TileSmem {
 };
 size_t gint_smem_needed(const Geom&) { return sizeof(TileSmem); }
 
+// The DMMA chains and their operand loads are volatile asm: left to itself the compiler sinks every shared load to
+// just before its DMMA (one operand register, fully serialised LDS -> DMMA -> LDS ...) and pairs the two k-steps of
+// an accumulator back to back.  Volatile asm keeps the written order: all loads of a cubelet, then the DMMAs.
 __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
-    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};" : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};" : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ double2 lds128(unsigned addr) {
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ double lds64(unsigned addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr) : "memory");
+    return v;
 }
 
-struct TileView {
-    int b, I, J, G;                  // batch, groups
-    int i0, j0, k0, ex, ey, ez;      // batch origin and extents (mesh points)
-    int nchunk;                      // stages of 4 cubelets
-    int nI, nJ;                      // atoms in the two groups
-    int nfI, nfJ;                    // fragments (8 orbitals) in the two groups
-    bool diag;
-};
 
+__device__ __forceinline__ void mbar_init(u64* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
 __device__ __forceinline__ u64 warp_or64(u64 v) {
     const unsigned lo = __reduce_or_sync(0xffffffffu, (unsigned)v), hi = __reduce_or_sync(0xffffffffu, (unsigned)(v >> 32));
     return (u64)lo | ((u64)hi << 32);
@@ -176,7 +195,7 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
         S.pair[a][bb] = pe;
     }
     // padding rows (orbital rows between the group's last orbital and the end of its last fragment) must hold zeros
-    for (int idx = tid; idx < 2 * 2 * 8 * GINT_LD; idx += blockDim.x) {
+    for (int idx = tid; idx < GINT_STAGES * 2 * 8 * GINT_LD; idx += blockDim.x) {
         const int col = idx % GINT_LD, r = (idx / GINT_LD) & 7, side = (idx / (8 * GINT_LD)) & 1, st = idx / (16 * GINT_LD);
         const int row = (side ? totJ : totI) + r;
         if (row < GINT_TILE_ORB) S.phi[st][side][row][col] = 0.0;
@@ -225,12 +244,17 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
         }
         if (pn > 0) {
             const int k7 = rank & 7, s = k7 < 4 ? k7 : 7 - k7, j = 2 * (rank >> 3) + (k7 >= 4);
-            const int W = s < (GINT_WARPS & 3) ? (GINT_WARPS >> 2) + 1 : (GINT_WARPS >> 2);
-            S.seg[s + 4 * (j % W) + GINT_WARPS * (j / W)] = r | (pcb << 8) | (pn << 16);
+            const int W = GINT_MMA_WARPS / 4;         // consumer warps per sub-partition
+            S.seg[s + 4 * (j % W) + GINT_MMA_WARPS * (j / W)] = r | (pcb << 8) | (pn << 16);
         }
     }
     __syncthreads();
     tv.nchunk = (S.ncub + 3) >> 2;
+    if (tid == 0) {
+        S.tv = tv;
+        for (int s = 0; s < GINT_STAGES; s++) { mbar_init(&S.full[s], GINT_EVAL_WARPS); mbar_init(&S.empty[s], GINT_MMA_WARPS); }
+    }
+    __syncthreads();
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -284,19 +308,19 @@ __device__ __forceinline__ void make_stage(const Geom& g, TileSmem& S, const Til
 // cubic in b = r/dr - i (reading R5), coefficients read with 128-bit loads.  vlocal scales side J by V dV.
 // A diagonal tile evaluates each atom once and writes both sides.
 template <bool VLOCAL>
-__device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, const TileView& tv, int st, int rank,
-                                           const double* __restrict__ tab) {
+__device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, const TileView& tv, int ps, int st, int rank,
+                                           const double* __restrict__ tab) {   // ps: ring slot of phi; st: parity of the point / item lists
     const int lane = threadIdx.x & 31;
     const int nitem = S.nitem[st], neval = S.neval[st];
     const bool two = tv.diag;
-    for (int base = 4 * rank; base < nitem; base += 4 * GINT_WARPS) {
+    for (int base = 4 * rank; base < nitem; base += 4 * GINT_EVAL_WARPS) {
         const int idx = base + (lane >> 3);
         const bool on = idx < nitem;
         const int it = on ? S.item[st][idx] : 0;
         const int slot = it >> 2, col = 8 * (it & 3) + (lane & 7);
         const int side = slot >> 3, a = slot & 7;
-        double* o0 = &S.phi[st][side][S.cstart[side][a]][col];
-        double* o1 = &S.phi[st][1][S.cstart[side][a]][col];
+        double* o0 = &S.phi[ps][side][S.cstart[side][a]][col];
+        double* o1 = &S.phi[ps][1][S.cstart[side][a]][col];
         if (base >= neval) {                        // the four items only need zeros
             const int norb = on ? S.cstart[side][a + 1] - S.cstart[side][a] : 0;
             for (int o = 0; o < norb; o++) { o0[o * GINT_LD] = 0.0; if (two) o1[o * GINT_LD] = 0.0; }
@@ -358,17 +382,33 @@ __device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, const Til
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Segments of a warp.
+// Producer / consumer plumbing.  Warp groups 2,3 (producers) evaluate orbital values into a ring of GINT_STAGES
+// shared-memory stages; warp groups 0,1 (consumers) run the DMMA chains.  full[s] completes when all producer warps
+// have written stage s, empty[s] when all consumer warps have read it.  setmaxnreg moves registers from the
+// producers (80 per thread) to the consumers (176), which hold the whole 104 x 104 block.
+__device__ __forceinline__ void mbar_arrive(u64* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(u64* bar, int parity) {
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
+                 :: "r"(a), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void producer_sync() { asm volatile("bar.sync 1, %0;" :: "n"(32 * GINT_EVAL_WARPS) : "memory"); }
+
+// Segments of a consumer warp.
 struct Seg {
-    int row, cb, n;                  // row fragment, first column fragment, column fragments (0 = unused)
+    int w;                           // row fragment | first column fragment << 8 | column fragments << 16 (0 = unused)
     u64 act;                         // cubelets on which the row fragment and some column fragment are both active
+    __device__ __forceinline__ int row() const { return w & 255; }
+    __device__ __forceinline__ int cb() const { return (w >> 8) & 255; }
+    __device__ __forceinline__ int n() const { return w >> 16; }
 };
 __device__ __forceinline__ Seg load_seg(const TileSmem& S, int slot) {
-    const int w = S.seg[slot];
-    Seg s; s.row = w & 255; s.cb = (w >> 8) & 255; s.n = w >> 16;
+    Seg s; s.w = S.seg[slot];
     u64 cm = 0;
-    for (int j = 0; j < s.n; j++) cm |= S.fmask[1][s.cb + j];
-    s.act = s.n ? (S.fmask[0][s.row] & cm) : 0ull;
+    for (int j = 0; j < s.n(); j++) cm |= S.fmask[1][s.cb() + j];
+    s.act = s.n() ? (S.fmask[0][s.row()] & cm) : 0ull;
     return s;
 }
 // 4-bit activity of a segment on the cubelets of stage c
@@ -385,21 +425,21 @@ __device__ __forceinline__ unsigned stage_bits(const TileSmem& S, int c, u64 act
 // active cubelet of the stage: one 128-bit shared load per operand fragment (points 2 lc, 2 lc + 1 of the lane's
 // orbital row) feeds two DMMA k-steps (k index lc <-> point 2 lc, then point 2 lc + 1).
 template <int N>
-__device__ __forceinline__ void vl_seg(double (&acc)[GINT_SEG_COLS][2], const double* __restrict__ pa, const double* __restrict__ pb, unsigned bits) {
+__device__ __forceinline__ void vl_seg(double (&acc)[GINT_SEG_COLS][2], unsigned pa, unsigned pb, unsigned bits) {
 #pragma unroll
     for (int q = 0; q < 4; q++) {
         if (!((bits >> q) & 1u)) continue;
-        const double2 a = *reinterpret_cast<const double2*>(pa + 8 * q);
+        const double2 a = lds128(pa + 64 * q);
         double2 bv[N];
 #pragma unroll
-        for (int j = 0; j < N; j++) bv[j] = *reinterpret_cast<const double2*>(pb + j * 8 * GINT_LD + 8 * q);
+        for (int j = 0; j < N; j++) bv[j] = lds128(pb + (j * 8 * GINT_LD + 8 * q) * 8);
 #pragma unroll
         for (int j = 0; j < N; j++) dmma884(acc[j], a.x, bv[j].x);
 #pragma unroll
         for (int j = 0; j < N; j++) dmma884(acc[j], a.y, bv[j].y);
     }
 }
-__device__ __forceinline__ void vl_seg_dispatch(int n, double (&acc)[GINT_SEG_COLS][2], const double* pa, const double* pb, unsigned bits) {
+__device__ __forceinline__ void vl_seg_dispatch(int n, double (&acc)[GINT_SEG_COLS][2], unsigned pa, unsigned pb, unsigned bits) {
     switch (n) {
         case 7: vl_seg<7>(acc, pa, pb, bits); break;
         case 6: vl_seg<6>(acc, pa, pb, bits); break;
@@ -409,6 +449,23 @@ __device__ __forceinline__ void vl_seg_dispatch(int n, double (&acc)[GINT_SEG_CO
         case 2: vl_seg<2>(acc, pa, pb, bits); break;
         case 1: vl_seg<1>(acc, pa, pb, bits); break;
         default: break;
+    }
+}
+
+// producer loop shared by both kernels: stage c of the tile goes to ring slot c % GINT_STAGES
+template <bool VLOCAL>
+__device__ __forceinline__ void producer_loop(const Geom& g, TileSmem& S, int nchunk, const double* __restrict__ tab, const double* __restrict__ V) {
+    const int pw = (threadIdx.x >> 5) - GINT_MMA_WARPS;
+    const TileView& tv = S.tv;
+    if (pw == 0) make_stage<VLOCAL>(g, S, tv, 0, V);
+    for (int c = 0; c < nchunk; c++) {
+        const int s = c % GINT_STAGES, k = c / GINT_STAGES;
+        producer_sync();              // the point / item lists of stage c are complete; all producers are done with stage c-1
+        if (pw == (c + 1) % GINT_EVAL_WARPS) make_stage<VLOCAL>(g, S, tv, c + 1, V);
+        if (k > 0) mbar_wait(&S.empty[s], (k - 1) & 1);
+        eval_stage<VLOCAL>(g, S, tv, s, c & 1, pw, tab);
+        __syncwarp();
+        if ((threadIdx.x & 31) == 0) mbar_arrive(&S.full[s]);
     }
 }
 
@@ -423,47 +480,55 @@ k_vlocal_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bst
               const unsigned int* __restrict__ coff, const double* __restrict__ V, double* __restrict__ Hc) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TileSmem& S = *reinterpret_cast<TileSmem*>(smem_raw);
-    TileView tv;
-    tile_setup(g, S, tv, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff);
-    if (tv.nchunk == 0) return;
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
-    const Seg sA = load_seg(S, warp), sB = load_seg(S, warp + GINT_WARPS);
-    double accA[GINT_SEG_COLS][2], accB[GINT_SEG_COLS][2];
+    {
+        TileView tv0;
+        tile_setup(g, S, tv0, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff);
+    }
+    const int nchunk = S.tv.nchunk;
+    if (nchunk == 0) return;
+    const int warp = threadIdx.x >> 5;
+    if (warp >= GINT_MMA_WARPS) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(GINT_REGS_EVAL));
+        producer_loop<true>(g, S, nchunk, tab, V);
+        return;
+    }
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(GINT_REGS_MMA));
+    const int lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
+    Seg sg[GINT_WARP_SEGS];
+    double acc[GINT_WARP_SEGS][GINT_SEG_COLS][2];
 #pragma unroll
-    for (int j = 0; j < GINT_SEG_COLS; j++) { accA[j][0] = accA[j][1] = 0.0; accB[j][0] = accB[j][1] = 0.0; }
-
-    if (warp < 2) make_stage<true>(g, S, tv, warp, V);
-    __syncthreads();
-    eval_stage<true>(g, S, tv, 0, warp, tab);
-    for (int c = 0; c < tv.nchunk; c++) {
-        const int st = c & 1;
-        __syncthreads();                       // stage st is complete; every warp has finished the MMAs of stage c-1
-        if (warp == (c + 2) % GINT_WARPS) make_stage<true>(g, S, tv, c + 2, V);
-        // half of the warps evaluate first, the other half multiply first, so that the FP64 tensor pipe has work
-        // while instructions of the evaluation issue
-        if (warp & 1) eval_stage<true>(g, S, tv, st ^ 1, warp, tab);
-        const unsigned bA = stage_bits(S, c, sA.act), bB = stage_bits(S, c, sB.act);
-        if (bA) vl_seg_dispatch(sA.n, accA, &S.phi[st][0][8 * sA.row + lr][2 * lc], &S.phi[st][1][8 * sA.cb + lr][2 * lc], bA);
-        if (bB) vl_seg_dispatch(sB.n, accB, &S.phi[st][0][8 * sB.row + lr][2 * lc], &S.phi[st][1][8 * sB.cb + lr][2 * lc], bB);
-        if (!(warp & 1)) eval_stage<true>(g, S, tv, st ^ 1, warp, tab);
+    for (int k = 0; k < GINT_WARP_SEGS; k++) {
+        sg[k] = load_seg(S, warp + GINT_MMA_WARPS * k);
+#pragma unroll
+        for (int j = 0; j < GINT_SEG_COLS; j++) { acc[k][j][0] = 0.0; acc[k][j][1] = 0.0; }
+    }
+    for (int c = 0; c < nchunk; c++) {
+        const int s = c % GINT_STAGES;
+        mbar_wait(&S.full[s], (c / GINT_STAGES) & 1);
+        const unsigned pa = smem_addr(&S.phi[s][0][lr][2 * lc]), pb = smem_addr(&S.phi[s][1][lr][2 * lc]);
+#pragma unroll
+        for (int k = 0; k < GINT_WARP_SEGS; k++) {
+            const unsigned bits = stage_bits(S, c, sg[k].act);
+            if (bits) vl_seg_dispatch(sg[k].n(), acc[k], pa + sg[k].row() * (64 * GINT_LD), pb + sg[k].cb() * (64 * GINT_LD), bits);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&S.empty[s]);
     }
     // flush: element (row, col) -> atom pair (a, b), orbitals (oa, ob) -> canonical block (transposed if the canonical
     // key is (b, a)).  Exact zeros (fragments never touched, atoms that do not overlap inside this batch) are skipped.
 #pragma unroll
-    for (int s = 0; s < 2; s++) {
-        const Seg& sg = s ? sB : sA;
-        if (sg.n == 0 || sg.act == 0ull) continue;
-        const int row = 8 * sg.row + lr;
+    for (int k = 0; k < GINT_WARP_SEGS; k++) {
+        if (sg[k].n() == 0 || sg[k].act == 0ull) continue;
+        const int row = 8 * sg[k].row() + lr;
         const int a = S.row_atom[0][row], oa = S.row_orb[0][row];
         if (a == 255) continue;
 #pragma unroll
         for (int j = 0; j < GINT_SEG_COLS; j++) {
-            if (j >= sg.n) break;
+            if (j >= sg[k].n()) break;
 #pragma unroll
             for (int e = 0; e < 2; e++) {
-                const double v = s ? accB[j][e] : accA[j][e];
-                const int col = 8 * (sg.cb + j) + 2 * lc + e;
+                const double v = acc[k][j][e];
+                const int col = 8 * (sg[k].cb() + j) + 2 * lc + e;
                 const int bb = S.row_atom[1][col], ob = S.row_orb[1][col];
                 if (bb == 255 || v == 0.0) continue;
                 const PairEnt pe = S.pair[a][bb];
@@ -479,25 +544,30 @@ k_vlocal_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bst
 // (registers): per cubelet X^T = Dh_seg^T Phi_I (8 orbitals of J x 8 points per column fragment) and
 // rho_g += sum_j X_jg Phi_J,jg.  Dh = canonical-half, symmetrised density blocks (k_sym_D).
 template <int N>
-__device__ __forceinline__ void rho_seg(const double (&d)[GINT_SEG_COLS][2], const double* __restrict__ pi, const double* __restrict__ pj,
-                                        unsigned bits, double (&part)[4][2]) {
+__device__ __forceinline__ void rho_cols(const double (&d)[GINT_SEG_COLS][2], int j0, double b0, double b1, unsigned pj, double& p0, double& p1) {
+    double2 f[N];
+#pragma unroll
+    for (int j = 0; j < N; j++) f[j] = lds128(pj + ((j0 + j) * 8 * GINT_LD) * 8);
+    double x[N][2];
+#pragma unroll
+    for (int j = 0; j < N; j++) { x[j][0] = 0.0; x[j][1] = 0.0; dmma884(x[j], d[j0 + j][0], b0); }
+#pragma unroll
+    for (int j = 0; j < N; j++) dmma884(x[j], d[j0 + j][1], b1);
+#pragma unroll
+    for (int j = 0; j < N; j++) { p0 = fma(x[j][0], f[j].x, p0); p1 = fma(x[j][1], f[j].y, p1); }
+}
+template <int N>
+__device__ __forceinline__ void rho_seg(const double (&d)[GINT_SEG_COLS][2], unsigned pi, unsigned pj, unsigned bits, double (&part)[4][2]) {
 #pragma unroll
     for (int q = 0; q < 4; q++) {
         if (!((bits >> q) & 1u)) continue;
-        const double b0 = pi[8 * q], b1 = pi[4 * GINT_LD + 8 * q];       // Phi_I[8 row + lc (+4)][point 8q + lr]
-        double2 f[N];
-#pragma unroll
-        for (int j = 0; j < N; j++) f[j] = *reinterpret_cast<const double2*>(pj + j * 8 * GINT_LD + 8 * q);
-        double x[N][2];
-#pragma unroll
-        for (int j = 0; j < N; j++) { x[j][0] = 0.0; x[j][1] = 0.0; dmma884(x[j], d[j][0], b0); }
-#pragma unroll
-        for (int j = 0; j < N; j++) dmma884(x[j], d[j][1], b1);
-#pragma unroll
-        for (int j = 0; j < N; j++) { part[q][0] = fma(x[j][0], f[j].x, part[q][0]); part[q][1] = fma(x[j][1], f[j].y, part[q][1]); }
+        const double b0 = lds64(pi + 64 * q), b1 = lds64(pi + (4 * GINT_LD + 8 * q) * 8);       // Phi_I[8 row + lc (+4)][point 8q + lr]
+        constexpr int N0 = N > 4 ? 4 : N;
+        rho_cols<N0>(d, 0, b0, b1, pj + 64 * q, part[q][0], part[q][1]);
+        if (N > 4) rho_cols<(N > 4 ? N - 4 : 1)>(d, 4, b0, b1, pj + 64 * q, part[q][0], part[q][1]);
     }
 }
-__device__ __forceinline__ void rho_seg_dispatch(int n, const double (&d)[GINT_SEG_COLS][2], const double* pi, const double* pj,
+__device__ __forceinline__ void rho_seg_dispatch(int n, const double (&d)[GINT_SEG_COLS][2], unsigned pi, unsigned pj,
                                                  unsigned bits, double (&part)[4][2]) {
     switch (n) {
         case 7: rho_seg<7>(d, pi, pj, bits, part); break;
@@ -518,8 +588,8 @@ __device__ __forceinline__ void load_dseg(const TileSmem& S, const Seg& sg, cons
 #pragma unroll
         for (int h = 0; h < 2; h++) {
             double v = 0.0;
-            if (j < sg.n) {
-                const int row = 8 * sg.row + 4 * h + lc, col = 8 * (sg.cb + j) + lr;
+            if (j < sg.n()) {
+                const int row = 8 * sg.row() + 4 * h + lc, col = 8 * (sg.cb() + j) + lr;
                 const int a = S.row_atom[0][row], bb = S.row_atom[1][col];
                 if (a != 255 && bb != 255) {
                     const PairEnt pe = S.pair[a][bb];
@@ -529,15 +599,6 @@ __device__ __forceinline__ void load_dseg(const TileSmem& S, const Seg& sg, cons
             d[j][h] = v;
         }
 }
-// sum over the 14 warps of the partial densities of stage c and add them to rho (one warp)
-__device__ __forceinline__ void rho_store(const Geom& g, const TileSmem& S, const TileView& tv, int c, double* __restrict__ rho) {
-    const int lane = threadIdx.x & 31;
-    double v = 0.0;
-#pragma unroll
-    for (int w = 0; w < GINT_WARPS; w++) v += S.red[c & 1][w][lane];
-    int gi, gj, gk;
-    if (v != 0.0 && stage_point(S, tv, c, lane, gi, gj, gk)) atomicAdd(rho + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk, v);
-}
 
 __global__ void __launch_bounds__(GINT_THREADS, 1)
 k_rho_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
@@ -546,39 +607,50 @@ k_rho_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart
            const unsigned int* __restrict__ coff, const double* __restrict__ Dh, double* __restrict__ rho) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TileSmem& S = *reinterpret_cast<TileSmem*>(smem_raw);
-    TileView tv;
-    tile_setup(g, S, tv, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff);
-    if (tv.nchunk == 0) return;
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
-    const Seg sA = load_seg(S, warp), sB = load_seg(S, warp + GINT_WARPS);
-    double dA[GINT_SEG_COLS][2], dB[GINT_SEG_COLS][2];
-    load_dseg(S, sA, Dh, dA);
-    load_dseg(S, sB, Dh, dB);
-    // lane -> point of the stage after the butterfly reduction below
-    const int pt = 8 * (lr >> 1) + 2 * lc + (lr & 1);
-
-    if (warp < 2) make_stage<false>(g, S, tv, warp, nullptr);
-    __syncthreads();
-    eval_stage<false>(g, S, tv, 0, warp, tab);
-    for (int c = 0; c < tv.nchunk; c++) {
-        const int st = c & 1;
-        __syncthreads();
-        if (warp == (c + 2) % GINT_WARPS) make_stage<false>(g, S, tv, c + 2, nullptr);
-        if (c > 0 && warp == (c + 3) % GINT_WARPS) rho_store(g, S, tv, c - 1, rho);
-        if (warp & 1) eval_stage<false>(g, S, tv, st ^ 1, warp, tab);
+    {
+        TileView tv0;
+        tile_setup(g, S, tv0, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff);
+    }
+    const int nchunk = S.tv.nchunk;
+    if (nchunk == 0) return;
+    const int warp = threadIdx.x >> 5;
+    if (warp >= GINT_MMA_WARPS) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(GINT_REGS_EVAL));
+        producer_loop<false>(g, S, nchunk, tab, nullptr);
+        return;
+    }
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(GINT_REGS_MMA));
+    const int lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
+    Seg sg[GINT_WARP_SEGS];
+    double d[GINT_WARP_SEGS][GINT_SEG_COLS][2];
+#pragma unroll
+    for (int k = 0; k < GINT_WARP_SEGS; k++) {
+        sg[k] = load_seg(S, warp + GINT_MMA_WARPS * k);
+        load_dseg(S, sg[k], Dh, d[k]);
+    }
+    for (int c = 0; c < nchunk; c++) {
+        const int s = c % GINT_STAGES;
         double part[4][2];
 #pragma unroll
         for (int q = 0; q < 4; q++) { part[q][0] = 0.0; part[q][1] = 0.0; }
-        const unsigned bA = stage_bits(S, c, sA.act), bB = stage_bits(S, c, sB.act);
-        if (bA) rho_seg_dispatch(sA.n, dA, &S.phi[st][0][8 * sA.row + lc][lr], &S.phi[st][1][8 * sA.cb + lr][2 * lc], bA, part);
-        if (bB) rho_seg_dispatch(sB.n, dB, &S.phi[st][0][8 * sB.row + lc][lr], &S.phi[st][1][8 * sB.cb + lr][2 * lc], bB, part);
+        mbar_wait(&S.full[s], (c / GINT_STAGES) & 1);
+        const unsigned pi = smem_addr(&S.phi[s][0][lc][lr]), pj = smem_addr(&S.phi[s][1][lr][2 * lc]);
+        unsigned any = 0;
+#pragma unroll
+        for (int k = 0; k < GINT_WARP_SEGS; k++) {
+            const unsigned bits = stage_bits(S, c, sg[k].act);
+            any |= bits;
+            if (bits) rho_seg_dispatch(sg[k].n(), d[k], pi + sg[k].row() * (64 * GINT_LD), pj + sg[k].cb() * (64 * GINT_LD), bits, part);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&S.empty[s]);
+        if (!any) continue;
         // part[q][e]: points 8q + 2lc + e, partial over the lane's orbital row lr -> reduce-scatter over lr (lane bits 2..4)
         double r4[4], r2[2], r1;
         {
             const bool hi = lane & 16;
 #pragma unroll
-            for (int i = 0; i < 4; i++) {     // value index t = 2q + e; keep t < 4 on lanes with bit 4 clear
+            for (int i = 0; i < 4; i++) {     // value index t = 2q + e; lanes with bit 4 clear keep t < 4
                 const double keep = hi ? part[2 + (i >> 1)][i & 1] : part[i >> 1][i & 1];
                 const double send = hi ? part[i >> 1][i & 1] : part[2 + (i >> 1)][i & 1];
                 r4[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
@@ -593,11 +665,11 @@ k_rho_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart
             const double keep = low ? r2[1] : r2[0], send = low ? r2[0] : r2[1];
             r1 = keep + __shfl_xor_sync(0xffffffffu, send, 4);
         }
-        S.red[st][warp][pt] = r1;
-        if (!(warp & 1)) eval_stage<false>(g, S, tv, st ^ 1, warp, tab);
+        // the lane now owns point 8 (lr >> 1) + 2 lc + (lr & 1) of the stage
+        int gi, gj, gk;
+        if (r1 != 0.0 && stage_point(S, S.tv, c, 8 * (lr >> 1) + 2 * lc + (lr & 1), gi, gj, gk))
+            atomicAdd(rho + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk, r1);
     }
-    __syncthreads();
-    if (warp == 0) rho_store(g, S, tv, tv.nchunk - 1, rho);
 }
 
 // ---------------------------------------------------------------------------------------------------
