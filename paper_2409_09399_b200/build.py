@@ -26,7 +26,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
-    cmd = [nvcc, *NVCC_FLAGS, *(("-Xptxas", "-v") if verbose else ()), "-o", LIB,
+    extra = os.environ.get("GINT_NVCC_EXTRA", "").split()      # developer switches (e.g. -DGINT_DBG_NO_MMA); empty in normal builds
+    cmd = [nvcc, *NVCC_FLAGS, *extra, *(("-Xptxas", "-v") if verbose else ()), "-o", LIB,
            *(os.path.join(CSRC, s) for s in SOURCES)]
     subprocess.check_call(cmd)
     return LIB

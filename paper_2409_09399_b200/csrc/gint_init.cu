@@ -309,9 +309,11 @@ static void free_ctx(gint_ctx* c) {
     delete c;
 }
 
-// ---- step 0: basis tables -> per-interval cubic coefficients in the local variable b = r/dr - i ------
-// R(b) = a y_i + b y_{i+1} + ((a^3-a) y2_i + (b^3-b) y2_{i+1}) dr^2/6, a = 1-b   (reading R5)
-//      = y_i + b [ (y_{i+1}-y_i) - dr^2/6 (2 y2_i + y2_{i+1}) ] + b^2 [ dr^2/2 y2_i ] + b^3 [ dr^2/6 (y2_{i+1}-y2_i) ]
+// ---- step 0: basis tables -> knot-major cells {y, y'' dr^2/6} ------------------------------------------------
+// R(r) = a y_i + b y_{i+1} + (a^3 - a) z_i + (b^3 - b) z_{i+1},  z = y'' dr^2/6,  b = r/dr - i, a = 1 - b   (reading R5)
+// Cell (species, knot i, shell k) sits at double2 index tab_off + i * n_shell + k, so that the two knots of an
+// interval are 2 * n_shell consecutive 16-byte cells.  The whole table (56 KB for the 5-shell, 701-knot basis of
+// BASELINE.json) is copied into shared memory by the contraction kernels when it fits.
 static int build_basis(gint_ctx* c, int n_species, const int* n_shell, const int* shell_l, const double* rcut, double dr,
                        const int* n_knot, const double* tab_y, const double* tab_y2) {
     c->n_species = n_species;
@@ -332,20 +334,15 @@ static int build_basis(gint_ctx* c, int n_species, const int* n_shell, const int
             S.l[k] = l; S.norb += 2 * l + 1;
         }
         if (S.norb > GINT_MAX_ORB) GINT_FAIL(GINT_ERR_UNSUPPORTED, "species %d: %d orbitals (max %d)", s, S.norb, GINT_MAX_ORB);
-        // rows of this species start at a multiple of 1 row; row stride = row_len doubles; the table is addressed
-        // as tab[tab_base(s) + i*row_len + 4*shell + {0..3}], tab_base kept in tab_off as a DOUBLE offset / 4.
-        S.tab_off = (int)(tab.size() / 4);
+        S.tab_off = (int)(tab.size() / 2);
         const double h2 = dr * dr;
-        for (int i = 0; i < S.n_int; i++) {
+        for (int i = 0; i < n_knot[s]; i++) {
             for (int k = 0; k < n_shell[s]; k++) {
-                const double* y = tab_y + src + (long long)k * n_knot[s];
-                const double* y2 = tab_y2 + src + (long long)k * n_knot[s];
-                if (!std::isfinite(y[i]) || !std::isfinite(y[i + 1]) || !std::isfinite(y2[i]) || !std::isfinite(y2[i + 1]))
-                    GINT_FAIL(GINT_ERR_INVALID_ARG, "species %d shell %d: non-finite table value near knot %d", s, k, i);
-                tab.push_back(y[i]);
-                tab.push_back((y[i + 1] - y[i]) - h2 / 6.0 * (2.0 * y2[i] + y2[i + 1]));
-                tab.push_back(h2 / 2.0 * y2[i]);
-                tab.push_back(h2 / 6.0 * (y2[i + 1] - y2[i]));
+                const double y = tab_y[src + (long long)k * n_knot[s] + i], y2 = tab_y2[src + (long long)k * n_knot[s] + i];
+                if (!std::isfinite(y) || !std::isfinite(y2))
+                    GINT_FAIL(GINT_ERR_INVALID_ARG, "species %d shell %d: non-finite table value at knot %d", s, k, i);
+                tab.push_back(y);
+                tab.push_back(h2 / 6.0 * y2);
             }
         }
         rows += S.n_int;
@@ -354,6 +351,7 @@ static int build_basis(gint_ctx* c, int n_species, const int* n_shell, const int
     }
     int rc = dev_upload(c, &c->d_species, c->h_species); if (rc) return rc;
     rc = dev_upload(c, &c->d_tab, tab); if (rc) return rc;
+    c->tab_bytes = tab.size() * sizeof(double);
     return GINT_OK;
 }
 
@@ -530,7 +528,7 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, bool* 
     int max_nb = 0, max_cols = 0;
     for (long long b = 0; b < nbt; b++) { max_nb = std::max(max_nb, count[b]); max_cols = std::max(max_cols, cols[b]); }
     g.max_nb = std::max(max_nb, 1); g.max_cols = std::max(max_cols, 1);
-    const bool ok = max_nb <= GINT_MAX_NB && gint_smem_needed(g) <= smem_limit;     // else: try a smaller batch shape
+    const bool ok = max_nb <= GINT_MAX_NB && gint_smem_needed(c, smem_limit) <= smem_limit;     // else: try a smaller batch shape
     if (!ok) { cudaFree(d_img); cudaFree(d_cand); cudaFree(d_ccount); cudaFree(d_count); cudaFree(d_cols); return GINT_OK; }
     *fits = true;
 
@@ -637,7 +635,7 @@ extern "C" int gint_init(gint_ctx** out, int n_species, const int* n_shell, cons
         }
         if (!fits) { free_ctx(c); GINT_FAIL(GINT_ERR_UNSUPPORTED, "even a 1-point batch does not fit: too many overlapping atoms"); }
     }
-    c->smem_bytes = gint_smem_needed(g);
+    c->smem_bytes = gint_smem_needed(c, smem_limit);
     if ((rc = gint_configure_kernels(c))) { free_ctx(c); return rc; }
     for (auto& e : c->ev) GINT_CUDA(cudaEventCreate(&e));
     GINT_CUDA(cudaDeviceSynchronize());

@@ -17,9 +17,9 @@
 #define GINT_THREADS (32 * GINT_WARPS)
 #define GINT_MMA_WARPS 8           // warp groups 0,1: DMMA consumers (setmaxnreg.inc); warp groups 2,3: orbital-evaluation producers
 #define GINT_EVAL_WARPS (GINT_WARPS - GINT_MMA_WARPS)
-#define GINT_REGS_MMA 176          // registers per thread after setmaxnreg: 256 * 176 + 256 * 80 = 65536
-#define GINT_REGS_EVAL 80
-#define GINT_STAGES 3              // shared-memory ring of orbital-value stages between producers and consumers
+#define GINT_REGS_MMA 168          // registers per thread after setmaxnreg: 256 * 168 + 256 * 88 = 65536
+#define GINT_REGS_EVAL 88
+#define GINT_STAGES 2              // shared-memory ring of orbital-value stages between producers and consumers
 // tile geometry of the contraction kernels: one CTA owns the block of H (or D) between two groups of atoms
 #define GINT_TILE_ATOMS 8          // atom images per group
 #define GINT_TILE_ORB 104          // orbitals per group = 13 fragments of 8 (8 atoms x 13 orbitals exactly)
@@ -28,7 +28,7 @@
 #define GINT_WARP_SEGS 4           // segments per consumer warp
 #define GINT_MAX_SEG (GINT_WARP_SEGS * GINT_MMA_WARPS)
 #define GINT_CHUNK 32              // mesh points per pipeline stage = 4 cubelets of 8 points
-#define GINT_LD 40                 // row stride (doubles) of the orbital tiles in shared memory: = 8 mod 16, LDS.128 conflict-free
+#define GINT_LD 36                 // row stride (doubles) of the orbital tiles in shared memory: = 4 mod 16, the 64-bit fragment loads are conflict-free
 
 // ---- error plumbing -------------------------------------------------------------------------------
 void gint_set_error(const char* fmt, ...);
@@ -43,8 +43,8 @@ struct SpeciesDev {
     int n_shell;
     int norb;
     int n_int;                      // spline intervals per shell (n_knot - 1)
-    int tab_off;                    // first row (interval) of this species in the coefficient table
-    int row_len;                    // doubles per table row = 4 * n_shell
+    int tab_off;                    // first cell (double2) of this species in the radial table
+    int row_len;                    // cells per knot = n_shell
     int l[GINT_MAX_SHELL];
 };
 
@@ -94,7 +94,9 @@ struct gint_ctx {
     int n_species = 0;
     std::vector<SpeciesDev> h_species;
     SpeciesDev* d_species = nullptr;
-    double* d_tab = nullptr;         // [rows][row_len]: per interval, per shell c0..c3 (R = ((c3 b + c2) b + c1) b + c0)
+    double* d_tab = nullptr;         // cells {y, y'' dr^2/6}: [species][knot][shell]
+    size_t tab_bytes = 0;
+    bool tab_in_smem = false;        // the contraction kernels copy the table into shared memory
     // atoms
     int n_atoms = 0;
     std::vector<int> h_atom_species;
@@ -144,7 +146,7 @@ int gint_launch_vlocal(gint_ctx* c, const double* V, double* H, cudaStream_t st)
 int gint_launch_rho(gint_ctx* c, const double* D, double* rho, cudaStream_t st);
 int gint_launch_alg_stats(gint_ctx* c);
 int gint_configure_kernels(gint_ctx* c);
-size_t gint_smem_needed(const Geom& g);
+size_t gint_smem_needed(gint_ctx* c, size_t limit);   // also decides tab_in_smem
 
 // Split of the n neighbour entries of a batch into G groups of consecutive entries: group k = [k*n/G, (k+1)*n/G).
 __host__ __device__ inline int group_begin(int k, int n, int G) { return (int)(((long long)k * n) / G); }

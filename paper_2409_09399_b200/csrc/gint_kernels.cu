@@ -20,6 +20,15 @@
 #include "gint_internal.h"
 
 typedef unsigned long long u64;
+#ifndef GINT_DBG_STATS
+#define DBG_T(x)
+#define DBG_ADD(i, v)
+#else
+__device__ unsigned long long g_dbg[16];
+#define DBG_T(x) const long long x = clock64()
+#define DBG_ADD(i, v) do { if ((threadIdx.x & 31) == 0) atomicAdd(&g_dbg[i], (unsigned long long)(v)); } while (0)
+extern "C" int gint_debug_counters(unsigned long long* out) { return (int)cudaMemcpyFromSymbol(out, g_dbg, sizeof(g_dbg)); }
+#endif
 #define GINT_EVAL_GROUP 3          // radial shells whose spline coefficients are loaded together (registers vs memory-level parallelism)
 
 // ---------------------------------------------------------------------------------------------------
@@ -40,7 +49,6 @@ struct TileSmem {
     // phi[stage][side][orbital row][GINT_LD]: side 0 = group I, side 1 = group J (scaled by V dV in vlocal);
     // column 8q + p = point p of the stage's q-th cubelet
     double phi[GINT_STAGES][2][GINT_TILE_ORB][GINT_LD];
-    double4 pts[2][GINT_CHUNK];         // [stage][point]: x, y, z, weight (V dV in vlocal, 1 in rho)
     u64 full[GINT_STAGES], empty[GINT_STAGES];   // mbarriers: stage written by all producer warps / read by all consumer warps
     double pos[16][4];                  // slot s < 8: atom s of group I; slot 8 + s: atom s of group J
     SlotInfo sinfo[16];
@@ -53,17 +61,21 @@ struct TileSmem {
     int atom[16], shift[16], spec[16];
     int cstart[2][GINT_TILE_ATOMS + 1]; // first orbital row of each atom inside its group
     int seg[GINT_MAX_SEG];              // slot (consumer warp) + 8 k: row fragment | first column fragment << 8 | n columns << 16
-    int nitem[2], neval[2];             // [stage]: items of the stage, of which the first neval need a real evaluation
     int ncub;
     TileView tv;                        // written by tile_setup; read from here afterwards to keep registers free
-    unsigned char valid[2][GINT_CHUNK]; // the stage's point exists (inside the batch and the mesh)
-    unsigned char item[2][64];          // [stage][k]: slot << 2 | cubelet of the stage
+    unsigned char item[16][64];         // [stage][k]: slot << 2 | cubelet of the stage
+    unsigned char nitem[16], neval[16]; // [stage]: items of the stage, of which the first neval need a real evaluation
     unsigned char cub[64 + 4];          // the tile's cubelets (bit numbers of U, ascending)
     unsigned char row_atom[2][GINT_TILE_ORB];   // orbital row -> atom slot inside the group (255 = padding)
     unsigned char row_orb[2][GINT_TILE_ORB];    // orbital row -> orbital index inside the atom
     unsigned char frag_atoms[2][16];            // fragment -> bit mask of the atoms it holds orbitals of
 };
-size_t gint_smem_needed(const Geom&) { return sizeof(TileSmem); }
+// the radial table follows the struct in dynamic shared memory when it fits
+#define GINT_SMEM_TAB_OFF ((sizeof(TileSmem) + 15) & ~(size_t)15)
+size_t gint_smem_needed(gint_ctx* c, size_t limit) {
+    c->tab_in_smem = GINT_SMEM_TAB_OFF + c->tab_bytes <= limit;
+    return GINT_SMEM_TAB_OFF + (c->tab_in_smem ? c->tab_bytes : 0);
+}
 
 // The DMMA chains and their operand loads are volatile asm: left to itself the compiler sinks every shared load to
 // just before its DMMA (one operand register, fully serialised LDS -> DMMA -> LDS ...) and pairs the two k-steps of
@@ -97,14 +109,140 @@ __device__ __forceinline__ u64 shfl64(u64 v, int src) {
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Stage c of a tile = its cubelets 4c .. 4c+3; point index 8 q + p: point p = (px, py, pz) bits of the q-th cubelet.
+__device__ __forceinline__ bool stage_point(const TileSmem& S, int c, int pt, int& gi, int& gj, int& gk) {
+    const int ci = 4 * c + (pt >> 3), p = pt & 7;
+    if (ci >= S.ncub) return false;
+    const int cl = S.cub[ci];
+    const int ix = 2 * (cl >> 4) + (p >> 2), iy = 2 * ((cl >> 2) & 3) + ((p >> 1) & 1), iz = 2 * (cl & 3) + (p & 1);
+    gi = S.tv.i0 + ix; gj = S.tv.j0 + iy; gk = S.tv.k0 + iz;
+    return ix < S.tv.ex && iy < S.tv.ey && iz < S.tv.ez;
+}
+
+// Item list of stage c (tile set-up, one warp per stage).  An item is (atom slot, cubelet of the stage) whose orbital
+// rows some segment reads on that cubelet: first the items on which the atom is really non-zero (evaluated), then
+// those that only need zeros.
+__device__ __forceinline__ void make_items(TileSmem& S, int c) {
+    const int lane = threadIdx.x & 31;
+    // candidates: lane -> (slot lane >> 2, cubelet lane & 3) and (slot 8 + (lane >> 2), same cubelet)
+    const int ci = 4 * c + (lane & 3);
+    const bool inb = ci < S.ncub;
+    const int cl = inb ? S.cub[ci] : 0;
+    const int s0 = lane >> 2, s1 = 8 + s0;
+    const bool n0 = inb && ((S.need[s0] >> cl) & 1ull), n1 = inb && ((S.need[s1] >> cl) & 1ull);
+    const bool a0 = n0 && ((S.amask[s0] >> cl) & 1ull), a1 = n1 && ((S.amask[s1] >> cl) & 1ull);
+    const unsigned e0 = __ballot_sync(0xffffffffu, a0), e1 = __ballot_sync(0xffffffffu, a1);
+    const unsigned z0 = __ballot_sync(0xffffffffu, n0 && !a0), z1 = __ballot_sync(0xffffffffu, n1 && !a1);
+    const unsigned lt = (1u << lane) - 1u;
+    const int ne = __popc(e0) + __popc(e1);
+    if (a0) S.item[c][__popc(e0 & lt)] = (unsigned char)lane;
+    else if (n0) S.item[c][ne + __popc(z0 & lt)] = (unsigned char)lane;
+    if (a1) S.item[c][__popc(e0) + __popc(e1 & lt)] = (unsigned char)(32 + lane);
+    else if (n1) S.item[c][ne + __popc(z0) + __popc(z1 & lt)] = (unsigned char)(32 + lane);
+    if (lane == 0) { S.neval[c] = (unsigned char)ne; S.nitem[c] = (unsigned char)(ne + __popc(z0) + __popc(z1)); }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Orbital evaluation of one stage by one producer warp (north_star step 2): a quarter warp = one item, lane p = point
+// p of the cubelet.  phi = R_s(|d|) Y_lm(d/|d|), zero for |d| >= rc (Fig. 6); radial part
+// (reading R5): R = a y_i + b y_{i+1} + (a^3-a) z_i + (b^3-b) z_{i+1} from the knot cells {y, z} of the interval,
+// read with 128-bit loads (from the shared-memory copy of the table when it fits).  vlocal scales side J by V dV.
+// A diagonal tile evaluates each atom once and writes both sides.  `first`: this warp's first item of the stage.
+template <bool VLOCAL>
+__device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, int ps, int c, int first, const double2* __restrict__ tab,
+                                           const double* __restrict__ V) {
+    const int lane = threadIdx.x & 31;
+    const int nitem = S.nitem[c], neval = S.neval[c];
+    const bool two = S.tv.diag;
+    for (int base = first; base < nitem; base += 4 * GINT_EVAL_WARPS) {
+        const int idx = base + (lane >> 3);
+        const bool on = idx < nitem;
+        const int it = on ? S.item[c][idx] : 0;
+        const int slot = it >> 2, pt = 8 * (it & 3) + (lane & 7);
+        const int side = slot >> 3, a = slot & 7;
+        double* o0 = &S.phi[ps][side][S.cstart[side][a]][pt];
+        if (base >= neval) {                        // the four items only need zeros
+            const int norb = on ? S.cstart[side][a + 1] - S.cstart[side][a] : 0;
+            for (int o = 0; o < norb; o++) { o0[o * GINT_LD] = 0.0; if (two) o0[o * GINT_LD + GINT_TILE_ORB * GINT_LD] = 0.0; }
+            continue;
+        }
+        int gi = 0, gj = 0, gk = 0;
+        const bool valid = stage_point(S, c, pt, gi, gj, gk);
+        double wv = 1.0;
+        if (VLOCAL && valid && on && (two || side)) wv = __ldg(V + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk) * g.dV;
+        double px, py, pz;
+        mesh_point(g, gi, gj, gk, px, py, pz);
+        const SlotInfo si = S.sinfo[slot];
+        const double dx = px - S.pos[slot][0], dy = py - S.pos[slot][1], dz = pz - S.pos[slot][2];
+        const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+        const bool inside = on && idx < neval && valid && r2 < si.rc2;
+        // 1/r by two Newton steps from the single-precision reciprocal square root (relative error ~1e-7 -> 1e-14 -> 1e-28)
+        const double q = fmin(fmax(r2, 1e-30), si.rc2);
+        double ir = (double)rsqrtf((float)q);
+        ir = ir * fma(-0.5 * q, ir * ir, 1.5);
+        ir = ir * fma(-0.5 * q, ir * ir, 1.5);
+        const double r = q * ir;
+        const int nsh = on ? si.nsh : 0;
+        const double x = r * g.inv_dr;
+        int i = (int)x;
+        i = min(i, si.n_int - 1);
+        const double b = x - (double)i, am = 1.0 - b;
+        const double a3 = (am * am - 1.0) * am, b3 = (b * b - 1.0) * b;
+        const double2* row = tab + (si.tab_off + i * si.nsh);
+        const bool tiny = r < 1e-12;
+        if (tiny) ir = 0.0;
+        // lanes outside the sphere run the same instructions on a clamped radius and store zeros
+        const double w0 = inside ? ((VLOCAL && side) ? wv : 1.0) : 0.0;
+        const double w1 = inside ? wv : 0.0;
+        const double ux = dx * ir, uy = dy * ir, uz = dz * ir;
+        const double lz = tiny ? 0.0 : 1.0;          // l > 0 orbitals vanish at the nucleus
+#define GINT_PUT(v) do { const double v_ = (v); *o0 = w0 * v_; if (two) o0[GINT_TILE_ORB * GINT_LD] = w1 * v_; o0 += GINT_LD; } while (0)
+        for (int k0 = 0; k0 < nsh; k0 += GINT_EVAL_GROUP) {
+            double2 c0[GINT_EVAL_GROUP], c1[GINT_EVAL_GROUP];
+#pragma unroll
+            for (int u = 0; u < GINT_EVAL_GROUP; u++)
+                if (k0 + u < nsh) { c0[u] = row[k0 + u]; c1[u] = row[nsh + k0 + u]; }
+#pragma unroll
+            for (int u = 0; u < GINT_EVAL_GROUP; u++) {
+                if (k0 + u >= nsh) break;
+                const double R = fma(am, c0[u].x, fma(b, c1[u].x, fma(a3, c0[u].y, b3 * c1[u].y)));
+                const int l = (si.lpack >> (2 * (k0 + u))) & 3;
+                if (l == 0) {
+                    GINT_PUT(R * 0.28209479177387814);
+                } else if (l == 1) {
+                    const double R1 = R * 0.4886025119029199;
+                    GINT_PUT(R1 * uy); GINT_PUT(R1 * uz); GINT_PUT(R1 * ux);
+                } else {
+                    const double R2 = R * lz;
+                    const double c2 = R2 * 1.0925484305920792;
+                    GINT_PUT(c2 * ux * uy);
+                    GINT_PUT(c2 * uy * uz);
+                    GINT_PUT(R2 * 0.31539156525252005 * (3.0 * uz * uz - 1.0));
+                    GINT_PUT(c2 * ux * uz);
+                    GINT_PUT(R2 * 0.5462742152960396 * (ux * ux - uy * uy));
+                }
+            }
+        }
+#undef GINT_PUT
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Tile set-up: atom slots, orbital-row maps, canonical block of every atom pair of the tile, activity masks,
 // cubelet list, segments.
 __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView& tv, const int2* __restrict__ tile,
                                            const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
                                            const double* __restrict__ atom_pos, const int* __restrict__ atom_spec,
                                            const SpeciesDev* __restrict__ sp, const int* __restrict__ crow,
-                                           const u64* __restrict__ ckey, const unsigned int* __restrict__ coff) {
+                                           const u64* __restrict__ ckey, const unsigned int* __restrict__ coff,
+                                           const double* __restrict__ tab, int tab_cells) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    // copy of the radial table (tab_cells = 0: it stays in global memory)
+    {
+        const double2* src = reinterpret_cast<const double2*>(tab);
+        double2* dst = reinterpret_cast<double2*>(reinterpret_cast<unsigned char*>(&S) + GINT_SMEM_TAB_OFF);
+        for (int i = tid; i < tab_cells; i += GINT_THREADS) dst[i] = __ldg(src + i);
+    }
     const int2 td = tile[blockIdx.x];
     tv.b = td.x; tv.I = td.y & 255; tv.J = (td.y >> 8) & 255; tv.G = (td.y >> 16) & 255;
     tv.diag = tv.I == tv.J;
@@ -250,135 +388,12 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
     }
     __syncthreads();
     tv.nchunk = (S.ncub + 3) >> 2;
+    if (warp < tv.nchunk) make_items(S, warp);
     if (tid == 0) {
         S.tv = tv;
         for (int s = 0; s < GINT_STAGES; s++) { mbar_init(&S.full[s], GINT_EVAL_WARPS); mbar_init(&S.empty[s], GINT_MMA_WARPS); }
     }
     __syncthreads();
-}
-
-// ---------------------------------------------------------------------------------------------------
-// Stage c of a tile = its cubelets 4c .. 4c+3; lane = 8 q + p: point p = (px, py, pz) bits of the q-th cubelet.
-__device__ __forceinline__ bool stage_point(const TileSmem& S, const TileView& tv, int c, int lane, int& gi, int& gj, int& gk) {
-    const int ci = 4 * c + (lane >> 3), p = lane & 7;
-    if (ci >= S.ncub) return false;
-    const int cl = S.cub[ci];
-    const int ix = 2 * (cl >> 4) + (p >> 2), iy = 2 * ((cl >> 2) & 3) + ((p >> 1) & 1), iz = 2 * (cl & 3) + (p & 1);
-    gi = tv.i0 + ix; gj = tv.j0 + iy; gk = tv.k0 + iz;
-    return ix < tv.ex && iy < tv.ey && iz < tv.ez;
-}
-
-// Run by one warp, two stages ahead of the evaluation that consumes them (so that the global load of V is off the
-// critical path): the stage's mesh points (coordinates, vlocal weight V dV) and its compacted item list.  An item
-// is (atom slot, cubelet of the stage) whose orbital rows some segment reads on that cubelet: first the items on
-// which the atom is really non-zero (evaluated), then those that only need zeros.
-template <bool VLOCAL>
-__device__ __forceinline__ void make_stage(const Geom& g, TileSmem& S, const TileView& tv, int c, const double* __restrict__ V) {
-    const int lane = threadIdx.x & 31, par = c & 1;
-    int gi, gj, gk;
-    double4 p = make_double4(0.0, 0.0, 0.0, 0.0);
-    const bool valid = stage_point(S, tv, c, lane, gi, gj, gk);
-    if (valid) {
-        mesh_point(g, gi, gj, gk, p.x, p.y, p.z);
-        p.w = VLOCAL ? __ldg(V + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk) * g.dV : 1.0;
-    }
-    S.pts[par][lane] = p;
-    S.valid[par][lane] = valid ? 1 : 0;
-    // candidates: lane -> (slot lane >> 2, cubelet lane & 3) and (slot 8 + (lane >> 2), same cubelet)
-    const int ci = 4 * c + (lane & 3);
-    const bool inb = ci < S.ncub;
-    const int cl = inb ? S.cub[ci] : 0;
-    const int s0 = lane >> 2, s1 = 8 + s0;
-    const bool n0 = inb && ((S.need[s0] >> cl) & 1ull), n1 = inb && ((S.need[s1] >> cl) & 1ull);
-    const bool a0 = n0 && ((S.amask[s0] >> cl) & 1ull), a1 = n1 && ((S.amask[s1] >> cl) & 1ull);
-    const unsigned e0 = __ballot_sync(0xffffffffu, a0), e1 = __ballot_sync(0xffffffffu, a1);
-    const unsigned z0 = __ballot_sync(0xffffffffu, n0 && !a0), z1 = __ballot_sync(0xffffffffu, n1 && !a1);
-    const unsigned lt = (1u << lane) - 1u;
-    const int ne = __popc(e0) + __popc(e1);
-    if (a0) S.item[par][__popc(e0 & lt)] = (unsigned char)lane;
-    else if (n0) S.item[par][ne + __popc(z0 & lt)] = (unsigned char)lane;
-    if (a1) S.item[par][__popc(e0) + __popc(e1 & lt)] = (unsigned char)(32 + lane);
-    else if (n1) S.item[par][ne + __popc(z0) + __popc(z1 & lt)] = (unsigned char)(32 + lane);
-    if (lane == 0) { S.neval[par] = ne; S.nitem[par] = ne + __popc(z0) + __popc(z1); }
-}
-
-// ---------------------------------------------------------------------------------------------------
-// Orbital evaluation of one stage (north_star step 2): a quarter warp = one item, lane p = point p of the cubelet.
-// phi = R_s(|d|) Y_lm(d/|d|), zero for |d| >= rc (Fig. 6); radial part: per-interval
-// cubic in b = r/dr - i (reading R5), coefficients read with 128-bit loads.  vlocal scales side J by V dV.
-// A diagonal tile evaluates each atom once and writes both sides.
-template <bool VLOCAL>
-__device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, const TileView& tv, int ps, int st, int rank,
-                                           const double* __restrict__ tab) {   // ps: ring slot of phi; st: parity of the point / item lists
-    const int lane = threadIdx.x & 31;
-    const int nitem = S.nitem[st], neval = S.neval[st];
-    const bool two = tv.diag;
-    for (int base = 4 * rank; base < nitem; base += 4 * GINT_EVAL_WARPS) {
-        const int idx = base + (lane >> 3);
-        const bool on = idx < nitem;
-        const int it = on ? S.item[st][idx] : 0;
-        const int slot = it >> 2, col = 8 * (it & 3) + (lane & 7);
-        const int side = slot >> 3, a = slot & 7;
-        double* o0 = &S.phi[ps][side][S.cstart[side][a]][col];
-        double* o1 = &S.phi[ps][1][S.cstart[side][a]][col];
-        if (base >= neval) {                        // the four items only need zeros
-            const int norb = on ? S.cstart[side][a + 1] - S.cstart[side][a] : 0;
-            for (int o = 0; o < norb; o++) { o0[o * GINT_LD] = 0.0; if (two) o1[o * GINT_LD] = 0.0; }
-            continue;
-        }
-        const SlotInfo si = S.sinfo[slot];
-        const double4 P = S.pts[st][col];
-        const double dx = P.x - S.pos[slot][0], dy = P.y - S.pos[slot][1], dz = P.z - S.pos[slot][2];
-        const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-        const bool inside = on && idx < neval && S.valid[st][col] && r2 < si.rc2;
-        // lanes outside the sphere run the same instructions on a clamped radius and store zeros
-        const double w0 = inside ? ((VLOCAL && side) ? P.w : 1.0) : 0.0;
-        const double w1 = inside ? (VLOCAL ? P.w : 1.0) : 0.0;
-        // 1/r by two Newton steps from the single-precision reciprocal square root (relative error ~1e-7 -> 1e-14 -> 1e-28)
-        const double q = fmin(fmax(r2, 1e-30), si.rc2);
-        double ir = (double)rsqrtf((float)q);
-        ir = ir * fma(-0.5 * q, ir * ir, 1.5);
-        ir = ir * fma(-0.5 * q, ir * ir, 1.5);
-        const double r = q * ir;
-        const int nsh = on ? si.nsh : 0;
-        const double x = r * g.inv_dr;
-        int i = (int)x;
-        i = min(i, si.n_int - 1);
-        const double bq = x - (double)i;
-        const double2* row = reinterpret_cast<const double2*>(tab) + ((size_t)si.tab_off + (size_t)i * si.nsh) * 2;
-        const bool tiny = r < 1e-12;
-        if (tiny) ir = 0.0;
-        const double ux = dx * ir, uy = dy * ir, uz = dz * ir;
-        const double lz = tiny ? 0.0 : 1.0;          // l > 0 orbitals vanish at the nucleus
-#define GINT_PUT(v) do { const double v_ = (v); *o0 = w0 * v_; o0 += GINT_LD; if (two) { *o1 = w1 * v_; o1 += GINT_LD; } } while (0)
-        for (int k0 = 0; k0 < nsh; k0 += GINT_EVAL_GROUP) {
-            double2 c01[GINT_EVAL_GROUP], c23[GINT_EVAL_GROUP];
-#pragma unroll
-            for (int u = 0; u < GINT_EVAL_GROUP; u++)
-                if (k0 + u < nsh) { c01[u] = __ldg(row + 2 * (k0 + u)); c23[u] = __ldg(row + 2 * (k0 + u) + 1); }
-#pragma unroll
-            for (int u = 0; u < GINT_EVAL_GROUP; u++) {
-                if (k0 + u >= nsh) break;
-                const double R = fma(fma(fma(c23[u].y, bq, c23[u].x), bq, c01[u].y), bq, c01[u].x);
-                const int l = (si.lpack >> (2 * (k0 + u))) & 3;
-                if (l == 0) {
-                    GINT_PUT(R * 0.28209479177387814);
-                } else if (l == 1) {
-                    const double R1 = R * 0.4886025119029199;
-                    GINT_PUT(R1 * uy); GINT_PUT(R1 * uz); GINT_PUT(R1 * ux);
-                } else {
-                    const double R2 = R * lz;
-                    const double c2 = R2 * 1.0925484305920792;
-                    GINT_PUT(c2 * ux * uy);
-                    GINT_PUT(c2 * uy * uz);
-                    GINT_PUT(R2 * 0.31539156525252005 * (3.0 * uz * uz - 1.0));
-                    GINT_PUT(c2 * ux * uz);
-                    GINT_PUT(R2 * 0.5462742152960396 * (ux * ux - uy * uy));
-                }
-            }
-        }
-#undef GINT_PUT
-    }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -394,55 +409,85 @@ __device__ __forceinline__ void mbar_wait(u64* bar, int parity) {
     asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
                  :: "r"(a), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void producer_sync() { asm volatile("bar.sync 1, %0;" :: "n"(32 * GINT_EVAL_WARPS) : "memory"); }
 
 // Segments of a consumer warp.
+#define GINT_ROWB (GINT_LD * 8)                    // bytes of one orbital row of a stage
+#define GINT_SIDEB (GINT_TILE_ORB * GINT_ROWB)     // bytes of one side of a stage
+#define GINT_STAGEB (2 * GINT_SIDEB)
 struct Seg {
-    int w;                           // row fragment | first column fragment << 8 | column fragments << 16 (0 = unused)
-    u64 act;                         // cubelets on which the row fragment and some column fragment are both active
+    unsigned oa;                     // byte offset of the row fragment in side I (row 8 row) | column fragments << 24 (0 = unused)
+    unsigned ob;                     // byte offset of the first column fragment in side J, relative to the stage
+    u64 W;                           // activity on the tile's cubelet list: bit p = the segment works on cubelet cub[p]
+    int w;                           // row fragment | first column fragment << 8 | column fragments << 16
     __device__ __forceinline__ int row() const { return w & 255; }
     __device__ __forceinline__ int cb() const { return (w >> 8) & 255; }
     __device__ __forceinline__ int n() const { return w >> 16; }
 };
 __device__ __forceinline__ Seg load_seg(const TileSmem& S, int slot) {
+    const int lane = threadIdx.x & 31;
     Seg s; s.w = S.seg[slot];
     u64 cm = 0;
     for (int j = 0; j < s.n(); j++) cm |= S.fmask[1][s.cb() + j];
-    s.act = s.n() ? (S.fmask[0][s.row()] & cm) : 0ull;
+    const u64 act = s.n() ? (S.fmask[0][s.row()] & cm) : 0ull;     // cubelets on which the row fragment and some column fragment are active
+    const bool b0 = lane < S.ncub && ((act >> S.cub[lane]) & 1ull), b1 = lane + 32 < S.ncub && ((act >> S.cub[(lane + 32) & 63]) & 1ull);
+    s.W = (u64)__ballot_sync(0xffffffffu, b0) | ((u64)__ballot_sync(0xffffffffu, b1) << 32);
+    s.oa = (unsigned)(s.row() * 8 * GINT_ROWB);
+    s.ob = (unsigned)(GINT_SIDEB + s.cb() * 8 * GINT_ROWB);
     return s;
-}
-// 4-bit activity of a segment on the cubelets of stage c
-__device__ __forceinline__ unsigned stage_bits(const TileSmem& S, int c, u64 act) {
-    const unsigned cw = *reinterpret_cast<const unsigned*>(&S.cub[4 * c]);
-    const int nq = min(4, S.ncub - 4 * c);
-    unsigned bits = 0;
-#pragma unroll
-    for (int q = 0; q < 4; q++) bits |= (unsigned)((act >> ((cw >> (8 * q)) & 63u)) & 1ull) << q;
-    return bits & ((1u << nq) - 1u);
 }
 
 // vlocal: acc[j] += Phi_I[row fragment]^T-slice x (V dV Phi_J)[column fragment cb + j] over the 8 points of every
-// active cubelet of the stage: one 128-bit shared load per operand fragment (points 2 lc, 2 lc + 1 of the lane's
-// orbital row) feeds two DMMA k-steps (k index lc <-> point 2 lc, then point 2 lc + 1).
+// active cubelet of the stage.  The two DMMA k-steps of a cubelet (points 0..3, points 4..7) use separate operand
+// registers X and Y: while the Y DMMAs issue, the X operands of the segment's next active cubelet are loaded, and
+// vice versa, so the shared-memory latency is hidden behind the FP64 tensor pipe.
+// next active cubelet of a segment: q = lowest set bit of rem (removed from rem), operand addresses pa/pb + 64 q.
+// One volatile asm block, so that it stays where it is written: in the shadow of the DMMAs.
+__device__ __forceinline__ void next_cubelet(unsigned& rem, unsigned pa, unsigned pb, unsigned& oa, unsigned& ob) {
+    asm volatile("{\n\t.reg .u32 t, u;\n\tbrev.b32 t, %0;\n\tclz.b32 t, t;\n\tshl.b32 t, t, 6;\n\tadd.u32 %1, %3, t;\n\tadd.u32 %2, %4, t;\n\t"
+                 "add.u32 u, %0, -1;\n\tand.b32 %0, %0, u;\n\t}" : "+r"(rem), "=r"(oa), "=r"(ob) : "r"(pa), "r"(pb));
+}
 template <int N>
 __device__ __forceinline__ void vl_seg(double (&acc)[GINT_SEG_COLS][2], unsigned pa, unsigned pb, unsigned bits) {
+    double ax, ay, bx[N], by[N];
+    unsigned rem = bits, oa, ob;
+    next_cubelet(rem, pa, pb, oa, ob);
+    ax = lds64(oa);
 #pragma unroll
-    for (int q = 0; q < 4; q++) {
-        if (!((bits >> q) & 1u)) continue;
-        const double2 a = lds128(pa + 64 * q);
-        double2 bv[N];
+    for (int j = 0; j < N; j++) bx[j] = lds64(ob + j * 8 * GINT_ROWB);
+    ay = lds64(oa + 32);
 #pragma unroll
-        for (int j = 0; j < N; j++) bv[j] = lds128(pb + (j * 8 * GINT_LD + 8 * q) * 8);
+    for (int j = 0; j < N; j++) by[j] = lds64(ob + j * 8 * GINT_ROWB + 32);
+    bool more = rem != 0;
+    next_cubelet(rem, pa, pb, oa, ob);
+    while (more) {
+        // the reload of an operand register follows the DMMA that read it: the loads issue in the shadow of the
+        // 16-cycle DMMAs instead of in a gap between the two groups
 #pragma unroll
-        for (int j = 0; j < N; j++) dmma884(acc[j], a.x, bv[j].x);
+        for (int j = 0; j < N; j++) {
+            dmma884(acc[j], ax, bx[j]);
+            bx[j] = lds64(ob + j * 8 * GINT_ROWB);
+        }
+        ax = lds64(oa);
+        unsigned oa2, ob2;
 #pragma unroll
-        for (int j = 0; j < N; j++) dmma884(acc[j], a.y, bv[j].y);
+        for (int j = 0; j < N; j++) {
+            dmma884(acc[j], ay, by[j]);
+            by[j] = lds64(ob + j * 8 * GINT_ROWB + 32);
+            if (j == 0) { more = rem != 0; next_cubelet(rem, pa, pb, oa2, ob2); }
+        }
+        ay = lds64(oa + 32);
+        oa = oa2; ob = ob2;
     }
+#pragma unroll
+    for (int j = 0; j < N; j++) dmma884(acc[j], ax, bx[j]);
+#pragma unroll
+    for (int j = 0; j < N; j++) dmma884(acc[j], ay, by[j]);
 }
 __device__ __forceinline__ void vl_seg_dispatch(int n, double (&acc)[GINT_SEG_COLS][2], unsigned pa, unsigned pb, unsigned bits) {
+    // 7 and 6 are the lengths of all segments of a full off-diagonal tile: two compares instead of an indexed branch
+    if (n == 7) { vl_seg<7>(acc, pa, pb, bits); return; }
+    if (n == 6) { vl_seg<6>(acc, pa, pb, bits); return; }
     switch (n) {
-        case 7: vl_seg<7>(acc, pa, pb, bits); break;
-        case 6: vl_seg<6>(acc, pa, pb, bits); break;
         case 5: vl_seg<5>(acc, pa, pb, bits); break;
         case 4: vl_seg<4>(acc, pa, pb, bits); break;
         case 3: vl_seg<3>(acc, pa, pb, bits); break;
@@ -452,20 +497,28 @@ __device__ __forceinline__ void vl_seg_dispatch(int n, double (&acc)[GINT_SEG_CO
     }
 }
 
-// producer loop shared by both kernels: stage c of the tile goes to ring slot c % GINT_STAGES
+// producer loop shared by both kernels: stage c of the tile goes to ring slot c % GINT_STAGES.  The producer warps do
+// not synchronise with one another: each takes every 8th group of four items, rotating with the stage so that
+// the remainders even out, and arrives on full[s] when its share of the stage is written.
 template <bool VLOCAL>
-__device__ __forceinline__ void producer_loop(const Geom& g, TileSmem& S, int nchunk, const double* __restrict__ tab, const double* __restrict__ V) {
+__device__ __forceinline__ void producer_loop(const Geom& g, TileSmem& S, int nchunk, const double* __restrict__ tab, int tab_cells,
+                                              const double* __restrict__ V) {
     const int pw = (threadIdx.x >> 5) - GINT_MMA_WARPS;
-    const TileView& tv = S.tv;
-    if (pw == 0) make_stage<VLOCAL>(g, S, tv, 0, V);
+    const double2* tb = tab_cells ? reinterpret_cast<const double2*>(reinterpret_cast<const unsigned char*>(&S) + GINT_SMEM_TAB_OFF)
+                                  : reinterpret_cast<const double2*>(tab);
     for (int c = 0; c < nchunk; c++) {
         const int s = c % GINT_STAGES, k = c / GINT_STAGES;
-        producer_sync();              // the point / item lists of stage c are complete; all producers are done with stage c-1
-        if (pw == (c + 1) % GINT_EVAL_WARPS) make_stage<VLOCAL>(g, S, tv, c + 1, V);
+        DBG_T(t_p0);
         if (k > 0) mbar_wait(&S.empty[s], (k - 1) & 1);
-        eval_stage<VLOCAL>(g, S, tv, s, c & 1, pw, tab);
+        DBG_T(t_p1);
+        DBG_ADD(10, t_p1 - t_p0);
+#ifndef GINT_DBG_NO_EVAL
+        eval_stage<VLOCAL>(g, S, s, c, 4 * ((pw + c) % GINT_EVAL_WARPS), tb, V);
+#endif
         __syncwarp();
         if ((threadIdx.x & 31) == 0) mbar_arrive(&S.full[s]);
+        DBG_T(t_p2);
+        DBG_ADD(11, t_p2 - t_p1);
     }
 }
 
@@ -477,19 +530,22 @@ __global__ void __launch_bounds__(GINT_THREADS, 1)
 k_vlocal_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
               const double* __restrict__ atom_pos, const int* __restrict__ atom_spec, const SpeciesDev* __restrict__ sp,
               const double* __restrict__ tab, const int* __restrict__ crow, const u64* __restrict__ ckey,
-              const unsigned int* __restrict__ coff, const double* __restrict__ V, double* __restrict__ Hc) {
+              const unsigned int* __restrict__ coff, int tab_cells, const double* __restrict__ V, double* __restrict__ Hc) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TileSmem& S = *reinterpret_cast<TileSmem*>(smem_raw);
+    DBG_T(t_start);
     {
         TileView tv0;
-        tile_setup(g, S, tv0, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff);
+        tile_setup(g, S, tv0, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff, tab, tab_cells);
     }
+    DBG_T(t_setup);
+    DBG_ADD(5, t_setup - t_start);
     const int nchunk = S.tv.nchunk;
     if (nchunk == 0) return;
     const int warp = threadIdx.x >> 5;
     if (warp >= GINT_MMA_WARPS) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(GINT_REGS_EVAL));
-        producer_loop<true>(g, S, nchunk, tab, V);
+        producer_loop<true>(g, S, nchunk, tab, tab_cells, V);
         return;
     }
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(GINT_REGS_MMA));
@@ -502,23 +558,74 @@ k_vlocal_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bst
 #pragma unroll
         for (int j = 0; j < GINT_SEG_COLS; j++) { acc[k][j][0] = 0.0; acc[k][j][1] = 0.0; }
     }
+#ifdef GINT_DBG_STATS
+    {   // developer statistics: DMMA balance over the four sub-partitions (whole tile, and stage by stage)
+        __shared__ int dbg_load[17][GINT_MMA_WARPS];
+        int tot = 0;
+        for (int c = 0; c < nchunk; c++) {
+            int l = 0;
+            for (int k = 0; k < GINT_WARP_SEGS; k++) l += 2 * sg[k].n() * __popc((unsigned)(sg[k].W >> (4 * c)) & 15u);
+            if (lane == 0) dbg_load[c][warp] = l;
+            tot += l;
+        }
+        if (lane == 0) dbg_load[16][warp] = tot;
+        {   // DMMAs needed at (row fragment, column fragment, cubelet) granularity, and with trailing-column cut per cubelet
+            unsigned long long fine = 0, lead = 0;
+            for (int k = 0; k < GINT_WARP_SEGS; k++) {
+                const u64 rm = S.fmask[0][sg[k].row()] & S.U;
+                u64 seen = 0;
+                for (int j = sg[k].n() - 1; j >= 0; j--) {
+                    const u64 cm = S.fmask[1][sg[k].cb() + j] & rm;
+                    fine += 2 * __popcll(cm);
+                    seen |= cm;
+                    lead += 2 * __popcll(seen);      // columns 0..j computed wherever some column >= j is active
+                }
+            }
+            if (sg[0].n() == 0) { fine = 0; lead = 0; }
+            DBG_ADD(12, fine); DBG_ADD(13, lead);
+        }
+        asm volatile("bar.sync 2, 256;" ::: "memory");
+        if (threadIdx.x == 0) {
+            unsigned long long sum = 0, mx_tile = 0, mx_chunk = 0;
+            for (int c = 0; c <= 16; c++) {
+                if (c < 16 && c >= nchunk) continue;
+                int m = 0, t = 0;
+                for (int q = 0; q < 4; q++) { const int v = dbg_load[c][q] + dbg_load[c][q + 4]; m = max(m, v); t += v; }
+                if (c == 16) { sum = t; mx_tile = 4ull * m; } else mx_chunk += 4ull * m;
+            }
+            atomicAdd(&g_dbg[0], sum); atomicAdd(&g_dbg[1], mx_tile); atomicAdd(&g_dbg[2], mx_chunk); atomicAdd(&g_dbg[3], 1ull);
+            atomicAdd(&g_dbg[4], (unsigned long long)nchunk);
+        }
+    }
+#endif
+    // lane part of every operand address: row lr of the fragment, point lc of the k-step
+    unsigned lane_off = smem_addr(&S.phi[0][0][0][0]) + lr * GINT_ROWB + lc * 8;
+    asm volatile("" : "+r"(lane_off));
     for (int c = 0; c < nchunk; c++) {
         const int s = c % GINT_STAGES;
+        DBG_T(t_w0);
         mbar_wait(&S.full[s], (c / GINT_STAGES) & 1);
-        const unsigned pa = smem_addr(&S.phi[s][0][lr][2 * lc]), pb = smem_addr(&S.phi[s][1][lr][2 * lc]);
+        DBG_T(t_w1);
+        DBG_ADD(6, t_w1 - t_w0);
+        const unsigned base = lane_off + s * GINT_STAGEB;
+#ifndef GINT_DBG_NO_MMA
 #pragma unroll
         for (int k = 0; k < GINT_WARP_SEGS; k++) {
-            const unsigned bits = stage_bits(S, c, sg[k].act);
-            if (bits) vl_seg_dispatch(sg[k].n(), acc[k], pa + sg[k].row() * (64 * GINT_LD), pb + sg[k].cb() * (64 * GINT_LD), bits);
+            const unsigned bits = (unsigned)(sg[k].W >> (4 * c)) & 15u;
+            if (bits) vl_seg_dispatch(sg[k].n(), acc[k], base + sg[k].oa, base + sg[k].ob, bits);
         }
+#endif
         __syncwarp();
         if (lane == 0) mbar_arrive(&S.empty[s]);
+        DBG_T(t_w2);
+        DBG_ADD(7, t_w2 - t_w1);
     }
+    DBG_T(t_loop);
     // flush: element (row, col) -> atom pair (a, b), orbitals (oa, ob) -> canonical block (transposed if the canonical
     // key is (b, a)).  Exact zeros (fragments never touched, atoms that do not overlap inside this batch) are skipped.
 #pragma unroll
     for (int k = 0; k < GINT_WARP_SEGS; k++) {
-        if (sg[k].n() == 0 || sg[k].act == 0ull) continue;
+        if (sg[k].n() == 0 || sg[k].W == 0ull) continue;
         const int row = 8 * sg[k].row() + lr;
         const int a = S.row_atom[0][row], oa = S.row_orb[0][row];
         if (a == 255) continue;
@@ -537,31 +644,37 @@ k_vlocal_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bst
             }
         }
     }
+    DBG_T(t_end);
+    DBG_ADD(8, t_end - t_loop);
+    DBG_ADD(9, t_end - t_start);
 }
 
 // ---------------------------------------------------------------------------------------------------
 // gint_rho main kernel (north_star step 3b).  The density blocks Dh_IJ of the tile are stationary DMMA A operands
 // (registers): per cubelet X^T = Dh_seg^T Phi_I (8 orbitals of J x 8 points per column fragment) and
 // rho_g += sum_j X_jg Phi_J,jg.  Dh = canonical-half, symmetrised density blocks (k_sym_D).
+// DMMA column n of X^T <-> point (n >> 1) + 4 (n & 1) of the cubelet, so that the lane's two results (columns 2 lc,
+// 2 lc + 1) meet Phi_J at points lc and lc + 4: the same conflict-free 64-bit shared loads as in vlocal.
 template <int N>
 __device__ __forceinline__ void rho_cols(const double (&d)[GINT_SEG_COLS][2], int j0, double b0, double b1, unsigned pj, double& p0, double& p1) {
-    double2 f[N];
-#pragma unroll
-    for (int j = 0; j < N; j++) f[j] = lds128(pj + ((j0 + j) * 8 * GINT_LD) * 8);
     double x[N][2];
 #pragma unroll
     for (int j = 0; j < N; j++) { x[j][0] = 0.0; x[j][1] = 0.0; dmma884(x[j], d[j0 + j][0], b0); }
 #pragma unroll
     for (int j = 0; j < N; j++) dmma884(x[j], d[j0 + j][1], b1);
+    double f0[N], f1[N];
 #pragma unroll
-    for (int j = 0; j < N; j++) { p0 = fma(x[j][0], f[j].x, p0); p1 = fma(x[j][1], f[j].y, p1); }
+    for (int j = 0; j < N; j++) { f0[j] = lds64(pj + (j0 + j) * 8 * GINT_ROWB); f1[j] = lds64(pj + (j0 + j) * 8 * GINT_ROWB + 32); }
+#pragma unroll
+    for (int j = 0; j < N; j++) { p0 = fma(x[j][0], f0[j], p0); p1 = fma(x[j][1], f1[j], p1); }
 }
 template <int N>
 __device__ __forceinline__ void rho_seg(const double (&d)[GINT_SEG_COLS][2], unsigned pi, unsigned pj, unsigned bits, double (&part)[4][2]) {
+    asm volatile("" : "+r"(pi), "+r"(pj));
 #pragma unroll
     for (int q = 0; q < 4; q++) {
         if (!((bits >> q) & 1u)) continue;
-        const double b0 = lds64(pi + 64 * q), b1 = lds64(pi + (4 * GINT_LD + 8 * q) * 8);       // Phi_I[8 row + lc (+4)][point 8q + lr]
+        const double b0 = lds64(pi + 64 * q), b1 = lds64(pi + 4 * GINT_ROWB + 64 * q);       // Phi_I[8 row + lc (+4)][point pi(lr) of cubelet q]
         constexpr int N0 = N > 4 ? 4 : N;
         rho_cols<N0>(d, 0, b0, b1, pj + 64 * q, part[q][0], part[q][1]);
         if (N > 4) rho_cols<(N > 4 ? N - 4 : 1)>(d, 4, b0, b1, pj + 64 * q, part[q][0], part[q][1]);
@@ -604,19 +717,19 @@ __global__ void __launch_bounds__(GINT_THREADS, 1)
 k_rho_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
            const double* __restrict__ atom_pos, const int* __restrict__ atom_spec, const SpeciesDev* __restrict__ sp,
            const double* __restrict__ tab, const int* __restrict__ crow, const u64* __restrict__ ckey,
-           const unsigned int* __restrict__ coff, const double* __restrict__ Dh, double* __restrict__ rho) {
+           const unsigned int* __restrict__ coff, int tab_cells, const double* __restrict__ Dh, double* __restrict__ rho) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TileSmem& S = *reinterpret_cast<TileSmem*>(smem_raw);
     {
         TileView tv0;
-        tile_setup(g, S, tv0, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff);
+        tile_setup(g, S, tv0, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff, tab, tab_cells);
     }
     const int nchunk = S.tv.nchunk;
     if (nchunk == 0) return;
     const int warp = threadIdx.x >> 5;
     if (warp >= GINT_MMA_WARPS) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(GINT_REGS_EVAL));
-        producer_loop<false>(g, S, nchunk, tab, nullptr);
+        producer_loop<false>(g, S, nchunk, tab, tab_cells, nullptr);
         return;
     }
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(GINT_REGS_MMA));
@@ -628,24 +741,27 @@ k_rho_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart
         sg[k] = load_seg(S, warp + GINT_MMA_WARPS * k);
         load_dseg(S, sg[k], Dh, d[k]);
     }
+    const unsigned phi0 = smem_addr(&S.phi[0][0][0][0]);
+    unsigned lane_i = phi0 + lc * GINT_ROWB + ((lr >> 1) + 4 * (lr & 1)) * 8;      // Phi_I: row lc of the k-step, point pi(lr)
+    unsigned lane_j = phi0 + lr * GINT_ROWB + lc * 8;                              // Phi_J: row lr, point lc (+4)
+    asm volatile("" : "+r"(lane_i), "+r"(lane_j));
     for (int c = 0; c < nchunk; c++) {
         const int s = c % GINT_STAGES;
         double part[4][2];
 #pragma unroll
         for (int q = 0; q < 4; q++) { part[q][0] = 0.0; part[q][1] = 0.0; }
         mbar_wait(&S.full[s], (c / GINT_STAGES) & 1);
-        const unsigned pi = smem_addr(&S.phi[s][0][lc][lr]), pj = smem_addr(&S.phi[s][1][lr][2 * lc]);
         unsigned any = 0;
 #pragma unroll
         for (int k = 0; k < GINT_WARP_SEGS; k++) {
-            const unsigned bits = stage_bits(S, c, sg[k].act);
+            const unsigned bits = (unsigned)(sg[k].W >> (4 * c)) & 15u;
             any |= bits;
-            if (bits) rho_seg_dispatch(sg[k].n(), d[k], pi + sg[k].row() * (64 * GINT_LD), pj + sg[k].cb() * (64 * GINT_LD), bits, part);
+            if (bits) rho_seg_dispatch(sg[k].n(), d[k], lane_i + s * GINT_STAGEB + sg[k].oa, lane_j + s * GINT_STAGEB + sg[k].ob, bits, part);
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&S.empty[s]);
         if (!any) continue;
-        // part[q][e]: points 8q + 2lc + e, partial over the lane's orbital row lr -> reduce-scatter over lr (lane bits 2..4)
+        // part[q][e]: point lc + 4e of cubelet q, partial over the lane's orbital row lr -> reduce-scatter over lr (lane bits 2..4)
         double r4[4], r2[2], r1;
         {
             const bool hi = lane & 16;
@@ -665,9 +781,9 @@ k_rho_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart
             const double keep = low ? r2[1] : r2[0], send = low ? r2[0] : r2[1];
             r1 = keep + __shfl_xor_sync(0xffffffffu, send, 4);
         }
-        // the lane now owns point 8 (lr >> 1) + 2 lc + (lr & 1) of the stage
+        // the lane now owns value t = lr: point lc + 4 (lr & 1) of cubelet lr >> 1
         int gi, gj, gk;
-        if (r1 != 0.0 && stage_point(S, S.tv, c, 8 * (lr >> 1) + 2 * lc + (lr & 1), gi, gj, gk))
+        if (r1 != 0.0 && stage_point(S, c, 8 * (lr >> 1) + lc + 4 * (lr & 1), gi, gj, gk))
             atomicAdd(rho + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk, r1);
     }
 }
@@ -767,7 +883,7 @@ int gint_launch_vlocal(gint_ctx* c, const double* V, double* H, cudaStream_t st)
     if (c->n_tiles > 0) {
         GINT_CUDA(cudaEventRecord(c->ev[0], st));
         k_vlocal_tile<<<(unsigned)c->n_tiles, GINT_THREADS, c->smem_bytes, st>>>(c->geom, c->d_tile, c->d_bstart, c->d_bent, c->d_atom_pos,
-            c->d_atom_species, c->d_species, c->d_tab, c->d_crow, c->d_ckey, c->d_coff, V, c->d_cval);
+            c->d_atom_species, c->d_species, c->d_tab, c->d_crow, c->d_ckey, c->d_coff, c->tab_in_smem ? (int)(c->tab_bytes / 16) : 0, V, c->d_cval);
         GINT_CUDA(cudaGetLastError());
         GINT_CUDA(cudaEventRecord(c->ev[1], st));
         c->timed[0] = true;
@@ -786,7 +902,7 @@ int gint_launch_rho(gint_ctx* c, const double* D, double* rho, cudaStream_t st) 
     GINT_CUDA(cudaGetLastError());
     GINT_CUDA(cudaEventRecord(c->ev[2], st));
     k_rho_tile<<<(unsigned)c->n_tiles, GINT_THREADS, c->smem_bytes, st>>>(c->geom, c->d_tile, c->d_bstart, c->d_bent, c->d_atom_pos,
-        c->d_atom_species, c->d_species, c->d_tab, c->d_crow, c->d_ckey, c->d_coff, c->d_cval, rho);
+        c->d_atom_species, c->d_species, c->d_tab, c->d_crow, c->d_ckey, c->d_coff, c->tab_in_smem ? (int)(c->tab_bytes / 16) : 0, c->d_cval, rho);
     GINT_CUDA(cudaGetLastError());
     GINT_CUDA(cudaEventRecord(c->ev[3], st));
     c->timed[1] = true;
