@@ -29,7 +29,7 @@ __device__ unsigned long long g_dbg[16];
 #define DBG_ADD(i, v) do { if ((threadIdx.x & 31) == 0) atomicAdd(&g_dbg[i], (unsigned long long)(v)); } while (0)
 extern "C" int gint_debug_counters(unsigned long long* out) { return (int)cudaMemcpyFromSymbol(out, g_dbg, sizeof(g_dbg)); }
 #endif
-#define GINT_EVAL_GROUP 3          // radial shells whose spline coefficients are loaded together (registers vs memory-level parallelism)
+#define GINT_EVAL_GROUP 5          // radial shells whose spline coefficients are loaded together (registers vs memory-level parallelism)
 
 // ---------------------------------------------------------------------------------------------------
 // shared memory of the tile kernels
@@ -49,6 +49,8 @@ struct TileSmem {
     // phi[stage][side][orbital row][GINT_LD]: side 0 = group I, side 1 = group J (scaled by V dV in vlocal);
     // column 8q + p = point p of the stage's q-th cubelet
     double phi[GINT_STAGES][2][GINT_TILE_ORB][GINT_LD];
+    double4 pts[512];                   // [cubelet id * 8 + p]: x, y, z of the batch's mesh points, weight V dV (vlocal) or 1 (rho);
+                                        // points outside the mesh: far away, weight 0
     u64 full[GINT_STAGES], empty[GINT_STAGES];   // mbarriers: stage written by all producer warps / read by all consumer warps
     double pos[16][4];                  // slot s < 8: atom s of group I; slot 8 + s: atom s of group J
     SlotInfo sinfo[16];
@@ -166,16 +168,12 @@ __device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, int ps, i
             for (int o = 0; o < norb; o++) { o0[o * GINT_LD] = 0.0; if (two) o0[o * GINT_LD + GINT_TILE_ORB * GINT_LD] = 0.0; }
             continue;
         }
-        int gi = 0, gj = 0, gk = 0;
-        const bool valid = stage_point(S, c, pt, gi, gj, gk);
-        double wv = 1.0;
-        if (VLOCAL && valid && on && (two || side)) wv = __ldg(V + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk) * g.dV;
-        double px, py, pz;
-        mesh_point(g, gi, gj, gk, px, py, pz);
+        const double4 P = S.pts[8 * S.cub[min(4 * c + (it & 3), 63)] + (lane & 7)];
+        const double wv = P.w;
         const SlotInfo si = S.sinfo[slot];
-        const double dx = px - S.pos[slot][0], dy = py - S.pos[slot][1], dz = pz - S.pos[slot][2];
+        const double dx = P.x - S.pos[slot][0], dy = P.y - S.pos[slot][1], dz = P.z - S.pos[slot][2];
         const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-        const bool inside = on && idx < neval && valid && r2 < si.rc2;
+        const bool inside = on && idx < neval && r2 < si.rc2;
         // 1/r by one Newton step from the single-precision reciprocal square root: relative error 2.4e-7 -> 1.5 e^2 = 9e-14,
         // three orders below the 1e-10 parity bar (a second step would cost four more dependent FP64 operations)
         const double q = fmin(fmax(r2, 1e-30), si.rc2);
@@ -195,31 +193,41 @@ __device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, int ps, i
         const double w0 = inside ? ((VLOCAL && side) ? wv : 1.0) : 0.0;
         const double w1 = inside ? wv : 0.0;
         const double ux = dx * ir, uy = dy * ir, uz = dz * ir;
-        const double lz = tiny ? 0.0 : 1.0;          // l > 0 orbitals vanish at the nucleus
-#define GINT_PUT(v) do { const double v_ = (v); *o0 = w0 * v_; if (two) o0[GINT_TILE_ORB * GINT_LD] = w1 * v_; o0 += GINT_LD; } while (0)
+        // Angular factors times the store weight, all independent of the radial values: the FP64 pipe is shared with the
+        // consumers' DMMAs, under which a DEPENDENT FP64 operation costs ~25 cycles but independent ones overlap (measured),
+        // so the evaluation is written as wide as the registers allow: every output is then one multiply R_k * yw[m].
+        double yw[9];
+        {
+            const double c1 = 0.4886025119029199 * w0, c2 = (tiny ? 0.0 : 1.0925484305920792) * w0;     // l > 0 orbitals vanish at the nucleus
+            const double c20 = (tiny ? 0.0 : 0.31539156525252005) * w0, c22 = (tiny ? 0.0 : 0.5462742152960396) * w0;
+            const double c2x = c2 * ux, c2y = c2 * uy;
+            yw[0] = 0.28209479177387814 * w0;
+            yw[1] = c1 * uy; yw[2] = c1 * uz; yw[3] = c1 * ux;
+            yw[4] = c2x * uy; yw[5] = c2y * uz; yw[6] = c20 * fma(3.0 * uz, uz, -1.0); yw[7] = c2x * uz; yw[8] = c22 * fma(ux, ux, -uy * uy);
+        }
+        const double wr = (two && inside) ? (VLOCAL ? wv : 1.0) : 0.0;      // diagonal tile: side J = wr / w0-scaled copy (w0 = 1 inside)
+#define GINT_PUT(m) do { const double v_ = R * yw[m]; *o0 = v_; if (two) o0[GINT_TILE_ORB * GINT_LD] = wr * v_; o0 += GINT_LD; } while (0)
         for (int k0 = 0; k0 < nsh; k0 += GINT_EVAL_GROUP) {
-            double2 c0[GINT_EVAL_GROUP], c1[GINT_EVAL_GROUP];
+            double Rk[GINT_EVAL_GROUP];
 #pragma unroll
-            for (int u = 0; u < GINT_EVAL_GROUP; u++)
-                if (k0 + u < nsh) { c0[u] = row[k0 + u]; c1[u] = row[nsh + k0 + u]; }
+            for (int u = 0; u < GINT_EVAL_GROUP; u++) {
+                Rk[u] = 0.0;
+                if (k0 + u < nsh) {
+                    const double2 c0 = row[k0 + u], c1 = row[nsh + k0 + u];
+                    Rk[u] = fma(am, c0.x, fma(b, c1.x, fma(a3, c0.y, b3 * c1.y)));
+                }
+            }
 #pragma unroll
             for (int u = 0; u < GINT_EVAL_GROUP; u++) {
                 if (k0 + u >= nsh) break;
-                const double R = fma(am, c0[u].x, fma(b, c1[u].x, fma(a3, c0[u].y, b3 * c1[u].y)));
+                const double R = Rk[u];
                 const int l = (si.lpack >> (2 * (k0 + u))) & 3;
                 if (l == 0) {
-                    GINT_PUT(R * 0.28209479177387814);
+                    GINT_PUT(0);
                 } else if (l == 1) {
-                    const double R1 = R * 0.4886025119029199;
-                    GINT_PUT(R1 * uy); GINT_PUT(R1 * uz); GINT_PUT(R1 * ux);
+                    GINT_PUT(1); GINT_PUT(2); GINT_PUT(3);
                 } else {
-                    const double R2 = R * lz;
-                    const double c2 = R2 * 1.0925484305920792;
-                    GINT_PUT(c2 * ux * uy);
-                    GINT_PUT(c2 * uy * uz);
-                    GINT_PUT(R2 * 0.31539156525252005 * (3.0 * uz * uz - 1.0));
-                    GINT_PUT(c2 * ux * uz);
-                    GINT_PUT(R2 * 0.5462742152960396 * (ux * ux - uy * uy));
+                    GINT_PUT(4); GINT_PUT(5); GINT_PUT(6); GINT_PUT(7); GINT_PUT(8);
                 }
             }
         }
@@ -235,7 +243,7 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
                                            const double* __restrict__ atom_pos, const int* __restrict__ atom_spec,
                                            const SpeciesDev* __restrict__ sp, const int* __restrict__ crow,
                                            const u64* __restrict__ ckey, const unsigned int* __restrict__ coff,
-                                           const double* __restrict__ tab, int tab_cells) {
+                                           const double* __restrict__ tab, int tab_cells, const double* __restrict__ V) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     // copy of the radial table (tab_cells = 0: it stays in global memory)
     {
@@ -255,6 +263,17 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
     tv.nI = group_begin(tv.I + 1, n, tv.G) - eI;
     tv.nJ = group_begin(tv.J + 1, n, tv.G) - eJ;
 
+    {   // mesh points of the batch, one per thread (V == nullptr: rho, weight 1)
+        const int cl = tid >> 3, pp = tid & 7;
+        const int ix = 2 * (cl >> 4) + (pp >> 2), iy = 2 * ((cl >> 2) & 3) + ((pp >> 1) & 1), iz = 2 * (cl & 3) + (pp & 1);
+        double4 P = make_double4(1e30, 0.0, 0.0, 0.0);
+        if (ix < tv.ex && iy < tv.ey && iz < tv.ez) {
+            const int gi = tv.i0 + ix, gj = tv.j0 + iy, gk = tv.k0 + iz;
+            mesh_point(g, gi, gj, gk, P.x, P.y, P.z);
+            P.w = V ? __ldg(V + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk) * g.dV : 1.0;
+        }
+        S.pts[tid] = P;
+    }
     if (tid < 16) {
         const int side = tid >> 3, a = tid & 7;
         const bool valid = a < (side ? tv.nJ : tv.nI);
@@ -536,7 +555,7 @@ k_vlocal_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bst
     DBG_T(t_start);
     {
         TileView tv0;
-        tile_setup(g, S, tv0, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff, tab, tab_cells);
+        tile_setup(g, S, tv0, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff, tab, tab_cells, V);
     }
     DBG_T(t_setup);
     DBG_ADD(5, t_setup - t_start);
@@ -722,7 +741,7 @@ k_rho_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart
     TileSmem& S = *reinterpret_cast<TileSmem*>(smem_raw);
     {
         TileView tv0;
-        tile_setup(g, S, tv0, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff, tab, tab_cells);
+        tile_setup(g, S, tv0, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff, tab, tab_cells, nullptr);
     }
     const int nchunk = S.tv.nchunk;
     if (nchunk == 0) return;
