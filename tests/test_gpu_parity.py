@@ -141,3 +141,55 @@ def test_empty_and_single_atom(torch_cuda):
     g.close()
     assert _rel(H, O.vlocal(w1, V, plist)) <= TOL
     assert _rel(rho, O.rho(w1, D, plist)) <= TOL
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Full-size configurations in the launch configuration bench.py times: sampled outputs the oracle computes one by one
+# (selected pair keys / mesh points are still the exact definition for those outputs), plus identity P4, which holds
+# at any size and ties the two kernels together.
+def _sampled_parity(torch, cfg, n_keys, n_pts):
+    w = W.make_workload(cfg)
+    plist = O.pairs(w)
+    g = _gint(w)
+    _check_pairs(g, plist)
+    V = W.make_potential(w)
+    D = W.make_density_blocks(w, *plist)
+    A, B, R, off = plist
+    rng = np.random.default_rng([2409, 9399, cfg, 77])
+    keys = np.unique(np.concatenate([rng.integers(0, len(A), n_keys), np.flatnonzero((A == B) & (np.abs(R).sum(1) == 0))[:8]])).astype(np.int64)
+    pts = np.unique(rng.integers(0, w.n_points, n_pts)).astype(np.int64)
+    V_d, D_d = torch.from_numpy(V).cuda(), torch.from_numpy(D).cuda()
+    H_d, rho_d = g.vlocal(V_d), g.rho(D_d)
+    H, rho = H_d.cpu().numpy(), rho_d.cpu().numpy()
+    H_or = O.vlocal(w, V, plist, sel=keys)
+    rho_or = O.rho(w, D, plist, sel=pts)
+    # the scale of the tolerance is the largest |H| (|rho|) of the whole result, as in north_star
+    Hmax, rmax = float(np.max(np.abs(H))), float(np.max(np.abs(rho)))
+    eH = max(float(np.max(np.abs(H[off[k]:off[k + 1]] - H_or[off[k]:off[k + 1]]))) for k in keys) / Hmax
+    er = float(np.max(np.abs(rho[pts] - rho_or[pts]))) / rmax
+    dV = abs(np.linalg.det(w.cell)) / w.n_points
+    lhs = float((V_d * rho_d).sum().item() * dV); rhs = float((D_d * H_d).sum().item())
+    g.close()
+    assert eH <= TOL, f"cfg{cfg} H parity on {len(keys)} sampled keys {eH:.3e}"
+    assert er <= TOL, f"cfg{cfg} rho parity on {len(pts)} sampled points {er:.3e}"
+    assert abs(lhs - rhs) <= 1e-11 * abs(lhs), f"cfg{cfg} identity P4 {abs(lhs - rhs) / abs(lhs):.3e}"
+
+
+def test_cfg2_bulk_sampled(torch_cuda):
+    """512-atom bulk diamond: up to 7 atom groups per batch (28 tiles), the largest dense contractions."""
+    _sampled_parity(torch_cuda, 2, 96, 4000)
+
+
+def test_cfg3_tbg_sampled(torch_cuda):
+    _sampled_parity(torch_cuda, 3, 128, 6000)
+
+
+def test_cfg4_tbg_headline_sampled(torch_cuda):
+    """The headline workload (10,444 atoms, 1.76e8 points) exactly as bench.py launches it."""
+    _sampled_parity(torch_cuda, 4, 96, 4000)
+
+
+def test_unsupported_batch_edge(torch_cuda):
+    from paper_2409_09399_b200.gint import GintError, batch_flag
+    with pytest.raises(GintError, match="batch edge"):
+        _gint(W.make_workload(0), flags=batch_flag(9, 8, 8))
