@@ -19,6 +19,10 @@
 #define GINT_EVAL_WARPS (GINT_WARPS - GINT_MMA_WARPS)
 #define GINT_REGS_MMA 168          // registers per thread after setmaxnreg: 256 * 168 + 256 * 88 = 65536
 #define GINT_REGS_EVAL 88
+#ifndef GINT_REGS_MMA_RHO
+#define GINT_REGS_MMA_RHO 184      // gint_rho: its consumers are the bottleneck and its producers have slack (measured: 168/88 93.6 ms, 184/72 91.8 ms at cfg3)
+#define GINT_REGS_EVAL_RHO 72
+#endif
 #define GINT_STAGES 2              // shared-memory ring of orbital-value stages between producers and consumers
 // tile geometry of the contraction kernels: one CTA owns the block of H (or D) between two groups of atoms
 #define GINT_TILE_ATOMS 8          // atom images per group

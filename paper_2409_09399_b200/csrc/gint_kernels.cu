@@ -747,11 +747,11 @@ k_rho_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart
     if (nchunk == 0) return;
     const int warp = threadIdx.x >> 5;
     if (warp >= GINT_MMA_WARPS) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(GINT_REGS_EVAL));
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(GINT_REGS_EVAL_RHO));
         producer_loop<false>(g, S, nchunk, tab, tab_cells, nullptr);
         return;
     }
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(GINT_REGS_MMA));
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(GINT_REGS_MMA_RHO));
     const int lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
     Seg sg[GINT_WARP_SEGS];
     double d[GINT_WARP_SEGS][GINT_SEG_COLS][2];
