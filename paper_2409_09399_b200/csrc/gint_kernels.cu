@@ -245,6 +245,7 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
                                            const u64* __restrict__ ckey, const unsigned int* __restrict__ coff,
                                            const double* __restrict__ tab, int tab_cells, const double* __restrict__ V) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    DBG_T(ts0);
     // copy of the radial table (tab_cells = 0: it stays in global memory)
     {
         const double2* src = reinterpret_cast<const double2*>(tab);
@@ -296,14 +297,17 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
         for (int k = 0; k < Sp->n_shell; k++) lp |= Sp->l[k] << (2 * k);
         si.lpack = lp;
         S.sinfo[tid] = si;
+        // first orbital row of each atom inside its group: prefix sum of norb over the 8 lanes of the side
+        const int norb = valid ? Sp->norb : 0;
+        int inc = norb;
+#pragma unroll
+        for (int dlt = 1; dlt < 8; dlt <<= 1) { const int t = __shfl_up_sync(0xffffu, inc, dlt, 8); if (a >= dlt) inc += t; }
+        S.cstart[side][a] = inc - norb;
+        if (a == 7) S.cstart[side][8] = inc;
     }
+    DBG_T(ts1);
     __syncthreads();
-    if (tid < 2) {
-        int o = 0;
-        const int na = tid ? tv.nJ : tv.nI;
-        for (int a = 0; a <= GINT_TILE_ATOMS; a++) { S.cstart[tid][a] = o; if (a < na) o += sp[S.spec[8 * tid + a]].norb; }
-    }
-    __syncthreads();
+    DBG_T(ts2);
     const int totI = S.cstart[0][GINT_TILE_ATOMS], totJ = S.cstart[1][GINT_TILE_ATOMS];
     tv.nfI = (totI + 7) >> 3;
     tv.nfJ = (totJ + 7) >> 3;
@@ -358,6 +362,7 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
         if (row < GINT_TILE_ORB) S.phi[st][side][row][col] = 0.0;
     }
     __syncthreads();
+    DBG_T(ts3);
     if (warp == 0) {
         // union masks, cubelet list, per-slot read sets
         const u64 vI = lane < tv.nfI ? S.fmask[0][lane] : 0ull;
@@ -406,6 +411,7 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
         }
     }
     __syncthreads();
+    DBG_T(ts4);
     tv.nchunk = (S.ncub + 3) >> 2;
     if (warp < tv.nchunk) make_items(S, warp);
     if (tid == 0) {
@@ -413,6 +419,7 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
         for (int s = 0; s < GINT_STAGES; s++) { mbar_init(&S.full[s], GINT_EVAL_WARPS); mbar_init(&S.empty[s], GINT_MMA_WARPS); }
     }
     __syncthreads();
+    DBG_T(ts5); DBG_ADD(12, ts1 - ts0); DBG_ADD(13, ts2 - ts1); DBG_ADD(14, ts3 - ts2); DBG_ADD(15, ts4 - ts3); DBG_ADD(0, ts5 - ts4);
 }
 
 // ---------------------------------------------------------------------------------------------------
