@@ -37,6 +37,20 @@ def alg_flops(st: dict) -> float:
     return float(st["alg_sum_n2"] + st["alg_sum_n"]) + float(st["alg_sum_n"]) + EVAL_FLOP_PER_INCIDENCE * st["alg_incidence"]
 
 
+def ncu_traffic(cfg: int, kernel: str):
+    """DRAM bytes (read + write) of one launch of `kernel` from the committed ncu capture (profiles/r1g_traffic.csv), or None."""
+    path = os.path.join(ROOT, "profiles", "r1g_traffic.csv")
+    try:
+        with open(path) as f:
+            for ln in f.read().splitlines()[1:]:
+                c, k, rd, wr = ln.split(",")[:4]
+                if int(c) == cfg and k == kernel:
+                    return int(rd) + int(wr)
+    except (OSError, ValueError):
+        pass
+    return None
+
+
 def max_over_ranks(values, device, world: int):
     """Element-wise maximum over all ranks (torch.distributed all-reduce; identity for one rank)."""
     if world <= 1:
@@ -287,7 +301,8 @@ def main():
             "alg_tflops_rho": F_alg / float(t_r.mean()) / 1e12,
             "identity_P4_rel": p4,
             "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                         "frac": achieved / FP64_PEAK_TFLOPS, "traffic": None,
+                         "frac": achieved / FP64_PEAK_TFLOPS, "traffic": ncu_traffic(args.cfg, dom),
+                         "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1g_final_kernels.md)",
                          "peak_source": "148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md; DMMA micro-benchmark reaches 37.1)",
                          "kernel_ms": {k: 1e3 * v for k, v in kt.items()}},
             "clocks": clocks,
