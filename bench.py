@@ -286,6 +286,15 @@ def main():
             cpu = {"value": val, "unit": "mesh points/s", **info}
         dom = "vlocal_main" if kt["vlocal_main"] >= kt["rho_main"] else "rho_main"
         achieved = F_alg / kt[dom] / 1e12
+        # context: the same kernel against the HBM roofline (measured copy bandwidth of this pool's B200s, MEASURED_PEAKS.json;
+        # 6650 GB/s is the profiling guide's fallback).  Algorithmic bytes: V + canonical H (vlocal) / canonical D + rho (rho).
+        try:
+            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+                hbm_peak, hbm_src = float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except (OSError, KeyError, ValueError):
+            hbm_peak, hbm_src = 6650.0, "fallback (B200_PROFILING.md)"
+        alg_bytes = 8.0 * (npts + st["n_canon"] * (g.n_values / max(1, g.n_pairs)))
+        hbm_achieved = alg_bytes / kt[dom] / 1e9
         line = {
             "metric": METRIC, "value": job_value(npts, t_step, world), "unit": "mesh points/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_step, "higher_is_better": True,
@@ -304,7 +313,9 @@ def main():
                          "frac": achieved / FP64_PEAK_TFLOPS, "traffic": ncu_traffic(args.cfg, dom),
                          "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1g_final_kernels.md)",
                          "peak_source": "148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md; DMMA micro-benchmark reaches 37.1)",
-                         "kernel_ms": {k: 1e3 * v for k, v in kt.items()}},
+                         "kernel_ms": {k: 1e3 * v for k, v in kt.items()},
+                         "hbm_context": {"achieved": hbm_achieved, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_achieved / hbm_peak,
+                                         "peak_source": hbm_src, "algorithmic_bytes": alg_bytes}},
             "clocks": clocks,
             "gpu_launches": args.steps * (st["launches_vlocal"] + st["launches_rho"]),
             "wall_s_timed_region": wall, "setup_s": t1 - t0,
