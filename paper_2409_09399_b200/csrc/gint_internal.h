@@ -17,8 +17,10 @@
 #define GINT_THREADS (32 * GINT_WARPS)
 #define GINT_MMA_WARPS 8           // warp groups 0,1: DMMA consumers (setmaxnreg.inc); warp groups 2,3: orbital-evaluation producers
 #define GINT_EVAL_WARPS (GINT_WARPS - GINT_MMA_WARPS)
+#ifndef GINT_REGS_MMA
 #define GINT_REGS_MMA 168          // registers per thread after setmaxnreg: 256 * 168 + 256 * 88 = 65536
 #define GINT_REGS_EVAL 88
+#endif
 #ifndef GINT_REGS_MMA_RHO
 #define GINT_REGS_MMA_RHO 184      // gint_rho: its consumers are the bottleneck and its producers have slack (measured: 168/88 93.6 ms, 184/72 91.8 ms at cfg3)
 #define GINT_REGS_EVAL_RHO 72

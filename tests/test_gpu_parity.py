@@ -193,3 +193,49 @@ def test_unsupported_batch_edge(torch_cuda):
     from paper_2409_09399_b200.gint import GintError, batch_flag
     with pytest.raises(GintError, match="batch edge"):
         _gint(W.make_workload(0), flags=batch_flag(9, 8, 8))
+
+
+def test_table_too_large_for_shared_memory(torch_cuda):
+    """Three species with rc = 9 (901 knots x 5 shells each): the radial table (216 KB) does not fit beside the tile in shared
+    memory, so the evaluation reads it from global memory -- the other table path of the kernels."""
+    torch = torch_cuda
+    bs = [W.make_basis(9.0, shells=((0, 0.5 + 0.1 * k), (0, 0.2), (1, 0.45), (1, 0.2), (2, 0.35))) for k in range(3)]
+    basis = W.Basis(3, np.array([5, 5, 5], np.int32), np.concatenate([b.shell_l for b in bs]), np.array([9.0, 9.0, 9.0]), W.DR,
+                    np.concatenate([b.n_knot for b in bs]), np.concatenate([b.tab_y for b in bs]), np.concatenate([b.tab_y2 for b in bs]))
+    cell = np.diag([22.0, 21.0, 20.0])
+    pos = np.array([[3.0, 4.0, 5.0], [9.5, 6.0, 8.0], [15.0, 14.0, 12.0], [6.0, 16.0, 3.0], [11.0, 11.0, 17.0]])
+    w = W.Workload("big-table", 93, cell, np.array([40, 38, 36], np.int32), np.array([0, 1, 2, 1, 0], np.int32), pos, basis)
+    plist = O.pairs(w)
+    g = _gint(w)
+    _check_pairs(g, plist)
+    rng = np.random.default_rng(21)
+    V = rng.standard_normal(w.n_points)
+    D = rng.standard_normal(int(plist[3][-1]))
+    H = g.vlocal(torch.from_numpy(V).cuda()).cpu().numpy()
+    rho = g.rho(torch.from_numpy(D).cuda()).cpu().numpy()
+    st = g.stats()
+    g.close()
+    assert st["smem_bytes"] < 200 * 1024          # the table was left out of shared memory
+    assert _rel(H, O.vlocal(w, V, plist)) <= TOL
+    assert _rel(rho, O.rho(w, D, plist)) <= TOL
+
+
+def test_dense_cell_falls_back_to_smaller_batches(torch_cuda):
+    """Tiny diamond cell with rc = 8.5 > a: more than 96 atom images touch an 8x8x8 batch, so gint_init must choose a smaller
+    batch shape by itself (flags = 0) and still be exact."""
+    torch = torch_cuda
+    w0 = W.make_workload(0)
+    w = W.Workload("dense", 94, w0.cell, np.array([16, 16, 16], np.int32), w0.atom_species, w0.atom_pos, W.make_basis(8.5))
+    plist = O.pairs(w)
+    g = _gint(w)
+    _check_pairs(g, plist)
+    st = g.stats()
+    assert st["batch_bx"] * st["batch_by"] * st["batch_bz"] < 512 and st["max_nb"] <= 96
+    rng = np.random.default_rng(22)
+    V = rng.standard_normal(w.n_points)
+    D = rng.standard_normal(int(plist[3][-1]))
+    H = g.vlocal(torch.from_numpy(V).cuda()).cpu().numpy()
+    rho = g.rho(torch.from_numpy(D).cuda()).cpu().numpy()
+    g.close()
+    assert _rel(H, O.vlocal(w, V, plist)) <= TOL
+    assert _rel(rho, O.rho(w, D, plist)) <= TOL
