@@ -29,7 +29,10 @@ __device__ unsigned long long g_dbg[16];
 #define DBG_ADD(i, v) do { if ((threadIdx.x & 31) == 0) atomicAdd(&g_dbg[i], (unsigned long long)(v)); } while (0)
 extern "C" int gint_debug_counters(unsigned long long* out) { return (int)cudaMemcpyFromSymbol(out, g_dbg, sizeof(g_dbg)); }
 #endif
-#define GINT_EVAL_GROUP 5          // radial shells whose spline coefficients are loaded together (registers vs memory-level parallelism)
+#ifndef GINT_EVAL_GROUP
+#define GINT_EVAL_GROUP 5          // radial shells whose spline cells are loaded together (registers vs memory-level parallelism)
+#define GINT_EVAL_GROUP_RHO 2      // gint_rho's producers run with 72 registers: measured 91.9 ms (5), 88.6 (3), 87.9 (2) at cfg3
+#endif
 
 // ---------------------------------------------------------------------------------------------------
 // shared memory of the tile kernels
@@ -154,6 +157,7 @@ template <bool VLOCAL>
 __device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, int ps, int c, int first, const double2* __restrict__ tab,
                                            const double* __restrict__ V) {
     const int lane = threadIdx.x & 31;
+    constexpr int GROUP = VLOCAL ? GINT_EVAL_GROUP : GINT_EVAL_GROUP_RHO;
     const int nitem = S.nitem[c], neval = S.neval[c];
     const bool two = S.tv.diag;
     for (int base = first; base < nitem; base += 4 * GINT_EVAL_WARPS) {
@@ -207,10 +211,10 @@ __device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, int ps, i
         }
         const double wr = (two && inside) ? (VLOCAL ? wv : 1.0) : 0.0;      // diagonal tile: side J = wr / w0-scaled copy (w0 = 1 inside)
 #define GINT_PUT(m) do { const double v_ = R * yw[m]; *o0 = v_; if (two) o0[GINT_TILE_ORB * GINT_LD] = wr * v_; o0 += GINT_LD; } while (0)
-        for (int k0 = 0; k0 < nsh; k0 += GINT_EVAL_GROUP) {
-            double Rk[GINT_EVAL_GROUP];
+        for (int k0 = 0; k0 < nsh; k0 += GROUP) {
+            double Rk[GROUP];
 #pragma unroll
-            for (int u = 0; u < GINT_EVAL_GROUP; u++) {
+            for (int u = 0; u < GROUP; u++) {
                 Rk[u] = 0.0;
                 if (k0 + u < nsh) {
                     const double2 c0 = row[k0 + u], c1 = row[nsh + k0 + u];
@@ -218,7 +222,7 @@ __device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, int ps, i
                 }
             }
 #pragma unroll
-            for (int u = 0; u < GINT_EVAL_GROUP; u++) {
+            for (int u = 0; u < GROUP; u++) {
                 if (k0 + u >= nsh) break;
                 const double R = Rk[u];
                 const int l = (si.lpack >> (2 * (k0 + u))) & 3;
