@@ -159,7 +159,7 @@ __device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, int ps, i
     const int lane = threadIdx.x & 31;
     constexpr int GROUP = VLOCAL ? GINT_EVAL_GROUP : GINT_EVAL_GROUP_RHO;
     const int nitem = S.nitem[c], neval = S.neval[c];
-    const bool two = S.tv.diag;
+    const bool two = VLOCAL && S.tv.diag;      // gint_rho reads side I twice in a diagonal tile instead
     for (int base = first; base < nitem; base += 4 * GINT_EVAL_WARPS) {
         const int idx = base + (lane >> 3);
         const bool on = idx < nitem;
@@ -453,7 +453,7 @@ struct Seg {
     __device__ __forceinline__ int cb() const { return (w >> 8) & 255; }
     __device__ __forceinline__ int n() const { return w >> 16; }
 };
-__device__ __forceinline__ Seg load_seg(const TileSmem& S, int slot) {
+__device__ __forceinline__ Seg load_seg(const TileSmem& S, int slot, bool j_is_i = false) {   // j_is_i: column operands from side I (rho, diagonal tile)
     const int lane = threadIdx.x & 31;
     Seg s; s.w = S.seg[slot];
     u64 cm = 0;
@@ -462,7 +462,7 @@ __device__ __forceinline__ Seg load_seg(const TileSmem& S, int slot) {
     const bool b0 = lane < S.ncub && ((act >> S.cub[lane]) & 1ull), b1 = lane + 32 < S.ncub && ((act >> S.cub[(lane + 32) & 63]) & 1ull);
     s.W = (u64)__ballot_sync(0xffffffffu, b0) | ((u64)__ballot_sync(0xffffffffu, b1) << 32);
     s.oa = (unsigned)(s.row() * 8 * GINT_ROWB);
-    s.ob = (unsigned)(GINT_SIDEB + s.cb() * 8 * GINT_ROWB);
+    s.ob = (unsigned)((j_is_i ? 0 : GINT_SIDEB) + s.cb() * 8 * GINT_ROWB);
     return s;
 }
 
@@ -768,7 +768,7 @@ k_rho_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart
     double d[GINT_WARP_SEGS][GINT_SEG_COLS][2];
 #pragma unroll
     for (int k = 0; k < GINT_WARP_SEGS; k++) {
-        sg[k] = load_seg(S, warp + GINT_MMA_WARPS * k);
+        sg[k] = load_seg(S, warp + GINT_MMA_WARPS * k, S.tv.diag);
         load_dseg(S, sg[k], Dh, d[k]);
     }
     const unsigned phi0 = smem_addr(&S.phi[0][0][0][0]);
