@@ -256,6 +256,7 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
         double2* dst = reinterpret_cast<double2*>(reinterpret_cast<unsigned char*>(&S) + GINT_SMEM_TAB_OFF);
         for (int i = tid; i < tab_cells; i += GINT_THREADS) dst[i] = __ldg(src + i);
     }
+    if (tid == GINT_THREADS - 32) for (int s = 0; s < GINT_STAGES; s++) { mbar_init(&S.full[s], GINT_EVAL_WARPS); mbar_init(&S.empty[s], GINT_MMA_WARPS); }
     const int2 td = tile[blockIdx.x];
     tv.b = td.x; tv.I = td.y & 255; tv.J = (td.y >> 8) & 255; tv.G = (td.y >> 16) & 255;
     tv.diag = tv.I == tv.J;
@@ -367,29 +368,32 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
     }
     __syncthreads();
     DBG_T(ts3);
-    if (warp == 0) {
-        // union masks, cubelet list, per-slot read sets
+    if (warp == 0 || warp == 2) {
+        // union masks (both warps), then warp 0: cubelet list; warp 2: per-slot read sets
         const u64 vI = lane < tv.nfI ? S.fmask[0][lane] : 0ull;
         const u64 vJ = lane < tv.nfJ ? S.fmask[1][lane] : 0ull;
         const u64 anyI = warp_or64(vI);
         const u64 h0 = warp_or64(lane < GINT_SEG_COLS ? vJ : 0ull) & anyI, h1 = warp_or64(lane >= GINT_SEG_COLS ? vJ : 0ull) & anyI;
         const u64 U = h0 | h1;
-        const unsigned Ulo = (unsigned)U, Uhi = (unsigned)(U >> 32), lt = (1u << lane) - 1u;
-        if ((Ulo >> lane) & 1u) S.cub[__popc(Ulo & lt)] = (unsigned char)lane;
-        if ((Uhi >> lane) & 1u) S.cub[__popc(Ulo) + __popc(Uhi & lt)] = (unsigned char)(32 + lane);
-        const int ncub = __popc(Ulo) + __popc(Uhi);
-        if (lane < 4) S.cub[ncub + lane] = 0;
-        u64 m = 0;
-        if (lane < 16) {
-            const int side = lane >> 3, a = lane & 7;
-            const int nf = side ? tv.nfJ : tv.nfI;
-            for (int f = 0; f < nf; f++)
-                if ((S.frag_atoms[side][f] >> a) & 1) m |= side ? (f < GINT_SEG_COLS ? h0 : h1) : (S.fmask[0][f] & U);
+        if (warp == 0) {
+            const unsigned Ulo = (unsigned)U, Uhi = (unsigned)(U >> 32), lt = (1u << lane) - 1u;
+            if ((Ulo >> lane) & 1u) S.cub[__popc(Ulo & lt)] = (unsigned char)lane;
+            if ((Uhi >> lane) & 1u) S.cub[__popc(Ulo) + __popc(Uhi & lt)] = (unsigned char)(32 + lane);
+            const int ncub = __popc(Ulo) + __popc(Uhi);
+            if (lane < 4) S.cub[ncub + lane] = 0;
+            if (lane == 0) { S.U = U; S.hmask[0] = h0; S.hmask[1] = h1; S.ncub = ncub; }
+        } else {
+            u64 m = 0;
+            if (lane < 16) {
+                const int side = lane >> 3, a = lane & 7;
+                const int nf = side ? tv.nfJ : tv.nfI;
+                for (int f = 0; f < nf; f++)
+                    if ((S.frag_atoms[side][f] >> a) & 1) m |= side ? (f < GINT_SEG_COLS ? h0 : h1) : (S.fmask[0][f] & U);
+            }
+            const u64 mj = shfl64(m, (lane + 8) & 31);
+            if (tv.diag) m = lane < 8 ? (m | mj) : 0ull;      // the atoms are evaluated once, for both sides
+            if (lane < 16) S.need[lane] = m;
         }
-        const u64 mj = shfl64(m, (lane + 8) & 31);
-        if (tv.diag) m = lane < 8 ? (m | mj) : 0ull;      // the atoms are evaluated once, for both sides
-        if (lane < 16) S.need[lane] = m;
-        if (lane == 0) { S.U = U; S.hmask[0] = h0; S.hmask[1] = h1; S.ncub = ncub; }
     } else if (warp == 1) {
         // segments: piece (row fragment r, half h) = columns [cb, cb + n); sorted by falling n and dealt to the
         // sub-partitions 0,1,2,3,3,2,1,0,... (warp w runs on sub-partition w % 4)
@@ -418,10 +422,7 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
     DBG_T(ts4);
     tv.nchunk = (S.ncub + 3) >> 2;
     if (warp < tv.nchunk) make_items(S, warp);
-    if (tid == 0) {
-        S.tv = tv;
-        for (int s = 0; s < GINT_STAGES; s++) { mbar_init(&S.full[s], GINT_EVAL_WARPS); mbar_init(&S.empty[s], GINT_MMA_WARPS); }
-    }
+    if (tid == GINT_THREADS - 1) S.tv = tv;      // a thread of the last warp: it has no item list to make (<= 16 stages, warp 15 only for 64 cubelets)
     __syncthreads();
     DBG_T(ts5); DBG_ADD(12, ts1 - ts0); DBG_ADD(13, ts2 - ts1); DBG_ADD(14, ts3 - ts2); DBG_ADD(15, ts4 - ts3); DBG_ADD(0, ts5 - ts4);
 }
