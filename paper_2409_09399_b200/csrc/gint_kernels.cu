@@ -250,14 +250,20 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
                                            const double* __restrict__ tab, int tab_cells, const double* __restrict__ V) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     DBG_T(ts0);
-    // copy of the radial table (tab_cells = 0: it stays in global memory)
+    const int2 td = tile[blockIdx.x];            // head of the dependent chain tile -> batch -> neighbour entries -> atoms: issue it first
+    // copy of the radial table (tab_cells = 0: it stays in global memory): 8 independent 16-byte loads per thread in flight
     {
         const double2* src = reinterpret_cast<const double2*>(tab);
         double2* dst = reinterpret_cast<double2*>(reinterpret_cast<unsigned char*>(&S) + GINT_SMEM_TAB_OFF);
-        for (int i = tid; i < tab_cells; i += GINT_THREADS) dst[i] = __ldg(src + i);
+        for (int i0 = tid; i0 < tab_cells; i0 += 8 * GINT_THREADS) {
+            double2 tmp[8];
+#pragma unroll
+            for (int u = 0; u < 8; u++) if (i0 + u * GINT_THREADS < tab_cells) tmp[u] = __ldg(src + i0 + u * GINT_THREADS);
+#pragma unroll
+            for (int u = 0; u < 8; u++) if (i0 + u * GINT_THREADS < tab_cells) dst[i0 + u * GINT_THREADS] = tmp[u];
+        }
     }
     if (tid == GINT_THREADS - 32) for (int s = 0; s < GINT_STAGES; s++) { mbar_init(&S.full[s], GINT_EVAL_WARPS); mbar_init(&S.empty[s], GINT_MMA_WARPS); }
-    const int2 td = tile[blockIdx.x];
     tv.b = td.x; tv.I = td.y & 255; tv.J = (td.y >> 8) & 255; tv.G = (td.y >> 16) & 255;
     tv.diag = tv.I == tv.J;
     const int b = tv.b;
