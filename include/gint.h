@@ -32,7 +32,7 @@ typedef struct gint_ctx gint_ctx;
 typedef enum gint_status {
     GINT_OK = 0,
     GINT_ERR_INVALID_ARG = -1,   /* NULL pointer, negative size, non-finite value, det(cell) <= 0, ...        */
-    GINT_ERR_UNSUPPORTED = -2,   /* l > 2, more than GINT_MAX_ORB orbitals per atom, batch edge > 8, device not sm_100 */
+    GINT_ERR_UNSUPPORTED = -2,   /* l > 2, more than GINT_MAX_ORB orbitals per atom, batch edge too large, device not sm_100 */
     GINT_ERR_CUDA = -3,          /* a CUDA runtime call failed (message holds cudaGetErrorString)             */
     GINT_ERR_OUT_OF_MEMORY = -4, /* host or device allocation failed                                          */
     GINT_ERR_BAD_STATE = -5      /* NULL / freed context                                                      */
@@ -41,9 +41,9 @@ typedef enum gint_status {
 #define GINT_MAX_L 2
 #define GINT_MAX_ORB 32          /* orbitals per atom (sum over shells of 2l+1) */
 
-/* flags of gint_init: three 8-bit fields override the grid-batch edge lengths (mesh points, 1..8 each) along a1,a2,a3;
- * 0 = choose automatically: 8x8x8 points, or the largest smaller shape whose batches have at most 96 neighbouring atom
- * images (PAPER.md:165 uses batches of 27..1000 points; Table 3 sweeps 125..512).  An edge > 8 is GINT_ERR_UNSUPPORTED. */
+/* flags of gint_init: three 8-bit fields override the grid-batch edge lengths (mesh points) along a1,a2,a3: 1..8, 1..8, 1..16;
+ * 0 = choose automatically: 8x8x16 points, or the largest smaller shape whose batches have at most 96 neighbouring atom
+ * images (PAPER.md:165 uses batches of 27..1000 points; Table 3 sweeps 125..512).  A larger edge is GINT_ERR_UNSUPPORTED. */
 #define GINT_FLAG_BATCH(bx, by, bz) ((unsigned long long)(bx) | ((unsigned long long)(by) << 8) | ((unsigned long long)(bz) << 16))
 
 /*

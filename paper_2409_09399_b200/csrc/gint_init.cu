@@ -172,7 +172,7 @@ __global__ void __launch_bounds__(256) k_batch_neighbours(Geom g, int cbx, int c
             const double dx = px - im.x, dy = py - im.y, dz = pz - im.z;
             const bool in = fma(dx, dx, fma(dy, dy, dz * dz)) < im.rc * im.rc;    // same expression as the orbital evaluation
             hits += in;
-            if (FILL && in) { const int cl = (qx >> 1) * 16 + (qj >> 1) * 4 + (qk >> 1); if (cl < 32) mlo |= 1u << cl; else mhi |= 1u << (cl - 32); }
+            if (FILL && in) { const int cl = (qx >> 1) * 16 + (qj >> 1) * 4 + qk / GINT_CZ; if (cl < 32) mlo |= 1u << cl; else mhi |= 1u << (cl - 32); }
         }
 #pragma unroll
         for (int d = 16; d; d >>= 1) hits += __shfl_xor_sync(0xffffffffu, hits, d);
@@ -459,7 +459,7 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, bool* 
     *fits = false;
     for (int i = 0; i < 3; i++) { g.bs[i] = std::min(bs[i], g.N[i]); g.nb[i] = (g.N[i] + g.bs[i] - 1) / g.bs[i]; }
     g.K = g.bs[0] * g.bs[1] * g.bs[2];
-    for (int i = 0; i < 3; i++) if (bs[i] < 1 || bs[i] > GINT_MAX_BS) GINT_FAIL(GINT_ERR_UNSUPPORTED, "batch edge %d (1..%d supported)", bs[i], GINT_MAX_BS);
+    for (int i = 0; i < 3; i++) if (bs[i] < 1 || bs[i] > (i == 2 ? GINT_MAX_BSZ : GINT_MAX_BS)) GINT_FAIL(GINT_ERR_UNSUPPORTED, "batch edge %d (1..%d supported)", bs[i], i == 2 ? GINT_MAX_BSZ : GINT_MAX_BS);
     const long long nbt = (long long)g.nb[0] * g.nb[1] * g.nb[2];
     if (nbt > 2000000000LL) GINT_FAIL(GINT_ERR_UNSUPPORTED, "%lld batches", nbt);
     c->n_batch_total = nbt;
@@ -628,7 +628,7 @@ extern "C" int gint_init(gint_ctx** out, int n_species, const int* n_shell, cons
         if ((rc = build_batches(c, bs, smem_limit, &fits))) { free_ctx(c); return rc; }
         if (!fits) { free_ctx(c); GINT_FAIL(GINT_ERR_UNSUPPORTED, "requested batch %dx%dx%d needs more shared memory than %zu bytes (or > %d neighbours)", bs[0], bs[1], bs[2], smem_limit, GINT_MAX_NB); }
     } else {
-        static const int shapes[][3] = {{8, 8, 8}, {4, 4, 8}, {4, 4, 4}, {2, 2, 4}, {1, 1, 4}, {1, 1, 1}};
+        static const int shapes[][3] = {{8, 8, GINT_MAX_BSZ}, {8, 8, 8}, {4, 4, 8}, {4, 4, 4}, {2, 2, 4}, {1, 1, 4}, {1, 1, 1}};
         for (auto& s : shapes) {
             if ((rc = build_batches(c, s, smem_limit, &fits))) { free_ctx(c); return rc; }
             if (fits) break;

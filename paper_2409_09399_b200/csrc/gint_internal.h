@@ -12,7 +12,12 @@
 
 #define GINT_MAX_SHELL 12          // radial shells per species
 #define GINT_MAX_NB 96             // neighbouring atom images per grid batch
-#define GINT_MAX_BS 8              // largest grid-batch edge (points): 4 x 4 x 4 cubelets of 2 x 2 x 2 points = one 64-bit mask
+#define GINT_MAX_BS 8              // largest grid-batch edge along a1, a2 (points)
+#ifndef GINT_CZ
+#define GINT_CZ 4                  // cubelet = 2 x 2 x GINT_CZ mesh points; a batch is at most 4 x 4 x 4 cubelets = one 64-bit mask
+#endif
+#define GINT_CPTS (4 * GINT_CZ)    // points per cubelet (8 or 16)
+#define GINT_MAX_BSZ (4 * GINT_CZ) // largest grid-batch edge along a3
 #define GINT_WARPS 16              // warps per CTA of the contraction kernels: 4 warp groups
 #define GINT_THREADS (32 * GINT_WARPS)
 #define GINT_MMA_WARPS 8           // warp groups 0,1: DMMA consumers (setmaxnreg.inc); warp groups 2,3: orbital-evaluation producers
@@ -33,7 +38,9 @@
 #define GINT_SEG_COLS 7            // column fragments of one segment (row fragment x <= 7 column fragments)
 #define GINT_WARP_SEGS 4           // segments per consumer warp
 #define GINT_MAX_SEG (GINT_WARP_SEGS * GINT_MMA_WARPS)
-#define GINT_CHUNK 32              // mesh points per pipeline stage = 4 cubelets of 8 points
+#define GINT_CHUNK 32              // mesh points per pipeline stage = 4 DMMA steps of 8 points
+#define GINT_CUBS (GINT_CHUNK / GINT_CPTS)      // cubelets per stage (4 or 2)
+#define GINT_MAX_CHUNKS (64 / GINT_CUBS)
 #define GINT_LD 36                 // row stride (doubles) of the orbital tiles in shared memory: = 4 mod 16, the 64-bit fragment loads are conflict-free
 
 // ---- error plumbing -------------------------------------------------------------------------------

@@ -52,7 +52,7 @@ struct TileSmem {
     // phi[stage][side][orbital row][GINT_LD]: side 0 = group I, side 1 = group J (scaled by V dV in vlocal);
     // column 8q + p = point p of the stage's q-th cubelet
     double phi[GINT_STAGES][2][GINT_TILE_ORB][GINT_LD];
-    double4 pts[512];                   // [cubelet id * 8 + p]: x, y, z of the batch's mesh points, weight V dV (vlocal) or 1 (rho);
+    double4 pts[64 * GINT_CPTS];                   // [cubelet id * 8 + p]: x, y, z of the batch's mesh points, weight V dV (vlocal) or 1 (rho);
                                         // points outside the mesh: far away, weight 0
     u64 full[GINT_STAGES], empty[GINT_STAGES];   // mbarriers: stage written by all producer warps / read by all consumer warps
     double pos[16][4];                  // slot s < 8: atom s of group I; slot 8 + s: atom s of group J
@@ -68,8 +68,8 @@ struct TileSmem {
     int seg[GINT_MAX_SEG];              // slot (consumer warp) + 8 k: row fragment | first column fragment << 8 | n columns << 16
     int ncub;
     TileView tv;                        // written by tile_setup; read from here afterwards to keep registers free
-    unsigned char item[16][64];         // [stage][k]: slot << 2 | cubelet of the stage
-    unsigned char nitem[16], neval[16]; // [stage]: items of the stage, of which the first neval need a real evaluation
+    unsigned char item[GINT_MAX_CHUNKS][16 * GINT_CUBS];         // [stage][k]: slot << 2 | cubelet of the stage
+    unsigned char nitem[GINT_MAX_CHUNKS], neval[GINT_MAX_CHUNKS]; // [stage]: items of the stage, of which the first neval need a real evaluation
     unsigned char cub[64 + 4];          // the tile's cubelets (bit numbers of U, ascending)
     unsigned char row_atom[2][GINT_TILE_ORB];   // orbital row -> atom slot inside the group (255 = padding)
     unsigned char row_orb[2][GINT_TILE_ORB];    // orbital row -> orbital index inside the atom
@@ -116,10 +116,10 @@ __device__ __forceinline__ u64 shfl64(u64 v, int src) {
 // ---------------------------------------------------------------------------------------------------
 // Stage c of a tile = its cubelets 4c .. 4c+3; point index 8 q + p: point p = (px, py, pz) bits of the q-th cubelet.
 __device__ __forceinline__ bool stage_point(const TileSmem& S, int c, int pt, int& gi, int& gj, int& gk) {
-    const int ci = 4 * c + (pt >> 3), p = pt & 7;
+    const int ci = GINT_CUBS * c + pt / GINT_CPTS, p = pt % GINT_CPTS;
     if (ci >= S.ncub) return false;
     const int cl = S.cub[ci];
-    const int ix = 2 * (cl >> 4) + (p >> 2), iy = 2 * ((cl >> 2) & 3) + ((p >> 1) & 1), iz = 2 * (cl & 3) + (p & 1);
+    const int ix = 2 * (cl >> 4) + p / (2 * GINT_CZ), iy = 2 * ((cl >> 2) & 3) + ((p / GINT_CZ) & 1), iz = GINT_CZ * (cl & 3) + p % GINT_CZ;
     gi = S.tv.i0 + ix; gj = S.tv.j0 + iy; gk = S.tv.k0 + iz;
     return ix < S.tv.ex && iy < S.tv.ey && iz < S.tv.ez;
 }
@@ -129,22 +129,34 @@ __device__ __forceinline__ bool stage_point(const TileSmem& S, int c, int pt, in
 // those that only need zeros.
 __device__ __forceinline__ void make_items(TileSmem& S, int c) {
     const int lane = threadIdx.x & 31;
-    // candidates: lane -> (slot lane >> 2, cubelet lane & 3) and (slot 8 + (lane >> 2), same cubelet)
-    const int ci = 4 * c + (lane & 3);
-    const bool inb = ci < S.ncub;
-    const int cl = inb ? S.cub[ci] : 0;
-    const int s0 = lane >> 2, s1 = 8 + s0;
-    const bool n0 = inb && ((S.need[s0] >> cl) & 1ull), n1 = inb && ((S.need[s1] >> cl) & 1ull);
-    const bool a0 = n0 && ((S.amask[s0] >> cl) & 1ull), a1 = n1 && ((S.amask[s1] >> cl) & 1ull);
-    const unsigned e0 = __ballot_sync(0xffffffffu, a0), e1 = __ballot_sync(0xffffffffu, a1);
-    const unsigned z0 = __ballot_sync(0xffffffffu, n0 && !a0), z1 = __ballot_sync(0xffffffffu, n1 && !a1);
+    // candidates (slot, cubelet of the stage): 16 * GINT_CUBS of them, NR per lane
+    constexpr int NR = (16 * GINT_CUBS + 31) / 32;
+    bool act[NR], need[NR];
+    unsigned eb[NR], zb[NR];
+    int ne = 0, nz = 0;
+#pragma unroll
+    for (int r = 0; r < NR; r++) {
+        const int cand = lane + 32 * r, slot = cand / GINT_CUBS, q = cand % GINT_CUBS;
+        const int ci = GINT_CUBS * c + q;
+        const bool inb = cand < 16 * GINT_CUBS && ci < S.ncub;
+        const int cl = inb ? S.cub[ci] : 0;
+        need[r] = inb && ((S.need[slot & 15] >> cl) & 1ull);
+        act[r] = need[r] && ((S.amask[slot & 15] >> cl) & 1ull);
+        eb[r] = __ballot_sync(0xffffffffu, act[r]);
+        zb[r] = __ballot_sync(0xffffffffu, need[r] && !act[r]);
+        ne += __popc(eb[r]); nz += __popc(zb[r]);
+    }
     const unsigned lt = (1u << lane) - 1u;
-    const int ne = __popc(e0) + __popc(e1);
-    if (a0) S.item[c][__popc(e0 & lt)] = (unsigned char)lane;
-    else if (n0) S.item[c][ne + __popc(z0 & lt)] = (unsigned char)lane;
-    if (a1) S.item[c][__popc(e0) + __popc(e1 & lt)] = (unsigned char)(32 + lane);
-    else if (n1) S.item[c][ne + __popc(z0) + __popc(z1 & lt)] = (unsigned char)(32 + lane);
-    if (lane == 0) { S.neval[c] = (unsigned char)ne; S.nitem[c] = (unsigned char)(ne + __popc(z0) + __popc(z1)); }
+    int pe = 0, pz = ne;
+#pragma unroll
+    for (int r = 0; r < NR; r++) {
+        const int cand = lane + 32 * r;
+        const unsigned char code = (unsigned char)(((cand / GINT_CUBS) << 2) | (cand % GINT_CUBS));
+        if (act[r]) S.item[c][pe + __popc(eb[r] & lt)] = code;
+        else if (need[r]) S.item[c][pz + __popc(zb[r] & lt)] = code;
+        pe += __popc(eb[r]); pz += __popc(zb[r]);
+    }
+    if (lane == 0) { S.neval[c] = (unsigned char)ne; S.nitem[c] = (unsigned char)(ne + nz); }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -160,11 +172,11 @@ __device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, int ps, i
     constexpr int GROUP = VLOCAL ? GINT_EVAL_GROUP : GINT_EVAL_GROUP_RHO;
     const int nitem = S.nitem[c], neval = S.neval[c];
     const bool two = VLOCAL && S.tv.diag;      // gint_rho reads side I twice in a diagonal tile instead
-    for (int base = first; base < nitem; base += 4 * GINT_EVAL_WARPS) {
-        const int idx = base + (lane >> 3);
+    for (int base = first; base < nitem; base += (32 / GINT_CPTS) * GINT_EVAL_WARPS) {
+        const int idx = base + lane / GINT_CPTS;
         const bool on = idx < nitem;
         const int it = on ? S.item[c][idx] : 0;
-        const int slot = it >> 2, pt = 8 * (it & 3) + (lane & 7);
+        const int slot = it >> 2, pt = GINT_CPTS * (it & 3) + lane % GINT_CPTS;
         const int side = slot >> 3, a = slot & 7;
         double* o0 = &S.phi[ps][side][S.cstart[side][a]][pt];
         if (base >= neval) {                        // the four items only need zeros
@@ -172,7 +184,7 @@ __device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, int ps, i
             for (int o = 0; o < norb; o++) { o0[o * GINT_LD] = 0.0; if (two) o0[o * GINT_LD + GINT_TILE_ORB * GINT_LD] = 0.0; }
             continue;
         }
-        const double4 P = S.pts[8 * S.cub[min(4 * c + (it & 3), 63)] + (lane & 7)];
+        const double4 P = S.pts[GINT_CPTS * S.cub[min(GINT_CUBS * c + (it & 3), 63)] + lane % GINT_CPTS];
         const double wv = P.w;
         const SlotInfo si = S.sinfo[slot];
         const double dx = P.x - S.pos[slot][0], dy = P.y - S.pos[slot][1], dz = P.z - S.pos[slot][2];
@@ -275,16 +287,16 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
     tv.nI = group_begin(tv.I + 1, n, tv.G) - eI;
     tv.nJ = group_begin(tv.J + 1, n, tv.G) - eJ;
 
-    {   // mesh points of the batch, one per thread (V == nullptr: rho, weight 1)
-        const int cl = tid >> 3, pp = tid & 7;
-        const int ix = 2 * (cl >> 4) + (pp >> 2), iy = 2 * ((cl >> 2) & 3) + ((pp >> 1) & 1), iz = 2 * (cl & 3) + (pp & 1);
+    for (int q = tid; q < 64 * GINT_CPTS; q += GINT_THREADS) {   // mesh points of the batch (V == nullptr: rho, weight 1)
+        const int cl = q / GINT_CPTS, pp = q % GINT_CPTS;
+        const int ix = 2 * (cl >> 4) + pp / (2 * GINT_CZ), iy = 2 * ((cl >> 2) & 3) + ((pp / GINT_CZ) & 1), iz = GINT_CZ * (cl & 3) + pp % GINT_CZ;
         double4 P = make_double4(1e30, 0.0, 0.0, 0.0);
         if (ix < tv.ex && iy < tv.ey && iz < tv.ez) {
             const int gi = tv.i0 + ix, gj = tv.j0 + iy, gk = tv.k0 + iz;
             mesh_point(g, gi, gj, gk, P.x, P.y, P.z);
             P.w = V ? __ldg(V + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk) * g.dV : 1.0;
         }
-        S.pts[tid] = P;
+        S.pts[q] = P;
     }
     if (tid < 16) {
         const int side = tid >> 3, a = tid & 7;
@@ -426,8 +438,8 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
     }
     __syncthreads();
     DBG_T(ts4);
-    tv.nchunk = (S.ncub + 3) >> 2;
-    if (warp < tv.nchunk) make_items(S, warp);
+    tv.nchunk = (S.ncub + GINT_CUBS - 1) / GINT_CUBS;
+    for (int c = warp; c < tv.nchunk; c += GINT_WARPS) make_items(S, c);
     if (tid == GINT_THREADS - 1) S.tv = tv;      // a thread of the last warp: it has no item list to make (<= 16 stages, warp 15 only for 64 cubelets)
     __syncthreads();
     DBG_T(ts5); DBG_ADD(12, ts1 - ts0); DBG_ADD(13, ts2 - ts1); DBG_ADD(14, ts3 - ts2); DBG_ADD(15, ts4 - ts3); DBG_ADD(0, ts5 - ts4);
@@ -479,6 +491,11 @@ __device__ __forceinline__ Seg load_seg(const TileSmem& S, int slot, bool j_is_i
 // vice versa, so the shared-memory latency is hidden behind the FP64 tensor pipe.
 // next active cubelet of a segment: q = lowest set bit of rem (removed from rem), operand addresses pa/pb + 64 q.
 // One volatile asm block, so that it stays where it is written: in the shadow of the DMMAs.
+// activity of a segment on the 8-point DMMA steps of stage c (a 16-point cubelet is two steps)
+__device__ __forceinline__ unsigned stage_steps(u64 W, int c) {
+    const unsigned b = (unsigned)(W >> (GINT_CUBS * c)) & ((1u << GINT_CUBS) - 1u);
+    return GINT_CPTS == 8 ? b : ((b & 1u) * 3u) | ((b & 2u) * 6u);
+}
 __device__ __forceinline__ void next_cubelet(unsigned& rem, unsigned pa, unsigned pb, unsigned& oa, unsigned& ob) {
     asm volatile("{\n\t.reg .u32 t, u;\n\tbrev.b32 t, %0;\n\tclz.b32 t, t;\n\tshl.b32 t, t, 6;\n\tadd.u32 %1, %3, t;\n\tadd.u32 %2, %4, t;\n\t"
                  "add.u32 u, %0, -1;\n\tand.b32 %0, %0, u;\n\t}" : "+r"(rem), "=r"(oa), "=r"(ob) : "r"(pa), "r"(pb));
@@ -550,7 +567,7 @@ __device__ __forceinline__ void producer_loop(const Geom& g, TileSmem& S, int nc
         DBG_T(t_p1);
         DBG_ADD(10, t_p1 - t_p0);
 #ifndef GINT_DBG_NO_EVAL
-        eval_stage<VLOCAL>(g, S, s, c, 4 * ((pw + c) % GINT_EVAL_WARPS), tb, V);
+        eval_stage<VLOCAL>(g, S, s, c, (32 / GINT_CPTS) * ((pw + c) % GINT_EVAL_WARPS), tb, V);
 #endif
         __syncwarp();
         if ((threadIdx.x & 31) == 0) mbar_arrive(&S.full[s]);
@@ -597,15 +614,15 @@ k_vlocal_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bst
     }
 #ifdef GINT_DBG_STATS
     {   // developer statistics: DMMA balance over the four sub-partitions (whole tile, and stage by stage)
-        __shared__ int dbg_load[17][GINT_MMA_WARPS];
+        __shared__ int dbg_load[GINT_MAX_CHUNKS + 1][GINT_MMA_WARPS];
         int tot = 0;
         for (int c = 0; c < nchunk; c++) {
             int l = 0;
-            for (int k = 0; k < GINT_WARP_SEGS; k++) l += 2 * sg[k].n() * __popc((unsigned)(sg[k].W >> (4 * c)) & 15u);
+            for (int k = 0; k < GINT_WARP_SEGS; k++) l += 2 * sg[k].n() * __popc(stage_steps(sg[k].W, c));
             if (lane == 0) dbg_load[c][warp] = l;
             tot += l;
         }
-        if (lane == 0) dbg_load[16][warp] = tot;
+        if (lane == 0) dbg_load[GINT_MAX_CHUNKS][warp] = tot;
         {   // DMMAs needed at (row fragment, column fragment, cubelet) granularity, and with trailing-column cut per cubelet
             unsigned long long fine = 0, lead = 0;
             for (int k = 0; k < GINT_WARP_SEGS; k++) {
@@ -624,11 +641,11 @@ k_vlocal_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bst
         asm volatile("bar.sync 2, 256;" ::: "memory");
         if (threadIdx.x == 0) {
             unsigned long long sum = 0, mx_tile = 0, mx_chunk = 0;
-            for (int c = 0; c <= 16; c++) {
-                if (c < 16 && c >= nchunk) continue;
+            for (int c = 0; c <= GINT_MAX_CHUNKS; c++) {
+                if (c < GINT_MAX_CHUNKS && c >= nchunk) continue;
                 int m = 0, t = 0;
                 for (int q = 0; q < 4; q++) { const int v = dbg_load[c][q] + dbg_load[c][q + 4]; m = max(m, v); t += v; }
-                if (c == 16) { sum = t; mx_tile = 4ull * m; } else mx_chunk += 4ull * m;
+                if (c == GINT_MAX_CHUNKS) { sum = t; mx_tile = 4ull * m; } else mx_chunk += 4ull * m;
             }
             atomicAdd(&g_dbg[0], sum); atomicAdd(&g_dbg[1], mx_tile); atomicAdd(&g_dbg[2], mx_chunk); atomicAdd(&g_dbg[3], 1ull);
             atomicAdd(&g_dbg[4], (unsigned long long)nchunk);
@@ -648,7 +665,7 @@ k_vlocal_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bst
 #ifndef GINT_DBG_NO_MMA
 #pragma unroll
         for (int k = 0; k < GINT_WARP_SEGS; k++) {
-            const unsigned bits = (unsigned)(sg[k].W >> (4 * c)) & 15u;
+            const unsigned bits = stage_steps(sg[k].W, c);
             if (bits) vl_seg_dispatch(sg[k].n(), acc[k], base + sg[k].oa, base + sg[k].ob, bits);
         }
 #endif
@@ -791,7 +808,7 @@ k_rho_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart
         unsigned any = 0;
 #pragma unroll
         for (int k = 0; k < GINT_WARP_SEGS; k++) {
-            const unsigned bits = (unsigned)(sg[k].W >> (4 * c)) & 15u;
+            const unsigned bits = stage_steps(sg[k].W, c);
             any |= bits;
             if (bits) rho_seg_dispatch(sg[k].n(), d[k], lane_i + s * GINT_STAGEB + sg[k].oa, lane_j + s * GINT_STAGEB + sg[k].ob, bits, part);
         }

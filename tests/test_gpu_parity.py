@@ -64,7 +64,7 @@ def test_cfg0_nonsymmetric_D(torch_cuda):
     _full_parity(torch_cuda, W.make_workload(0), seed_extra=7)
 
 
-@pytest.mark.parametrize("shape", [(2, 2, 2), (3, 3, 5), (5, 2, 3), (1, 1, 1), (4, 2, 7)])
+@pytest.mark.parametrize("shape", [(2, 2, 2), (3, 3, 5), (5, 2, 3), (1, 1, 1), (4, 2, 7), (8, 8, 16), (3, 5, 13), (8, 8, 8)])
 def test_cfg0_batch_shapes(torch_cuda, shape):
     """Ragged edge batches (24 is not a multiple of 5 or 7) and other batch shapes give the same result."""
     from paper_2409_09399_b200.gint import batch_flag
