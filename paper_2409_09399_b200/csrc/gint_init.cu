@@ -148,7 +148,7 @@ __global__ void __launch_bounds__(256) k_batch_neighbours(Geom g, int cbx, int c
                                                           int* __restrict__ bgroups) {
     __shared__ int s_act[FILL ? 8 : 1][FILL ? GINT_MAX_NB : 1];
     __shared__ int s_img[FILL ? 8 : 1][FILL ? GINT_MAX_NB : 1];
-    __shared__ unsigned s_mlo[FILL ? 8 : 1][FILL ? GINT_MAX_NB : 1], s_mhi[FILL ? 8 : 1][FILL ? GINT_MAX_NB : 1];
+    __shared__ unsigned long long s_mlo[FILL ? 8 : 1][FILL ? GINT_MAX_NB : 1], s_mhi[FILL ? 8 : 1][FILL ? GINT_MAX_NB : 1];
     const int w = threadIdx.x >> 5;
     const long long b = (long long)blockIdx.x * 8 + w;
     const int lane = threadIdx.x & 31;
@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(256) k_batch_neighbours(Geom g, int cbx, int c
         const int qi = cand[(size_t)cell * cap + c];
         const ImageDev im = img[qi];
         int hits = 0;
-        unsigned mlo = 0, mhi = 0;
+        unsigned mw[4] = {0u, 0u, 0u, 0u};
         for (int q = lane; q < Kb; q += 32) {
             const int qk = q % ez, qj = (q / ez) % ey, qx = q / (ez * ey);
             double px, py, pz;
@@ -172,13 +172,20 @@ __global__ void __launch_bounds__(256) k_batch_neighbours(Geom g, int cbx, int c
             const double dx = px - im.x, dy = py - im.y, dz = pz - im.z;
             const bool in = fma(dx, dx, fma(dy, dy, dz * dz)) < im.rc * im.rc;    // same expression as the orbital evaluation
             hits += in;
-            if (FILL && in) { const int cl = (qx >> 1) * 16 + (qj >> 1) * 4 + qk / GINT_CZ; if (cl < 32) mlo |= 1u << cl; else mhi |= 1u << (cl - 32); }
+            if (FILL && in) {
+                const int cl = ((qx >> 1) * 4 + (qj >> 1)) * GINT_NCZ + qk / GINT_CZ;
+#pragma unroll
+                for (int wd = 0; wd < 4; wd++) if ((cl >> 5) == wd) mw[wd] |= 1u << (cl & 31);
+            }
         }
 #pragma unroll
         for (int d = 16; d; d >>= 1) hits += __shfl_xor_sync(0xffffffffu, hits, d);
-        if (FILL) { mlo = __reduce_or_sync(0xffffffffu, mlo); mhi = __reduce_or_sync(0xffffffffu, mhi); }
+        if (FILL) {
+#pragma unroll
+            for (int wd = 0; wd < 4; wd++) mw[wd] = __reduce_or_sync(0xffffffffu, mw[wd]);
+        }
         if (hits > 0) {
-            if (FILL && lane == 0 && n < GINT_MAX_NB) { s_act[w][n] = hits; s_img[w][n] = qi; s_mlo[w][n] = mlo; s_mhi[w][n] = mhi; }
+            if (FILL && lane == 0 && n < GINT_MAX_NB) { s_act[w][n] = hits; s_img[w][n] = qi; s_mlo[w][n] = (unsigned long long)mw[0] | ((unsigned long long)mw[1] << 32); s_mhi[w][n] = (unsigned long long)mw[2] | ((unsigned long long)mw[3] << 32); }
             n++;
             ncol += sp[spec[im.atom]].norb;
         }
@@ -195,7 +202,7 @@ __global__ void __launch_bounds__(256) k_batch_neighbours(Geom g, int cbx, int c
         for (int j = 0; j < n; j++) { const int aj = s_act[w][j]; rank += (aj > a) || (aj == a && j < e); }
         const ImageDev im = img[s_img[w][e]];
         bent[base + rank].atom = im.atom; bent[base + rank].shift = im.shift;
-        bent[base + rank].mask = (unsigned long long)s_mlo[w][e] | ((unsigned long long)s_mhi[w][e] << 32);
+        bent[base + rank].mask[0] = s_mlo[w][e]; bent[base + rank].mask[1] = s_mhi[w][e];
     }
     __syncwarp();
     if (lane == 0) {

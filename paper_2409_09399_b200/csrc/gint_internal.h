@@ -14,10 +14,12 @@
 #define GINT_MAX_NB 96             // neighbouring atom images per grid batch
 #define GINT_MAX_BS 8              // largest grid-batch edge along a1, a2 (points)
 #ifndef GINT_CZ
-#define GINT_CZ 4                  // cubelet = 2 x 2 x GINT_CZ mesh points; a batch is at most 4 x 4 x 4 cubelets = one 64-bit mask
+#define GINT_CZ 2                  // cubelet = 2 x 2 x GINT_CZ mesh points
+#define GINT_NCZ 8                 // a batch is at most 4 x 4 x GINT_NCZ cubelets: one 128-bit activity mask
 #endif
 #define GINT_CPTS (4 * GINT_CZ)    // points per cubelet (8 or 16)
-#define GINT_MAX_BSZ (4 * GINT_CZ) // largest grid-batch edge along a3
+#define GINT_NCUB (16 * GINT_NCZ)  // cubelets per batch (at most 128)
+#define GINT_MAX_BSZ (GINT_NCZ * GINT_CZ) // largest grid-batch edge along a3
 #define GINT_WARPS 16              // warps per CTA of the contraction kernels: 4 warp groups
 #define GINT_THREADS (32 * GINT_WARPS)
 #define GINT_MMA_WARPS 8           // warp groups 0,1: DMMA consumers (setmaxnreg.inc); warp groups 2,3: orbital-evaluation producers
@@ -40,7 +42,7 @@
 #define GINT_MAX_SEG (GINT_WARP_SEGS * GINT_MMA_WARPS)
 #define GINT_CHUNK 32              // mesh points per pipeline stage = 4 DMMA steps of 8 points
 #define GINT_CUBS (GINT_CHUNK / GINT_CPTS)      // cubelets per stage (4 or 2)
-#define GINT_MAX_CHUNKS (64 / GINT_CUBS)
+#define GINT_MAX_CHUNKS (GINT_NCUB / GINT_CUBS)
 #define GINT_LD 36                 // row stride (doubles) of the orbital tiles in shared memory: = 4 mod 16, the 64-bit fragment loads are conflict-free
 
 // ---- error plumbing -------------------------------------------------------------------------------
@@ -83,7 +85,7 @@ struct Geom {
 struct NeighEntry {
     int atom;
     int shift;                      // (t1+64) | (t2+64)<<8 | (t3+64)<<16
-    unsigned long long mask;        // bit (cx*16 + cy*4 + cz): cubelet (2x2x2 points) of the batch with a point inside the sphere
+    unsigned long long mask[2];     // bit ((cx*4 + cy)*GINT_NCZ + cz) of the 128: cubelet of the batch with a point inside the sphere
 };
 
 __host__ __device__ inline int pack_shift(int t1, int t2, int t3) { return (t1 + 64) | ((t2 + 64) << 8) | ((t3 + 64) << 16); }

@@ -1,8 +1,8 @@
 // gint_kernels.cu -- the per-call hot path (north_star steps 2 and 3), fp64, sm_100a.
 //
-// Work decomposition.  The mesh is cut into grid batches (default 8x8x8 points) whose neighbouring
-// atom images were listed by gint_init, most active first, each with a 64-bit ACTIVITY MASK over the
-// batch's 4x4x4 "cubelets" of 2x2x2 mesh points (bit set = some point of the cubelet lies inside the atom's cutoff
+// Work decomposition.  The mesh is cut into grid batches (default 8x8x16 points) whose neighbouring
+// atom images were listed by gint_init, most active first, each with a 128-bit ACTIVITY MASK over the
+// batch's 4x4x8 "cubelets" of 2x2x2 mesh points (bit set = some point of the cubelet lies inside the atom's cutoff
 // sphere; Fig. 6: everything else is zero padding).  The neighbours of a batch are split into G
 // groups of at most 8 atoms / 104 orbitals.  One CTA owns one TILE = (batch, group I, group J), I <= J: the
 // 104 x 104 block of Phi_I^T diag(V dV) Phi_J (gint_vlocal, Eq. 2) or of the density blocks D_IJ
@@ -20,6 +20,13 @@
 #include "gint_internal.h"
 
 typedef unsigned long long u64;
+// activity mask over the (at most 128) cubelets of a batch
+struct cmask { u64 lo, hi; };
+__device__ __forceinline__ cmask operator|(cmask a, cmask b) { return cmask{a.lo | b.lo, a.hi | b.hi}; }
+__device__ __forceinline__ cmask operator&(cmask a, cmask b) { return cmask{a.lo & b.lo, a.hi & b.hi}; }
+__device__ __forceinline__ cmask& operator|=(cmask& a, cmask b) { a.lo |= b.lo; a.hi |= b.hi; return a; }
+__device__ __forceinline__ bool cbit(const cmask& m, int i) { return ((i < 64 ? m.lo >> i : m.hi >> (i - 64)) & 1ull) != 0; }
+__device__ __forceinline__ cmask czero() { return cmask{0ull, 0ull}; }
 #ifndef GINT_DBG_STATS
 #define DBG_T(x)
 #define DBG_ADD(i, v)
@@ -52,25 +59,26 @@ struct TileSmem {
     // phi[stage][side][orbital row][GINT_LD]: side 0 = group I, side 1 = group J (scaled by V dV in vlocal);
     // column 8q + p = point p of the stage's q-th cubelet
     double phi[GINT_STAGES][2][GINT_TILE_ORB][GINT_LD];
-    double4 pts[64 * GINT_CPTS];                   // [cubelet id * 8 + p]: x, y, z of the batch's mesh points, weight V dV (vlocal) or 1 (rho);
+    double4 pts[GINT_NCUB * GINT_CPTS];                   // [cubelet id * 8 + p]: x, y, z of the batch's mesh points, weight V dV (vlocal) or 1 (rho);
                                         // points outside the mesh: far away, weight 0
     u64 full[GINT_STAGES], empty[GINT_STAGES];   // mbarriers: stage written by all producer warps / read by all consumer warps
     double pos[16][4];                  // slot s < 8: atom s of group I; slot 8 + s: atom s of group J
     SlotInfo sinfo[16];
-    u64 amask[16];                      // cubelets on which the slot's atom is non-zero
-    u64 need[16];                       // cubelets on which the slot's orbital rows are read by some segment
-    u64 fmask[2][16];                   // [side][fragment]: OR of amask over the atoms with orbitals in the fragment
-    u64 hmask[2];                       // side J: OR of fmask over the column fragments 0..6 / 7..12
-    u64 U;                              // cubelets the tile walks over: (any I fragment) & (any J fragment)
+    cmask amask[16];                      // cubelets on which the slot's atom is non-zero
+    cmask need[16];                       // cubelets on which the slot's orbital rows are read by some segment
+    cmask fmask[2][16];                   // [side][fragment]: OR of amask over the atoms with orbitals in the fragment
+    cmask hmask[2];                       // side J: OR of fmask over the column fragments 0..6 / 7..12
+    cmask U;                            // cubelets the tile walks over: (any I fragment) & (any J fragment)
     PairEnt pair[GINT_TILE_ATOMS][GINT_TILE_ATOMS];   // canonical block of (I atom a, J atom b)
     int atom[16], shift[16], spec[16];
     int cstart[2][GINT_TILE_ATOMS + 1]; // first orbital row of each atom inside its group
+    u64 segWhi[GINT_MAX_SEG];           // second half (list positions 64..127) of the segments' activity words
     int seg[GINT_MAX_SEG];              // slot (consumer warp) + 8 k: row fragment | first column fragment << 8 | n columns << 16
     int ncub;
     TileView tv;                        // written by tile_setup; read from here afterwards to keep registers free
     unsigned char item[GINT_MAX_CHUNKS][16 * GINT_CUBS];         // [stage][k]: slot << 2 | cubelet of the stage
     unsigned char nitem[GINT_MAX_CHUNKS], neval[GINT_MAX_CHUNKS]; // [stage]: items of the stage, of which the first neval need a real evaluation
-    unsigned char cub[64 + 4];          // the tile's cubelets (bit numbers of U, ascending)
+    unsigned char cub[GINT_NCUB + 4];          // the tile's cubelets (bit numbers of U, ascending)
     unsigned char row_atom[2][GINT_TILE_ORB];   // orbital row -> atom slot inside the group (255 = padding)
     unsigned char row_orb[2][GINT_TILE_ORB];    // orbital row -> orbital index inside the atom
     unsigned char frag_atoms[2][16];            // fragment -> bit mask of the atoms it holds orbitals of
@@ -108,6 +116,7 @@ __device__ __forceinline__ u64 warp_or64(u64 v) {
     const unsigned lo = __reduce_or_sync(0xffffffffu, (unsigned)v), hi = __reduce_or_sync(0xffffffffu, (unsigned)(v >> 32));
     return (u64)lo | ((u64)hi << 32);
 }
+__device__ __forceinline__ cmask warp_orc(cmask v) { return cmask{warp_or64(v.lo), warp_or64(v.hi)}; }
 __device__ __forceinline__ u64 shfl64(u64 v, int src) {
     const unsigned lo = __shfl_sync(0xffffffffu, (unsigned)v, src), hi = __shfl_sync(0xffffffffu, (unsigned)(v >> 32), src);
     return (u64)lo | ((u64)hi << 32);
@@ -119,7 +128,7 @@ __device__ __forceinline__ bool stage_point(const TileSmem& S, int c, int pt, in
     const int ci = GINT_CUBS * c + pt / GINT_CPTS, p = pt % GINT_CPTS;
     if (ci >= S.ncub) return false;
     const int cl = S.cub[ci];
-    const int ix = 2 * (cl >> 4) + p / (2 * GINT_CZ), iy = 2 * ((cl >> 2) & 3) + ((p / GINT_CZ) & 1), iz = GINT_CZ * (cl & 3) + p % GINT_CZ;
+    const int ix = 2 * (cl / (4 * GINT_NCZ)) + p / (2 * GINT_CZ), iy = 2 * ((cl / GINT_NCZ) & 3) + ((p / GINT_CZ) & 1), iz = GINT_CZ * (cl % GINT_NCZ) + p % GINT_CZ;
     gi = S.tv.i0 + ix; gj = S.tv.j0 + iy; gk = S.tv.k0 + iz;
     return ix < S.tv.ex && iy < S.tv.ey && iz < S.tv.ez;
 }
@@ -140,8 +149,8 @@ __device__ __forceinline__ void make_items(TileSmem& S, int c) {
         const int ci = GINT_CUBS * c + q;
         const bool inb = cand < 16 * GINT_CUBS && ci < S.ncub;
         const int cl = inb ? S.cub[ci] : 0;
-        need[r] = inb && ((S.need[slot & 15] >> cl) & 1ull);
-        act[r] = need[r] && ((S.amask[slot & 15] >> cl) & 1ull);
+        need[r] = inb && cbit(S.need[slot & 15], cl);
+        act[r] = need[r] && cbit(S.amask[slot & 15], cl);
         eb[r] = __ballot_sync(0xffffffffu, act[r]);
         zb[r] = __ballot_sync(0xffffffffu, need[r] && !act[r]);
         ne += __popc(eb[r]); nz += __popc(zb[r]);
@@ -184,7 +193,7 @@ __device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, int ps, i
             for (int o = 0; o < norb; o++) { o0[o * GINT_LD] = 0.0; if (two) o0[o * GINT_LD + GINT_TILE_ORB * GINT_LD] = 0.0; }
             continue;
         }
-        const double4 P = S.pts[GINT_CPTS * S.cub[min(GINT_CUBS * c + (it & 3), 63)] + lane % GINT_CPTS];
+        const double4 P = S.pts[GINT_CPTS * S.cub[min(GINT_CUBS * c + (it & 3), GINT_NCUB - 1)] + lane % GINT_CPTS];
         const double wv = P.w;
         const SlotInfo si = S.sinfo[slot];
         const double dx = P.x - S.pos[slot][0], dy = P.y - S.pos[slot][1], dz = P.z - S.pos[slot][2];
@@ -287,9 +296,9 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
     tv.nI = group_begin(tv.I + 1, n, tv.G) - eI;
     tv.nJ = group_begin(tv.J + 1, n, tv.G) - eJ;
 
-    for (int q = tid; q < 64 * GINT_CPTS; q += GINT_THREADS) {   // mesh points of the batch (V == nullptr: rho, weight 1)
+    for (int q = tid; q < GINT_NCUB * GINT_CPTS; q += GINT_THREADS) {   // mesh points of the batch (V == nullptr: rho, weight 1)
         const int cl = q / GINT_CPTS, pp = q % GINT_CPTS;
-        const int ix = 2 * (cl >> 4) + pp / (2 * GINT_CZ), iy = 2 * ((cl >> 2) & 3) + ((pp / GINT_CZ) & 1), iz = GINT_CZ * (cl & 3) + pp % GINT_CZ;
+        const int ix = 2 * (cl / (4 * GINT_NCZ)) + pp / (2 * GINT_CZ), iy = 2 * ((cl / GINT_NCZ) & 3) + ((pp / GINT_CZ) & 1), iz = GINT_CZ * (cl % GINT_NCZ) + pp % GINT_CZ;
         double4 P = make_double4(1e30, 0.0, 0.0, 0.0);
         if (ix < tv.ex && iy < tv.ey && iz < tv.ez) {
             const int gi = tv.i0 + ix, gj = tv.j0 + iy, gk = tv.k0 + iz;
@@ -303,11 +312,11 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
         const bool valid = a < (side ? tv.nJ : tv.nI);
         int atom = 0, shift = pack_shift(0, 0, 0), spec = 0;
         double x = 0, y = 0, z = 0;
-        u64 m = 0;
+        cmask m = czero();
         if (valid) {
             const NeighEntry e = bent[e0 + (side ? eJ : eI) + a];
             int t1, t2, t3; unpack_shift(e.shift, t1, t2, t3);
-            atom = e.atom; shift = e.shift; spec = atom_spec[atom]; m = e.mask;
+            atom = e.atom; shift = e.shift; spec = atom_spec[atom]; m = cmask{e.mask[0], e.mask[1]};
             x = atom_pos[3 * atom + 0] + t1 * g.a[0] + t2 * g.a[3] + t3 * g.a[6];
             y = atom_pos[3 * atom + 1] + t1 * g.a[1] + t2 * g.a[4] + t3 * g.a[7];
             z = atom_pos[3 * atom + 2] + t1 * g.a[2] + t2 * g.a[5] + t3 * g.a[8];
@@ -343,7 +352,7 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
     } else if (tid < 2 * GINT_TILE_ORB + 32) {
         const int q = tid - 2 * GINT_TILE_ORB, side = q >> 4, f = q & 15;
         unsigned m = 0;
-        u64 fm = 0;
+        cmask fm = czero();
         for (int k = 0; k < GINT_TILE_ATOMS; k++)
             if (S.cstart[side][k] < 8 * f + 8 && S.cstart[side][k + 1] > 8 * f) { m |= 1u << k; fm |= S.amask[8 * side + k]; }
         S.frag_atoms[side][f] = (unsigned char)m;
@@ -388,28 +397,33 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
     DBG_T(ts3);
     if (warp == 0 || warp == 2) {
         // union masks (both warps), then warp 0: cubelet list; warp 2: per-slot read sets
-        const u64 vI = lane < tv.nfI ? S.fmask[0][lane] : 0ull;
-        const u64 vJ = lane < tv.nfJ ? S.fmask[1][lane] : 0ull;
-        const u64 anyI = warp_or64(vI);
-        const u64 h0 = warp_or64(lane < GINT_SEG_COLS ? vJ : 0ull) & anyI, h1 = warp_or64(lane >= GINT_SEG_COLS ? vJ : 0ull) & anyI;
-        const u64 U = h0 | h1;
+        const cmask vI = lane < tv.nfI ? S.fmask[0][lane] : czero();
+        const cmask vJ = lane < tv.nfJ ? S.fmask[1][lane] : czero();
+        const cmask anyI = warp_orc(vI);
+        const cmask h0 = warp_orc(lane < GINT_SEG_COLS ? vJ : czero()) & anyI, h1 = warp_orc(lane >= GINT_SEG_COLS ? vJ : czero()) & anyI;
+        const cmask U = h0 | h1;
         if (warp == 0) {
-            const unsigned Ulo = (unsigned)U, Uhi = (unsigned)(U >> 32), lt = (1u << lane) - 1u;
-            if ((Ulo >> lane) & 1u) S.cub[__popc(Ulo & lt)] = (unsigned char)lane;
-            if ((Uhi >> lane) & 1u) S.cub[__popc(Ulo) + __popc(Uhi & lt)] = (unsigned char)(32 + lane);
-            const int ncub = __popc(Ulo) + __popc(Uhi);
+            const unsigned Uw[4] = {(unsigned)U.lo, (unsigned)(U.lo >> 32), (unsigned)U.hi, (unsigned)(U.hi >> 32)};
+            const unsigned lt = (1u << lane) - 1u;
+            int before = 0;
+#pragma unroll
+            for (int wd = 0; wd < 4; wd++) {
+                if ((Uw[wd] >> lane) & 1u) S.cub[before + __popc(Uw[wd] & lt)] = (unsigned char)(32 * wd + lane);
+                before += __popc(Uw[wd]);
+            }
+            const int ncub = before;
             if (lane < 4) S.cub[ncub + lane] = 0;
             if (lane == 0) { S.U = U; S.hmask[0] = h0; S.hmask[1] = h1; S.ncub = ncub; }
         } else {
-            u64 m = 0;
+            cmask m = czero();
             if (lane < 16) {
                 const int side = lane >> 3, a = lane & 7;
                 const int nf = side ? tv.nfJ : tv.nfI;
                 for (int f = 0; f < nf; f++)
                     if ((S.frag_atoms[side][f] >> a) & 1) m |= side ? (f < GINT_SEG_COLS ? h0 : h1) : (S.fmask[0][f] & U);
             }
-            const u64 mj = shfl64(m, (lane + 8) & 31);
-            if (tv.diag) m = lane < 8 ? (m | mj) : 0ull;      // the atoms are evaluated once, for both sides
+            const cmask mj = cmask{shfl64(m.lo, (lane + 8) & 31), shfl64(m.hi, (lane + 8) & 31)};
+            if (tv.diag) m = lane < 8 ? (m | mj) : czero();      // the atoms are evaluated once, for both sides
             if (lane < 16) S.need[lane] = m;
         }
     } else if (warp == 1) {
@@ -472,28 +486,29 @@ struct Seg {
     __device__ __forceinline__ int cb() const { return (w >> 8) & 255; }
     __device__ __forceinline__ int n() const { return w >> 16; }
 };
-__device__ __forceinline__ Seg load_seg(const TileSmem& S, int slot, bool j_is_i = false) {   // j_is_i: column operands from side I (rho, diagonal tile)
+__device__ __forceinline__ Seg load_seg(TileSmem& S, int slot, bool j_is_i = false) {   // j_is_i: column operands from side I (rho, diagonal tile)
     const int lane = threadIdx.x & 31;
     Seg s; s.w = S.seg[slot];
-    u64 cm = 0;
+    cmask cm = czero();
     for (int j = 0; j < s.n(); j++) cm |= S.fmask[1][s.cb() + j];
-    const u64 act = s.n() ? (S.fmask[0][s.row()] & cm) : 0ull;     // cubelets on which the row fragment and some column fragment are active
-    const bool b0 = lane < S.ncub && ((act >> S.cub[lane]) & 1ull), b1 = lane + 32 < S.ncub && ((act >> S.cub[(lane + 32) & 63]) & 1ull);
-    s.W = (u64)__ballot_sync(0xffffffffu, b0) | ((u64)__ballot_sync(0xffffffffu, b1) << 32);
+    const cmask act = s.n() ? (S.fmask[0][s.row()] & cm) : czero();     // cubelets on which the row fragment and some column fragment are active
+    unsigned wb[4];
+#pragma unroll
+    for (int wd = 0; wd < 4; wd++) {
+        const int pp = 32 * wd + lane;
+        wb[wd] = __ballot_sync(0xffffffffu, pp < S.ncub && cbit(act, S.cub[min(pp, GINT_NCUB - 1)]));
+    }
+    s.W = (u64)wb[0] | ((u64)wb[1] << 32);
+    if (lane == 0) S.segWhi[slot] = (u64)wb[2] | ((u64)wb[3] << 32);      // list positions 64..127: fetched when the tile gets there
+    __syncwarp();
     s.oa = (unsigned)(s.row() * 8 * GINT_ROWB);
     s.ob = (unsigned)((j_is_i ? 0 : GINT_SIDEB) + s.cb() * 8 * GINT_ROWB);
     return s;
 }
 
-// vlocal: acc[j] += Phi_I[row fragment]^T-slice x (V dV Phi_J)[column fragment cb + j] over the 8 points of every
-// active cubelet of the stage.  The two DMMA k-steps of a cubelet (points 0..3, points 4..7) use separate operand
-// registers X and Y: while the Y DMMAs issue, the X operands of the segment's next active cubelet are loaded, and
-// vice versa, so the shared-memory latency is hidden behind the FP64 tensor pipe.
-// next active cubelet of a segment: q = lowest set bit of rem (removed from rem), operand addresses pa/pb + 64 q.
-// One volatile asm block, so that it stays where it is written: in the shadow of the DMMAs.
 // activity of a segment on the 8-point DMMA steps of stage c (a 16-point cubelet is two steps)
 __device__ __forceinline__ unsigned stage_steps(u64 W, int c) {
-    const unsigned b = (unsigned)(W >> (GINT_CUBS * c)) & ((1u << GINT_CUBS) - 1u);
+    const unsigned b = (unsigned)(W >> ((GINT_CUBS * c) & 63)) & ((1u << GINT_CUBS) - 1u);
     return GINT_CPTS == 8 ? b : ((b & 1u) * 3u) | ((b & 2u) * 6u);
 }
 __device__ __forceinline__ void next_cubelet(unsigned& rem, unsigned pa, unsigned pb, unsigned& oa, unsigned& ob) {
@@ -626,13 +641,13 @@ k_vlocal_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bst
         {   // DMMAs needed at (row fragment, column fragment, cubelet) granularity, and with trailing-column cut per cubelet
             unsigned long long fine = 0, lead = 0;
             for (int k = 0; k < GINT_WARP_SEGS; k++) {
-                const u64 rm = S.fmask[0][sg[k].row()] & S.U;
-                u64 seen = 0;
+                const cmask rm = S.fmask[0][sg[k].row()] & S.U;
+                cmask seen = czero();
                 for (int j = sg[k].n() - 1; j >= 0; j--) {
-                    const u64 cm = S.fmask[1][sg[k].cb() + j] & rm;
-                    fine += 2 * __popcll(cm);
+                    const cmask cm = S.fmask[1][sg[k].cb() + j] & rm;
+                    fine += 2 * (__popcll(cm.lo) + __popcll(cm.hi));
                     seen |= cm;
-                    lead += 2 * __popcll(seen);      // columns 0..j computed wherever some column >= j is active
+                    lead += 2 * (__popcll(seen.lo) + __popcll(seen.hi));      // columns 0..j computed wherever some column >= j is active
                 }
             }
             if (sg[0].n() == 0) { fine = 0; lead = 0; }
@@ -657,6 +672,10 @@ k_vlocal_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bst
     asm volatile("" : "+r"(lane_off));
     for (int c = 0; c < nchunk; c++) {
         const int s = c % GINT_STAGES;
+        if (c == 64 / GINT_CUBS) {      // the activity words cover 64 list positions: switch to the second half
+#pragma unroll
+            for (int k = 0; k < GINT_WARP_SEGS; k++) sg[k].W = S.segWhi[warp + GINT_MMA_WARPS * k];
+        }
         DBG_T(t_w0);
         mbar_wait(&S.full[s], (c / GINT_STAGES) & 1);
         DBG_T(t_w1);
@@ -679,7 +698,7 @@ k_vlocal_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bst
     // key is (b, a)).  Exact zeros (fragments never touched, atoms that do not overlap inside this batch) are skipped.
 #pragma unroll
     for (int k = 0; k < GINT_WARP_SEGS; k++) {
-        if (sg[k].n() == 0 || sg[k].W == 0ull) continue;
+        if (sg[k].n() == 0) continue;
         const int row = 8 * sg[k].row() + lr;
         const int a = S.row_atom[0][row], oa = S.row_orb[0][row];
         if (a == 255) continue;
@@ -801,6 +820,10 @@ k_rho_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart
     asm volatile("" : "+r"(lane_i), "+r"(lane_j));
     for (int c = 0; c < nchunk; c++) {
         const int s = c % GINT_STAGES;
+        if (c == 64 / GINT_CUBS) {      // the activity words cover 64 list positions: switch to the second half
+#pragma unroll
+            for (int k = 0; k < GINT_WARP_SEGS; k++) sg[k].W = S.segWhi[warp + GINT_MMA_WARPS * k];
+        }
         double part[4][2];
 #pragma unroll
         for (int q = 0; q < 4; q++) { part[q][0] = 0.0; part[q][1] = 0.0; }
