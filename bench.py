@@ -38,8 +38,8 @@ def alg_flops(st: dict) -> float:
 
 
 def ncu_traffic(cfg: int, kernel: str):
-    """DRAM bytes (read + write) of one launch of `kernel` from the committed ncu capture (profiles/r1g_traffic.csv), or None."""
-    path = os.path.join(ROOT, "profiles", "r1g_traffic.csv")
+    """DRAM bytes (read + write) of one launch of `kernel` from the committed ncu capture (profiles/r1h_traffic.csv), or None."""
+    path = os.path.join(ROOT, "profiles", "r1h_traffic.csv")
     try:
         with open(path) as f:
             for ln in f.read().splitlines()[1:]:
@@ -311,7 +311,7 @@ def main():
             "identity_P4_rel": p4,
             "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                          "frac": achieved / FP64_PEAK_TFLOPS, "traffic": ncu_traffic(args.cfg, dom),
-                         "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1g_final_kernels.md)",
+                         "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1h_final_kernels.md)",
                          "peak_source": "148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md; DMMA micro-benchmark reaches 37.1)",
                          "kernel_ms": {k: 1e3 * v for k, v in kt.items()},
                          "hbm_context": {"achieved": hbm_achieved, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_achieved / hbm_peak,
