@@ -11,6 +11,8 @@ None of these tests calls the CUDA path.  Each pin is independent of the oracle'
   P6  brute force on 2 atoms in a skew cell with self-images: numpy loops over every mesh point x every
       image in a fixed +-3 shell, radial part by scipy.interpolate.CubicSpline (clamped), angular part
       from scipy.special.sph_harm_y -- no lists, no lens boxes, no code shared with the oracle
+  P6b the same brute force on a skew 3-atom cell with TWO species that differ in rc, in the number of knots
+      and in their shell sets (s,p,d / s,s,p): pins the per-species table offsets and shell look-ups
   P7  invariances: translation by one mesh step, atom permutation, linearity in V and D
   P9  pair counts against a KD-tree count; lexicographic key order
   Y   real spherical harmonics: orthonormal under Gauss-Legendre x uniform-phi quadrature
@@ -62,7 +64,7 @@ def brute_phi(basis, species, d):
         l = int(basis.shell_l[sh0 + s])
         y = basis.tab_y[tab0 + s * nk: tab0 + (s + 1) * nk]
         # end slopes of the analytic functions: R'(0) = N delta_{l,1} (y[1]/dr to O(dr^2) for l=1), R'(rc) = 0
-        d0 = basis.norm[s] if (l == 1 and basis.norm) else 0.0
+        d0 = basis.norm[sh0 + s] if (l == 1 and basis.norm) else 0.0
         cs = CubicSpline(knots, y, bc_type=((1, d0), (1, 0.0)))
         R = np.where(inside, cs(np.minimum(r, rc)), 0.0)
         for ylm in real_ylm_scipy(l, ux, uy, uz):
@@ -319,6 +321,77 @@ def test_P6_brute_force_rho(skew):
     sel = np.array([0, 7, 1234, w.n_points - 1], np.int64)
     part = O.rho(w, D, pl, sel=sel)
     assert np.array_equal(part[sel], rho[sel]) and np.count_nonzero(part) <= len(sel)
+
+
+# ----------------------------------------------------------------------------- P6b brute force, two species
+def two_species_workload():
+    """Skew cell, 3 atoms, species 0 = (s,p,d) with rc 3.0 (301 knots), species 1 = (s,s,p) with rc 2.5 (251 knots):
+    different cutoffs, table lengths, shell sets and orbital counts (9 / 5); atoms outside the home cell; self images."""
+    b0 = W.make_basis(3.0, shells=((0, 0.7), (1, 0.5), (2, 0.45)))
+    b1 = W.make_basis(2.5, shells=((0, 0.9), (0, 0.3), (1, 0.6)))
+    basis = W.Basis(2, np.array([3, 3], np.int32), np.concatenate([b0.shell_l, b1.shell_l]), np.array([3.0, 2.5]), W.DR,
+                    np.concatenate([b0.n_knot, b1.n_knot]), np.concatenate([b0.tab_y, b1.tab_y]),
+                    np.concatenate([b0.tab_y2, b1.tab_y2]), norm=b0.norm + b1.norm)
+    cell = np.array([[4.9, 0.2, 0.0], [1.3, 4.4, 0.1], [0.3, -0.6, 5.1]])
+    pos = np.array([[0.2, 0.4, 0.5], [2.6, 2.9, 3.1], [6.3, -0.8, 4.0]])
+    return W.Workload("skew-3-two-species", 96, cell, np.array([12, 11, 13], np.int32), np.array([0, 1, 1], np.int32), pos, basis)
+
+
+@pytest.fixture(scope="module")
+def skew2():
+    w = two_species_workload()
+    S_ = 3
+    pts = mesh_points(w)
+    Phi = {}
+    for A in range(w.n_atoms):
+        for t in itertools.product(range(-S_, S_ + 1), repeat=3):
+            v = brute_phi(w.basis, int(w.atom_species[A]), pts - w.atom_pos[A] - np.array(t) @ w.cell)
+            if np.any(v != 0.0):
+                Phi[(A, t)] = v
+    return dict(w=w, Phi=Phi, keys=brute_pairs(w, S_))
+
+
+def test_P6b_two_species_phi_and_pairs(skew2):
+    w = skew2["w"]
+    assert w.basis.norb == [9, 5] and list(w.basis.n_knot) == [301, 251]
+    rng = np.random.default_rng(31)
+    for sp in (0, 1):
+        for _ in range(40):
+            d = rng.normal(size=3) * 1.2
+            assert np.allclose(O.phi(w.basis, sp, d), brute_phi(w.basis, sp, d), rtol=0, atol=1e-12)
+    A, B, R, off = O.pairs(w)
+    got = [(int(a), int(b), int(r[0]), int(r[1]), int(r[2])) for a, b, r in zip(A, B, R)]
+    assert got == skew2["keys"]
+    no = np.array(w.basis.norb)[w.atom_species]
+    assert np.array_equal(np.diff(off), no[A] * no[B])
+    assert {(int(a), int(b)) for a, b in zip(w.atom_species[A], w.atom_species[B])} == {(0, 0), (0, 1), (1, 0), (1, 1)}
+
+
+def test_P6b_two_species_brute_force_H_and_rho(skew2):
+    w, Phi, keys = skew2["w"], skew2["Phi"], skew2["keys"]
+    pl = O.pairs(w)
+    off = pl[3]
+    no = np.array(w.basis.norb)[w.atom_species]
+    rng = np.random.default_rng(32)
+    V = rng.normal(size=w.n_points)
+    D = rng.normal(size=int(off[-1]))                        # every ordered block independent
+    H = O.vlocal(w, V, pl)
+    rho = O.rho(w, D, pl)
+    Href = np.zeros_like(H)
+    rref = np.zeros(w.n_points)
+    for p, (A, B, n1, n2, n3) in enumerate(keys):
+        blk = np.zeros((no[A], no[B]))
+        Dp = D[off[p]:off[p + 1]].reshape(no[A], no[B])
+        for (A2, t), pa in Phi.items():
+            if A2 != A:
+                continue
+            pb = Phi.get((B, (t[0] + n1, t[1] + n2, t[2] + n3)))
+            if pb is not None:
+                blk += pa.T @ (V[:, None] * pb)
+                rref += ((pa @ Dp) * pb).sum(1)
+        Href[off[p]:off[p + 1]] = (blk * dV(w)).ravel()
+    assert np.abs(H - Href).max() <= 1e-12 * np.abs(Href).max()
+    assert np.abs(rho - rref).max() <= 1e-12 * np.abs(rref).max()
 
 
 # ----------------------------------------------------------------------------- P7 invariances
