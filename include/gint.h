@@ -125,11 +125,17 @@ enum {
     GINT_STAT_ALG_SUM_N = 11,     /* sum_g n_g,   n_g = orbitals non-zero at g                              */
     GINT_STAT_ALG_SUM_N2 = 12,    /* sum_g n_g^2                                                            */
     GINT_STAT_NONEMPTY_POINTS = 13,
-    GINT_STAT_SMEM_BYTES = 14,    /* dynamic shared memory of the contraction kernels                       */
+    GINT_STAT_SMEM_BYTES = 14,    /* dynamic shared memory of the contraction kernels (TMA ring + tile contexts) */
     GINT_STAT_DEVICE_BYTES = 15,  /* device memory owned by the context                                     */
     GINT_STAT_LAUNCHES_VLOCAL = 16, /* kernels one gint_vlocal call launches (memsets not counted)          */
     GINT_STAT_LAUNCHES_RHO = 17,  /* kernels one gint_rho call launches                                     */
-    GINT_N_STATS = 18
+    GINT_STAT_SMEM_EVAL = 18,     /* dynamic shared memory of the orbital-evaluation kernel                 */
+    GINT_STAT_TAB_IN_SMEM = 19,   /* 1: the evaluation kernel reads the radial table from shared memory     */
+    GINT_STAT_PHI_BYTES = 20,     /* orbital values one call evaluates and writes (all waves), bytes        */
+    GINT_STAT_PHI_SCRATCH_BYTES = 21, /* size of the context's orbital-value scratch buffer (one wave)      */
+    GINT_STAT_N_WAVES = 22,       /* waves (evaluate + contract launches) per call                          */
+    GINT_STAT_N_TILES = 23,       /* (batch, group pair) tiles per call                                     */
+    GINT_N_STATS = 24
 };
 int gint_stats(gint_ctx* ctx, long long* out);
 

@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdarg>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -310,7 +311,8 @@ static void free_ctx(gint_ctx* c) {
     cudaFree(c->d_species); cudaFree(c->d_tab); cudaFree(c->d_atom_pos); cudaFree(c->d_atom_species);
     cudaFree(c->d_poff); cudaFree(c->d_pcanon); cudaFree(c->d_pflag); cudaFree(c->d_pnA);
     cudaFree(c->d_crow); cudaFree(c->d_ckey); cudaFree(c->d_coff); cudaFree(c->d_cpub); cudaFree(c->d_cmir); cudaFree(c->d_cval);
-    cudaFree(c->d_bstart); cudaFree(c->d_bent); cudaFree(c->d_tile);
+    cudaFree(c->d_bstart); cudaFree(c->d_bent); cudaFree(c->d_tile); cudaFree(c->d_tstart); cudaFree(c->d_gstart);
+    cudaFree(c->d_goff); cudaFree(c->d_phi); cudaFree(c->d_queue);
     cudaFree(c->d_stage_in); cudaFree(c->d_stage_out);
     for (auto& e : c->ev) if (e) cudaEventDestroy(e);
     delete c;
@@ -461,7 +463,7 @@ static int build_pairs(gint_ctx* c) {
 // ---- step a2: grid batches and their neighbour lists ------------------------------------------------------
 // Tries one batch shape: fills geom.bs/nb/K/LD/max_cols/max_nb and the CSR neighbour table.  Returns
 // GINT_ERR_UNSUPPORTED (without message) when the orbital tile of the largest batch does not fit in `smem_limit`.
-static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, bool* fits) {
+static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, size_t phi_cap, bool* fits) {
     Geom& g = c->geom;
     *fits = false;
     for (int i = 0; i < 3; i++) { g.bs[i] = std::min(bs[i], g.N[i]); g.nb[i] = (g.N[i] + g.bs[i] - 1) / g.bs[i]; }
@@ -491,9 +493,7 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, bool* 
             if (!ok) continue;
             if (std::abs(t1) > 60 || std::abs(t2) > 60 || std::abs(t3) > 60) GINT_FAIL(GINT_ERR_UNSUPPORTED, "atom %d lies more than 60 cells away from the home cell", A);
             ImageDev im;
-            im.x = p[0] + t1 * g.a[0] + t2 * g.a[3] + t3 * g.a[6];
-            im.y = p[1] + t1 * g.a[1] + t2 * g.a[4] + t3 * g.a[7];
-            im.z = p[2] + t1 * g.a[2] + t2 * g.a[5] + t3 * g.a[8];
+            image_pos(g, p, t1, t2, t3, im.x, im.y, im.z);      // the same fma chain as on the device
             im.rc = rc; im.atom = A; im.shift = pack_shift(t1, t2, t3);
             img.push_back(im);
         }
@@ -545,25 +545,29 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, bool* 
     if ((rc = device_excl_scan(d_count, nbt, c->d_bstart, &n_ent))) return rc;
     c->n_entries = n_ent;
     if ((rc = dev_alloc(c, &c->d_bent, (size_t)n_ent))) return rc;
-    int *d_bgroups = nullptr, *d_tcount = nullptr, *d_tstart = nullptr;
+    int *d_bgroups = nullptr, *d_tcount = nullptr;
     GINT_CUDA(cudaMalloc(&d_bgroups, sizeof(int) * nbt));
     GINT_CUDA(cudaMalloc(&d_tcount, sizeof(int) * nbt));
-    GINT_CUDA(cudaMalloc(&d_tstart, sizeof(int) * (nbt + 1)));
+    if ((rc = dev_alloc(c, &c->d_tstart, (size_t)nbt + 1))) return rc;
+    if ((rc = dev_alloc(c, &c->d_gstart, (size_t)nbt + 1))) return rc;
     k_batch_neighbours<true><<<gridB, 256>>>(g, cb[0], cb[1], cb[2], nc[1], nc[2], d_img, cap, d_cand, d_ccount, nbt, d_count, d_cols,
                                              c->d_species, c->d_atom_species, c->d_bstart, c->d_bent, d_bgroups);
     GINT_CUDA(cudaGetLastError());
     const unsigned gridT = (unsigned)((nbt + 255) / 256);
     k_tiles_count<<<gridT, 256>>>(nbt, d_bgroups, d_tcount);
     GINT_CUDA(cudaGetLastError());
-    long long n_tiles = 0;
-    if ((rc = device_excl_scan(d_tcount, nbt, d_tstart, &n_tiles))) return rc;
+    long long n_tiles = 0, n_groups = 0;
+    if ((rc = device_excl_scan(d_tcount, nbt, c->d_tstart, &n_tiles))) return rc;
+    if ((rc = device_excl_scan(d_bgroups, nbt, c->d_gstart, &n_groups))) return rc;
     c->n_tiles = n_tiles;
     if ((rc = dev_alloc(c, &c->d_tile, (size_t)n_tiles))) return rc;
-    k_tiles_fill<<<gridT, 256>>>(nbt, d_bgroups, d_tstart, c->d_tile);
+    k_tiles_fill<<<gridT, 256>>>(nbt, d_bgroups, c->d_tstart, c->d_tile);
     GINT_CUDA(cudaGetLastError());
     GINT_CUDA(cudaDeviceSynchronize());
     cudaFree(d_img); cudaFree(d_cand); cudaFree(d_ccount); cudaFree(d_count); cudaFree(d_cols);
-    cudaFree(d_bgroups); cudaFree(d_tcount); cudaFree(d_tstart);
+    cudaFree(d_bgroups); cudaFree(d_tcount);
+    // orbital-value ("Phi") layout: offsets of every (batch, group) slot array, waves, scratch buffer
+    if ((rc = gint_build_phi_layout(c, nullptr, phi_cap))) return rc;
 
     c->padded_macs = 0; c->n_batch = 0;
     for (long long b = 0; b < nbt; b++) {
@@ -628,24 +632,29 @@ extern "C" int gint_init(gint_ctx** out, int n_species, const int* n_shell, cons
     if ((rc = build_pairs(c))) { free_ctx(c); return rc; }
 
     const size_t smem_limit = prop.sharedMemPerBlockOptin;
+    // scratch for the orbital values of one wave of batches: at most 16 GiB and a quarter of the free device memory
+    size_t mem_free = 0, mem_total = 0;
+    GINT_CUDA(cudaMemGetInfo(&mem_free, &mem_total));
+    size_t phi_cap = std::min<size_t>((size_t)16 << 30, mem_free / 4);
+    if (const char* e = getenv("GINT_PHI_CAP_MB")) { const long long mb = atoll(e); if (mb > 0) phi_cap = (size_t)mb << 20; }   // developer knob (tests use it to force several waves)
     const int fx = (int)(flags & 255), fy = (int)((flags >> 8) & 255), fz = (int)((flags >> 16) & 255);
     bool fits = false;
     if (fx || fy || fz) {
         const int bs[3] = {fx ? fx : 8, fy ? fy : 8, fz ? fz : 8};
-        if ((rc = build_batches(c, bs, smem_limit, &fits))) { free_ctx(c); return rc; }
+        if ((rc = build_batches(c, bs, smem_limit, phi_cap, &fits))) { free_ctx(c); return rc; }
         if (!fits) { free_ctx(c); GINT_FAIL(GINT_ERR_UNSUPPORTED, "requested batch %dx%dx%d needs more shared memory than %zu bytes (or > %d neighbours)", bs[0], bs[1], bs[2], smem_limit, GINT_MAX_NB); }
     } else {
         static const int shapes[][3] = {{8, 8, GINT_MAX_BSZ}, {8, 8, 8}, {4, 4, 8}, {4, 4, 4}, {2, 2, 4}, {1, 1, 4}, {1, 1, 1}};
         for (auto& s : shapes) {
-            if ((rc = build_batches(c, s, smem_limit, &fits))) { free_ctx(c); return rc; }
+            if ((rc = build_batches(c, s, smem_limit, phi_cap, &fits))) { free_ctx(c); return rc; }
             if (fits) break;
         }
         if (!fits) { free_ctx(c); GINT_FAIL(GINT_ERR_UNSUPPORTED, "even a 1-point batch does not fit: too many overlapping atoms"); }
     }
     c->smem_bytes = gint_smem_needed(c, smem_limit);
     if ((rc = gint_configure_kernels(c))) { free_ctx(c); return rc; }
-    for (auto& e : c->ev) GINT_CUDA(cudaEventCreate(&e));
-    GINT_CUDA(cudaDeviceSynchronize());
+    for (auto& e : c->ev) if (cudaEventCreate(&e) != cudaSuccess) { free_ctx(c); GINT_FAIL(GINT_ERR_CUDA, "cudaEventCreate failed"); }
+    if (cudaDeviceSynchronize() != cudaSuccess) { free_ctx(c); GINT_FAIL(GINT_ERR_CUDA, "gint_init: device error %s", cudaGetErrorString(cudaGetLastError())); }
     *out = c;
     return GINT_OK;
 }
@@ -691,7 +700,10 @@ extern "C" int gint_stats(gint_ctx* ctx, long long* out) {
     out[GINT_STAT_ALG_INCIDENCE] = ctx->alg[0]; out[GINT_STAT_ALG_SUM_N] = ctx->alg[1]; out[GINT_STAT_ALG_SUM_N2] = ctx->alg[2];
     out[GINT_STAT_NONEMPTY_POINTS] = ctx->alg[3];
     out[GINT_STAT_SMEM_BYTES] = (long long)ctx->smem_bytes; out[GINT_STAT_DEVICE_BYTES] = (long long)ctx->device_bytes;
-    out[GINT_STAT_LAUNCHES_VLOCAL] = 2; out[GINT_STAT_LAUNCHES_RHO] = 2;
+    out[GINT_STAT_LAUNCHES_VLOCAL] = 1 + 2 * (long long)ctx->waves.size(); out[GINT_STAT_LAUNCHES_RHO] = 1 + 2 * (long long)ctx->waves.size();
+    out[GINT_STAT_SMEM_EVAL] = (long long)ctx->smem_eval; out[GINT_STAT_TAB_IN_SMEM] = ctx->tab_in_smem ? 1 : 0;
+    out[GINT_STAT_PHI_BYTES] = (long long)(ctx->phi_rows_total * GINT_ROW_BYTES); out[GINT_STAT_PHI_SCRATCH_BYTES] = (long long)ctx->phi_bytes;
+    out[GINT_STAT_N_WAVES] = (long long)ctx->waves.size(); out[GINT_STAT_N_TILES] = ctx->n_tiles;
     return GINT_OK;
 }
 

@@ -12,38 +12,36 @@
 
 #define GINT_MAX_SHELL 12          // radial shells per species
 #define GINT_MAX_NB 96             // neighbouring atom images per grid batch
+#define GINT_MAX_GROUPS 32         // atom groups per batch (96 atoms of <= 32 orbitals in groups of <= 104 orbitals)
 #define GINT_MAX_BS 8              // largest grid-batch edge along a1, a2 (points)
-#ifndef GINT_CZ
-#define GINT_CZ 2                  // cubelet = 2 x 2 x GINT_CZ mesh points
+#define GINT_CZ 2                  // cubelet = 2 x 2 x 2 mesh points = the 8 columns of one DMMA operand pair
 #define GINT_NCZ 8                 // a batch is at most 4 x 4 x GINT_NCZ cubelets: one 128-bit activity mask
-#endif
-#define GINT_CPTS (4 * GINT_CZ)    // points per cubelet (8 or 16)
+#define GINT_CPTS 8                // points per cubelet
 #define GINT_NCUB (16 * GINT_NCZ)  // cubelets per batch (at most 128)
 #define GINT_MAX_BSZ (GINT_NCZ * GINT_CZ) // largest grid-batch edge along a3
-#define GINT_WARPS 16              // warps per CTA of the contraction kernels: 4 warp groups
-#define GINT_THREADS (32 * GINT_WARPS)
-#define GINT_MMA_WARPS 8           // warp groups 0,1: DMMA consumers (setmaxnreg.inc); warp groups 2,3: orbital-evaluation producers
-#define GINT_EVAL_WARPS (GINT_WARPS - GINT_MMA_WARPS)
-#ifndef GINT_REGS_MMA
-#define GINT_REGS_MMA 168          // registers per thread after setmaxnreg: 256 * 168 + 256 * 88 = 65536
-#define GINT_REGS_EVAL 88
-#endif
-#ifndef GINT_REGS_MMA_RHO
-#define GINT_REGS_MMA_RHO 184      // gint_rho: its consumers are the bottleneck and its producers have slack (measured: 168/88 93.6 ms, 184/72 91.8 ms at cfg3)
-#define GINT_REGS_EVAL_RHO 72
-#endif
-#define GINT_STAGES 2              // shared-memory ring of orbital-value stages between producers and consumers
-// tile geometry of the contraction kernels: one CTA owns the block of H (or D) between two groups of atoms
+// tile geometry of the contraction kernels: one tile = the block of H (or D) between two groups of atoms of one batch
 #define GINT_TILE_ATOMS 8          // atom images per group
 #define GINT_TILE_ORB 104          // orbitals per group = 13 fragments of 8 (8 atoms x 13 orbitals exactly)
 #define GINT_TILE_FRAG 13
 #define GINT_SEG_COLS 7            // column fragments of one segment (row fragment x <= 7 column fragments)
 #define GINT_WARP_SEGS 4           // segments per consumer warp
+#define GINT_MMA_WARPS 8           // warp groups 0,1: DMMA consumers
 #define GINT_MAX_SEG (GINT_WARP_SEGS * GINT_MMA_WARPS)
-#define GINT_CHUNK 32              // mesh points per pipeline stage = 4 DMMA steps of 8 points
-#define GINT_CUBS (GINT_CHUNK / GINT_CPTS)      // cubelets per stage (4 or 2)
-#define GINT_MAX_CHUNKS (GINT_NCUB / GINT_CUBS)
-#define GINT_LD 36                 // row stride (doubles) of the orbital tiles in shared memory: = 4 mod 16, the 64-bit fragment loads are conflict-free
+#define GINT_AUX_WARPS 4           // warp group 2: warp 8 = TMA issuer (+ rho reducer), warps 9..11 = tile set-up
+#define GINT_SETUP_THREADS 96
+#define GINT_CTA_THREADS (32 * (GINT_MMA_WARPS + GINT_AUX_WARPS))
+#define GINT_REGS_MMA 224          // registers per thread after setmaxnreg: 256 * 224 + 128 * 56 = 64512 <= 65536
+#define GINT_REGS_AUX 56
+// orbital values ("Phi") in global memory: one SLOT per (atom group, active cubelet) = [orbital row][8 points] doubles,
+// rows padded to whole fragments; 64 bytes per row = the unit of all Phi offsets
+#define GINT_ROW_BYTES 64
+#define GINT_SLOT_MAX_BYTES (GINT_TILE_ORB * GINT_ROW_BYTES)   // 6656
+// shared-memory ring of the contraction kernels: a stage = GINT_SC cubelets x (slot of group I, slot of group J)
+#define GINT_SC 2
+#define GINT_NS 6
+#define GINT_STAGE_BYTES (GINT_SC * 2 * GINT_SLOT_MAX_BYTES)   // 26624
+#define GINT_NCTX 3                // tile contexts in flight per CTA (set-up runs ahead of the TMA issuer, which runs ahead of the consumers)
+#define GINT_EVAL_THREADS 256      // orbital-evaluation kernel
 
 // ---- error plumbing -------------------------------------------------------------------------------
 void gint_set_error(const char* fmt, ...);
@@ -102,6 +100,15 @@ __host__ __device__ inline void mesh_point(const Geom& g, int i, int j, int k, d
     z = fma(w, g.step[8], fma(v, g.step[5], u * g.step[2]));
 }
 
+// Position of atom image (A, t): tau_A + t1 a1 + t2 a2 + t3 a3, with explicit fma so that host and device agree bit by bit
+// (the neighbour pass, the activity masks and the orbital evaluation all take the |d| < rc decision on these numbers).
+__host__ __device__ inline void image_pos(const Geom& g, const double* p, int t1, int t2, int t3, double& x, double& y, double& z) {
+    const double u = (double)t1, v = (double)t2, w = (double)t3;
+    x = fma(w, g.a[6], fma(v, g.a[3], fma(u, g.a[0], p[0])));
+    y = fma(w, g.a[7], fma(v, g.a[4], fma(u, g.a[1], p[1])));
+    z = fma(w, g.a[8], fma(v, g.a[5], fma(u, g.a[2], p[2])));
+}
+
 struct gint_ctx {
     int device = 0;
     Geom geom{};
@@ -142,8 +149,20 @@ struct gint_ctx {
     int* d_order = nullptr;          // [n_batch_total] batch ids: non-empty first (mesh order), then empty ones
     long long n_tiles = 0;
     int2* d_tile = nullptr;          // [n_tiles] {batch id, I | J<<8 | G<<16}: group pair (I <= J) of G groups of the batch
+    int* d_tstart = nullptr;         // [n_batch_total+1] first tile of each batch
+    int* d_gstart = nullptr;         // [n_batch_total+1] first atom group of each batch (CSR into d_goff)
+    unsigned long long* d_goff = nullptr; // [sum G] Phi offset (rows of 64 bytes, whole mesh) of each (batch, group) slot array
+    // waves: contiguous batch ranges whose orbital values fit the Phi scratch buffer
+    struct Wave { long long b0, b1, t0, t1; unsigned long long row0, rows; };
+    std::vector<Wave> waves;
+    double* d_phi = nullptr;         // Phi scratch of one wave
+    size_t phi_bytes = 0;
+    unsigned long long phi_rows_total = 0;
+    int* d_queue = nullptr;          // [waves] tile-queue heads
+    int n_sm = 0;
     long long padded_macs = 0;
-    size_t smem_bytes = 0;
+    size_t smem_bytes = 0;           // contraction kernels
+    size_t smem_eval = 0;            // evaluation kernel
     size_t device_bytes = 0;
     // lazily computed statistics
     bool have_alg = false;
@@ -162,6 +181,7 @@ int gint_launch_rho(gint_ctx* c, const double* D, double* rho, cudaStream_t st);
 int gint_launch_alg_stats(gint_ctx* c);
 int gint_configure_kernels(gint_ctx* c);
 size_t gint_smem_needed(gint_ctx* c, size_t limit);   // also decides tab_in_smem
+int gint_build_phi_layout(gint_ctx* c, const int* d_bgroups, size_t phi_cap_bytes);   // Phi offsets of every (batch, group), waves, scratch
 
 // Split of the n neighbour entries of a batch into G groups of consecutive entries: group k = [k*n/G, (k+1)*n/G).
 __host__ __device__ inline int group_begin(int k, int n, int G) { return (int)(((long long)k * n) / G); }

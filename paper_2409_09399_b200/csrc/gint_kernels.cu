@@ -4,19 +4,28 @@
 // atom images were listed by gint_init, most active first, each with a 128-bit ACTIVITY MASK over the
 // batch's 4x4x8 "cubelets" of 2x2x2 mesh points (bit set = some point of the cubelet lies inside the atom's cutoff
 // sphere; Fig. 6: everything else is zero padding).  The neighbours of a batch are split into G
-// groups of at most 8 atoms / 104 orbitals.  One CTA owns one TILE = (batch, group I, group J), I <= J: the
-// 104 x 104 block of Phi_I^T diag(V dV) Phi_J (gint_vlocal, Eq. 2) or of the density blocks D_IJ
-// (gint_rho, Eq. 3).  That block stays in REGISTERS (DMMA accumulators, resp. stationary DMMA
-// operands): the 13 x 13 fragments (8 x 8 orbitals) of the block are cut into SEGMENTS of one row fragment x up to
-// 7 column fragments, four segments per consumer warp, dealt to the 8 consumer warps so that the four SM sub-partitions carry equal
-// numbers of DMMAs; in a diagonal tile (I == J) only the fragments on or above the atom diagonal are segments.
-// The CTA walks over the cubelets on which both groups are active, 4 cubelets (32 points) per pipeline stage: the
-// orbital values of the needed (atom, cubelet) items are evaluated into shared memory (the paper's orbital-value
-// kernel, never written to global memory; items compacted so that a quarter warp = one atom on one
-// cubelet), then every warp runs the DMMA chains (mma.sync m8n8k4 f64 = DMMA.8x8x4) of its segments on the cubelets
-// where the segment is active -- straight-line code specialised on the segment length, one bit test per cubelet.
-// Only one of each mirror pair of blocks, (A,B,n) / (B,A,-n), is accumulated ("canonical half"); small
-// streaming kernels convert between the public pair-list layout and the canonical layout.
+// groups of at most 8 atoms / 104 orbitals = 13 FRAGMENTS of 8 orbital rows.
+//
+// Step 2 (k_eval_phi, the paper's orbital-value kernel): every (batch, atom, active cubelet) is
+// evaluated exactly ONCE per call into a "Phi" scratch buffer laid out as the contraction kernels read it: one SLOT
+// per (atom group, cubelet on which the group is active) = [orbital row][8 points] doubles.  The scratch holds one
+// WAVE of batches (a few GB; re-read through L2 by the tiles that follow immediately).
+//
+// Step 3 (k_vlocal_tiles / k_rho_tiles): persistent CTAs, one per SM, pull TILES = (batch, group I, group J), I <= J,
+// from a queue in batch order (tiles sharing a group run at the same time on different SMs, so their slots hit L2).
+// Per CTA three roles run decoupled through mbarriers:
+//   * set-up warps (9..11) prepare the next tiles' contexts (atom slots, canonical block of every atom pair, the list of
+//     cubelets on which both groups are active with per-cubelet fragment activity, the segment plan, V dV weights);
+//   * the issuer warp (8) streams the slots of the tile's cubelets into a shared-memory ring with TMA bulk copies
+//     (cp.async.bulk, complete_tx on the stage's mbarrier) and, in gint_rho, reduces the consumers' partial densities;
+//   * 8 consumer warps (setmaxnreg 232) keep the 104 x 104 block of Phi_I^T diag(V dV) Phi_J (gint_vlocal, Eq. 2
+//     PAPER.md:66) or of the density blocks D_IJ (gint_rho, Eq. 3) in REGISTERS as DMMA accumulators /
+//     stationary operands: the 13 x 13 fragments are cut into SEGMENTS of one row fragment x up to 7 column
+//     fragments, four per warp, dealt so that the four SM sub-partitions carry equal numbers of DMMAs.  Per cubelet a
+//     segment issues mma.sync.m8n8k4.f64 (DMMA.8x8x4) only for the (row fragment, column fragment) pairs that are
+//     both active there: one R2P sets seven predicates from the activity word, loads and DMMAs are predicated.
+// Only one of each mirror pair of blocks, (A,B,n) / (B,A,-n), is accumulated ("canonical half"); small streaming
+// kernels convert between the public pair-list layout and the canonical layout.
 #include "gint_internal.h"
 
 typedef unsigned long long u64;
@@ -27,6 +36,25 @@ __device__ __forceinline__ cmask operator&(cmask a, cmask b) { return cmask{a.lo
 __device__ __forceinline__ cmask& operator|=(cmask& a, cmask b) { a.lo |= b.lo; a.hi |= b.hi; return a; }
 __device__ __forceinline__ bool cbit(const cmask& m, int i) { return ((i < 64 ? m.lo >> i : m.hi >> (i - 64)) & 1ull) != 0; }
 __device__ __forceinline__ cmask czero() { return cmask{0ull, 0ull}; }
+__device__ __forceinline__ int ccount(const cmask& m) { return __popcll(m.lo) + __popcll(m.hi); }
+// number of set bits below bit i
+__device__ __forceinline__ int crank(const cmask& m, int i) {
+    return i < 64 ? __popcll(m.lo & ((1ull << i) - 1ull)) : __popcll(m.lo) + __popcll(m.hi & ((1ull << (i - 64)) - 1ull));
+}
+// position of the i-th set bit (i < ccount(m))
+__device__ __forceinline__ int cselect(const cmask& m, int i) {
+    const unsigned w0 = (unsigned)m.lo, w1 = (unsigned)(m.lo >> 32), w2 = (unsigned)m.hi, w3 = (unsigned)(m.hi >> 32);
+    const int c0 = __popc(w0), c1 = c0 + __popc(w1), c2 = c1 + __popc(w2);
+    const int k = (i >= c0) + (i >= c1) + (i >= c2);
+    const unsigned w = k == 0 ? w0 : (k == 1 ? w1 : (k == 2 ? w2 : w3));
+    const int skip = k == 0 ? 0 : (k == 1 ? c0 : (k == 2 ? c1 : c2));
+    return 32 * k + (int)__fns(w, 0, i - skip + 1);
+}
+// cubelet id -> first point of the cubelet inside the batch; point p of a cubelet = (px, py, pz) bits
+__device__ __forceinline__ void cubelet_point(int cl, int p, int& ix, int& iy, int& iz) {
+    ix = 2 * (cl / (4 * GINT_NCZ)) + (p >> 2); iy = 2 * ((cl / GINT_NCZ) & 3) + ((p >> 1) & 1); iz = GINT_CZ * (cl % GINT_NCZ) + (p & 1);
+}
+
 #ifndef GINT_DBG_STATS
 #define DBG_T(x)
 #define DBG_ADD(i, v)
@@ -35,192 +63,146 @@ __device__ unsigned long long g_dbg[16];
 #define DBG_T(x) const long long x = clock64()
 #define DBG_ADD(i, v) do { if ((threadIdx.x & 31) == 0) atomicAdd(&g_dbg[i], (unsigned long long)(v)); } while (0)
 extern "C" int gint_debug_counters(unsigned long long* out) { return (int)cudaMemcpyFromSymbol(out, g_dbg, sizeof(g_dbg)); }
-#endif
-#ifndef GINT_EVAL_GROUP
-#define GINT_EVAL_GROUP 5          // radial shells whose spline cells are loaded together (registers vs memory-level parallelism)
-#define GINT_EVAL_GROUP_RHO 2      // gint_rho's producers run with 72 registers: measured 91.9 ms (5), 88.6 (3), 87.9 (2) at cfg3
+extern "C" int gint_debug_reset() { unsigned long long z[16] = {0}; return (int)cudaMemcpyToSymbol(g_dbg, z, sizeof(z)); }
 #endif
 
 // ---------------------------------------------------------------------------------------------------
-// shared memory of the tile kernels
-struct PairEnt { unsigned off; unsigned short sr, sc; };   // element (oa, ob) of the atom pair at off + oa*sr + ob*sc; off = ~0u: none
-struct SlotInfo { double rc2; int n_int, nsh, tab_off, lpack; };   // lpack: 2 bits of l per shell
-
-struct TileView {
-    int b, I, J, G;                  // batch, groups
-    int i0, j0, k0, ex, ey, ez;      // batch origin and extents (mesh points)
-    int nchunk;                      // stages of 4 cubelets
-    int nI, nJ;                      // atoms in the two groups
-    int nfI, nfJ;                    // fragments (8 orbitals) in the two groups
-    bool diag;
-};
-
-struct TileSmem {
-    // phi[stage][side][orbital row][GINT_LD]: side 0 = group I, side 1 = group J (scaled by V dV in vlocal);
-    // column 8q + p = point p of the stage's q-th cubelet
-    double phi[GINT_STAGES][2][GINT_TILE_ORB][GINT_LD];
-    double4 pts[GINT_NCUB * GINT_CPTS];                   // [cubelet id * 8 + p]: x, y, z of the batch's mesh points, weight V dV (vlocal) or 1 (rho);
-                                        // points outside the mesh: far away, weight 0
-    u64 full[GINT_STAGES], empty[GINT_STAGES];   // mbarriers: stage written by all producer warps / read by all consumer warps
-    double pos[16][4];                  // slot s < 8: atom s of group I; slot 8 + s: atom s of group J
-    SlotInfo sinfo[16];
-    cmask amask[16];                      // cubelets on which the slot's atom is non-zero
-    cmask need[16];                       // cubelets on which the slot's orbital rows are read by some segment
-    cmask fmask[2][16];                   // [side][fragment]: OR of amask over the atoms with orbitals in the fragment
-    cmask hmask[2];                       // side J: OR of fmask over the column fragments 0..6 / 7..12
-    cmask U;                            // cubelets the tile walks over: (any I fragment) & (any J fragment)
-    PairEnt pair[GINT_TILE_ATOMS][GINT_TILE_ATOMS];   // canonical block of (I atom a, J atom b)
-    int atom[16], shift[16], spec[16];
-    int cstart[2][GINT_TILE_ATOMS + 1]; // first orbital row of each atom inside its group
-    u64 segWhi[GINT_MAX_SEG];           // second half (list positions 64..127) of the segments' activity words
-    int seg[GINT_MAX_SEG];              // slot (consumer warp) + 8 k: row fragment | first column fragment << 8 | n columns << 16
-    int ncub;
-    TileView tv;                        // written by tile_setup; read from here afterwards to keep registers free
-    unsigned char item[GINT_MAX_CHUNKS][16 * GINT_CUBS];         // [stage][k]: slot << 2 | cubelet of the stage
-    unsigned char nitem[GINT_MAX_CHUNKS], neval[GINT_MAX_CHUNKS]; // [stage]: items of the stage, of which the first neval need a real evaluation
-    unsigned char cub[GINT_NCUB + 4];          // the tile's cubelets (bit numbers of U, ascending)
-    unsigned char row_atom[2][GINT_TILE_ORB];   // orbital row -> atom slot inside the group (255 = padding)
-    unsigned char row_orb[2][GINT_TILE_ORB];    // orbital row -> orbital index inside the atom
-    unsigned char frag_atoms[2][16];            // fragment -> bit mask of the atoms it holds orbitals of
-};
-// the radial table follows the struct in dynamic shared memory when it fits
-#define GINT_SMEM_TAB_OFF ((sizeof(TileSmem) + 15) & ~(size_t)15)
-size_t gint_smem_needed(gint_ctx* c, size_t limit) {
-    c->tab_in_smem = GINT_SMEM_TAB_OFF + c->tab_bytes <= limit;
-    return GINT_SMEM_TAB_OFF + (c->tab_in_smem ? c->tab_bytes : 0);
-}
-
-// The DMMA chains and their operand loads are volatile asm: left to itself the compiler sinks every shared load to
-// just before its DMMA (one operand register, fully serialised LDS -> DMMA -> LDS ...) and pairs the two k-steps of
-// an accumulator back to back.  Volatile asm keeps the written order: all loads of a cubelet, then the DMMAs.
-__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};" : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
-}
+// PTX helpers
 __device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ double2 lds128(unsigned addr) {
-    double2 v;
-    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory");
-    return v;
-}
-__device__ __forceinline__ double lds64(unsigned addr) {
-    double v;
-    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr) : "memory");
-    return v;
-}
-
-
 __device__ __forceinline__ void mbar_init(u64* bar, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_addr(bar)), "r"(count) : "memory");
 }
-__device__ __forceinline__ u64 warp_or64(u64 v) {
-    const unsigned lo = __reduce_or_sync(0xffffffffu, (unsigned)v), hi = __reduce_or_sync(0xffffffffu, (unsigned)(v >> 32));
-    return (u64)lo | ((u64)hi << 32);
+__device__ __forceinline__ void mbar_arrive(u64* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(smem_addr(bar)) : "memory");
 }
-__device__ __forceinline__ cmask warp_orc(cmask v) { return cmask{warp_or64(v.lo), warp_or64(v.hi)}; }
-__device__ __forceinline__ u64 shfl64(u64 v, int src) {
-    const unsigned lo = __shfl_sync(0xffffffffu, (unsigned)v, src), hi = __shfl_sync(0xffffffffu, (unsigned)(v >> 32), src);
-    return (u64)lo | ((u64)hi << 32);
+__device__ __forceinline__ void mbar_expect_tx(u64* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(smem_addr(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_wait(u64* bar, int parity) {
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
+                 :: "r"(smem_addr(bar)), "r"(parity) : "memory");
+}
+// TMA bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP.S.G)
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, u64* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(dst), "l"(src), "r"(bytes), "r"(smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void setup_sync() { asm volatile("bar.sync 1, %0;" :: "n"(GINT_SETUP_THREADS) : "memory"); }
 
 // ---------------------------------------------------------------------------------------------------
-// Stage c of a tile = its cubelets 4c .. 4c+3; point index 8 q + p: point p = (px, py, pz) bits of the q-th cubelet.
-__device__ __forceinline__ bool stage_point(const TileSmem& S, int c, int pt, int& gi, int& gj, int& gk) {
-    const int ci = GINT_CUBS * c + pt / GINT_CPTS, p = pt % GINT_CPTS;
-    if (ci >= S.ncub) return false;
-    const int cl = S.cub[ci];
-    const int ix = 2 * (cl / (4 * GINT_NCZ)) + p / (2 * GINT_CZ), iy = 2 * ((cl / GINT_NCZ) & 3) + ((p / GINT_CZ) & 1), iz = GINT_CZ * (cl % GINT_NCZ) + p % GINT_CZ;
-    gi = S.tv.i0 + ix; gj = S.tv.j0 + iy; gk = S.tv.k0 + iz;
-    return ix < S.tv.ex && iy < S.tv.ey && iz < S.tv.ez;
-}
+// Step 2: orbital evaluation, once per (batch, atom, active cubelet).
+// phi = R_s(|d|) Y_lm(d/|d|), zero for |d| >= rc (Fig. 6); radial part (reading R5):
+// R = a y_i + b y_{i+1} + (a^3-a) z_i + (b^3-b) z_{i+1} from the knot cells {y, z} of the interval, read with 128-bit
+// loads from the shared-memory copy of the table when it fits.  A quarter warp = one (atom, cubelet) item, lane = point.
+struct EvalSmem {
+    double pos[GINT_MAX_NB][4];             // image position, rc^2
+    cmask amask[GINT_MAX_NB];
+    int tab_off[GINT_MAX_NB], n_int[GINT_MAX_NB], nsh[GINT_MAX_NB], lpack[GINT_MAX_NB];
+    int row0[GINT_MAX_NB], norb[GINT_MAX_NB], grp[GINT_MAX_NB];
+    int item0[GINT_MAX_NB + 1];             // prefix sums of the atoms' active cubelets
+    int zitem0[GINT_MAX_NB + 1];            // prefix sums of the atoms' (group slot) pairs
+    cmask gmask[GINT_MAX_GROUPS];
+    u64 gbase[GINT_MAX_GROUPS];             // first row of the group's slot array in the wave's Phi scratch
+    int gR[GINT_MAX_GROUPS], gfirst[GINT_MAX_GROUPS], gcnt[GINT_MAX_GROUPS], gns[GINT_MAX_GROUPS];
+};
+#define GINT_EVAL_TAB_OFF ((sizeof(EvalSmem) + 15) & ~(size_t)15)
 
-// Item list of stage c (tile set-up, one warp per stage).  An item is (atom slot, cubelet of the stage) whose orbital
-// rows some segment reads on that cubelet: first the items on which the atom is really non-zero (evaluated), then
-// those that only need zeros.
-__device__ __forceinline__ void make_items(TileSmem& S, int c) {
-    const int lane = threadIdx.x & 31;
-    // candidates (slot, cubelet of the stage): 16 * GINT_CUBS of them, NR per lane
-    constexpr int NR = (16 * GINT_CUBS + 31) / 32;
-    bool act[NR], need[NR];
-    unsigned eb[NR], zb[NR];
-    int ne = 0, nz = 0;
+template <bool TAB_SMEM>
+__global__ void __launch_bounds__(GINT_EVAL_THREADS)
+k_eval_phi(Geom g, long long b0, const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
+           const int* __restrict__ gstart, const u64* __restrict__ goff, u64 wave_row0,
+           const double* __restrict__ atom_pos, const int* __restrict__ atom_spec, const SpeciesDev* __restrict__ sp,
+           const double* __restrict__ tab, int tab_cells, double* __restrict__ phi) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    EvalSmem& S = *reinterpret_cast<EvalSmem*>(smem_raw);
+    const long long b = b0 + blockIdx.x;
+    const int e0 = bstart[b], n = bstart[b + 1] - e0;
+    if (n == 0) return;
+    const int tid = threadIdx.x;
+    const int G = gstart[b + 1] - gstart[b];
+    if (TAB_SMEM) {
+        const double2* src = reinterpret_cast<const double2*>(tab);
+        double2* dst = reinterpret_cast<double2*>(smem_raw + GINT_EVAL_TAB_OFF);
+        for (int i0 = tid; i0 < tab_cells; i0 += 8 * GINT_EVAL_THREADS) {
+            double2 tmp[8];
 #pragma unroll
-    for (int r = 0; r < NR; r++) {
-        const int cand = lane + 32 * r, slot = cand / GINT_CUBS, q = cand % GINT_CUBS;
-        const int ci = GINT_CUBS * c + q;
-        const bool inb = cand < 16 * GINT_CUBS && ci < S.ncub;
-        const int cl = inb ? S.cub[ci] : 0;
-        need[r] = inb && cbit(S.need[slot & 15], cl);
-        act[r] = need[r] && cbit(S.amask[slot & 15], cl);
-        eb[r] = __ballot_sync(0xffffffffu, act[r]);
-        zb[r] = __ballot_sync(0xffffffffu, need[r] && !act[r]);
-        ne += __popc(eb[r]); nz += __popc(zb[r]);
-    }
-    const unsigned lt = (1u << lane) - 1u;
-    int pe = 0, pz = ne;
+            for (int u = 0; u < 8; u++) if (i0 + u * GINT_EVAL_THREADS < tab_cells) tmp[u] = __ldg(src + i0 + u * GINT_EVAL_THREADS);
 #pragma unroll
-    for (int r = 0; r < NR; r++) {
-        const int cand = lane + 32 * r;
-        const unsigned char code = (unsigned char)(((cand / GINT_CUBS) << 2) | (cand % GINT_CUBS));
-        if (act[r]) S.item[c][pe + __popc(eb[r] & lt)] = code;
-        else if (need[r]) S.item[c][pz + __popc(zb[r] & lt)] = code;
-        pe += __popc(eb[r]); pz += __popc(zb[r]);
-    }
-    if (lane == 0) { S.neval[c] = (unsigned char)ne; S.nitem[c] = (unsigned char)(ne + nz); }
-}
-
-// ---------------------------------------------------------------------------------------------------
-// Orbital evaluation of one stage by one producer warp (north_star step 2): a quarter warp = one item, lane p = point
-// p of the cubelet.  phi = R_s(|d|) Y_lm(d/|d|), zero for |d| >= rc (Fig. 6); radial part
-// (reading R5): R = a y_i + b y_{i+1} + (a^3-a) z_i + (b^3-b) z_{i+1} from the knot cells {y, z} of the interval,
-// read with 128-bit loads (from the shared-memory copy of the table when it fits).  vlocal scales side J by V dV.
-// A diagonal tile evaluates each atom once and writes both sides.  `first`: this warp's first item of the stage.
-template <bool VLOCAL>
-__device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, int ps, int c, int first, const double2* __restrict__ tab,
-                                           const double* __restrict__ V) {
-    const int lane = threadIdx.x & 31;
-    constexpr int GROUP = VLOCAL ? GINT_EVAL_GROUP : GINT_EVAL_GROUP_RHO;
-    const int nitem = S.nitem[c], neval = S.neval[c];
-    const bool two = VLOCAL && S.tv.diag;      // gint_rho reads side I twice in a diagonal tile instead
-    for (int base = first; base < nitem; base += (32 / GINT_CPTS) * GINT_EVAL_WARPS) {
-        const int idx = base + lane / GINT_CPTS;
-        const bool on = idx < nitem;
-        const int it = on ? S.item[c][idx] : 0;
-        const int slot = it >> 2, pt = GINT_CPTS * (it & 3) + lane % GINT_CPTS;
-        const int side = slot >> 3, a = slot & 7;
-        double* o0 = &S.phi[ps][side][S.cstart[side][a]][pt];
-        if (base >= neval) {                        // the four items only need zeros
-            const int norb = on ? S.cstart[side][a + 1] - S.cstart[side][a] : 0;
-            for (int o = 0; o < norb; o++) { o0[o * GINT_LD] = 0.0; if (two) o0[o * GINT_LD + GINT_TILE_ORB * GINT_LD] = 0.0; }
-            continue;
+            for (int u = 0; u < 8; u++) if (i0 + u * GINT_EVAL_THREADS < tab_cells) dst[i0 + u * GINT_EVAL_THREADS] = tmp[u];
         }
-        const double4 P = S.pts[GINT_CPTS * S.cub[min(GINT_CUBS * c + (it & 3), GINT_NCUB - 1)] + lane % GINT_CPTS];
-        const double wv = P.w;
-        const SlotInfo si = S.sinfo[slot];
-        const double dx = P.x - S.pos[slot][0], dy = P.y - S.pos[slot][1], dz = P.z - S.pos[slot][2];
+    }
+    const int bz = (int)(b % g.nb[2]), by = (int)((b / g.nb[2]) % g.nb[1]), bx = (int)(b / ((long long)g.nb[2] * g.nb[1]));
+    const int i0 = bx * g.bs[0], j0 = by * g.bs[1], k0 = bz * g.bs[2];
+    if (tid < n) {
+        const NeighEntry e = bent[e0 + tid];
+        int t1, t2, t3; unpack_shift(e.shift, t1, t2, t3);
+        double x, y, z;
+        image_pos(g, atom_pos + 3 * e.atom, t1, t2, t3, x, y, z);
+        const SpeciesDev* Sp = sp + atom_spec[e.atom];
+        S.pos[tid][0] = x; S.pos[tid][1] = y; S.pos[tid][2] = z; S.pos[tid][3] = Sp->rc * Sp->rc;
+        S.amask[tid] = cmask{e.mask[0], e.mask[1]};
+        S.tab_off[tid] = Sp->tab_off; S.n_int[tid] = Sp->n_int; S.nsh[tid] = Sp->n_shell; S.norb[tid] = Sp->norb;
+        int lp = 0;
+        for (int k = 0; k < Sp->n_shell; k++) lp |= Sp->l[k] << (2 * k);
+        S.lpack[tid] = lp;
+    }
+    __syncthreads();
+    if (tid < G) {      // one thread per group: entry range, rows, union mask
+        const int k = tid, f = group_begin(k, n, G), l = group_begin(k + 1, n, G);
+        cmask m = czero();
+        int rows = 0;
+        for (int e = f; e < l; e++) { m |= S.amask[e]; S.row0[e] = rows; S.grp[e] = k; rows += S.norb[e]; }
+        S.gmask[k] = m; S.gfirst[k] = f; S.gcnt[k] = l - f; S.gR[k] = (rows + 7) & ~7; S.gns[k] = ccount(m);
+        S.gbase[k] = goff[gstart[b] + k] - wave_row0;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        int a = 0, z = 0;
+        for (int e = 0; e < n; e++) { S.item0[e] = a; S.zitem0[e] = z; a += ccount(S.amask[e]); z += S.gns[S.grp[e]]; }
+        S.item0[n] = a; S.zitem0[n] = z;
+    }
+    __syncthreads();
+    const double2* tb = TAB_SMEM ? reinterpret_cast<const double2*>(smem_raw + GINT_EVAL_TAB_OFF) : reinterpret_cast<const double2*>(tab);
+    const int qw = tid >> 3, pl = tid & 7;
+    // ---- pass A: the active (atom, cubelet) items, compacted: every quarter warp evaluates one
+    const int n_items = S.item0[n];
+    for (int it0 = 0; it0 < n_items; it0 += GINT_EVAL_THREADS / 8) {
+        const int it = it0 + qw;
+        const bool on = it < n_items;
+        int e = 0;
+        if (on) {       // entry of the item: last e with item0[e] <= it
+            int lo = 0, hi = n - 1;
+            while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (S.item0[mid] <= it) lo = mid; else hi = mid - 1; }
+            e = lo;
+        }
+        const int k = S.grp[e];
+        const int cl = on ? cselect(S.amask[e], it - S.item0[e]) : 0;
+        const int slot = crank(S.gmask[k], cl);
+        int ix, iy, iz; cubelet_point(cl, pl, ix, iy, iz);
+        double px, py, pz;
+        mesh_point(g, i0 + ix, j0 + iy, k0 + iz, px, py, pz);
+        const double dx = px - S.pos[e][0], dy = py - S.pos[e][1], dz = pz - S.pos[e][2];
+        const double rc2 = S.pos[e][3];
         const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-        const bool inside = on && idx < neval && r2 < si.rc2;
+        const bool inside = on && r2 < rc2;
         // 1/r by one Newton step from the single-precision reciprocal square root: relative error 2.4e-7 -> 1.5 e^2 = 9e-14,
-        // three orders below the 1e-10 parity bar (a second step would cost four more dependent FP64 operations)
-        const double q = fmin(fmax(r2, 1e-30), si.rc2);
+        // three orders below the 1e-10 parity bar
+        const double q = fmin(fmax(r2, 1e-30), rc2);
         double ir = (double)rsqrtf((float)q);
         ir = ir * fma(-0.5 * q, ir * ir, 1.5);
         const double r = q * ir;
-        const int nsh = on ? si.nsh : 0;
+        const int nsh = on ? S.nsh[e] : 0;
         const double x = r * g.inv_dr;
         int i = (int)x;
-        i = min(i, si.n_int - 1);
-        const double b = x - (double)i, am = 1.0 - b;
-        const double a3 = (am * am - 1.0) * am, b3 = (b * b - 1.0) * b;
-        const double2* row = tab + (si.tab_off + i * si.nsh);
+        i = min(i, S.n_int[e] - 1);
+        const double bb = x - (double)i, am = 1.0 - bb;
+        const double a3 = (am * am - 1.0) * am, b3 = (bb * bb - 1.0) * bb;
+        const double2* row = tb + (S.tab_off[e] + i * nsh);
         const bool tiny = r < 1e-12;
         if (tiny) ir = 0.0;
         // lanes outside the sphere run the same instructions on a clamped radius and store zeros
-        const double w0 = inside ? ((VLOCAL && side) ? wv : 1.0) : 0.0;
-        const double w1 = inside ? wv : 0.0;
+        const double w0 = inside ? 1.0 : 0.0;
         const double ux = dx * ir, uy = dy * ir, uz = dz * ir;
-        // Angular factors times the store weight, all independent of the radial values: the FP64 pipe is shared with the
-        // consumers' DMMAs, under which a DEPENDENT FP64 operation costs ~25 cycles but independent ones overlap (measured),
-        // so the evaluation is written as wide as the registers allow: every output is then one multiply R_k * yw[m].
         double yw[9];
         {
             const double c1 = 0.4886025119029199 * w0, c2 = (tiny ? 0.0 : 1.0925484305920792) * w0;     // l > 0 orbitals vanish at the nucleus
@@ -230,142 +212,136 @@ __device__ __forceinline__ void eval_stage(const Geom& g, TileSmem& S, int ps, i
             yw[1] = c1 * uy; yw[2] = c1 * uz; yw[3] = c1 * ux;
             yw[4] = c2x * uy; yw[5] = c2y * uz; yw[6] = c20 * fma(3.0 * uz, uz, -1.0); yw[7] = c2x * uz; yw[8] = c22 * fma(ux, ux, -uy * uy);
         }
-        const double wr = (two && inside) ? (VLOCAL ? wv : 1.0) : 0.0;      // diagonal tile: side J = wr / w0-scaled copy (w0 = 1 inside)
-#define GINT_PUT(m) do { const double v_ = R * yw[m]; *o0 = v_; if (two) o0[GINT_TILE_ORB * GINT_LD] = wr * v_; o0 += GINT_LD; } while (0)
-        for (int k0 = 0; k0 < nsh; k0 += GROUP) {
-            double Rk[GROUP];
-#pragma unroll
-            for (int u = 0; u < GROUP; u++) {
-                Rk[u] = 0.0;
-                if (k0 + u < nsh) {
-                    const double2 c0 = row[k0 + u], c1 = row[nsh + k0 + u];
-                    Rk[u] = fma(am, c0.x, fma(b, c1.x, fma(a3, c0.y, b3 * c1.y)));
-                }
-            }
-#pragma unroll
-            for (int u = 0; u < GROUP; u++) {
-                if (k0 + u >= nsh) break;
-                const double R = Rk[u];
-                const int l = (si.lpack >> (2 * (k0 + u))) & 3;
-                if (l == 0) {
-                    GINT_PUT(0);
-                } else if (l == 1) {
-                    GINT_PUT(1); GINT_PUT(2); GINT_PUT(3);
-                } else {
-                    GINT_PUT(4); GINT_PUT(5); GINT_PUT(6); GINT_PUT(7); GINT_PUT(8);
-                }
+        double* o0 = phi + ((S.gbase[k] + (u64)slot * S.gR[k] + S.row0[e]) << 3) + pl;
+        const int lpack = S.lpack[e];
+#define GINT_PUT(m) do { *o0 = R * yw[m]; o0 += 8; } while (0)
+        for (int s = 0; s < nsh; s++) {
+            const double2 c0 = row[s], c1 = row[nsh + s];
+            const double R = fma(am, c0.x, fma(bb, c1.x, fma(a3, c0.y, b3 * c1.y)));
+            const int l = (lpack >> (2 * s)) & 3;
+            if (l == 0) {
+                GINT_PUT(0);
+            } else if (l == 1) {
+                GINT_PUT(1); GINT_PUT(2); GINT_PUT(3);
+            } else {
+                GINT_PUT(4); GINT_PUT(5); GINT_PUT(6); GINT_PUT(7); GINT_PUT(8);
             }
         }
 #undef GINT_PUT
     }
+    // ---- pass B: zero rows.  Inside a slot, a fragment that holds orbitals of an active atom is read whole by the
+    // contraction kernels: the rows of its inactive atoms and the padding rows behind the group's last orbital are zeros.
+    const int n_z = S.zitem0[n];
+    for (int it = qw; it < n_z; it += GINT_EVAL_THREADS / 8) {
+        int lo = 0, hi = n - 1;
+        while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (S.zitem0[mid] <= it) lo = mid; else hi = mid - 1; }
+        const int e = lo, k = S.grp[e], slot = it - S.zitem0[e];
+        const int cl = cselect(S.gmask[k], slot);
+        const bool act = cbit(S.amask[e], cl);
+        const int f = S.gfirst[k], cnt = S.gcnt[k];
+        const bool last = e == f + cnt - 1;
+        int r0 = S.row0[e], r1 = r0 + S.norb[e];
+        if (act) r0 = r1;                               // an active atom's own rows were written by pass A
+        if (last) r1 = S.gR[k];                         // padding rows
+        if (r0 >= r1) continue;
+        unsigned fact = 0;                              // fragments with an active atom
+        for (int a = f; a < f + cnt; a++)
+            if (cbit(S.amask[a], cl)) { const int q0 = S.row0[a] >> 3, q1 = (S.row0[a] + S.norb[a] - 1) >> 3; fact |= (2u << q1) - (1u << q0); }
+        double* o0 = phi + ((S.gbase[k] + (u64)slot * S.gR[k]) << 3) + pl;
+        for (int rr = r0; rr < r1; rr++) if ((fact >> (rr >> 3)) & 1u) o0[rr << 3] = 0.0;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Tile set-up: atom slots, orbital-row maps, canonical block of every atom pair of the tile, activity masks,
-// cubelet list, segments.
-__device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView& tv, const int2* __restrict__ tile,
-                                           const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
-                                           const double* __restrict__ atom_pos, const int* __restrict__ atom_spec,
-                                           const SpeciesDev* __restrict__ sp, const int* __restrict__ crow,
-                                           const u64* __restrict__ ckey, const unsigned int* __restrict__ coff,
-                                           const double* __restrict__ tab, int tab_cells, const double* __restrict__ V) {
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    DBG_T(ts0);
-    const int2 td = tile[blockIdx.x];            // head of the dependent chain tile -> batch -> neighbour entries -> atoms: issue it first
-    // copy of the radial table (tab_cells = 0: it stays in global memory): 8 independent 16-byte loads per thread in flight
-    {
-        const double2* src = reinterpret_cast<const double2*>(tab);
-        double2* dst = reinterpret_cast<double2*>(reinterpret_cast<unsigned char*>(&S) + GINT_SMEM_TAB_OFF);
-        for (int i0 = tid; i0 < tab_cells; i0 += 8 * GINT_THREADS) {
-            double2 tmp[8];
-#pragma unroll
-            for (int u = 0; u < 8; u++) if (i0 + u * GINT_THREADS < tab_cells) tmp[u] = __ldg(src + i0 + u * GINT_THREADS);
-#pragma unroll
-            for (int u = 0; u < 8; u++) if (i0 + u * GINT_THREADS < tab_cells) dst[i0 + u * GINT_THREADS] = tmp[u];
-        }
-    }
-    if (tid == GINT_THREADS - 32) for (int s = 0; s < GINT_STAGES; s++) { mbar_init(&S.full[s], GINT_EVAL_WARPS); mbar_init(&S.empty[s], GINT_MMA_WARPS); }
-    tv.b = td.x; tv.I = td.y & 255; tv.J = (td.y >> 8) & 255; tv.G = (td.y >> 16) & 255;
-    tv.diag = tv.I == tv.J;
-    const int b = tv.b;
-    const int bz = b % g.nb[2], by = (b / g.nb[2]) % g.nb[1], bx = b / (g.nb[2] * g.nb[1]);
-    tv.i0 = bx * g.bs[0]; tv.j0 = by * g.bs[1]; tv.k0 = bz * g.bs[2];
-    tv.ex = min(g.bs[0], g.N[0] - tv.i0); tv.ey = min(g.bs[1], g.N[1] - tv.j0); tv.ez = min(g.bs[2], g.N[2] - tv.k0);
-    const int e0 = bstart[b], n = bstart[b + 1] - e0;
-    const int eI = group_begin(tv.I, n, tv.G), eJ = group_begin(tv.J, n, tv.G);
-    tv.nI = group_begin(tv.I + 1, n, tv.G) - eI;
-    tv.nJ = group_begin(tv.J + 1, n, tv.G) - eJ;
+// shared memory of the contraction kernels
+struct PairEnt { unsigned off; unsigned short sr, sc; };   // element (oa, ob) of the atom pair at off + oa*sr + ob*sc; off = ~0u: none
 
-    for (int q = tid; q < GINT_NCUB * GINT_CPTS; q += GINT_THREADS) {   // mesh points of the batch (V == nullptr: rho, weight 1)
-        const int cl = q / GINT_CPTS, pp = q % GINT_CPTS;
-        const int ix = 2 * (cl / (4 * GINT_NCZ)) + pp / (2 * GINT_CZ), iy = 2 * ((cl / GINT_NCZ) & 3) + ((pp / GINT_CZ) & 1), iz = GINT_CZ * (cl % GINT_NCZ) + pp % GINT_CZ;
-        double4 P = make_double4(1e30, 0.0, 0.0, 0.0);
-        if (ix < tv.ex && iy < tv.ey && iz < tv.ez) {
-            const int gi = tv.i0 + ix, gj = tv.j0 + iy, gk = tv.k0 + iz;
-            mesh_point(g, gi, gj, gk, P.x, P.y, P.z);
-            P.w = V ? __ldg(V + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk) * g.dV : 1.0;
-        }
-        S.pts[q] = P;
-    }
-    if (tid < 16) {
-        const int side = tid >> 3, a = tid & 7;
-        const bool valid = a < (side ? tv.nJ : tv.nI);
-        int atom = 0, shift = pack_shift(0, 0, 0), spec = 0;
-        double x = 0, y = 0, z = 0;
+struct alignas(16) TileCtx {
+    int valid;                          // 0: the queue is empty, the roles leave
+    int ncub, nstage;                   // cubelets the tile walks over; ring stages of GINT_SC cubelets
+    int nI, nJ, nfI, nfJ, RI, RJ, diag;
+    int i0, j0, k0, ex, ey, ez;         // batch origin and extents (mesh points)
+    const double *srcI, *srcJ;          // slot arrays of the two groups
+    int seg[GINT_MAX_SEG];              // consumer warp w, segment k at [w + 8 k]: row fragment | first column fragment << 8 | n columns << 16
+    unsigned cubinfo[GINT_NCUB];        // per listed cubelet: active row fragments of I | active column fragments of J << 16
+    unsigned short slotI[GINT_NCUB], slotJ[GINT_NCUB];     // slot of the listed cubelet inside the groups' slot arrays
+    unsigned char cub[GINT_NCUB];       // the listed cubelets (bit numbers of the batch's masks, ascending)
+    PairEnt pair[GINT_TILE_ATOMS][GINT_TILE_ATOMS];   // canonical block of (I atom a, J atom b)
+    unsigned char row_atom[2][GINT_TILE_ORB];   // orbital row -> atom slot inside the group (255 = padding)
+    unsigned char row_orb[2][GINT_TILE_ORB];    // orbital row -> orbital index inside the atom
+    alignas(16) double pw[GINT_NCUB][GINT_CPTS];    // gint_vlocal: V dV at the listed cubelets' points (0 outside the mesh);
+                                        // gint_rho: the tile's density at those points (summed by the issuer warp)
+};
+struct SetupScratch {                   // private to the set-up warps
+    cmask amask[16];                    // slot s < 8: atom s of group I; slot 8 + s: atom s of group J
+    cmask fmask[2][16];                 // [side][fragment]: OR of amask over the atoms with orbitals in the fragment
+    int atom[16], shift[16];
+    int cstart[2][GINT_TILE_ATOMS + 1]; // first orbital row of each atom inside its group
+    int tile;
+};
+static_assert(GINT_SC == 2, "the density reduction of the consumers is written for two cubelets per stage");
+struct alignas(128) TileSmem {
+    unsigned char ring[GINT_NS][GINT_STAGE_BYTES];     // stage: [cubelet q][side][row][8 points]
+    TileCtx ctx[GINT_NCTX];
+    SetupScratch ss;
+    double part[GINT_NS][GINT_MMA_WARPS][GINT_SC * GINT_CPTS];   // gint_rho: per stage, the consumer warps' partial densities
+    u64 full[GINT_NS], empty[GINT_NS];             // stage filled by TMA / read by all consumer warps
+    u64 ctx_full[GINT_NCTX], ctx_free[GINT_NCTX];  // context written by the set-up warps / released by consumers and issuer
+    int hist[GINT_NS];                  // issuer: context | stage of the tile << 8 of what each ring slot holds
+};
+
+size_t gint_smem_needed(gint_ctx* c, size_t limit) {
+    c->tab_in_smem = GINT_EVAL_TAB_OFF + c->tab_bytes <= 72 * 1024 && GINT_EVAL_TAB_OFF + c->tab_bytes <= limit;   // three evaluation CTAs per SM
+    c->smem_eval = GINT_EVAL_TAB_OFF + (c->tab_in_smem ? c->tab_bytes : 0);
+    return sizeof(TileSmem) + 128;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Tile set-up by the 96 threads of warps 9..11: everything the issuer and the consumers need for one tile.
+template <bool VLOCAL>
+__device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileCtx& X, const int2 td, const int* __restrict__ bstart,
+                                           const NeighEntry* __restrict__ bent, const int* __restrict__ gstart,
+                                           const u64* __restrict__ goff, u64 wave_row0, const double* __restrict__ phi,
+                                           const int* __restrict__ atom_spec, const SpeciesDev* __restrict__ sp,
+                                           const int* __restrict__ crow, const u64* __restrict__ ckey,
+                                           const unsigned int* __restrict__ coff, const double* __restrict__ V) {
+    const int sid = threadIdx.x - 32 * (GINT_MMA_WARPS + 1), lane = threadIdx.x & 31, sw = sid >> 5;
+    SetupScratch& Q = S.ss;
+    const int b = td.x, I = td.y & 255, J = (td.y >> 8) & 255, G = (td.y >> 16) & 255;
+    const bool diag = I == J;
+    const int e0 = bstart[b], n = bstart[b + 1] - e0;
+    const int eI = group_begin(I, n, G), eJ = group_begin(J, n, G);
+    const int nI = group_begin(I + 1, n, G) - eI, nJ = group_begin(J + 1, n, G) - eJ;
+    if (sid < 16) {
+        const int side = sid >> 3, a = sid & 7;
+        const bool valid = a < (side ? nJ : nI);
+        int atom = 0, shift = pack_shift(0, 0, 0), norb = 0;
         cmask m = czero();
         if (valid) {
             const NeighEntry e = bent[e0 + (side ? eJ : eI) + a];
-            int t1, t2, t3; unpack_shift(e.shift, t1, t2, t3);
-            atom = e.atom; shift = e.shift; spec = atom_spec[atom]; m = cmask{e.mask[0], e.mask[1]};
-            x = atom_pos[3 * atom + 0] + t1 * g.a[0] + t2 * g.a[3] + t3 * g.a[6];
-            y = atom_pos[3 * atom + 1] + t1 * g.a[1] + t2 * g.a[4] + t3 * g.a[7];
-            z = atom_pos[3 * atom + 2] + t1 * g.a[2] + t2 * g.a[5] + t3 * g.a[8];
+            atom = e.atom; shift = e.shift; m = cmask{e.mask[0], e.mask[1]};
+            norb = sp[atom_spec[atom]].norb;
         }
-        S.pos[tid][0] = x; S.pos[tid][1] = y; S.pos[tid][2] = z; S.pos[tid][3] = 0.0;
-        S.spec[tid] = spec; S.atom[tid] = atom; S.shift[tid] = shift; S.amask[tid] = m;
-        const SpeciesDev* Sp = sp + spec;
-        SlotInfo si; si.rc2 = Sp->rc * Sp->rc; si.n_int = Sp->n_int; si.nsh = valid ? Sp->n_shell : 0; si.tab_off = Sp->tab_off;
-        int lp = 0;
-        for (int k = 0; k < Sp->n_shell; k++) lp |= Sp->l[k] << (2 * k);
-        si.lpack = lp;
-        S.sinfo[tid] = si;
-        // first orbital row of each atom inside its group: prefix sum of norb over the 8 lanes of the side
-        const int norb = valid ? Sp->norb : 0;
+        Q.atom[sid] = atom; Q.shift[sid] = shift; Q.amask[sid] = m;
         int inc = norb;
 #pragma unroll
         for (int dlt = 1; dlt < 8; dlt <<= 1) { const int t = __shfl_up_sync(0xffffu, inc, dlt, 8); if (a >= dlt) inc += t; }
-        S.cstart[side][a] = inc - norb;
-        if (a == 7) S.cstart[side][8] = inc;
+        Q.cstart[side][a] = inc - norb;
+        if (a == 7) Q.cstart[side][8] = inc;
     }
-    DBG_T(ts1);
-    __syncthreads();
-    DBG_T(ts2);
-    const int totI = S.cstart[0][GINT_TILE_ATOMS], totJ = S.cstart[1][GINT_TILE_ATOMS];
-    tv.nfI = (totI + 7) >> 3;
-    tv.nfJ = (totJ + 7) >> 3;
-    if (tid < 2 * GINT_TILE_ORB) {
-        const int side = tid / GINT_TILE_ORB, row = tid - side * GINT_TILE_ORB;
-        int a = 255, o = 0;
-        for (int k = 0; k < GINT_TILE_ATOMS; k++)
-            if (row >= S.cstart[side][k] && row < S.cstart[side][k + 1]) { a = k; o = row - S.cstart[side][k]; }
-        S.row_atom[side][row] = (unsigned char)a; S.row_orb[side][row] = (unsigned char)o;
-    } else if (tid < 2 * GINT_TILE_ORB + 32) {
-        const int q = tid - 2 * GINT_TILE_ORB, side = q >> 4, f = q & 15;
-        unsigned m = 0;
-        cmask fm = czero();
-        for (int k = 0; k < GINT_TILE_ATOMS; k++)
-            if (S.cstart[side][k] < 8 * f + 8 && S.cstart[side][k + 1] > 8 * f) { m |= 1u << k; fm |= S.amask[8 * side + k]; }
-        S.frag_atoms[side][f] = (unsigned char)m;
-        S.fmask[side][f] = fm;
-    } else if (tid >= 256 && tid < 256 + 64) {
-        const int q = tid - 256, a = q >> 3, bb = q & 7;
+    setup_sync();
+    const int totI = Q.cstart[0][GINT_TILE_ATOMS], totJ = Q.cstart[1][GINT_TILE_ATOMS];
+    const int nfI = (totI + 7) >> 3, nfJ = (totJ + 7) >> 3;
+    if (sid < 64) {
+        // canonical block of every atom pair of the tile: binary search in row A of the canonical key list
+        const int a = sid >> 3, bb = sid & 7;
         PairEnt pe; pe.off = 0xffffffffu; pe.sr = 0; pe.sc = 0;
         // diagonal tile: only pairs a <= b are accumulated (a == b is the full on-site block)
-        if (a < tv.nI && bb < tv.nJ && !(tv.diag && a > bb)) {
-            int A = S.atom[a], B = S.atom[8 + bb];
-            const int nA = S.cstart[0][a + 1] - S.cstart[0][a], nB = S.cstart[1][bb + 1] - S.cstart[1][bb];
+        if (a < nI && bb < nJ && !(diag && a > bb)) {
+            int A = Q.atom[a], B = Q.atom[8 + bb];
+            const int nA = Q.cstart[0][a + 1] - Q.cstart[0][a], nB = Q.cstart[1][bb + 1] - Q.cstart[1][bb];
             int ta1, ta2, ta3, tb1, tb2, tb3;
-            unpack_shift(S.shift[a], ta1, ta2, ta3); unpack_shift(S.shift[8 + bb], tb1, tb2, tb3);
+            unpack_shift(Q.shift[a], ta1, ta2, ta3); unpack_shift(Q.shift[8 + bb], tb1, tb2, tb3);
             int n1 = tb1 - ta1, n2 = tb2 - ta2, n3 = tb3 - ta3;
             const bool ge0 = n1 > 0 || (n1 == 0 && (n2 > 0 || (n2 == 0 && n3 >= 0)));
             bool tr = false;
@@ -385,58 +361,56 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
             // canonical key (b, a): the stored block is nB x nA and holds the transpose
             pe.sr = (unsigned short)(tr ? 1 : nB); pe.sc = (unsigned short)(tr ? nA : 1);
         }
-        S.pair[a][bb] = pe;
-    }
-    // padding rows (orbital rows between the group's last orbital and the end of its last fragment) must hold zeros
-    for (int idx = tid; idx < GINT_STAGES * 2 * 8 * GINT_LD; idx += blockDim.x) {
-        const int col = idx % GINT_LD, r = (idx / GINT_LD) & 7, side = (idx / (8 * GINT_LD)) & 1, st = idx / (16 * GINT_LD);
-        const int row = (side ? totJ : totI) + r;
-        if (row < GINT_TILE_ORB) S.phi[st][side][row][col] = 0.0;
-    }
-    __syncthreads();
-    DBG_T(ts3);
-    if (warp == 0 || warp == 2) {
-        // union masks (both warps), then warp 0: cubelet list; warp 2: per-slot read sets
-        const cmask vI = lane < tv.nfI ? S.fmask[0][lane] : czero();
-        const cmask vJ = lane < tv.nfJ ? S.fmask[1][lane] : czero();
-        const cmask anyI = warp_orc(vI);
-        const cmask h0 = warp_orc(lane < GINT_SEG_COLS ? vJ : czero()) & anyI, h1 = warp_orc(lane >= GINT_SEG_COLS ? vJ : czero()) & anyI;
-        const cmask U = h0 | h1;
-        if (warp == 0) {
-            const unsigned Uw[4] = {(unsigned)U.lo, (unsigned)(U.lo >> 32), (unsigned)U.hi, (unsigned)(U.hi >> 32)};
-            const unsigned lt = (1u << lane) - 1u;
-            int before = 0;
-#pragma unroll
-            for (int wd = 0; wd < 4; wd++) {
-                if ((Uw[wd] >> lane) & 1u) S.cub[before + __popc(Uw[wd] & lt)] = (unsigned char)(32 * wd + lane);
-                before += __popc(Uw[wd]);
-            }
-            const int ncub = before;
-            if (lane < 4) S.cub[ncub + lane] = 0;
-            if (lane == 0) { S.U = U; S.hmask[0] = h0; S.hmask[1] = h1; S.ncub = ncub; }
-        } else {
-            cmask m = czero();
-            if (lane < 16) {
-                const int side = lane >> 3, a = lane & 7;
-                const int nf = side ? tv.nfJ : tv.nfI;
-                for (int f = 0; f < nf; f++)
-                    if ((S.frag_atoms[side][f] >> a) & 1) m |= side ? (f < GINT_SEG_COLS ? h0 : h1) : (S.fmask[0][f] & U);
-            }
-            const cmask mj = cmask{shfl64(m.lo, (lane + 8) & 31), shfl64(m.hi, (lane + 8) & 31)};
-            if (tv.diag) m = lane < 8 ? (m | mj) : czero();      // the atoms are evaluated once, for both sides
-            if (lane < 16) S.need[lane] = m;
+        X.pair[a][bb] = pe;
+    } else {
+        // fragment masks, then the row maps
+        const int q = sid - 64, side = q >> 4, f = q & 15;
+        cmask fm = czero();
+        for (int k = 0; k < GINT_TILE_ATOMS; k++)
+            if (Q.cstart[side][k] < 8 * f + 8 && Q.cstart[side][k + 1] > 8 * f) fm |= Q.amask[8 * side + k];
+        Q.fmask[side][f] = fm;
+        for (int idx = q; idx < 2 * GINT_TILE_ORB; idx += 32) {
+            const int sd = idx / GINT_TILE_ORB, row = idx - sd * GINT_TILE_ORB;
+            int a = 255, o = 0;
+            for (int k = 0; k < GINT_TILE_ATOMS; k++)
+                if (row >= Q.cstart[sd][k] && row < Q.cstart[sd][k + 1]) { a = k; o = row - Q.cstart[sd][k]; }
+            X.row_atom[sd][row] = (unsigned char)a; X.row_orb[sd][row] = (unsigned char)o;
         }
-    } else if (warp == 1) {
+    }
+    setup_sync();
+    if (sw == 0) {
+        // cubelet list: the cubelets on which both groups are active, with their slots in the two slot arrays
+        cmask mI = czero(), mJ = czero();
+        if (lane < 8) mI = Q.amask[lane]; else if (lane < 16) mJ = Q.amask[lane];
+        mI.lo = __reduce_or_sync(0xffffffffu, (unsigned)mI.lo) | ((u64)__reduce_or_sync(0xffffffffu, (unsigned)(mI.lo >> 32)) << 32);
+        mI.hi = __reduce_or_sync(0xffffffffu, (unsigned)mI.hi) | ((u64)__reduce_or_sync(0xffffffffu, (unsigned)(mI.hi >> 32)) << 32);
+        mJ.lo = __reduce_or_sync(0xffffffffu, (unsigned)mJ.lo) | ((u64)__reduce_or_sync(0xffffffffu, (unsigned)(mJ.lo >> 32)) << 32);
+        mJ.hi = __reduce_or_sync(0xffffffffu, (unsigned)mJ.hi) | ((u64)__reduce_or_sync(0xffffffffu, (unsigned)(mJ.hi >> 32)) << 32);
+        const cmask U = mI & mJ;
+        const unsigned Uw[4] = {(unsigned)U.lo, (unsigned)(U.lo >> 32), (unsigned)U.hi, (unsigned)(U.hi >> 32)};
+        const unsigned lt = (1u << lane) - 1u;
+        int before = 0;
+#pragma unroll
+        for (int wd = 0; wd < 4; wd++) {
+            if ((Uw[wd] >> lane) & 1u) {
+                const int pos = before + __popc(Uw[wd] & lt), cl = 32 * wd + lane;
+                X.cub[pos] = (unsigned char)cl;
+                X.slotI[pos] = (unsigned short)crank(mI, cl); X.slotJ[pos] = (unsigned short)crank(mJ, cl);
+            }
+            before += __popc(Uw[wd]);
+        }
+        if (lane == 0) { X.ncub = before; X.nstage = (before + GINT_SC - 1) / GINT_SC; }
+    } else if (sw == 1) {
         // segments: piece (row fragment r, half h) = columns [cb, cb + n); sorted by falling n and dealt to the
-        // sub-partitions 0,1,2,3,3,2,1,0,... (warp w runs on sub-partition w % 4)
-        if (lane < GINT_MAX_SEG) S.seg[lane] = 0;
+        // sub-partitions 0,1,2,3,3,2,1,0,... (consumer warp w runs on sub-partition w % 4)
+        X.seg[lane] = 0;
         __syncwarp();
         int pn = 0, pcb = 0;
         const int r = lane >> 1, h = lane & 1;
-        if (lane < 2 * GINT_TILE_FRAG && r < tv.nfI) {
-            const int cf = tv.diag ? (S.cstart[1][S.row_atom[0][8 * r]] >> 3) : 0;
-            if (h == 0) { pcb = cf; pn = min(GINT_SEG_COLS, tv.nfJ) - cf; }
-            else { pcb = max(GINT_SEG_COLS, cf); pn = tv.nfJ - pcb; }
+        if (lane < 2 * GINT_TILE_FRAG && r < nfI) {
+            const int cf = diag ? (Q.cstart[1][X.row_atom[0][8 * r]] >> 3) : 0;
+            if (h == 0) { pcb = cf; pn = min(GINT_SEG_COLS, nfJ) - cf; }
+            else { pcb = max(GINT_SEG_COLS, cf); pn = nfJ - pcb; }
             pn = max(pn, 0);
         }
         int rank = 0;
@@ -446,422 +420,423 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileView&
         }
         if (pn > 0) {
             const int k7 = rank & 7, s = k7 < 4 ? k7 : 7 - k7, j = 2 * (rank >> 3) + (k7 >= 4);
-            const int W = GINT_MMA_WARPS / 4;         // consumer warps per sub-partition
-            S.seg[s + 4 * (j % W) + GINT_MMA_WARPS * (j / W)] = r | (pcb << 8) | (pn << 16);
+            X.seg[s + 4 * (j & 1) + GINT_MMA_WARPS * (j >> 1)] = r | (pcb << 8) | (pn << 16);
         }
+    } else if (lane == 0) {
+        const int bz = b % g.nb[2], by = (b / g.nb[2]) % g.nb[1], bx = b / (g.nb[2] * g.nb[1]);
+        X.i0 = bx * g.bs[0]; X.j0 = by * g.bs[1]; X.k0 = bz * g.bs[2];
+        X.ex = min(g.bs[0], g.N[0] - X.i0); X.ey = min(g.bs[1], g.N[1] - X.j0); X.ez = min(g.bs[2], g.N[2] - X.k0);
+        X.nI = nI; X.nJ = nJ; X.nfI = nfI; X.nfJ = nfJ; X.RI = 8 * nfI; X.RJ = 8 * nfJ; X.diag = diag;
+        X.srcI = phi + ((goff[gstart[b] + I] - wave_row0) << 3);
+        X.srcJ = phi + ((goff[gstart[b] + J] - wave_row0) << 3);
+        X.valid = 1;
     }
-    __syncthreads();
-    DBG_T(ts4);
-    tv.nchunk = (S.ncub + GINT_CUBS - 1) / GINT_CUBS;
-    for (int c = warp; c < tv.nchunk; c += GINT_WARPS) make_items(S, c);
-    if (tid == GINT_THREADS - 1) S.tv = tv;      // a thread of the last warp: it has no item list to make (<= 16 stages, warp 15 only for 64 cubelets)
-    __syncthreads();
-    DBG_T(ts5); DBG_ADD(12, ts1 - ts0); DBG_ADD(13, ts2 - ts1); DBG_ADD(14, ts3 - ts2); DBG_ADD(15, ts4 - ts3); DBG_ADD(0, ts5 - ts4);
+    setup_sync();
+    // per listed cubelet: which fragments are active, and the points' weights
+    const int ncub = X.ncub;
+    const int bi0 = X.i0, bj0 = X.j0, bk0 = X.k0, ex = X.ex, ey = X.ey, ez = X.ez;
+    for (int pos = sid; pos < ncub; pos += GINT_SETUP_THREADS) {
+        const int cl = X.cub[pos];
+        unsigned info = 0;
+        for (int f = 0; f < nfI; f++) info |= (unsigned)cbit(Q.fmask[0][f], cl) << f;
+        for (int f = 0; f < nfJ; f++) info |= (unsigned)cbit(Q.fmask[1][f], cl) << (16 + f);
+        X.cubinfo[pos] = info;
+    }
+    for (int idx = sid; idx < ncub * GINT_CPTS; idx += GINT_SETUP_THREADS) {
+        double w = 0.0;
+        if (VLOCAL) {
+            int ix, iy, iz; cubelet_point(X.cub[idx >> 3], idx & 7, ix, iy, iz);
+            if (ix < ex && iy < ey && iz < ez) w = __ldg(V + ((size_t)(bi0 + ix) * g.N[1] + (bj0 + iy)) * g.N[2] + (bk0 + iz)) * g.dV;
+        }
+        X.pw[0][idx] = w;
+    }
+    setup_sync();
+}
+
+template <bool VLOCAL>
+__device__ __forceinline__ void setup_role(const Geom& g, TileSmem& S, const int2* __restrict__ tile, int n_tiles, int* __restrict__ queue,
+                                           const int* __restrict__ bstart, const NeighEntry* __restrict__ bent, const int* __restrict__ gstart,
+                                           const u64* __restrict__ goff, u64 wave_row0, const double* __restrict__ phi,
+                                           const int* __restrict__ atom_spec, const SpeciesDev* __restrict__ sp,
+                                           const int* __restrict__ crow, const u64* __restrict__ ckey,
+                                           const unsigned int* __restrict__ coff, const double* __restrict__ V) {
+    const int sid = threadIdx.x - 32 * (GINT_MMA_WARPS + 1);
+    for (int t = 0;; t++) {
+        const int c = t % GINT_NCTX;
+        if (t >= GINT_NCTX) mbar_wait(&S.ctx_free[c], ((t / GINT_NCTX) - 1) & 1);
+        if (sid == 0) S.ss.tile = atomicAdd(queue, 1);
+        setup_sync();
+        const int ti = S.ss.tile;
+        if (ti >= n_tiles) {
+            if (sid == 0) { S.ctx[c].valid = 0; mbar_arrive(&S.ctx_full[c]); }
+            return;
+        }
+        tile_setup<VLOCAL>(g, S, S.ctx[c], tile[ti], bstart, bent, gstart, goff, wave_row0, phi, atom_spec, sp, crow, ckey, coff, V);
+        if (sid == 0) mbar_arrive(&S.ctx_full[c]);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Producer / consumer plumbing.  Warp groups 2,3 (producers) evaluate orbital values into a ring of GINT_STAGES
-// shared-memory stages; warp groups 0,1 (consumers) run the DMMA chains.  full[s] completes when all producer warps
-// have written stage s, empty[s] when all consumer warps have read it.  setmaxnreg moves registers from the
-// producers (80 per thread) to the consumers (176), which hold the whole 104 x 104 block.
-__device__ __forceinline__ void mbar_arrive(u64* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(u64* bar, int parity) {
-    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
-    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
-                 :: "r"(a), "r"(parity) : "memory");
+// Issuer warp: streams the tile's slots into the ring; in gint_rho it also retires the stages: sums the consumer
+// warps' partial densities in fixed order into the tile's density, which it adds to rho when the tile is complete
+// (one red.global.add.f64 per mesh point per tile).
+template <bool VLOCAL>
+__device__ __forceinline__ void retire_stage(const Geom& g, TileSmem& S, int gr, double* __restrict__ rho) {
+    const int lane = threadIdx.x & 31, s = gr % GINT_NS;
+    mbar_wait(&S.empty[s], (gr / GINT_NS) & 1);
+    if (VLOCAL) return;
+    const int h = S.hist[s], c = h & 255, st = h >> 8;
+    TileCtx& X = S.ctx[c];
+    const int ncs = min(GINT_SC, X.ncub - st * GINT_SC);
+    if (lane < ncs * GINT_CPTS) {
+        double v = 0.0;
+#pragma unroll
+        for (int w = 0; w < GINT_MMA_WARPS; w++) v += S.part[s][w][lane];
+        X.pw[0][st * GINT_SC * GINT_CPTS + lane] += v;
+    }
+    if (st == X.nstage - 1) {
+        __syncwarp();
+        const int npt = X.ncub * GINT_CPTS;
+        for (int idx = lane; idx < npt; idx += 32) {
+            const double v = X.pw[0][idx];
+            int ix, iy, iz; cubelet_point(X.cub[idx >> 3], idx & 7, ix, iy, iz);
+            if (v != 0.0 && ix < X.ex && iy < X.ey && iz < X.ez)
+                atomicAdd(rho + ((size_t)(X.i0 + ix) * g.N[1] + (X.j0 + iy)) * g.N[2] + (X.k0 + iz), v);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&S.ctx_free[c]);
+    }
 }
 
-// Segments of a consumer warp.
-#define GINT_ROWB (GINT_LD * 8)                    // bytes of one orbital row of a stage
-#define GINT_SIDEB (GINT_TILE_ORB * GINT_ROWB)     // bytes of one side of a stage
-#define GINT_STAGEB (2 * GINT_SIDEB)
+template <bool VLOCAL>
+__device__ __forceinline__ void issuer_role(const Geom& g, TileSmem& S, double* __restrict__ rho) {
+    const int lane = threadIdx.x & 31;
+    int gi = 0, gr = 0;                 // stages issued / retired
+    int tile_end[GINT_NCTX];
+#pragma unroll
+    for (int c = 0; c < GINT_NCTX; c++) tile_end[c] = 0;
+    for (int t = 0;; t++) {
+        const int c = t % GINT_NCTX;
+        // the set-up warps can only rebuild this context when its previous tile is retired
+        if (!VLOCAL) {
+            int te = 0;
+#pragma unroll
+            for (int k = 0; k < GINT_NCTX; k++) if (k == c) te = tile_end[k];
+            while (gr < te) { retire_stage<VLOCAL>(g, S, gr, rho); gr++; }
+        }
+        mbar_wait(&S.ctx_full[c], (t / GINT_NCTX) & 1);
+        TileCtx& X = S.ctx[c];
+        if (!X.valid) break;
+        const int nstage = X.nstage, ncub = X.ncub;
+        const unsigned bI = (unsigned)X.RI * GINT_ROW_BYTES, bJ = X.diag ? 0u : (unsigned)X.RJ * GINT_ROW_BYTES;
+        const double *srcI = X.srcI, *srcJ = X.srcJ;
+        for (int st = 0; st < nstage; st++, gi++) {
+            const int s = gi % GINT_NS;
+            while (gi - gr >= GINT_NS) { retire_stage<VLOCAL>(g, S, gr, rho); gr++; }
+            const int ncs = min(GINT_SC, ncub - st * GINT_SC);
+            if (lane == 0) { mbar_expect_tx(&S.full[s], (unsigned)ncs * (bI + bJ)); S.hist[s] = c | (st << 8); }
+            __syncwarp();
+            if (lane < ncs) {
+                const int pos = st * GINT_SC + lane;
+                const unsigned dst = smem_addr(&S.ring[s][lane * 2 * GINT_SLOT_MAX_BYTES]);
+                bulk_g2s(dst, reinterpret_cast<const unsigned char*>(srcI) + (size_t)X.slotI[pos] * bI, bI, &S.full[s]);
+                if (bJ) bulk_g2s(dst + GINT_SLOT_MAX_BYTES, reinterpret_cast<const unsigned char*>(srcJ) + (size_t)X.slotJ[pos] * bJ, bJ, &S.full[s]);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < GINT_NCTX; k++) if (k == c) tile_end[k] = gi;
+        if (nstage == 0 || VLOCAL) { __syncwarp(); if (lane == 0) mbar_arrive(&S.ctx_free[c]); }
+    }
+    while (gr < gi) { retire_stage<VLOCAL>(g, S, gr, rho); gr++; }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Consumers.  DMMA.8x8x4 fragment layouts (mma.sync.m8n8k4.f64): A[m = lane / 4][k = lane % 4], B[k = lane % 4][n = lane / 4],
+// C[m = lane / 4][n = 2 (lane % 4) + {0, 1}].  A slot row holds the 8 points of a cubelet; the two k-steps of a cubelet
+// take points {0,2,4,6} and {1,3,5,7}, so that one 128-bit load fetches a lane's operands of both steps.
+__device__ __forceinline__ double2 lds128(unsigned addr) {
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory");
+    return v;
+}
 struct Seg {
-    unsigned oa;                     // byte offset of the row fragment in side I (row 8 row) | column fragments << 24 (0 = unused)
-    unsigned ob;                     // byte offset of the first column fragment in side J, relative to the stage
-    u64 W;                           // activity on the tile's cubelet list: bit p = the segment works on cubelet cub[p]
-    int w;                           // row fragment | first column fragment << 8 | column fragments << 16
+    unsigned oa, ob;                 // byte offsets of the row fragment (side I) and of the first column fragment (side J) inside a cubelet of a stage
+    int w;                           // row fragment | first column fragment << 8 | column fragments << 16 (0: unused)
     __device__ __forceinline__ int row() const { return w & 255; }
     __device__ __forceinline__ int cb() const { return (w >> 8) & 255; }
     __device__ __forceinline__ int n() const { return w >> 16; }
 };
-__device__ __forceinline__ Seg load_seg(TileSmem& S, int slot, bool j_is_i = false) {   // j_is_i: column operands from side I (rho, diagonal tile)
-    const int lane = threadIdx.x & 31;
-    Seg s; s.w = S.seg[slot];
-    cmask cm = czero();
-    for (int j = 0; j < s.n(); j++) cm |= S.fmask[1][s.cb() + j];
-    const cmask act = s.n() ? (S.fmask[0][s.row()] & cm) : czero();     // cubelets on which the row fragment and some column fragment are active
-    unsigned wb[4];
-#pragma unroll
-    for (int wd = 0; wd < 4; wd++) {
-        const int pp = 32 * wd + lane;
-        wb[wd] = __ballot_sync(0xffffffffu, pp < S.ncub && cbit(act, S.cub[min(pp, GINT_NCUB - 1)]));
-    }
-    s.W = (u64)wb[0] | ((u64)wb[1] << 32);
-    if (lane == 0) S.segWhi[slot] = (u64)wb[2] | ((u64)wb[3] << 32);      // list positions 64..127: fetched when the tile gets there
-    __syncwarp();
-    s.oa = (unsigned)(s.row() * 8 * GINT_ROWB);
-    s.ob = (unsigned)((j_is_i ? 0 : GINT_SIDEB) + s.cb() * 8 * GINT_ROWB);
+__device__ __forceinline__ Seg load_seg(const TileCtx& X, int slot) {
+    Seg s; s.w = X.seg[slot];
+    s.oa = (unsigned)(s.row() * 8 * GINT_ROW_BYTES);
+    s.ob = (unsigned)((X.diag ? 0 : GINT_SLOT_MAX_BYTES) + s.cb() * 8 * GINT_ROW_BYTES);
     return s;
 }
 
-// activity of a segment on the 8-point DMMA steps of stage c (a 16-point cubelet is two steps)
-__device__ __forceinline__ unsigned stage_steps(u64 W, int c) {
-    const unsigned b = (unsigned)(W >> ((GINT_CUBS * c) & 63)) & ((1u << GINT_CUBS) - 1u);
-    return GINT_CPTS == 8 ? b : ((b & 1u) * 3u) | ((b & 2u) * 6u);
-}
-__device__ __forceinline__ void next_cubelet(unsigned& rem, unsigned pa, unsigned pb, unsigned& oa, unsigned& ob) {
-    asm volatile("{\n\t.reg .u32 t, u;\n\tbrev.b32 t, %0;\n\tclz.b32 t, t;\n\tshl.b32 t, t, 6;\n\tadd.u32 %1, %3, t;\n\tadd.u32 %2, %4, t;\n\t"
-                 "add.u32 u, %0, -1;\n\tand.b32 %0, %0, u;\n\t}" : "+r"(rem), "=r"(oa), "=r"(ob) : "r"(pa), "r"(pb));
-}
-template <int N>
-__device__ __forceinline__ void vl_seg(double (&acc)[GINT_SEG_COLS][2], unsigned pa, unsigned pb, unsigned bits) {
-    double ax, ay, bx[N], by[N];
-    unsigned rem = bits, oa, ob;
-    next_cubelet(rem, pa, pb, oa, ob);
-    ax = lds64(oa);
-#pragma unroll
-    for (int j = 0; j < N; j++) bx[j] = lds64(ob + j * 8 * GINT_ROWB);
-    ay = lds64(oa + 32);
-#pragma unroll
-    for (int j = 0; j < N; j++) by[j] = lds64(ob + j * 8 * GINT_ROWB + 32);
-    bool more = rem != 0;
-    next_cubelet(rem, pa, pb, oa, ob);
-    while (more) {
-        // the reload of an operand register follows the DMMA that read it: the loads issue in the shadow of the
-        // 16-cycle DMMAs instead of in a gap between the two groups
-#pragma unroll
-        for (int j = 0; j < N; j++) {
-            dmma884(acc[j], ax, bx[j]);
-            bx[j] = lds64(ob + j * 8 * GINT_ROWB);
-        }
-        ax = lds64(oa);
-        unsigned oa2, ob2;
-#pragma unroll
-        for (int j = 0; j < N; j++) {
-            dmma884(acc[j], ay, by[j]);
-            by[j] = lds64(ob + j * 8 * GINT_ROWB + 32);
-            if (j == 0) { more = rem != 0; next_cubelet(rem, pa, pb, oa2, ob2); }
-        }
-        ay = lds64(oa + 32);
-        oa = oa2; ob = ob2;
-    }
-#pragma unroll
-    for (int j = 0; j < N; j++) dmma884(acc[j], ax, bx[j]);
-#pragma unroll
-    for (int j = 0; j < N; j++) dmma884(acc[j], ay, by[j]);
-}
-__device__ __forceinline__ void vl_seg_dispatch(int n, double (&acc)[GINT_SEG_COLS][2], unsigned pa, unsigned pb, unsigned bits) {
-    // 7 and 6 are the lengths of all segments of a full off-diagonal tile: two compares instead of an indexed branch
-    if (n == 7) { vl_seg<7>(acc, pa, pb, bits); return; }
-    if (n == 6) { vl_seg<6>(acc, pa, pb, bits); return; }
-    switch (n) {
-        case 5: vl_seg<5>(acc, pa, pb, bits); break;
-        case 4: vl_seg<4>(acc, pa, pb, bits); break;
-        case 3: vl_seg<3>(acc, pa, pb, bits); break;
-        case 2: vl_seg<2>(acc, pa, pb, bits); break;
-        case 1: vl_seg<1>(acc, pa, pb, bits); break;
-        default: break;
-    }
+// gint_vlocal, one segment on one cubelet: acc[j] += (w . Phi_I[row fragment])^T Phi_J[column fragment j] for the active j.
+// pa, pb: lane addresses of the row fragment / first column fragment; m: activity bits of the segment's columns.
+// Only the DMMAs are predicated: a predicated load would leave its destination "maybe defined", which keeps the register
+// live across the whole loop (ptxas then spills); inactive fragments of a slot hold finite values or are never multiplied.
+__device__ __forceinline__ void vl_seg(double (&acc)[GINT_SEG_COLS][2], unsigned pa, unsigned pb, unsigned pw, unsigned m) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p0, p1, p2, p3, p4, p5, p6;\n\t"
+        ".reg .f64 ax, ay, wx, wy, bx0, by0, bx1, by1, bx2, by2, bx3, by3, bx4, by4, bx5, by5, bx6, by6;\n\t"
+        ".reg .b32 t;\n\t"
+        "and.b32 t, %17, 1;  setp.ne.u32 p0, t, 0;\n\t"
+        "and.b32 t, %17, 2;  setp.ne.u32 p1, t, 0;\n\t"
+        "and.b32 t, %17, 4;  setp.ne.u32 p2, t, 0;\n\t"
+        "and.b32 t, %17, 8;  setp.ne.u32 p3, t, 0;\n\t"
+        "and.b32 t, %17, 16; setp.ne.u32 p4, t, 0;\n\t"
+        "and.b32 t, %17, 32; setp.ne.u32 p5, t, 0;\n\t"
+        "and.b32 t, %17, 64; setp.ne.u32 p6, t, 0;\n\t"
+        "ld.shared.v2.f64 {ax, ay}, [%14];\n\t"
+        "ld.shared.v2.f64 {wx, wy}, [%16];\n\t"
+        "ld.shared.v2.f64 {bx0, by0}, [%15];\n\t"
+        "ld.shared.v2.f64 {bx1, by1}, [%15 + 512];\n\t"
+        "ld.shared.v2.f64 {bx2, by2}, [%15 + 1024];\n\t"
+        "ld.shared.v2.f64 {bx3, by3}, [%15 + 1536];\n\t"
+        "ld.shared.v2.f64 {bx4, by4}, [%15 + 2048];\n\t"
+        "ld.shared.v2.f64 {bx5, by5}, [%15 + 2560];\n\t"
+        "ld.shared.v2.f64 {bx6, by6}, [%15 + 3072];\n\t"
+        "mul.f64 ax, ax, wx;\n\t"
+        "mul.f64 ay, ay, wy;\n\t"
+        "@p0 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{ax},{bx0},{%0,%1};\n\t"
+        "@p1 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{ax},{bx1},{%2,%3};\n\t"
+        "@p2 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{ax},{bx2},{%4,%5};\n\t"
+        "@p3 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{ax},{bx3},{%6,%7};\n\t"
+        "@p4 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%8,%9},{ax},{bx4},{%8,%9};\n\t"
+        "@p5 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%10,%11},{ax},{bx5},{%10,%11};\n\t"
+        "@p6 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%12,%13},{ax},{bx6},{%12,%13};\n\t"
+        "@p0 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{ay},{by0},{%0,%1};\n\t"
+        "@p1 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{ay},{by1},{%2,%3};\n\t"
+        "@p2 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{ay},{by2},{%4,%5};\n\t"
+        "@p3 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{ay},{by3},{%6,%7};\n\t"
+        "@p4 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%8,%9},{ay},{by4},{%8,%9};\n\t"
+        "@p5 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%10,%11},{ay},{by5},{%10,%11};\n\t"
+        "@p6 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%12,%13},{ay},{by6},{%12,%13};\n\t"
+        "}"
+        : "+d"(acc[0][0]), "+d"(acc[0][1]), "+d"(acc[1][0]), "+d"(acc[1][1]), "+d"(acc[2][0]), "+d"(acc[2][1]), "+d"(acc[3][0]), "+d"(acc[3][1]),
+          "+d"(acc[4][0]), "+d"(acc[4][1]), "+d"(acc[5][0]), "+d"(acc[5][1]), "+d"(acc[6][0]), "+d"(acc[6][1])
+        : "r"(pa), "r"(pb), "r"(pw), "r"(m)
+        : "memory");
 }
 
-// producer loop shared by both kernels: stage c of the tile goes to ring slot c % GINT_STAGES.  The producer warps do
-// not synchronise with one another: each takes every 8th group of four items, rotating with the stage so that
-// the remainders even out, and arrives on full[s] when its share of the stage is written.
-template <bool VLOCAL>
-__device__ __forceinline__ void producer_loop(const Geom& g, TileSmem& S, int nchunk, const double* __restrict__ tab, int tab_cells,
-                                              const double* __restrict__ V) {
-    const int pw = (threadIdx.x >> 5) - GINT_MMA_WARPS;
-    const double2* tb = tab_cells ? reinterpret_cast<const double2*>(reinterpret_cast<const unsigned char*>(&S) + GINT_SMEM_TAB_OFF)
-                                  : reinterpret_cast<const double2*>(tab);
-    for (int c = 0; c < nchunk; c++) {
-        const int s = c % GINT_STAGES, k = c / GINT_STAGES;
-        DBG_T(t_p0);
-        if (k > 0) mbar_wait(&S.empty[s], (k - 1) & 1);
-        DBG_T(t_p1);
-        DBG_ADD(10, t_p1 - t_p0);
-#ifndef GINT_DBG_NO_EVAL
-        eval_stage<VLOCAL>(g, S, s, c, (32 / GINT_CPTS) * ((pw + c) % GINT_EVAL_WARPS), tb, V);
-#endif
-        __syncwarp();
-        if ((threadIdx.x & 31) == 0) mbar_arrive(&S.full[s]);
-        DBG_T(t_p2);
-        DBG_ADD(11, t_p2 - t_p1);
-    }
+// gint_rho, one segment on one cubelet: Y = sum_j D[row fragment][column fragment j] Phi_J[column fragment j]  (8 orbitals of I x 8 points),
+// then rho_g += sum_i Phi_I[i][g] Y[i][g].  d[j][h]: stationary A operands D[8 row + lane / 4][8 (cb + j) + 4 h + lane % 4].
+// pj: lane address of Phi_J[8 cb + lane % 4][point lane / 4]; pi: of Phi_I[8 row + lane / 4][points 2 (lane % 4), + 1].
+__device__ __forceinline__ void rho_seg(const double (&d)[GINT_SEG_COLS][2], unsigned pi, unsigned pj, unsigned m, double& r0, double& r1) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p0, p1, p2, p3, p4, p5, p6;\n\t"
+        ".reg .f64 fx, fy, ya0, ya1, yb0, yb1, b00, b01, b10, b11, b20, b21, b30, b31, b40, b41, b50, b51, b60, b61;\n\t"
+        ".reg .b32 t;\n\t"
+        "and.b32 t, %18, 1;  setp.ne.u32 p0, t, 0;\n\t"
+        "and.b32 t, %18, 2;  setp.ne.u32 p1, t, 0;\n\t"
+        "and.b32 t, %18, 4;  setp.ne.u32 p2, t, 0;\n\t"
+        "and.b32 t, %18, 8;  setp.ne.u32 p3, t, 0;\n\t"
+        "and.b32 t, %18, 16; setp.ne.u32 p4, t, 0;\n\t"
+        "and.b32 t, %18, 32; setp.ne.u32 p5, t, 0;\n\t"
+        "and.b32 t, %18, 64; setp.ne.u32 p6, t, 0;\n\t"
+        "ld.shared.f64 b00, [%17];\n\t"
+        "ld.shared.f64 b01, [%17 + 256];\n\t"
+        "ld.shared.f64 b10, [%17 + 512];\n\t"
+        "ld.shared.f64 b11, [%17 + 768];\n\t"
+        "ld.shared.f64 b20, [%17 + 1024];\n\t"
+        "ld.shared.f64 b21, [%17 + 1280];\n\t"
+        "ld.shared.f64 b30, [%17 + 1536];\n\t"
+        "ld.shared.f64 b31, [%17 + 1792];\n\t"
+        "ld.shared.f64 b40, [%17 + 2048];\n\t"
+        "ld.shared.f64 b41, [%17 + 2304];\n\t"
+        "ld.shared.f64 b50, [%17 + 2560];\n\t"
+        "ld.shared.f64 b51, [%17 + 2816];\n\t"
+        "ld.shared.f64 b60, [%17 + 3072];\n\t"
+        "ld.shared.f64 b61, [%17 + 3328];\n\t"
+        "ld.shared.v2.f64 {fx, fy}, [%16];\n\t"
+        "mov.f64 ya0, 0d0000000000000000; mov.f64 ya1, 0d0000000000000000;\n\t"
+        "mov.f64 yb0, 0d0000000000000000; mov.f64 yb1, 0d0000000000000000;\n\t"
+        "@p0 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%2},{b00},{ya0,ya1};\n\t"
+        "@p1 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {yb0,yb1},{%4},{b10},{yb0,yb1};\n\t"
+        "@p0 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%3},{b01},{ya0,ya1};\n\t"
+        "@p1 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {yb0,yb1},{%5},{b11},{yb0,yb1};\n\t"
+        "@p2 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%6},{b20},{ya0,ya1};\n\t"
+        "@p3 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {yb0,yb1},{%8},{b30},{yb0,yb1};\n\t"
+        "@p2 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%7},{b21},{ya0,ya1};\n\t"
+        "@p3 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {yb0,yb1},{%9},{b31},{yb0,yb1};\n\t"
+        "@p4 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%10},{b40},{ya0,ya1};\n\t"
+        "@p5 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {yb0,yb1},{%12},{b50},{yb0,yb1};\n\t"
+        "@p4 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%11},{b41},{ya0,ya1};\n\t"
+        "@p5 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {yb0,yb1},{%13},{b51},{yb0,yb1};\n\t"
+        "@p6 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%14},{b60},{ya0,ya1};\n\t"
+        "@p6 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%15},{b61},{ya0,ya1};\n\t"
+        "add.f64 ya0, ya0, yb0;\n\t"
+        "add.f64 ya1, ya1, yb1;\n\t"
+        "fma.rn.f64 %0, ya0, fx, %0;\n\t"
+        "fma.rn.f64 %1, ya1, fy, %1;\n\t"
+        "}"
+        : "+d"(r0), "+d"(r1)
+        : "d"(d[0][0]), "d"(d[0][1]), "d"(d[1][0]), "d"(d[1][1]), "d"(d[2][0]), "d"(d[2][1]), "d"(d[3][0]), "d"(d[3][1]),
+          "d"(d[4][0]), "d"(d[4][1]), "d"(d[5][0]), "d"(d[5][1]), "d"(d[6][0]), "d"(d[6][1]), "r"(pi), "r"(pj), "r"(m)
+        : "memory");
 }
 
-// ---------------------------------------------------------------------------------------------------
-// gint_vlocal main kernel (north_star step 3a): W_IJ = Phi_I^T diag(V dV) Phi_J accumulated over the whole batch in
-// DMMA accumulators, then added to the canonical-half value array with fp64 reductions (red.global.add.f64):
-// one reduction per element per batch.
-__global__ void __launch_bounds__(GINT_THREADS, 1)
-k_vlocal_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
-              const double* __restrict__ atom_pos, const int* __restrict__ atom_spec, const SpeciesDev* __restrict__ sp,
-              const double* __restrict__ tab, const int* __restrict__ crow, const u64* __restrict__ ckey,
-              const unsigned int* __restrict__ coff, int tab_cells, const double* __restrict__ V, double* __restrict__ Hc) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    TileSmem& S = *reinterpret_cast<TileSmem*>(smem_raw);
-    DBG_T(t_start);
-    {
-        TileView tv0;
-        tile_setup(g, S, tv0, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff, tab, tab_cells, V);
-    }
-    DBG_T(t_setup);
-    DBG_ADD(5, t_setup - t_start);
-    const int nchunk = S.tv.nchunk;
-    if (nchunk == 0) return;
-    const int warp = threadIdx.x >> 5;
-    if (warp >= GINT_MMA_WARPS) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(GINT_REGS_EVAL));
-        producer_loop<true>(g, S, nchunk, tab, tab_cells, V);
-        return;
-    }
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(GINT_REGS_MMA));
+// stationary operand of a segment (gint_rho): d[j][h] = Dh[orbital row 8 row + lr of I][orbital column 8 (cb + j) + 4 h + lc of J]
+__device__ __forceinline__ void load_dseg(const TileCtx& X, const Seg& sg, const double* __restrict__ Dh, double (&d)[GINT_SEG_COLS][2]) {
     const int lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
-    Seg sg[GINT_WARP_SEGS];
-    double acc[GINT_WARP_SEGS][GINT_SEG_COLS][2];
-#pragma unroll
-    for (int k = 0; k < GINT_WARP_SEGS; k++) {
-        sg[k] = load_seg(S, warp + GINT_MMA_WARPS * k);
-#pragma unroll
-        for (int j = 0; j < GINT_SEG_COLS; j++) { acc[k][j][0] = 0.0; acc[k][j][1] = 0.0; }
-    }
-#ifdef GINT_DBG_STATS
-    {   // developer statistics: DMMA balance over the four sub-partitions (whole tile, and stage by stage)
-        __shared__ int dbg_load[GINT_MAX_CHUNKS + 1][GINT_MMA_WARPS];
-        int tot = 0;
-        for (int c = 0; c < nchunk; c++) {
-            int l = 0;
-            for (int k = 0; k < GINT_WARP_SEGS; k++) l += 2 * sg[k].n() * __popc(stage_steps(sg[k].W, c));
-            if (lane == 0) dbg_load[c][warp] = l;
-            tot += l;
-        }
-        if (lane == 0) dbg_load[GINT_MAX_CHUNKS][warp] = tot;
-        {   // DMMAs needed at (row fragment, column fragment, cubelet) granularity, and with trailing-column cut per cubelet
-            unsigned long long fine = 0, lead = 0;
-            for (int k = 0; k < GINT_WARP_SEGS; k++) {
-                const cmask rm = S.fmask[0][sg[k].row()] & S.U;
-                cmask seen = czero();
-                for (int j = sg[k].n() - 1; j >= 0; j--) {
-                    const cmask cm = S.fmask[1][sg[k].cb() + j] & rm;
-                    fine += 2 * (__popcll(cm.lo) + __popcll(cm.hi));
-                    seen |= cm;
-                    lead += 2 * (__popcll(seen.lo) + __popcll(seen.hi));      // columns 0..j computed wherever some column >= j is active
-                }
-            }
-            if (sg[0].n() == 0) { fine = 0; lead = 0; }
-            DBG_ADD(12, fine); DBG_ADD(13, lead);
-        }
-        asm volatile("bar.sync 2, 256;" ::: "memory");
-        if (threadIdx.x == 0) {
-            unsigned long long sum = 0, mx_tile = 0, mx_chunk = 0;
-            for (int c = 0; c <= GINT_MAX_CHUNKS; c++) {
-                if (c < GINT_MAX_CHUNKS && c >= nchunk) continue;
-                int m = 0, t = 0;
-                for (int q = 0; q < 4; q++) { const int v = dbg_load[c][q] + dbg_load[c][q + 4]; m = max(m, v); t += v; }
-                if (c == GINT_MAX_CHUNKS) { sum = t; mx_tile = 4ull * m; } else mx_chunk += 4ull * m;
-            }
-            atomicAdd(&g_dbg[0], sum); atomicAdd(&g_dbg[1], mx_tile); atomicAdd(&g_dbg[2], mx_chunk); atomicAdd(&g_dbg[3], 1ull);
-            atomicAdd(&g_dbg[4], (unsigned long long)nchunk);
-        }
-    }
-#endif
-    // lane part of every operand address: row lr of the fragment, point lc of the k-step
-    unsigned lane_off = smem_addr(&S.phi[0][0][0][0]) + lr * GINT_ROWB + lc * 8;
-    asm volatile("" : "+r"(lane_off));
-    for (int c = 0; c < nchunk; c++) {
-        const int s = c % GINT_STAGES;
-        if (c == 64 / GINT_CUBS) {      // the activity words cover 64 list positions: switch to the second half
-#pragma unroll
-            for (int k = 0; k < GINT_WARP_SEGS; k++) sg[k].W = S.segWhi[warp + GINT_MMA_WARPS * k];
-        }
-        DBG_T(t_w0);
-        mbar_wait(&S.full[s], (c / GINT_STAGES) & 1);
-        DBG_T(t_w1);
-        DBG_ADD(6, t_w1 - t_w0);
-        const unsigned base = lane_off + s * GINT_STAGEB;
-#ifndef GINT_DBG_NO_MMA
-#pragma unroll
-        for (int k = 0; k < GINT_WARP_SEGS; k++) {
-            const unsigned bits = stage_steps(sg[k].W, c);
-            if (bits) vl_seg_dispatch(sg[k].n(), acc[k], base + sg[k].oa, base + sg[k].ob, bits);
-        }
-#endif
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&S.empty[s]);
-        DBG_T(t_w2);
-        DBG_ADD(7, t_w2 - t_w1);
-    }
-    DBG_T(t_loop);
-    // flush: element (row, col) -> atom pair (a, b), orbitals (oa, ob) -> canonical block (transposed if the canonical
-    // key is (b, a)).  Exact zeros (fragments never touched, atoms that do not overlap inside this batch) are skipped.
-#pragma unroll
-    for (int k = 0; k < GINT_WARP_SEGS; k++) {
-        if (sg[k].n() == 0) continue;
-        const int row = 8 * sg[k].row() + lr;
-        const int a = S.row_atom[0][row], oa = S.row_orb[0][row];
-        if (a == 255) continue;
-#pragma unroll
-        for (int j = 0; j < GINT_SEG_COLS; j++) {
-            if (j >= sg[k].n()) break;
-#pragma unroll
-            for (int e = 0; e < 2; e++) {
-                const double v = acc[k][j][e];
-                const int col = 8 * (sg[k].cb() + j) + 2 * lc + e;
-                const int bb = S.row_atom[1][col], ob = S.row_orb[1][col];
-                if (bb == 255 || v == 0.0) continue;
-                const PairEnt pe = S.pair[a][bb];
-                if (pe.off == 0xffffffffu) continue;
-                atomicAdd(Hc + pe.off + oa * pe.sr + ob * pe.sc, v);
-            }
-        }
-    }
-    DBG_T(t_end);
-    DBG_ADD(8, t_end - t_loop);
-    DBG_ADD(9, t_end - t_start);
-}
-
-// ---------------------------------------------------------------------------------------------------
-// gint_rho main kernel (north_star step 3b).  The density blocks Dh_IJ of the tile are stationary DMMA A operands
-// (registers): per cubelet X^T = Dh_seg^T Phi_I (8 orbitals of J x 8 points per column fragment) and
-// rho_g += sum_j X_jg Phi_J,jg.  Dh = canonical-half, symmetrised density blocks (k_sym_D).
-// DMMA column n of X^T <-> point (n >> 1) + 4 (n & 1) of the cubelet, so that the lane's two results (columns 2 lc,
-// 2 lc + 1) meet Phi_J at points lc and lc + 4: the same conflict-free 64-bit shared loads as in vlocal.
-template <int N>
-__device__ __forceinline__ void rho_cols(const double (&d)[GINT_SEG_COLS][2], int j0, double b0, double b1, unsigned pj, double& p0, double& p1) {
-    double x[N][2];
-#pragma unroll
-    for (int j = 0; j < N; j++) { x[j][0] = 0.0; x[j][1] = 0.0; dmma884(x[j], d[j0 + j][0], b0); }
-#pragma unroll
-    for (int j = 0; j < N; j++) dmma884(x[j], d[j0 + j][1], b1);
-    double f0[N], f1[N];
-#pragma unroll
-    for (int j = 0; j < N; j++) { f0[j] = lds64(pj + (j0 + j) * 8 * GINT_ROWB); f1[j] = lds64(pj + (j0 + j) * 8 * GINT_ROWB + 32); }
-#pragma unroll
-    for (int j = 0; j < N; j++) { p0 = fma(x[j][0], f0[j], p0); p1 = fma(x[j][1], f1[j], p1); }
-}
-template <int N>
-__device__ __forceinline__ void rho_seg(const double (&d)[GINT_SEG_COLS][2], unsigned pi, unsigned pj, unsigned bits, double (&part)[4][2]) {
-    asm volatile("" : "+r"(pi), "+r"(pj));
-#pragma unroll
-    for (int q = 0; q < 4; q++) {
-        if (!((bits >> q) & 1u)) continue;
-        const double b0 = lds64(pi + 64 * q), b1 = lds64(pi + 4 * GINT_ROWB + 64 * q);       // Phi_I[8 row + lc (+4)][point pi(lr) of cubelet q]
-        constexpr int N0 = N > 4 ? 4 : N;
-        rho_cols<N0>(d, 0, b0, b1, pj + 64 * q, part[q][0], part[q][1]);
-        if (N > 4) rho_cols<(N > 4 ? N - 4 : 1)>(d, 4, b0, b1, pj + 64 * q, part[q][0], part[q][1]);
-    }
-}
-__device__ __forceinline__ void rho_seg_dispatch(int n, const double (&d)[GINT_SEG_COLS][2], unsigned pi, unsigned pj,
-                                                 unsigned bits, double (&part)[4][2]) {
-    switch (n) {
-        case 7: rho_seg<7>(d, pi, pj, bits, part); break;
-        case 6: rho_seg<6>(d, pi, pj, bits, part); break;
-        case 5: rho_seg<5>(d, pi, pj, bits, part); break;
-        case 4: rho_seg<4>(d, pi, pj, bits, part); break;
-        case 3: rho_seg<3>(d, pi, pj, bits, part); break;
-        case 2: rho_seg<2>(d, pi, pj, bits, part); break;
-        case 1: rho_seg<1>(d, pi, pj, bits, part); break;
-        default: break;
-    }
-}
-// stationary operand of a segment: d[j][h] = Dh[orbital row 8 row + 4h + lc of I][orbital column 8 (cb + j) + lr of J]
-__device__ __forceinline__ void load_dseg(const TileSmem& S, const Seg& sg, const double* __restrict__ Dh, double (&d)[GINT_SEG_COLS][2]) {
-    const int lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
+    const int row = 8 * sg.row() + lr;
+    const int a = X.row_atom[0][row], oa = X.row_orb[0][row];
 #pragma unroll
     for (int j = 0; j < GINT_SEG_COLS; j++)
 #pragma unroll
         for (int h = 0; h < 2; h++) {
             double v = 0.0;
-            if (j < sg.n()) {
-                const int row = 8 * sg.row() + 4 * h + lc, col = 8 * (sg.cb() + j) + lr;
-                const int a = S.row_atom[0][row], bb = S.row_atom[1][col];
-                if (a != 255 && bb != 255) {
-                    const PairEnt pe = S.pair[a][bb];
-                    if (pe.off != 0xffffffffu) v = __ldg(Dh + pe.off + S.row_orb[0][row] * pe.sr + S.row_orb[1][col] * pe.sc);
+            if (j < sg.n() && a != 255) {
+                const int col = 8 * (sg.cb() + j) + 4 * h + lc;
+                const int bb = X.row_atom[1][col];
+                if (bb != 255) {
+                    const PairEnt pe = X.pair[a][bb];
+                    if (pe.off != 0xffffffffu) v = __ldg(Dh + pe.off + oa * pe.sr + X.row_orb[1][col] * pe.sc);
                 }
             }
             d[j][h] = v;
         }
 }
 
-__global__ void __launch_bounds__(GINT_THREADS, 1)
-k_rho_tile(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
-           const double* __restrict__ atom_pos, const int* __restrict__ atom_spec, const SpeciesDev* __restrict__ sp,
-           const double* __restrict__ tab, const int* __restrict__ crow, const u64* __restrict__ ckey,
-           const unsigned int* __restrict__ coff, int tab_cells, const double* __restrict__ Dh, double* __restrict__ rho) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    TileSmem& S = *reinterpret_cast<TileSmem*>(smem_raw);
-    {
-        TileView tv0;
-        tile_setup(g, S, tv0, tile, bstart, bent, atom_pos, atom_spec, sp, crow, ckey, coff, tab, tab_cells, nullptr);
-    }
-    const int nchunk = S.tv.nchunk;
-    if (nchunk == 0) return;
-    const int warp = threadIdx.x >> 5;
-    if (warp >= GINT_MMA_WARPS) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(GINT_REGS_EVAL_RHO));
-        producer_loop<false>(g, S, nchunk, tab, tab_cells, nullptr);
-        return;
-    }
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(GINT_REGS_MMA_RHO));
-    const int lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
-    Seg sg[GINT_WARP_SEGS];
-    double d[GINT_WARP_SEGS][GINT_SEG_COLS][2];
-#pragma unroll
-    for (int k = 0; k < GINT_WARP_SEGS; k++) {
-        sg[k] = load_seg(S, warp + GINT_MMA_WARPS * k, S.tv.diag);
-        load_dseg(S, sg[k], Dh, d[k]);
-    }
-    const unsigned phi0 = smem_addr(&S.phi[0][0][0][0]);
-    unsigned lane_i = phi0 + lc * GINT_ROWB + ((lr >> 1) + 4 * (lr & 1)) * 8;      // Phi_I: row lc of the k-step, point pi(lr)
-    unsigned lane_j = phi0 + lr * GINT_ROWB + lc * 8;                              // Phi_J: row lr, point lc (+4)
-    asm volatile("" : "+r"(lane_i), "+r"(lane_j));
-    for (int c = 0; c < nchunk; c++) {
-        const int s = c % GINT_STAGES;
-        if (c == 64 / GINT_CUBS) {      // the activity words cover 64 list positions: switch to the second half
-#pragma unroll
-            for (int k = 0; k < GINT_WARP_SEGS; k++) sg[k].W = S.segWhi[warp + GINT_MMA_WARPS * k];
-        }
-        double part[4][2];
-#pragma unroll
-        for (int q = 0; q < 4; q++) { part[q][0] = 0.0; part[q][1] = 0.0; }
-        mbar_wait(&S.full[s], (c / GINT_STAGES) & 1);
-        unsigned any = 0;
+template <bool VLOCAL>
+__device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restrict__ Dh, double* __restrict__ Hc) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
+    const unsigned ring0 = smem_addr(&S.ring[0][0]);
+    // lane parts of the operand addresses
+    const unsigned lane_v = lr * GINT_ROW_BYTES + lc * 16;                 // row lr of a fragment, points 2 lc, 2 lc + 1
+    const unsigned lane_j = lc * GINT_ROW_BYTES + lr * 8;                  // gint_rho B operand: row lc of the k-step, point lr
+    int gs = 0;                                                            // ring stages consumed
+    for (int t = 0;; t++) {
+        const int c = t % GINT_NCTX;
+        mbar_wait(&S.ctx_full[c], (t / GINT_NCTX) & 1);
+        const TileCtx& X = S.ctx[c];
+        if (!X.valid) break;
+        DBG_T(t_tile0);
+        Seg sg[GINT_WARP_SEGS];
+        double acc[GINT_WARP_SEGS][GINT_SEG_COLS][2];      // gint_vlocal: accumulators; gint_rho: stationary D operands
 #pragma unroll
         for (int k = 0; k < GINT_WARP_SEGS; k++) {
-            const unsigned bits = stage_steps(sg[k].W, c);
-            any |= bits;
-            if (bits) rho_seg_dispatch(sg[k].n(), d[k], lane_i + s * GINT_STAGEB + sg[k].oa, lane_j + s * GINT_STAGEB + sg[k].ob, bits, part);
+            sg[k] = load_seg(X, warp + GINT_MMA_WARPS * k);
+            if (VLOCAL) {
+#pragma unroll
+                for (int j = 0; j < GINT_SEG_COLS; j++) { acc[k][j][0] = 0.0; acc[k][j][1] = 0.0; }
+            } else {
+                load_dseg(X, sg[k], Dh, acc[k]);
+            }
+        }
+        const int nstage = X.nstage, ncub = X.ncub;
+        const unsigned pw0 = smem_addr(&X.pw[0][0]) + lc * 16;
+        DBG_T(t_tile1);
+        DBG_ADD(0, t_tile1 - t_tile0);
+        for (int st = 0; st < nstage; st++, gs++) {
+            const int s = gs % GINT_NS;
+            DBG_T(t_w0);
+            mbar_wait(&S.full[s], (gs / GINT_NS) & 1);
+            DBG_T(t_w1);
+            DBG_ADD(1, t_w1 - t_w0);
+            double part[GINT_SC][2];
+#pragma unroll
+            for (int q = 0; q < GINT_SC; q++) { part[q][0] = 0.0; part[q][1] = 0.0; }
+#pragma unroll
+            for (int q = 0; q < GINT_SC; q++) {
+                const int pos = st * GINT_SC + q;
+                if (pos < ncub) {
+                    const unsigned info = X.cubinfo[pos];
+                    const unsigned base = ring0 + s * GINT_STAGE_BYTES + q * 2 * GINT_SLOT_MAX_BYTES;
+#pragma unroll
+                    for (int k = 0; k < GINT_WARP_SEGS; k++) {
+                        const unsigned m = ((info >> sg[k].row()) & 1u) ? ((info >> (16 + sg[k].cb())) & ((1u << sg[k].n()) - 1u)) : 0u;
+                        if (m) {
+                            if (VLOCAL) vl_seg(acc[k], base + sg[k].oa + lane_v, base + sg[k].ob + lane_v, pw0 + pos * 64, m);
+                            else rho_seg(acc[k], base + sg[k].oa + lane_v, base + sg[k].ob + lane_j, m, part[q][0], part[q][1]);
+                        }
+                    }
+                }
+            }
+            if (!VLOCAL) {
+                // part[q][e]: point 2 lc + e of cubelet q, partial over the lane's orbital row lr -> sum over lr (lane bits 2..4)
+                const bool hi = lane & 16, mid = lane & 8;
+                double r2[2];
+#pragma unroll
+                for (int e = 0; e < 2; e++) {
+                    const double keep = hi ? part[GINT_SC - 1][e] : part[0][e], send = hi ? part[0][e] : part[GINT_SC - 1][e];
+                    r2[e] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+                }
+                const double keep = mid ? r2[1] : r2[0], send = mid ? r2[0] : r2[1];
+                double r1 = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+                r1 += __shfl_xor_sync(0xffffffffu, r1, 4);
+                // the lane holds cubelet (lane >> 4) & 1, point 2 lc + ((lane >> 3) & 1)
+                if (!(lane & 4)) S.part[s][warp][((lane >> 4) & 1) * GINT_CPTS + 2 * lc + ((lane >> 3) & 1)] = r1;
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&S.empty[s]);
+            DBG_T(t_w2);
+            DBG_ADD(2, t_w2 - t_w1);
+        }
+        DBG_T(t_loop);
+        if (VLOCAL) {
+            // flush: element (row, col) -> atom pair (a, b), orbitals (oa, ob) -> canonical block (transposed if the canonical
+            // key is (b, a)).  Exact zeros (fragments never touched, atoms that do not overlap inside this batch) are skipped.
+#pragma unroll
+            for (int k = 0; k < GINT_WARP_SEGS; k++) {
+                if (sg[k].n() == 0) continue;
+                const int row = 8 * sg[k].row() + lr;
+                const int a = X.row_atom[0][row], oa = X.row_orb[0][row];
+                if (a == 255) continue;
+#pragma unroll
+                for (int j = 0; j < GINT_SEG_COLS; j++) {
+                    if (j >= sg[k].n()) break;
+#pragma unroll
+                    for (int e = 0; e < 2; e++) {
+                        const double v = acc[k][j][e];
+                        const int col = 8 * (sg[k].cb() + j) + 2 * lc + e;
+                        const int bb = X.row_atom[1][col], ob = X.row_orb[1][col];
+                        if (bb == 255 || v == 0.0) continue;
+                        const PairEnt pe = X.pair[a][bb];
+                        if (pe.off == 0xffffffffu) continue;
+                        atomicAdd(Hc + pe.off + oa * pe.sr + ob * pe.sc, v);
+                    }
+                }
+            }
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(&S.empty[s]);
-        if (!any) continue;
-        // part[q][e]: point lc + 4e of cubelet q, partial over the lane's orbital row lr -> reduce-scatter over lr (lane bits 2..4)
-        double r4[4], r2[2], r1;
-        {
-            const bool hi = lane & 16;
-#pragma unroll
-            for (int i = 0; i < 4; i++) {     // value index t = 2q + e; lanes with bit 4 clear keep t < 4
-                const double keep = hi ? part[2 + (i >> 1)][i & 1] : part[i >> 1][i & 1];
-                const double send = hi ? part[i >> 1][i & 1] : part[2 + (i >> 1)][i & 1];
-                r4[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-            }
-            const bool mid = lane & 8;
-#pragma unroll
-            for (int i = 0; i < 2; i++) {
-                const double keep = mid ? r4[2 + i] : r4[i], send = mid ? r4[i] : r4[2 + i];
-                r2[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-            }
-            const bool low = lane & 4;
-            const double keep = low ? r2[1] : r2[0], send = low ? r2[0] : r2[1];
-            r1 = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-        }
-        // the lane now owns value t = lr: point lc + 4 (lr & 1) of cubelet lr >> 1
-        int gi, gj, gk;
-        if (r1 != 0.0 && stage_point(S, c, 8 * (lr >> 1) + lc + 4 * (lr & 1), gi, gj, gk))
-            atomicAdd(rho + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk, r1);
+        if (lane == 0) mbar_arrive(&S.ctx_free[c]);
+        DBG_T(t_end);
+        DBG_ADD(3, t_end - t_loop);
+        DBG_ADD(4, t_end - t_tile0);
+        DBG_ADD(5, 1);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// gint_vlocal / gint_rho main kernels (north_star step 3): persistent, one CTA per SM.
+template <bool VLOCAL>
+__global__ void __launch_bounds__(GINT_CTA_THREADS, 1)
+k_tiles(Geom g, const int2* __restrict__ tile, int n_tiles, int* __restrict__ queue, const int* __restrict__ bstart,
+        const NeighEntry* __restrict__ bent, const int* __restrict__ gstart, const u64* __restrict__ goff, u64 wave_row0,
+        const double* __restrict__ phi, const int* __restrict__ atom_spec, const SpeciesDev* __restrict__ sp,
+        const int* __restrict__ crow, const u64* __restrict__ ckey, const unsigned int* __restrict__ coff,
+        const double* __restrict__ in /* V or Dh */, double* __restrict__ out /* Hc or rho */) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    TileSmem& S = *reinterpret_cast<TileSmem*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~(uintptr_t)127);
+    const int warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < GINT_NS; s++) { mbar_init(&S.full[s], 1); mbar_init(&S.empty[s], GINT_MMA_WARPS); }
+        for (int c = 0; c < GINT_NCTX; c++) { mbar_init(&S.ctx_full[c], 1); mbar_init(&S.ctx_free[c], GINT_MMA_WARPS + 1); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (warp < GINT_MMA_WARPS) {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(GINT_REGS_MMA));
+        consumer_role<VLOCAL>(S, in, out);
+    } else {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(GINT_REGS_AUX));
+        if (warp == GINT_MMA_WARPS) issuer_role<VLOCAL>(g, S, out);
+        else setup_role<VLOCAL>(g, S, tile, n_tiles, queue, bstart, bent, gstart, goff, wave_row0, phi, atom_spec, sp, crow, ckey, coff, in);
     }
 }
 
@@ -909,6 +884,76 @@ __global__ void __launch_bounds__(256) k_sym_D(long long n_canon, const long lon
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Phi layout (gint_init): rows of every (batch, group) slot array = (cubelets on which the group is active) x (orbital rows
+// padded to whole fragments).  One thread per batch.
+__global__ void __launch_bounds__(128) k_phi_rows(long long n_batch_total, const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
+                                                  const int* __restrict__ gstart, const int* __restrict__ atom_spec,
+                                                  const SpeciesDev* __restrict__ sp, unsigned* __restrict__ grows) {
+    const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= n_batch_total) return;
+    const int e0 = bstart[b], n = bstart[b + 1] - e0, G = gstart[b + 1] - gstart[b];
+    for (int k = 0; k < G; k++) {
+        cmask m = czero();
+        int rows = 0;
+        for (int e = group_begin(k, n, G); e < group_begin(k + 1, n, G); e++) {
+            const NeighEntry en = bent[e0 + e];
+            m |= cmask{en.mask[0], en.mask[1]};
+            rows += sp[atom_spec[en.atom]].norb;
+        }
+        grows[gstart[b] + k] = (unsigned)(ccount(m) * ((rows + 7) & ~7));
+    }
+}
+
+int gint_build_phi_layout(gint_ctx* c, const int* d_bgroups, size_t phi_cap_bytes) {
+    (void)d_bgroups;
+    const long long nbt = c->n_batch_total;
+    std::vector<int> gs(nbt + 1);
+    GINT_CUDA(cudaMemcpy(gs.data(), c->d_gstart, sizeof(int) * (nbt + 1), cudaMemcpyDeviceToHost));
+    const long long ng = gs[nbt];
+    unsigned* d_grows = nullptr;
+    GINT_CUDA(cudaMalloc(&d_grows, sizeof(unsigned) * (ng ? ng : 1)));
+    if (nbt > 0) k_phi_rows<<<(unsigned)((nbt + 127) / 128), 128>>>(nbt, c->d_bstart, c->d_bent, c->d_gstart, c->d_atom_species, c->d_species, d_grows);
+    GINT_CUDA(cudaGetLastError());
+    std::vector<unsigned> grows(ng);
+    if (ng) GINT_CUDA(cudaMemcpy(grows.data(), d_grows, sizeof(unsigned) * ng, cudaMemcpyDeviceToHost));
+    GINT_CUDA(cudaFree(d_grows));
+    std::vector<unsigned long long> goff(ng + 1);
+    unsigned long long acc = 0;
+    for (long long i = 0; i < ng; i++) { goff[i] = acc; acc += grows[i]; }
+    goff[ng] = acc;
+    c->phi_rows_total = acc;
+    std::vector<int> ts(nbt + 1);
+    GINT_CUDA(cudaMemcpy(ts.data(), c->d_tstart, sizeof(int) * (nbt + 1), cudaMemcpyDeviceToHost));
+    // waves: contiguous batch ranges of at most cap rows
+    const unsigned long long cap_rows = std::max<unsigned long long>(phi_cap_bytes / GINT_ROW_BYTES, 1);
+    c->waves.clear();
+    unsigned long long max_rows = 0;
+    long long b = 0;
+    while (b < nbt) {
+        gint_ctx::Wave w; w.b0 = b; w.row0 = goff[gs[b]];
+        unsigned long long rows = 0;
+        while (b < nbt) {
+            const unsigned long long br = goff[gs[b + 1]] - goff[gs[b]];
+            if (br > cap_rows) GINT_FAIL(GINT_ERR_OUT_OF_MEMORY, "orbital values of one batch (%llu bytes) exceed the scratch buffer", br * GINT_ROW_BYTES);
+            if (rows + br > cap_rows) break;
+            rows += br; b++;
+        }
+        w.b1 = b; w.rows = rows; w.t0 = ts[w.b0]; w.t1 = ts[w.b1];
+        if (w.t1 > w.t0) { c->waves.push_back(w); max_rows = std::max(max_rows, rows); }
+    }
+    goff.pop_back();
+    if (goff.empty()) goff.push_back(0);
+    GINT_CUDA(cudaMalloc((void**)&c->d_goff, sizeof(unsigned long long) * goff.size()));
+    GINT_CUDA(cudaMemcpy(c->d_goff, goff.data(), sizeof(unsigned long long) * goff.size(), cudaMemcpyHostToDevice));
+    c->device_bytes += sizeof(unsigned long long) * goff.size();
+    c->phi_bytes = (size_t)std::max<unsigned long long>(max_rows, 1) * GINT_ROW_BYTES;
+    GINT_CUDA(cudaMalloc((void**)&c->d_phi, c->phi_bytes));
+    c->device_bytes += c->phi_bytes;
+    GINT_CUDA(cudaMalloc((void**)&c->d_queue, sizeof(int) * (c->waves.size() + 1)));
+    return GINT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
 // algorithmic work counters (for the roofline numerator): per mesh point, the atoms with |d| < rc.
 __global__ void __launch_bounds__(128) k_alg_stats(Geom g, const int* __restrict__ bstart,
                                                    const NeighEntry* __restrict__ bent, const double* __restrict__ atom_pos,
@@ -928,9 +973,9 @@ __global__ void __launch_bounds__(128) k_alg_stats(Geom g, const int* __restrict
             for (int e = bstart[b]; e < bstart[b + 1]; e++) {
                 const NeighEntry en = bent[e];
                 int t1, t2, t3; unpack_shift(en.shift, t1, t2, t3);
-                const double dx = x - (atom_pos[3 * en.atom + 0] + t1 * g.a[0] + t2 * g.a[3] + t3 * g.a[6]);
-                const double dy = y - (atom_pos[3 * en.atom + 1] + t1 * g.a[1] + t2 * g.a[4] + t3 * g.a[7]);
-                const double dz = z - (atom_pos[3 * en.atom + 2] + t1 * g.a[2] + t2 * g.a[5] + t3 * g.a[8]);
+                double ax, ay, az;
+                image_pos(g, atom_pos + 3 * en.atom, t1, t2, t3, ax, ay, az);
+                const double dx = x - ax, dy = y - ay, dz = z - az;
                 const SpeciesDev* Sp = sp + atom_spec[en.atom];
                 if (fma(dx, dx, fma(dy, dy, dz * dz)) < Sp->rc * Sp->rc) { na++; no += Sp->norb; }
             }
@@ -947,9 +992,40 @@ __global__ void __launch_bounds__(128) k_alg_stats(Geom g, const int* __restrict
 // ---------------------------------------------------------------------------------------------------
 // host-side launchers
 int gint_configure_kernels(gint_ctx* c) {
-    const int smem = (int)c->smem_bytes;
-    GINT_CUDA(cudaFuncSetAttribute(k_vlocal_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    GINT_CUDA(cudaFuncSetAttribute(k_rho_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    // per function and device, not per context: set to what the kernels can ever need on this device
+    cudaDeviceProp prop;
+    GINT_CUDA(cudaGetDeviceProperties(&prop, c->device));
+    const int lim = (int)prop.sharedMemPerBlockOptin;
+    GINT_CUDA(cudaFuncSetAttribute(k_tiles<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim));
+    GINT_CUDA(cudaFuncSetAttribute(k_tiles<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim));
+    GINT_CUDA(cudaFuncSetAttribute(k_eval_phi<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim));
+    GINT_CUDA(cudaFuncSetAttribute(k_eval_phi<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim));
+    c->n_sm = prop.multiProcessorCount;
+    return GINT_OK;
+}
+
+// one wave: evaluate the orbital values of its batches, then contract its tiles
+template <bool VLOCAL>
+static int launch_waves(gint_ctx* c, const double* in, double* out, cudaStream_t st) {
+    if (c->waves.empty()) return GINT_OK;
+    GINT_CUDA(cudaMemsetAsync(c->d_queue, 0, sizeof(int) * c->waves.size(), st));
+    const int tab_cells = (int)(c->tab_bytes / 16);
+    for (size_t w = 0; w < c->waves.size(); w++) {
+        const gint_ctx::Wave& W = c->waves[w];
+        const unsigned nb = (unsigned)(W.b1 - W.b0);
+        if (c->tab_in_smem)
+            k_eval_phi<true><<<nb, GINT_EVAL_THREADS, c->smem_eval, st>>>(c->geom, W.b0, c->d_bstart, c->d_bent, c->d_gstart, c->d_goff, W.row0,
+                c->d_atom_pos, c->d_atom_species, c->d_species, c->d_tab, tab_cells, c->d_phi);
+        else
+            k_eval_phi<false><<<nb, GINT_EVAL_THREADS, c->smem_eval, st>>>(c->geom, W.b0, c->d_bstart, c->d_bent, c->d_gstart, c->d_goff, W.row0,
+                c->d_atom_pos, c->d_atom_species, c->d_species, c->d_tab, tab_cells, c->d_phi);
+        GINT_CUDA(cudaGetLastError());
+        const int nt = (int)(W.t1 - W.t0);
+        const unsigned grid = (unsigned)std::min<long long>(c->n_sm, nt);
+        k_tiles<VLOCAL><<<grid, GINT_CTA_THREADS, c->smem_bytes, st>>>(c->geom, c->d_tile + W.t0, nt, c->d_queue + w, c->d_bstart, c->d_bent,
+            c->d_gstart, c->d_goff, W.row0, c->d_phi, c->d_atom_species, c->d_species, c->d_crow, c->d_ckey, c->d_coff, in, out);
+        GINT_CUDA(cudaGetLastError());
+    }
     return GINT_OK;
 }
 
@@ -959,9 +1035,8 @@ int gint_launch_vlocal(gint_ctx* c, const double* V, double* H, cudaStream_t st)
     GINT_CUDA(cudaMemsetAsync(c->d_cval, 0, sizeof(double) * (size_t)c->n_cvalues, st));
     if (c->n_tiles > 0) {
         GINT_CUDA(cudaEventRecord(c->ev[0], st));
-        k_vlocal_tile<<<(unsigned)c->n_tiles, GINT_THREADS, c->smem_bytes, st>>>(c->geom, c->d_tile, c->d_bstart, c->d_bent, c->d_atom_pos,
-            c->d_atom_species, c->d_species, c->d_tab, c->d_crow, c->d_ckey, c->d_coff, c->tab_in_smem ? (int)(c->tab_bytes / 16) : 0, V, c->d_cval);
-        GINT_CUDA(cudaGetLastError());
+        int rc = launch_waves<true>(c, V, c->d_cval, st);
+        if (rc) return rc;
         GINT_CUDA(cudaEventRecord(c->ev[1], st));
         c->timed[0] = true;
     }
@@ -978,9 +1053,8 @@ int gint_launch_rho(gint_ctx* c, const double* D, double* rho, cudaStream_t st) 
     k_sym_D<<<(unsigned)((c->n_canon + 7) / 8), 256, 0, st>>>(c->n_canon, c->d_poff, c->d_cpub, c->d_cmir, c->d_pnA, c->d_coff, D, c->d_cval);
     GINT_CUDA(cudaGetLastError());
     GINT_CUDA(cudaEventRecord(c->ev[2], st));
-    k_rho_tile<<<(unsigned)c->n_tiles, GINT_THREADS, c->smem_bytes, st>>>(c->geom, c->d_tile, c->d_bstart, c->d_bent, c->d_atom_pos,
-        c->d_atom_species, c->d_species, c->d_tab, c->d_crow, c->d_ckey, c->d_coff, c->tab_in_smem ? (int)(c->tab_bytes / 16) : 0, c->d_cval, rho);
-    GINT_CUDA(cudaGetLastError());
+    int rc = launch_waves<false>(c, c->d_cval, rho, st);
+    if (rc) return rc;
     GINT_CUDA(cudaEventRecord(c->ev[3], st));
     c->timed[1] = true;
     return GINT_OK;

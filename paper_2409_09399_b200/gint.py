@@ -17,7 +17,8 @@ _lib = None
 
 STAT_NAMES = ("n_batch", "n_batch_empty", "batch_bx", "batch_by", "batch_bz", "neigh_entries", "max_nb", "max_cols",
               "padded_macs", "n_canon", "alg_incidence", "alg_sum_n", "alg_sum_n2", "nonempty_points", "smem_bytes",
-              "device_bytes", "launches_vlocal", "launches_rho")
+              "device_bytes", "launches_vlocal", "launches_rho", "smem_eval", "tab_in_smem", "phi_bytes", "phi_scratch_bytes",
+              "n_waves", "n_tiles")
 
 EXPORTS = ("gint_init", "gint_n_orb", "gint_n_pairs", "gint_get_pairs", "gint_vlocal", "gint_rho", "gint_vlocal_host",
            "gint_rho_host", "gint_stats", "gint_kernel_times", "gint_free", "gint_last_error")
@@ -110,10 +111,9 @@ class Gint:
         return {"vlocal_main": float(out[0]), "rho_main": float(out[1])}
 
     # ------------------------------------------------------------------ device path
-    @staticmethod
-    def _stream():
+    def _stream(self):
         import torch
-        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+        return C.c_void_p(torch.cuda.current_stream(self.device).cuda_stream)
 
     def _dev_check(self, t, n, name):
         import torch
