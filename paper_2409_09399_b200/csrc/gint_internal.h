@@ -23,14 +23,14 @@
 #define GINT_TILE_ATOMS 8          // atom images per group
 #define GINT_TILE_ORB 104          // orbitals per group = 13 fragments of 8 (8 atoms x 13 orbitals exactly)
 #define GINT_TILE_FRAG 13
-#define GINT_SEG_COLS 7            // column fragments of one segment (row fragment x <= 7 column fragments)
-#define GINT_WARP_SEGS 4           // segments per consumer warp
-#define GINT_MMA_WARPS 8           // warp groups 0,1: DMMA consumers
-#define GINT_MAX_SEG (GINT_WARP_SEGS * GINT_MMA_WARPS)
-#define GINT_AUX_WARPS 4           // warp group 2: warp 8 = TMA issuer (+ rho reducer), warps 9..11 = tile set-up
+#define GINT_SEG_COLS 7            // column fragments of one segment
+#define GINT_MMA_WARPS 12          // warp groups 0,1,2: DMMA consumers, three per SM sub-partition; each owns up to GINT_WARP_BLOCKS blocks
+                                   // of 2 row fragments x 4 (block 0) or 3 (blocks 1, 2) column fragments of the tile
+#define GINT_WARP_BLOCKS 3
+#define GINT_AUX_WARPS 4           // warp group 3: warp 12 = TMA issuer (+ rho reducer), warps 13..15 = tile set-up
 #define GINT_SETUP_THREADS 96
 #define GINT_CTA_THREADS (32 * (GINT_MMA_WARPS + GINT_AUX_WARPS))
-#define GINT_REGS_MMA 224          // registers per thread after setmaxnreg: 256 * 224 + 128 * 56 = 64512 <= 65536
+#define GINT_REGS_MMA 152          // registers per thread after setmaxnreg: 384 * 152 + 128 * 56 = 65536
 #define GINT_REGS_AUX 56
 // orbital values ("Phi") in global memory: one SLOT per (atom group, active cubelet) = [orbital row][8 points] doubles,
 // rows padded to whole fragments; 64 bytes per row = the unit of all Phi offsets

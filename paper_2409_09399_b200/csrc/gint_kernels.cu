@@ -61,7 +61,7 @@ __device__ __forceinline__ void cubelet_point(int cl, int p, int& ix, int& iy, i
 #else
 __device__ unsigned long long g_dbg[16];
 #define DBG_T(x) const long long x = clock64()
-#define DBG_ADD(i, v) do { if ((threadIdx.x & 31) == 0) atomicAdd(&g_dbg[i], (unsigned long long)(v)); } while (0)
+#define DBG_ADD(i, v) dbg_acc[i] += (unsigned long long)(v)
 extern "C" int gint_debug_counters(unsigned long long* out) { return (int)cudaMemcpyFromSymbol(out, g_dbg, sizeof(g_dbg)); }
 extern "C" int gint_debug_reset() { unsigned long long z[16] = {0}; return (int)cudaMemcpyToSymbol(g_dbg, z, sizeof(z)); }
 #endif
@@ -229,8 +229,9 @@ k_eval_phi(Geom g, long long b0, const int* __restrict__ bstart, const NeighEntr
         }
 #undef GINT_PUT
     }
-    // ---- pass B: zero rows.  Inside a slot, a fragment that holds orbitals of an active atom is read whole by the
-    // contraction kernels: the rows of its inactive atoms and the padding rows behind the group's last orbital are zeros.
+    // ---- pass B: zero rows.  The contraction kernels read a slot in blocks of fragments and only test whether SOME row and SOME
+    // column fragment of a block is active on the cubelet: every row of a slot that no active atom owns (inactive atoms, the padding
+    // rows behind the group's last orbital) must hold zeros.
     const int n_z = S.zitem0[n];
     for (int it = qw; it < n_z; it += GINT_EVAL_THREADS / 8) {
         int lo = 0, hi = n - 1;
@@ -238,17 +239,12 @@ k_eval_phi(Geom g, long long b0, const int* __restrict__ bstart, const NeighEntr
         const int e = lo, k = S.grp[e], slot = it - S.zitem0[e];
         const int cl = cselect(S.gmask[k], slot);
         const bool act = cbit(S.amask[e], cl);
-        const int f = S.gfirst[k], cnt = S.gcnt[k];
-        const bool last = e == f + cnt - 1;
+        const bool last = e == S.gfirst[k] + S.gcnt[k] - 1;
         int r0 = S.row0[e], r1 = r0 + S.norb[e];
         if (act) r0 = r1;                               // an active atom's own rows were written by pass A
         if (last) r1 = S.gR[k];                         // padding rows
-        if (r0 >= r1) continue;
-        unsigned fact = 0;                              // fragments with an active atom
-        for (int a = f; a < f + cnt; a++)
-            if (cbit(S.amask[a], cl)) { const int q0 = S.row0[a] >> 3, q1 = (S.row0[a] + S.norb[a] - 1) >> 3; fact |= (2u << q1) - (1u << q0); }
         double* o0 = phi + ((S.gbase[k] + (u64)slot * S.gR[k]) << 3) + pl;
-        for (int rr = r0; rr < r1; rr++) if ((fact >> (rr >> 3)) & 1u) o0[rr << 3] = 0.0;
+        for (int rr = r0; rr < r1; rr++) o0[rr << 3] = 0.0;
     }
 }
 
@@ -262,7 +258,9 @@ struct alignas(16) TileCtx {
     int nI, nJ, nfI, nfJ, RI, RJ, diag;
     int i0, j0, k0, ex, ey, ez;         // batch origin and extents (mesh points)
     const double *srcI, *srcJ;          // slot arrays of the two groups
-    int seg[GINT_MAX_SEG];              // consumer warp w, segment k at [w + 8 k]: row fragment | first column fragment << 8 | n columns << 16
+    unsigned blk[GINT_WARP_BLOCKS][GINT_MMA_WARPS];   // consumer warp w, block k: first row fragment | second row present << 4 | first column
+                                        // fragment << 5 | n column fragments << 9   (n = 0: unused).  Block 0 holds up to 4 columns, blocks 1, 2 up to 3.
+    int zero;                           // always 0: the consumers' opaque loop condition (keeps ptxas from predicating the DMMA blocks)
     unsigned cubinfo[GINT_NCUB];        // per listed cubelet: active row fragments of I | active column fragments of J << 16
     unsigned short slotI[GINT_NCUB], slotJ[GINT_NCUB];     // slot of the listed cubelet inside the groups' slot arrays
     unsigned char cub[GINT_NCUB];       // the listed cubelets (bit numbers of the batch's masks, ascending)
@@ -400,41 +398,71 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileCtx& 
             before += __popc(Uw[wd]);
         }
         if (lane == 0) { X.ncub = before; X.nstage = (before + GINT_SC - 1) / GINT_SC; }
-    } else if (sw == 1) {
-        // segments: piece (row fragment r, half h) = columns [cb, cb + n); sorted by falling n and dealt to the
-        // sub-partitions 0,1,2,3,3,2,1,0,... (consumer warp w runs on sub-partition w % 4)
-        X.seg[lane] = 0;
-        __syncwarp();
-        int pn = 0, pcb = 0;
-        const int r = lane >> 1, h = lane & 1;
-        if (lane < 2 * GINT_TILE_FRAG && r < nfI) {
-            const int cf = diag ? (Q.cstart[1][X.row_atom[0][8 * r]] >> 3) : 0;
-            if (h == 0) { pcb = cf; pn = min(GINT_SEG_COLS, nfJ) - cf; }
-            else { pcb = max(GINT_SEG_COLS, cf); pn = nfJ - pcb; }
-            pn = max(pn, 0);
-        }
-        int rank = 0;
-        for (int j = 0; j < 2 * GINT_TILE_FRAG; j++) {
-            const int nj = __shfl_sync(0xffffffffu, pn, j);
-            rank += (nj > pn) || (nj == pn && j < lane);
-        }
-        if (pn > 0) {
-            const int k7 = rank & 7, s = k7 < 4 ? k7 : 7 - k7, j = 2 * (rank >> 3) + (k7 >= 4);
-            X.seg[s + 4 * (j & 1) + GINT_MMA_WARPS * (j >> 1)] = r | (pcb << 8) | (pn << 16);
-        }
-    } else if (lane == 0) {
+    } else if (sid == 32) {
         const int bz = b % g.nb[2], by = (b / g.nb[2]) % g.nb[1], bx = b / (g.nb[2] * g.nb[1]);
         X.i0 = bx * g.bs[0]; X.j0 = by * g.bs[1]; X.k0 = bz * g.bs[2];
         X.ex = min(g.bs[0], g.N[0] - X.i0); X.ey = min(g.bs[1], g.N[1] - X.j0); X.ez = min(g.bs[2], g.N[2] - X.k0);
         X.nI = nI; X.nJ = nJ; X.nfI = nfI; X.nfJ = nfJ; X.RI = 8 * nfI; X.RJ = 8 * nfJ; X.diag = diag;
         X.srcI = phi + ((goff[gstart[b] + I] - wave_row0) << 3);
         X.srcJ = phi + ((goff[gstart[b] + J] - wave_row0) << 3);
-        X.valid = 1;
+        X.valid = 1; X.zero = 0;
+    } else if (sid == 64) {
+        // Block plan.  The 13 x 13 fragments of the tile are cut into blocks of two adjacent row fragments x 3 or 4 adjacent column
+        // fragments (neighbours are sorted by falling activity, so the fragments of a block have similar activity masks).  A block is
+        // worked on a cubelet iff one of its rows and one of its columns are active there; its cost = 4 n DMMAs per such cubelet.
+        // In a diagonal tile only blocks that reach the atom diagonal or lie above it exist.  Blocks are dealt heaviest first to the
+        // least loaded SM sub-partition (consumer warp w runs on sub-partition w % 4) and there to the least loaded warp with a free slot.
+        for (int k = 0; k < GINT_WARP_BLOCKS; k++) for (int w = 0; w < GINT_MMA_WARPS; w++) X.blk[k][w] = 0;
+        unsigned desc[28];
+        int wgt[28], np = 0;
+        // column groups of 3 fragments; one group of 4 (the first: the densest columns) when 3 does not divide evenly, else a last group of 2
+        const int ng = nfJ <= 4 ? 1 : (nfJ + 2) / 3 - (nfJ % 3 == 1);
+        for (int r0 = 0; r0 < nfI; r0 += 2) {
+            const bool has1 = r0 + 1 < nfI;
+            const int cf0 = diag ? (Q.cstart[1][X.row_atom[0][8 * r0]] >> 3) : 0;
+            const cmask rm = has1 ? (Q.fmask[0][r0] | Q.fmask[0][r0 + 1]) : Q.fmask[0][r0];
+            int c0 = 0;
+            for (int gi = 0; gi < ng; gi++) {
+                const int n = ng == 1 ? nfJ : ((gi == 0 && nfJ % 3 == 1) ? 4 : min(3, nfJ - c0));
+                if (c0 + n > cf0) {                    // the block holds a fragment on or above the diagonal
+                    cmask cm = czero();
+                    for (int j = 0; j < n; j++) cm |= Q.fmask[1][c0 + j];
+                    desc[np] = (unsigned)r0 | ((unsigned)has1 << 4) | ((unsigned)c0 << 5) | ((unsigned)n << 9);
+                    wgt[np] = ccount(rm & cm) * n * (has1 ? 2 : 1);
+                    np++;
+                }
+                c0 += n;
+            }
+        }
+        for (int i = 1; i < np; i++) {      // insertion sort by falling weight
+            const unsigned d = desc[i]; const int w = wgt[i];
+            int j = i - 1;
+            while (j >= 0 && wgt[j] < w) { desc[j + 1] = desc[j]; wgt[j + 1] = wgt[j]; j--; }
+            desc[j + 1] = d; wgt[j + 1] = w;
+        }
+        int lsm[4] = {0, 0, 0, 0}, lw[GINT_MMA_WARPS], used[GINT_MMA_WARPS];
+        for (int w = 0; w < GINT_MMA_WARPS; w++) { lw[w] = 0; used[w] = 0; }      // used: bit k = block slot k taken
+        for (int pass = 0; pass < 2; pass++)            // the 4-column blocks first: only block slot 0 holds them (at most 7 of them, 12 slots)
+            for (int i = 0; i < np; i++) {
+                const bool wide = ((desc[i] >> 9) & 15u) > 3;
+                if (wide != (pass == 0)) continue;
+                int best = -1;
+                for (int w = 0; w < GINT_MMA_WARPS; w++) {
+                    const bool free_slot = wide ? !(used[w] & 1) : used[w] != 7;
+                    if (!free_slot) continue;
+                    if (best < 0 || lsm[w & 3] < lsm[best & 3] || (lsm[w & 3] == lsm[best & 3] && lw[w] < lw[best])) best = w;
+                }
+                if (best < 0) __trap();     // cannot happen: at most 28 blocks for 36 slots
+                int k = 0;
+                if (!wide) k = !(used[best] & 2) ? 1 : (!(used[best] & 4) ? 2 : 0);
+                used[best] |= 1 << k; lsm[best & 3] += wgt[i]; lw[best] += wgt[i];
+                X.blk[k][best] = desc[i];
+            }
     }
     setup_sync();
-    // per listed cubelet: which fragments are active, and the points' weights
     const int ncub = X.ncub;
     const int bi0 = X.i0, bj0 = X.j0, bk0 = X.k0, ex = X.ex, ey = X.ey, ez = X.ez;
+    // per listed cubelet: which fragments are active, and the points' weights
     for (int pos = sid; pos < ncub; pos += GINT_SETUP_THREADS) {
         const int cl = X.cub[pos];
         unsigned info = 0;
@@ -534,9 +562,15 @@ __device__ __forceinline__ void issuer_role(const Geom& g, TileSmem& S, double* 
             const int s = gi % GINT_NS;
             while (gi - gr >= GINT_NS) { retire_stage<VLOCAL>(g, S, gr, rho); gr++; }
             const int ncs = min(GINT_SC, ncub - st * GINT_SC);
+#ifdef GINT_DBG_NO_TMA
+            if (lane == 0) { mbar_arrive(&S.full[s]); S.hist[s] = c | (st << 8); }
+            __syncwarp();
+            if (false) {
+#else
             if (lane == 0) { mbar_expect_tx(&S.full[s], (unsigned)ncs * (bI + bJ)); S.hist[s] = c | (st << 8); }
             __syncwarp();
             if (lane < ncs) {
+#endif
                 const int pos = st * GINT_SC + lane;
                 const unsigned dst = smem_addr(&S.ring[s][lane * 2 * GINT_SLOT_MAX_BYTES]);
                 bulk_g2s(dst, reinterpret_cast<const unsigned char*>(srcI) + (size_t)X.slotI[pos] * bI, bI, &S.full[s]);
@@ -559,139 +593,196 @@ __device__ __forceinline__ double2 lds128(unsigned addr) {
     asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory");
     return v;
 }
-struct Seg {
-    unsigned oa, ob;                 // byte offsets of the row fragment (side I) and of the first column fragment (side J) inside a cubelet of a stage
-    int w;                           // row fragment | first column fragment << 8 | column fragments << 16 (0: unused)
-    __device__ __forceinline__ int row() const { return w & 255; }
-    __device__ __forceinline__ int cb() const { return (w >> 8) & 255; }
-    __device__ __forceinline__ int n() const { return w >> 16; }
+__device__ __forceinline__ double lds64(unsigned addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr) : "memory");
+    return v;
+}
+#define GINT_DMMA(c0, c1, a, b) "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {" c0 "," c1 "},{" a "},{" b "},{" c0 "," c1 "};\n\t"
+// A DMMA that is predicated off still occupies the FP64 tensor pipe for its 16 cycles (measured), and ptxas turns a
+// forward branch over a few DMMAs into predication.  So every skippable DMMA sequence is written as a loop with an opaque,
+// never-taken back edge (q == 0 at run time): ptxas keeps the branch, and skipped work costs no pipe time.  Taken
+// branches cost a warp ~15-20 cycles each, so the unit of skipping is a whole block (2 x 3..4 fragments) on a cubelet,
+// with three straight-line variants: both rows, only row 0, only row 1.
+//
+// gint_vlocal block, both rows: c[r][j] += a_r b_j over the two k-steps (x, y) of the cubelet.  All x-steps first: the two DMMAs
+// of one accumulator are 2 N apart (a dependent DMMA waits 26 cycles, an independent one issues every 16).
+template <int N>
+__device__ __forceinline__ void vl_blk2(double (&c)[2][4][2], double a0x, double a0y, double a1x, double a1y, const double2 (&b)[4], int q) {
+    if (N == 4) {
+        asm volatile(
+            "{\n\t.reg .pred pq;\n\tsetp.ne.s32 pq, %28, 0;\n\tL_%=:\n\t"
+            GINT_DMMA("%0", "%1", "%16", "%20") GINT_DMMA("%8", "%9", "%18", "%20") GINT_DMMA("%2", "%3", "%16", "%22") GINT_DMMA("%10", "%11", "%18", "%22")
+            GINT_DMMA("%4", "%5", "%16", "%24") GINT_DMMA("%12", "%13", "%18", "%24") GINT_DMMA("%6", "%7", "%16", "%26") GINT_DMMA("%14", "%15", "%18", "%26")
+            GINT_DMMA("%0", "%1", "%17", "%21") GINT_DMMA("%8", "%9", "%19", "%21") GINT_DMMA("%2", "%3", "%17", "%23") GINT_DMMA("%10", "%11", "%19", "%23")
+            GINT_DMMA("%4", "%5", "%17", "%25") GINT_DMMA("%12", "%13", "%19", "%25") GINT_DMMA("%6", "%7", "%17", "%27") GINT_DMMA("%14", "%15", "%19", "%27")
+            "@pq bra.uni L_%=;\n\t}"
+            : "+d"(c[0][0][0]), "+d"(c[0][0][1]), "+d"(c[0][1][0]), "+d"(c[0][1][1]), "+d"(c[0][2][0]), "+d"(c[0][2][1]), "+d"(c[0][3][0]), "+d"(c[0][3][1]),
+              "+d"(c[1][0][0]), "+d"(c[1][0][1]), "+d"(c[1][1][0]), "+d"(c[1][1][1]), "+d"(c[1][2][0]), "+d"(c[1][2][1]), "+d"(c[1][3][0]), "+d"(c[1][3][1])
+            : "d"(a0x), "d"(a0y), "d"(a1x), "d"(a1y), "d"(b[0].x), "d"(b[0].y), "d"(b[1].x), "d"(b[1].y), "d"(b[2].x), "d"(b[2].y), "d"(b[3].x), "d"(b[3].y), "r"(q));
+    } else {
+        asm volatile(
+            "{\n\t.reg .pred pq;\n\tsetp.ne.s32 pq, %22, 0;\n\tL_%=:\n\t"
+            GINT_DMMA("%0", "%1", "%12", "%16") GINT_DMMA("%6", "%7", "%14", "%16") GINT_DMMA("%2", "%3", "%12", "%18") GINT_DMMA("%8", "%9", "%14", "%18")
+            GINT_DMMA("%4", "%5", "%12", "%20") GINT_DMMA("%10", "%11", "%14", "%20")
+            GINT_DMMA("%0", "%1", "%13", "%17") GINT_DMMA("%6", "%7", "%15", "%17") GINT_DMMA("%2", "%3", "%13", "%19") GINT_DMMA("%8", "%9", "%15", "%19")
+            GINT_DMMA("%4", "%5", "%13", "%21") GINT_DMMA("%10", "%11", "%15", "%21")
+            "@pq bra.uni L_%=;\n\t}"
+            : "+d"(c[0][0][0]), "+d"(c[0][0][1]), "+d"(c[0][1][0]), "+d"(c[0][1][1]), "+d"(c[0][2][0]), "+d"(c[0][2][1]),
+              "+d"(c[1][0][0]), "+d"(c[1][0][1]), "+d"(c[1][1][0]), "+d"(c[1][1][1]), "+d"(c[1][2][0]), "+d"(c[1][2][1])
+            : "d"(a0x), "d"(a0y), "d"(a1x), "d"(a1y), "d"(b[0].x), "d"(b[0].y), "d"(b[1].x), "d"(b[1].y), "d"(b[2].x), "d"(b[2].y), "r"(q));
+    }
+}
+// one row of a block
+template <int N>
+__device__ __forceinline__ void vl_blk1(double (&c)[4][2], double ax, double ay, const double2 (&b)[4], int q) {
+    if (N == 4) {
+        asm volatile(
+            "{\n\t.reg .pred pq;\n\tsetp.ne.s32 pq, %18, 0;\n\tL_%=:\n\t"
+            GINT_DMMA("%0", "%1", "%8", "%10") GINT_DMMA("%2", "%3", "%8", "%12") GINT_DMMA("%4", "%5", "%8", "%14") GINT_DMMA("%6", "%7", "%8", "%16")
+            GINT_DMMA("%0", "%1", "%9", "%11") GINT_DMMA("%2", "%3", "%9", "%13") GINT_DMMA("%4", "%5", "%9", "%15") GINT_DMMA("%6", "%7", "%9", "%17")
+            "@pq bra.uni L_%=;\n\t}"
+            : "+d"(c[0][0]), "+d"(c[0][1]), "+d"(c[1][0]), "+d"(c[1][1]), "+d"(c[2][0]), "+d"(c[2][1]), "+d"(c[3][0]), "+d"(c[3][1])
+            : "d"(ax), "d"(ay), "d"(b[0].x), "d"(b[0].y), "d"(b[1].x), "d"(b[1].y), "d"(b[2].x), "d"(b[2].y), "d"(b[3].x), "d"(b[3].y), "r"(q));
+    } else {
+        asm volatile(
+            "{\n\t.reg .pred pq;\n\tsetp.ne.s32 pq, %14, 0;\n\tL_%=:\n\t"
+            GINT_DMMA("%0", "%1", "%6", "%8") GINT_DMMA("%2", "%3", "%6", "%10") GINT_DMMA("%4", "%5", "%6", "%12")
+            GINT_DMMA("%0", "%1", "%7", "%9") GINT_DMMA("%2", "%3", "%7", "%11") GINT_DMMA("%4", "%5", "%7", "%13")
+            "@pq bra.uni L_%=;\n\t}"
+            : "+d"(c[0][0]), "+d"(c[0][1]), "+d"(c[1][0]), "+d"(c[1][1]), "+d"(c[2][0]), "+d"(c[2][1])
+            : "d"(ax), "d"(ay), "d"(b[0].x), "d"(b[0].y), "d"(b[1].x), "d"(b[1].y), "d"(b[2].x), "d"(b[2].y), "r"(q));
+    }
+}
+// gint_rho block, both rows: y_r += sum_j D[r][j] b_j (two chains, interleaved).  d[r][j][h]: stationary A operands, bx/by[j]: the two k-steps of column j.
+template <int N>
+__device__ __forceinline__ void rho_blk2(const double (&d)[2][4][2], const double (&bx)[4], const double (&by)[4], int q, double (&y0)[2], double (&y1)[2]) {
+    if (N == 4) {
+        asm volatile(
+            "{\n\t.reg .pred pq;\n\tsetp.ne.s32 pq, %28, 0;\n\tL_%=:\n\t"
+            GINT_DMMA("%0", "%1", "%4", "%20") GINT_DMMA("%2", "%3", "%12", "%20") GINT_DMMA("%0", "%1", "%5", "%24") GINT_DMMA("%2", "%3", "%13", "%24")
+            GINT_DMMA("%0", "%1", "%6", "%21") GINT_DMMA("%2", "%3", "%14", "%21") GINT_DMMA("%0", "%1", "%7", "%25") GINT_DMMA("%2", "%3", "%15", "%25")
+            GINT_DMMA("%0", "%1", "%8", "%22") GINT_DMMA("%2", "%3", "%16", "%22") GINT_DMMA("%0", "%1", "%9", "%26") GINT_DMMA("%2", "%3", "%17", "%26")
+            GINT_DMMA("%0", "%1", "%10", "%23") GINT_DMMA("%2", "%3", "%18", "%23") GINT_DMMA("%0", "%1", "%11", "%27") GINT_DMMA("%2", "%3", "%19", "%27")
+            "@pq bra.uni L_%=;\n\t}"
+            : "+d"(y0[0]), "+d"(y0[1]), "+d"(y1[0]), "+d"(y1[1])
+            : "d"(d[0][0][0]), "d"(d[0][0][1]), "d"(d[0][1][0]), "d"(d[0][1][1]), "d"(d[0][2][0]), "d"(d[0][2][1]), "d"(d[0][3][0]), "d"(d[0][3][1]),
+              "d"(d[1][0][0]), "d"(d[1][0][1]), "d"(d[1][1][0]), "d"(d[1][1][1]), "d"(d[1][2][0]), "d"(d[1][2][1]), "d"(d[1][3][0]), "d"(d[1][3][1]),
+              "d"(bx[0]), "d"(bx[1]), "d"(bx[2]), "d"(bx[3]), "d"(by[0]), "d"(by[1]), "d"(by[2]), "d"(by[3]), "r"(q));
+    } else {
+        asm volatile(
+            "{\n\t.reg .pred pq;\n\tsetp.ne.s32 pq, %22, 0;\n\tL_%=:\n\t"
+            GINT_DMMA("%0", "%1", "%4", "%16") GINT_DMMA("%2", "%3", "%10", "%16") GINT_DMMA("%0", "%1", "%5", "%19") GINT_DMMA("%2", "%3", "%11", "%19")
+            GINT_DMMA("%0", "%1", "%6", "%17") GINT_DMMA("%2", "%3", "%12", "%17") GINT_DMMA("%0", "%1", "%7", "%20") GINT_DMMA("%2", "%3", "%13", "%20")
+            GINT_DMMA("%0", "%1", "%8", "%18") GINT_DMMA("%2", "%3", "%14", "%18") GINT_DMMA("%0", "%1", "%9", "%21") GINT_DMMA("%2", "%3", "%15", "%21")
+            "@pq bra.uni L_%=;\n\t}"
+            : "+d"(y0[0]), "+d"(y0[1]), "+d"(y1[0]), "+d"(y1[1])
+            : "d"(d[0][0][0]), "d"(d[0][0][1]), "d"(d[0][1][0]), "d"(d[0][1][1]), "d"(d[0][2][0]), "d"(d[0][2][1]),
+              "d"(d[1][0][0]), "d"(d[1][0][1]), "d"(d[1][1][0]), "d"(d[1][1][1]), "d"(d[1][2][0]), "d"(d[1][2][1]),
+              "d"(bx[0]), "d"(bx[1]), "d"(bx[2]), "d"(by[0]), "d"(by[1]), "d"(by[2]), "r"(q));
+    }
+}
+// one row of a block: two chains (the x and the y k-steps), summed by the caller
+template <int N>
+__device__ __forceinline__ void rho_blk1(const double (&d)[4][2], const double (&bx)[4], const double (&by)[4], int q, double (&ya)[2], double (&yb)[2]) {
+    if (N == 4) {
+        asm volatile(
+            "{\n\t.reg .pred pq;\n\tsetp.ne.s32 pq, %20, 0;\n\tL_%=:\n\t"
+            GINT_DMMA("%0", "%1", "%4", "%12") GINT_DMMA("%2", "%3", "%5", "%16") GINT_DMMA("%0", "%1", "%6", "%13") GINT_DMMA("%2", "%3", "%7", "%17")
+            GINT_DMMA("%0", "%1", "%8", "%14") GINT_DMMA("%2", "%3", "%9", "%18") GINT_DMMA("%0", "%1", "%10", "%15") GINT_DMMA("%2", "%3", "%11", "%19")
+            "@pq bra.uni L_%=;\n\t}"
+            : "+d"(ya[0]), "+d"(ya[1]), "+d"(yb[0]), "+d"(yb[1])
+            : "d"(d[0][0]), "d"(d[0][1]), "d"(d[1][0]), "d"(d[1][1]), "d"(d[2][0]), "d"(d[2][1]), "d"(d[3][0]), "d"(d[3][1]),
+              "d"(bx[0]), "d"(bx[1]), "d"(bx[2]), "d"(bx[3]), "d"(by[0]), "d"(by[1]), "d"(by[2]), "d"(by[3]), "r"(q));
+    } else {
+        asm volatile(
+            "{\n\t.reg .pred pq;\n\tsetp.ne.s32 pq, %16, 0;\n\tL_%=:\n\t"
+            GINT_DMMA("%0", "%1", "%4", "%10") GINT_DMMA("%2", "%3", "%5", "%13") GINT_DMMA("%0", "%1", "%6", "%11") GINT_DMMA("%2", "%3", "%7", "%14")
+            GINT_DMMA("%0", "%1", "%8", "%12") GINT_DMMA("%2", "%3", "%9", "%15")
+            "@pq bra.uni L_%=;\n\t}"
+            : "+d"(ya[0]), "+d"(ya[1]), "+d"(yb[0]), "+d"(yb[1])
+            : "d"(d[0][0]), "d"(d[0][1]), "d"(d[1][0]), "d"(d[1][1]), "d"(d[2][0]), "d"(d[2][1]),
+              "d"(bx[0]), "d"(bx[1]), "d"(bx[2]), "d"(by[0]), "d"(by[1]), "d"(by[2]), "r"(q));
+    }
+}
+
+// Blocks of a consumer warp.
+#define GINT_FRAG_BYTES (8 * GINT_ROW_BYTES)
+struct Blk {
+    unsigned oa, ob;                 // byte offsets of the first row fragment (side I) and of the first column fragment (side J) inside a cubelet of a stage
+    unsigned d;                      // descriptor (TileCtx::blk)
+    __device__ __forceinline__ int row() const { return d & 15; }
+    __device__ __forceinline__ bool has1() const { return (d >> 4) & 1u; }
+    __device__ __forceinline__ int c0() const { return (d >> 5) & 15; }
+    __device__ __forceinline__ int n() const { return (d >> 9) & 7; }
 };
-__device__ __forceinline__ Seg load_seg(const TileCtx& X, int slot) {
-    Seg s; s.w = X.seg[slot];
-    s.oa = (unsigned)(s.row() * 8 * GINT_ROW_BYTES);
-    s.ob = (unsigned)((X.diag ? 0 : GINT_SLOT_MAX_BYTES) + s.cb() * 8 * GINT_ROW_BYTES);
+__device__ __forceinline__ Blk load_blk(const TileCtx& X, unsigned desc) {
+    Blk s; s.d = desc;
+    s.oa = (unsigned)(s.row() * GINT_FRAG_BYTES);
+    s.ob = (unsigned)((X.diag ? 0 : GINT_SLOT_MAX_BYTES) + s.c0() * GINT_FRAG_BYTES);
     return s;
 }
 
-// gint_vlocal, one segment on one cubelet: acc[j] += (w . Phi_I[row fragment])^T Phi_J[column fragment j] for the active j.
-// pa, pb: lane addresses of the row fragment / first column fragment; m: activity bits of the segment's columns.
-// Only the DMMAs are predicated: a predicated load would leave its destination "maybe defined", which keeps the register
-// live across the whole loop (ptxas then spills); inactive fragments of a slot hold finite values or are never multiplied.
-__device__ __forceinline__ void vl_seg(double (&acc)[GINT_SEG_COLS][2], unsigned pa, unsigned pb, unsigned pw, unsigned m) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p0, p1, p2, p3, p4, p5, p6;\n\t"
-        ".reg .f64 ax, ay, wx, wy, bx0, by0, bx1, by1, bx2, by2, bx3, by3, bx4, by4, bx5, by5, bx6, by6;\n\t"
-        ".reg .b32 t;\n\t"
-        "and.b32 t, %17, 1;  setp.ne.u32 p0, t, 0;\n\t"
-        "and.b32 t, %17, 2;  setp.ne.u32 p1, t, 0;\n\t"
-        "and.b32 t, %17, 4;  setp.ne.u32 p2, t, 0;\n\t"
-        "and.b32 t, %17, 8;  setp.ne.u32 p3, t, 0;\n\t"
-        "and.b32 t, %17, 16; setp.ne.u32 p4, t, 0;\n\t"
-        "and.b32 t, %17, 32; setp.ne.u32 p5, t, 0;\n\t"
-        "and.b32 t, %17, 64; setp.ne.u32 p6, t, 0;\n\t"
-        "ld.shared.v2.f64 {ax, ay}, [%14];\n\t"
-        "ld.shared.v2.f64 {wx, wy}, [%16];\n\t"
-        "ld.shared.v2.f64 {bx0, by0}, [%15];\n\t"
-        "ld.shared.v2.f64 {bx1, by1}, [%15 + 512];\n\t"
-        "ld.shared.v2.f64 {bx2, by2}, [%15 + 1024];\n\t"
-        "ld.shared.v2.f64 {bx3, by3}, [%15 + 1536];\n\t"
-        "ld.shared.v2.f64 {bx4, by4}, [%15 + 2048];\n\t"
-        "ld.shared.v2.f64 {bx5, by5}, [%15 + 2560];\n\t"
-        "ld.shared.v2.f64 {bx6, by6}, [%15 + 3072];\n\t"
-        "mul.f64 ax, ax, wx;\n\t"
-        "mul.f64 ay, ay, wy;\n\t"
-        "@p0 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{ax},{bx0},{%0,%1};\n\t"
-        "@p1 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{ax},{bx1},{%2,%3};\n\t"
-        "@p2 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{ax},{bx2},{%4,%5};\n\t"
-        "@p3 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{ax},{bx3},{%6,%7};\n\t"
-        "@p4 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%8,%9},{ax},{bx4},{%8,%9};\n\t"
-        "@p5 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%10,%11},{ax},{bx5},{%10,%11};\n\t"
-        "@p6 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%12,%13},{ax},{bx6},{%12,%13};\n\t"
-        "@p0 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{ay},{by0},{%0,%1};\n\t"
-        "@p1 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{ay},{by1},{%2,%3};\n\t"
-        "@p2 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{ay},{by2},{%4,%5};\n\t"
-        "@p3 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{ay},{by3},{%6,%7};\n\t"
-        "@p4 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%8,%9},{ay},{by4},{%8,%9};\n\t"
-        "@p5 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%10,%11},{ay},{by5},{%10,%11};\n\t"
-        "@p6 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%12,%13},{ay},{by6},{%12,%13};\n\t"
-        "}"
-        : "+d"(acc[0][0]), "+d"(acc[0][1]), "+d"(acc[1][0]), "+d"(acc[1][1]), "+d"(acc[2][0]), "+d"(acc[2][1]), "+d"(acc[3][0]), "+d"(acc[3][1]),
-          "+d"(acc[4][0]), "+d"(acc[4][1]), "+d"(acc[5][0]), "+d"(acc[5][1]), "+d"(acc[6][0]), "+d"(acc[6][1])
-        : "r"(pa), "r"(pb), "r"(pw), "r"(m)
-        : "memory");
-}
-
-// gint_rho, one segment on one cubelet: Y = sum_j D[row fragment][column fragment j] Phi_J[column fragment j]  (8 orbitals of I x 8 points),
-// then rho_g += sum_i Phi_I[i][g] Y[i][g].  d[j][h]: stationary A operands D[8 row + lane / 4][8 (cb + j) + 4 h + lane % 4].
-// pj: lane address of Phi_J[8 cb + lane % 4][point lane / 4]; pi: of Phi_I[8 row + lane / 4][points 2 (lane % 4), + 1].
-__device__ __forceinline__ void rho_seg(const double (&d)[GINT_SEG_COLS][2], unsigned pi, unsigned pj, unsigned m, double& r0, double& r1) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p0, p1, p2, p3, p4, p5, p6;\n\t"
-        ".reg .f64 fx, fy, ya0, ya1, yb0, yb1, b00, b01, b10, b11, b20, b21, b30, b31, b40, b41, b50, b51, b60, b61;\n\t"
-        ".reg .b32 t;\n\t"
-        "and.b32 t, %18, 1;  setp.ne.u32 p0, t, 0;\n\t"
-        "and.b32 t, %18, 2;  setp.ne.u32 p1, t, 0;\n\t"
-        "and.b32 t, %18, 4;  setp.ne.u32 p2, t, 0;\n\t"
-        "and.b32 t, %18, 8;  setp.ne.u32 p3, t, 0;\n\t"
-        "and.b32 t, %18, 16; setp.ne.u32 p4, t, 0;\n\t"
-        "and.b32 t, %18, 32; setp.ne.u32 p5, t, 0;\n\t"
-        "and.b32 t, %18, 64; setp.ne.u32 p6, t, 0;\n\t"
-        "ld.shared.f64 b00, [%17];\n\t"
-        "ld.shared.f64 b01, [%17 + 256];\n\t"
-        "ld.shared.f64 b10, [%17 + 512];\n\t"
-        "ld.shared.f64 b11, [%17 + 768];\n\t"
-        "ld.shared.f64 b20, [%17 + 1024];\n\t"
-        "ld.shared.f64 b21, [%17 + 1280];\n\t"
-        "ld.shared.f64 b30, [%17 + 1536];\n\t"
-        "ld.shared.f64 b31, [%17 + 1792];\n\t"
-        "ld.shared.f64 b40, [%17 + 2048];\n\t"
-        "ld.shared.f64 b41, [%17 + 2304];\n\t"
-        "ld.shared.f64 b50, [%17 + 2560];\n\t"
-        "ld.shared.f64 b51, [%17 + 2816];\n\t"
-        "ld.shared.f64 b60, [%17 + 3072];\n\t"
-        "ld.shared.f64 b61, [%17 + 3328];\n\t"
-        "ld.shared.v2.f64 {fx, fy}, [%16];\n\t"
-        "mov.f64 ya0, 0d0000000000000000; mov.f64 ya1, 0d0000000000000000;\n\t"
-        "mov.f64 yb0, 0d0000000000000000; mov.f64 yb1, 0d0000000000000000;\n\t"
-        "@p0 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%2},{b00},{ya0,ya1};\n\t"
-        "@p1 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {yb0,yb1},{%4},{b10},{yb0,yb1};\n\t"
-        "@p0 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%3},{b01},{ya0,ya1};\n\t"
-        "@p1 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {yb0,yb1},{%5},{b11},{yb0,yb1};\n\t"
-        "@p2 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%6},{b20},{ya0,ya1};\n\t"
-        "@p3 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {yb0,yb1},{%8},{b30},{yb0,yb1};\n\t"
-        "@p2 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%7},{b21},{ya0,ya1};\n\t"
-        "@p3 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {yb0,yb1},{%9},{b31},{yb0,yb1};\n\t"
-        "@p4 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%10},{b40},{ya0,ya1};\n\t"
-        "@p5 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {yb0,yb1},{%12},{b50},{yb0,yb1};\n\t"
-        "@p4 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%11},{b41},{ya0,ya1};\n\t"
-        "@p5 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {yb0,yb1},{%13},{b51},{yb0,yb1};\n\t"
-        "@p6 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%14},{b60},{ya0,ya1};\n\t"
-        "@p6 mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {ya0,ya1},{%15},{b61},{ya0,ya1};\n\t"
-        "add.f64 ya0, ya0, yb0;\n\t"
-        "add.f64 ya1, ya1, yb1;\n\t"
-        "fma.rn.f64 %0, ya0, fx, %0;\n\t"
-        "fma.rn.f64 %1, ya1, fy, %1;\n\t"
-        "}"
-        : "+d"(r0), "+d"(r1)
-        : "d"(d[0][0]), "d"(d[0][1]), "d"(d[1][0]), "d"(d[1][1]), "d"(d[2][0]), "d"(d[2][1]), "d"(d[3][0]), "d"(d[3][1]),
-          "d"(d[4][0]), "d"(d[4][1]), "d"(d[5][0]), "d"(d[5][1]), "d"(d[6][0]), "d"(d[6][1]), "r"(pi), "r"(pj), "r"(m)
-        : "memory");
-}
-
-// stationary operand of a segment (gint_rho): d[j][h] = Dh[orbital row 8 row + lr of I][orbital column 8 (cb + j) + 4 h + lc of J]
-__device__ __forceinline__ void load_dseg(const TileCtx& X, const Seg& sg, const double* __restrict__ Dh, double (&d)[GINT_SEG_COLS][2]) {
-    const int lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
-    const int row = 8 * sg.row() + lr;
-    const int a = X.row_atom[0][row], oa = X.row_orb[0][row];
+// gint_vlocal, one block on one cubelet.  pa, pb: lane addresses of the first row fragment / first column fragment; ra, rb: the rows are active.
+template <int NMAX>
+__device__ __forceinline__ void vl_visit(double (&acc)[2][4][2], int n, unsigned pa, unsigned pb, unsigned pw, bool ra, bool rb, int q) {
+    double2 b[4];
 #pragma unroll
-    for (int j = 0; j < GINT_SEG_COLS; j++)
+    for (int j = 0; j < 4; j++) b[j] = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int j = 0; j < NMAX; j++) b[j] = lds128(pb + j * GINT_FRAG_BYTES);
+    const double2 w = lds128(pw);
+    double2 a0 = lds128(pa), a1 = lds128(pa + GINT_FRAG_BYTES);
+    a0.x *= w.x; a0.y *= w.y; a1.x *= w.x; a1.y *= w.y;
+    if (NMAX == 4 && n == 4) {
+        if (ra && rb) vl_blk2<4>(acc, a0.x, a0.y, a1.x, a1.y, b, q);
+        else if (ra) vl_blk1<4>(acc[0], a0.x, a0.y, b, q);
+        else vl_blk1<4>(acc[1], a1.x, a1.y, b, q);
+    } else {            // 3 columns (a narrower block of a small group runs its unused columns on whatever the slot holds there; never flushed)
+        if (ra && rb) vl_blk2<3>(acc, a0.x, a0.y, a1.x, a1.y, b, q);
+        else if (ra) vl_blk1<3>(acc[0], a0.x, a0.y, b, q);
+        else vl_blk1<3>(acc[1], a1.x, a1.y, b, q);
+    }
+}
+// gint_rho, one block on one cubelet: Y_r = sum_j D[row r][column j] Phi_J[column j] (8 orbitals of I x 8 points), then
+// rho_g += sum_i Phi_I[i][g] Y_r[i][g].  pj: lane address of Phi_J[8 c0 + lane % 4][point lane / 4]; pi: of Phi_I[8 row + lane / 4][points 2 (lane % 4), + 1].
+template <int NMAX>
+__device__ __forceinline__ void rho_visit(const double (&d)[2][4][2], int n, unsigned pi, unsigned pj, bool ra, bool rb, int q, double& r0, double& r1) {
+    double bx[4], by[4];
+#pragma unroll
+    for (int j = 0; j < 4; j++) { bx[j] = 0.0; by[j] = 0.0; }
+#pragma unroll
+    for (int j = 0; j < NMAX; j++) { bx[j] = lds64(pj + j * GINT_FRAG_BYTES); by[j] = lds64(pj + j * GINT_FRAG_BYTES + 4 * GINT_ROW_BYTES); }
+#pragma unroll
+    for (int j = 1; j < 3; j++) if (j >= n) { bx[j] = 0.0; by[j] = 0.0; }      // a narrower block: D is zero there, the operand must be finite
+    const double2 f0 = lds128(pi), f1 = lds128(pi + GINT_FRAG_BYTES);
+    double y0[2] = {0.0, 0.0}, y1[2] = {0.0, 0.0};
+    const bool wide = NMAX == 4 && n == 4;
+    if (ra && rb) {
+        if (wide) rho_blk2<4>(d, bx, by, q, y0, y1); else rho_blk2<3>(d, bx, by, q, y0, y1);
+        r0 = fma(y0[0], f0.x, r0); r1 = fma(y0[1], f0.y, r1);
+        r0 = fma(y1[0], f1.x, r0); r1 = fma(y1[1], f1.y, r1);
+    } else if (ra) {        // an inactive row fragment of a slot may hold anything: its Phi_I values must not be touched
+        if (wide) rho_blk1<4>(d[0], bx, by, q, y0, y1); else rho_blk1<3>(d[0], bx, by, q, y0, y1);
+        r0 = fma(y0[0] + y1[0], f0.x, r0); r1 = fma(y0[1] + y1[1], f0.y, r1);
+    } else {
+        if (wide) rho_blk1<4>(d[1], bx, by, q, y0, y1); else rho_blk1<3>(d[1], bx, by, q, y0, y1);
+        r0 = fma(y0[0] + y1[0], f1.x, r0); r1 = fma(y0[1] + y1[1], f1.y, r1);
+    }
+}
+
+// stationary operands of a row fragment (gint_rho): d[j][h] = Dh[orbital row 8 row + lr of I][orbital column 8 (c0 + j) + 4 h + lc of J]
+__device__ __forceinline__ void load_drow(const TileCtx& X, int rowf, int c0, int n, const double* __restrict__ Dh, double (&d)[4][2]) {
+    const int lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
+    const int row = 8 * rowf + lr;
+    const int a = row < GINT_TILE_ORB ? X.row_atom[0][row] : 255, oa = row < GINT_TILE_ORB ? X.row_orb[0][row] : 0;
+#pragma unroll
+    for (int j = 0; j < 4; j++)
 #pragma unroll
         for (int h = 0; h < 2; h++) {
             double v = 0.0;
-            if (j < sg.n() && a != 255) {
-                const int col = 8 * (sg.cb() + j) + 4 * h + lc;
+            if (j < n && a != 255) {
+                const int col = 8 * (c0 + j) + 4 * h + lc;
                 const int bb = X.row_atom[1][col];
                 if (bb != 255) {
                     const PairEnt pe = X.pair[a][bb];
@@ -700,6 +791,28 @@ __device__ __forceinline__ void load_dseg(const TileCtx& X, const Seg& sg, const
             }
             d[j][h] = v;
         }
+}
+// flush of a row fragment's accumulators (gint_vlocal): element (row, col) -> atom pair (a, b), orbitals (oa, ob) -> canonical block
+// (transposed if the canonical key is (b, a)).  Exact zeros (fragments never touched, atoms that do not overlap inside this batch) are skipped.
+__device__ __forceinline__ void flush_row(const TileCtx& X, int rowf, int c0, int n, const double (&acc)[4][2], double* __restrict__ Hc) {
+    const int lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
+    const int row = 8 * rowf + lr;
+    const int a = X.row_atom[0][row], oa = X.row_orb[0][row];
+    if (a == 255) return;
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        if (j >= n) break;
+#pragma unroll
+        for (int e = 0; e < 2; e++) {
+            const double v = acc[j][e];
+            const int col = 8 * (c0 + j) + 2 * lc + e;
+            const int bb = X.row_atom[1][col], ob = X.row_orb[1][col];
+            if (bb == 255 || v == 0.0) continue;
+            const PairEnt pe = X.pair[a][bb];
+            if (pe.off == 0xffffffffu) continue;
+            atomicAdd(Hc + pe.off + oa * pe.sr + ob * pe.sc, v);
+        }
+    }
 }
 
 template <bool VLOCAL>
@@ -710,22 +823,29 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
     const unsigned lane_v = lr * GINT_ROW_BYTES + lc * 16;                 // row lr of a fragment, points 2 lc, 2 lc + 1
     const unsigned lane_j = lc * GINT_ROW_BYTES + lr * 8;                  // gint_rho B operand: row lc of the k-step, point lr
     int gs = 0;                                                            // ring stages consumed
+#ifdef GINT_DBG_STATS
+    unsigned long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#endif
     for (int t = 0;; t++) {
         const int c = t % GINT_NCTX;
+        DBG_T(t_ctx0);
         mbar_wait(&S.ctx_full[c], (t / GINT_NCTX) & 1);
         const TileCtx& X = S.ctx[c];
         if (!X.valid) break;
         DBG_T(t_tile0);
-        Seg sg[GINT_WARP_SEGS];
-        double acc[GINT_WARP_SEGS][GINT_SEG_COLS][2];      // gint_vlocal: accumulators; gint_rho: stationary D operands
+        DBG_ADD(7, t_tile0 - t_ctx0);
+        Blk bk[GINT_WARP_BLOCKS];
+        double acc[GINT_WARP_BLOCKS][2][4][2];      // gint_vlocal: accumulators; gint_rho: stationary D operands (column 3 of blocks 1, 2 is never touched)
+        const int q = X.zero;
 #pragma unroll
-        for (int k = 0; k < GINT_WARP_SEGS; k++) {
-            sg[k] = load_seg(X, warp + GINT_MMA_WARPS * k);
+        for (int k = 0; k < GINT_WARP_BLOCKS; k++) {
+            bk[k] = load_blk(X, X.blk[k][warp]);
             if (VLOCAL) {
 #pragma unroll
-                for (int j = 0; j < GINT_SEG_COLS; j++) { acc[k][j][0] = 0.0; acc[k][j][1] = 0.0; }
+                for (int j = 0; j < 4; j++) { acc[k][0][j][0] = 0.0; acc[k][0][j][1] = 0.0; acc[k][1][j][0] = 0.0; acc[k][1][j][1] = 0.0; }
             } else {
-                load_dseg(X, sg[k], Dh, acc[k]);
+                load_drow(X, bk[k].row(), bk[k].c0(), bk[k].n(), Dh, acc[k][0]);
+                load_drow(X, bk[k].row() + 1, bk[k].c0(), bk[k].has1() ? bk[k].n() : 0, Dh, acc[k][1]);
             }
         }
         const int nstage = X.nstage, ncub = X.ncub;
@@ -740,19 +860,30 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
             DBG_ADD(1, t_w1 - t_w0);
             double part[GINT_SC][2];
 #pragma unroll
-            for (int q = 0; q < GINT_SC; q++) { part[q][0] = 0.0; part[q][1] = 0.0; }
+            for (int qq = 0; qq < GINT_SC; qq++) { part[qq][0] = 0.0; part[qq][1] = 0.0; }
 #pragma unroll
-            for (int q = 0; q < GINT_SC; q++) {
-                const int pos = st * GINT_SC + q;
+            for (int qq = 0; qq < GINT_SC; qq++) {
+                const int pos = st * GINT_SC + qq;
+#ifdef GINT_DBG_NO_MMA
+                if (false) {
+#else
                 if (pos < ncub) {
+#endif
                     const unsigned info = X.cubinfo[pos];
-                    const unsigned base = ring0 + s * GINT_STAGE_BYTES + q * 2 * GINT_SLOT_MAX_BYTES;
+                    const unsigned base = ring0 + s * GINT_STAGE_BYTES + qq * 2 * GINT_SLOT_MAX_BYTES;
 #pragma unroll
-                    for (int k = 0; k < GINT_WARP_SEGS; k++) {
-                        const unsigned m = ((info >> sg[k].row()) & 1u) ? ((info >> (16 + sg[k].cb())) & ((1u << sg[k].n()) - 1u)) : 0u;
-                        if (m) {
-                            if (VLOCAL) vl_seg(acc[k], base + sg[k].oa + lane_v, base + sg[k].ob + lane_v, pw0 + pos * 64, m);
-                            else rho_seg(acc[k], base + sg[k].oa + lane_v, base + sg[k].ob + lane_j, m, part[q][0], part[q][1]);
+                    for (int k = 0; k < GINT_WARP_BLOCKS; k++) {
+                        const unsigned rr = (info >> bk[k].row()) & (bk[k].has1() ? 3u : 1u);
+                        const unsigned cm = (info >> (16 + bk[k].c0())) & ((1u << bk[k].n()) - 1u);
+                        if (rr && cm) {
+                            DBG_ADD(6, (rr == 3u ? 4 : 2) * bk[k].n());
+                            if (VLOCAL) {
+                                if (k == 0) vl_visit<4>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_v, pw0 + pos * 64, rr & 1u, rr & 2u, q);
+                                else vl_visit<3>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_v, pw0 + pos * 64, rr & 1u, rr & 2u, q);
+                            } else {
+                                if (k == 0) rho_visit<4>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_j, rr & 1u, rr & 2u, q, part[qq][0], part[qq][1]);
+                                else rho_visit<3>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_j, rr & 1u, rr & 2u, q, part[qq][0], part[qq][1]);
+                            }
                         }
                     }
                 }
@@ -779,28 +910,11 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
         }
         DBG_T(t_loop);
         if (VLOCAL) {
-            // flush: element (row, col) -> atom pair (a, b), orbitals (oa, ob) -> canonical block (transposed if the canonical
-            // key is (b, a)).  Exact zeros (fragments never touched, atoms that do not overlap inside this batch) are skipped.
 #pragma unroll
-            for (int k = 0; k < GINT_WARP_SEGS; k++) {
-                if (sg[k].n() == 0) continue;
-                const int row = 8 * sg[k].row() + lr;
-                const int a = X.row_atom[0][row], oa = X.row_orb[0][row];
-                if (a == 255) continue;
-#pragma unroll
-                for (int j = 0; j < GINT_SEG_COLS; j++) {
-                    if (j >= sg[k].n()) break;
-#pragma unroll
-                    for (int e = 0; e < 2; e++) {
-                        const double v = acc[k][j][e];
-                        const int col = 8 * (sg[k].cb() + j) + 2 * lc + e;
-                        const int bb = X.row_atom[1][col], ob = X.row_orb[1][col];
-                        if (bb == 255 || v == 0.0) continue;
-                        const PairEnt pe = X.pair[a][bb];
-                        if (pe.off == 0xffffffffu) continue;
-                        atomicAdd(Hc + pe.off + oa * pe.sr + ob * pe.sc, v);
-                    }
-                }
+            for (int k = 0; k < GINT_WARP_BLOCKS; k++) {
+                if (bk[k].n() == 0) continue;
+                flush_row(X, bk[k].row(), bk[k].c0(), bk[k].n(), acc[k][0], Hc);
+                if (bk[k].has1()) flush_row(X, bk[k].row() + 1, bk[k].c0(), bk[k].n(), acc[k][1], Hc);
             }
         }
         __syncwarp();
@@ -810,6 +924,9 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
         DBG_ADD(4, t_end - t_tile0);
         DBG_ADD(5, 1);
     }
+#ifdef GINT_DBG_STATS
+    if (lane == 0) for (int i = 0; i < 8; i++) atomicAdd(&g_dbg[i], dbg_acc[i]);
+#endif
 }
 
 // ---------------------------------------------------------------------------------------------------
