@@ -145,6 +145,10 @@ int gint_stats(gint_ctx* ctx, long long* out);
  * is -1 when that call has not been made yet. */
 int gint_kernel_times(gint_ctx* ctx, double out[2]);
 
+/* The same, split by kernel: out[0] / out[1] = orbital-evaluation kernels / tile-contraction kernels (summed over the waves) of the
+ * last gint_vlocal call, out[2] / out[3] = of the last gint_rho call; -1 when that call has not been made yet. */
+int gint_phase_times(gint_ctx* ctx, double out[4]);
+
 int gint_free(gint_ctx* ctx);
 
 const char* gint_last_error(void);

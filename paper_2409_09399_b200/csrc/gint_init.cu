@@ -315,6 +315,7 @@ static void free_ctx(gint_ctx* c) {
     cudaFree(c->d_goff); cudaFree(c->d_phi); cudaFree(c->d_queue);
     cudaFree(c->d_stage_in); cudaFree(c->d_stage_out);
     for (auto& e : c->ev) if (e) cudaEventDestroy(e);
+    for (auto& v : c->ev_wave) for (auto& e : v) if (e) cudaEventDestroy(e);
     delete c;
 }
 
@@ -718,6 +719,27 @@ extern "C" int gint_kernel_times(gint_ctx* ctx, double out[2]) {
         GINT_CUDA(cudaEventSynchronize(ctx->ev[2 * k + 1]));
         GINT_CUDA(cudaEventElapsedTime(&ms, ctx->ev[2 * k], ctx->ev[2 * k + 1]));
         out[k] = 1e-3 * (double)ms;
+    }
+    return GINT_OK;
+}
+
+extern "C" int gint_phase_times(gint_ctx* ctx, double out[4]) {
+    if (!ctx) GINT_FAIL(GINT_ERR_BAD_STATE, "NULL context");
+    if (!out) GINT_FAIL(GINT_ERR_INVALID_ARG, "NULL output");
+    GINT_CUDA(cudaSetDevice(ctx->device));
+    for (int k = 0; k < 2; k++) {
+        out[2 * k] = out[2 * k + 1] = -1.0;
+        if (!ctx->timed[k] || ctx->ev_wave[k].empty()) continue;
+        double te = 0.0, tt = 0.0;
+        cudaEvent_t prev = ctx->ev[2 * k];
+        for (size_t w = 0; w < ctx->ev_wave[k].size(); w++) {
+            float ms = 0.f;
+            GINT_CUDA(cudaEventSynchronize(ctx->ev_wave[k][w]));
+            GINT_CUDA(cudaEventElapsedTime(&ms, prev, ctx->ev_wave[k][w]));
+            ((w & 1) ? tt : te) += 1e-3 * (double)ms;
+            prev = ctx->ev_wave[k][w];
+        }
+        out[2 * k] = te; out[2 * k + 1] = tt;
     }
     return GINT_OK;
 }

@@ -170,6 +170,8 @@ struct gint_ctx {
     // CUDA events around the two main kernels (gint_kernel_times)
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     bool timed[2] = {false, false};
+    // per-wave events (gint_phase_times): [call][2 * wave] after the evaluation kernel, [call][2 * wave + 1] after the tile kernel
+    std::vector<cudaEvent_t> ev_wave[2];
     // host-path staging
     double* d_stage_in = nullptr; size_t stage_in_n = 0;
     double* d_stage_out = nullptr; size_t stage_out_n = 0;

@@ -60,10 +60,12 @@ __device__ __forceinline__ void cubelet_point(int cl, int p, int& ix, int& iy, i
 #define DBG_ADD(i, v)
 #else
 __device__ unsigned long long g_dbg[16];
+__device__ unsigned long long g_dbgw[16][8];
 #define DBG_T(x) const long long x = clock64()
 #define DBG_ADD(i, v) dbg_acc[i] += (unsigned long long)(v)
 extern "C" int gint_debug_counters(unsigned long long* out) { return (int)cudaMemcpyFromSymbol(out, g_dbg, sizeof(g_dbg)); }
-extern "C" int gint_debug_reset() { unsigned long long z[16] = {0}; return (int)cudaMemcpyToSymbol(g_dbg, z, sizeof(z)); }
+extern "C" int gint_debug_warp_counters(unsigned long long* out) { return (int)cudaMemcpyFromSymbol(out, g_dbgw, sizeof(g_dbgw)); }
+extern "C" int gint_debug_reset() { unsigned long long z[16 * 8] = {0}; cudaMemcpyToSymbol(g_dbgw, z, sizeof(z)); return (int)cudaMemcpyToSymbol(g_dbg, z, 16 * 8); }
 #endif
 
 // ---------------------------------------------------------------------------------------------------
@@ -107,12 +109,15 @@ struct EvalSmem {
 };
 #define GINT_EVAL_TAB_OFF ((sizeof(EvalSmem) + 15) & ~(size_t)15)
 
+// gint_vlocal (V != nullptr) stores sqrt(|V dV|) phi: the contraction Phi_I^T diag(V dV) Phi_J then needs no FP64 multiply, only
+// the sign of V at the point, which the consumers apply to one operand with an integer XOR (an FP64 multiply queues behind the
+// other warps' DMMAs in the shared FP64 pipe).  Points outside the mesh (ragged edge batches) get weight 0.
 template <bool TAB_SMEM>
 __global__ void __launch_bounds__(GINT_EVAL_THREADS)
 k_eval_phi(Geom g, long long b0, const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
            const int* __restrict__ gstart, const u64* __restrict__ goff, u64 wave_row0,
            const double* __restrict__ atom_pos, const int* __restrict__ atom_spec, const SpeciesDev* __restrict__ sp,
-           const double* __restrict__ tab, int tab_cells, double* __restrict__ phi) {
+           const double* __restrict__ tab, int tab_cells, const double* __restrict__ V, double* __restrict__ phi) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     EvalSmem& S = *reinterpret_cast<EvalSmem*>(smem_raw);
     const long long b = b0 + blockIdx.x;
@@ -201,7 +206,12 @@ k_eval_phi(Geom g, long long b0, const int* __restrict__ bstart, const NeighEntr
         const bool tiny = r < 1e-12;
         if (tiny) ir = 0.0;
         // lanes outside the sphere run the same instructions on a clamped radius and store zeros
-        const double w0 = inside ? 1.0 : 0.0;
+        double w0 = inside ? 1.0 : 0.0;
+        if (V) {
+            const int gi = i0 + ix, gj = j0 + iy, gk = k0 + iz;
+            const bool in_mesh = gi < g.N[0] && gj < g.N[1] && gk < g.N[2];
+            w0 = (inside && in_mesh) ? sqrt(fabs(__ldg(V + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk) * g.dV)) : 0.0;
+        }
         const double ux = dx * ir, uy = dy * ir, uz = dz * ir;
         double yw[9];
         {
@@ -267,8 +277,9 @@ struct alignas(16) TileCtx {
     PairEnt pair[GINT_TILE_ATOMS][GINT_TILE_ATOMS];   // canonical block of (I atom a, J atom b)
     unsigned char row_atom[2][GINT_TILE_ORB];   // orbital row -> atom slot inside the group (255 = padding)
     unsigned char row_orb[2][GINT_TILE_ORB];    // orbital row -> orbital index inside the atom
-    alignas(16) double pw[GINT_NCUB][GINT_CPTS];    // gint_vlocal: V dV at the listed cubelets' points (0 outside the mesh);
-                                        // gint_rho: the tile's density at those points (summed by the issuer warp)
+    unsigned char vis[GINT_NCUB][16];   // per listed cubelet and consumer warp: bits 2k, 2k+1 = rows of the warp's block k to work on there (0: skip)
+    unsigned char sgn[GINT_NCUB];       // gint_vlocal: bit p = V < 0 at point p of the listed cubelet
+    alignas(16) double pw[GINT_NCUB][GINT_CPTS];    // gint_rho: the tile's density at the listed cubelets' points (summed by the issuer warp)
 };
 struct SetupScratch {                   // private to the set-up warps
     cmask amask[16];                    // slot s < 8: atom s of group I; slot 8 + s: atom s of group J
@@ -460,6 +471,28 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileCtx& 
             }
     }
     setup_sync();
+#ifdef GINT_DBG_STATS
+    if (VLOCAL && sid == 1) {
+        // DMMAs per tile at several granularities of skipping (debug statistics)
+        unsigned long long fine = 0, atomx = 0, dense = 0, rowp = 0, rowf = 0;
+        cmask mJ = czero();
+        for (int cc = 0; cc < nfJ; cc++) mJ |= Q.fmask[1][cc];
+        for (int r = 0; r < nfI; r++) {
+            const int cf = diag ? (Q.cstart[1][X.row_atom[0][8 * r]] >> 3) : 0;
+            for (int cc = cf; cc < nfJ; cc++) fine += 2ull * ccount(Q.fmask[0][r] & Q.fmask[1][cc]);
+            dense += 2ull * (nfJ - cf) * X.ncub;
+            rowf += 2ull * (nfJ - cf) * ccount(Q.fmask[0][r] & mJ);
+            const cmask rp = Q.fmask[0][r & ~1] | Q.fmask[0][min(r | 1, nfI - 1)];
+            rowp += 2ull * (nfJ - cf) * ccount(rp & mJ);
+        }
+        for (int a = 0; a < nI; a++) for (int bb = (diag ? a : 0); bb < nJ; bb++) {
+            const unsigned long long na = Q.cstart[0][a + 1] - Q.cstart[0][a], nb2 = Q.cstart[1][bb + 1] - Q.cstart[1][bb];
+            const unsigned long long el = (diag && a == bb) ? na * (na + 1) / 2 : na * nb2;       // orbital pairs
+            atomx += el * ccount(Q.amask[a] & Q.amask[8 + bb]);                                     // x cubelets (8 points each)
+        }
+        atomicAdd(&g_dbg[8], fine); atomicAdd(&g_dbg[9], atomx); atomicAdd(&g_dbg[10], dense); atomicAdd(&g_dbg[11], rowp); atomicAdd(&g_dbg[12], rowf);
+    }
+#endif
     const int ncub = X.ncub;
     const int bi0 = X.i0, bj0 = X.j0, bk0 = X.k0, ex = X.ex, ey = X.ey, ez = X.ez;
     // per listed cubelet: which fragments are active, and the points' weights
@@ -470,13 +503,34 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileCtx& 
         for (int f = 0; f < nfJ; f++) info |= (unsigned)cbit(Q.fmask[1][f], cl) << (16 + f);
         X.cubinfo[pos] = info;
     }
-    for (int idx = sid; idx < ncub * GINT_CPTS; idx += GINT_SETUP_THREADS) {
-        double w = 0.0;
-        if (VLOCAL) {
-            int ix, iy, iz; cubelet_point(X.cub[idx >> 3], idx & 7, ix, iy, iz);
-            if (ix < ex && iy < ey && iz < ez) w = __ldg(V + ((size_t)(bi0 + ix) * g.N[1] + (bj0 + iy)) * g.N[2] + (bk0 + iz)) * g.dV;
+    if (VLOCAL) {
+        for (int pos = sid; pos < ncub; pos += GINT_SETUP_THREADS) {
+            const int cl = X.cub[pos];
+            unsigned sg = 0;
+#pragma unroll
+            for (int pp = 0; pp < GINT_CPTS; pp++) {
+                int ix, iy, iz; cubelet_point(cl, pp, ix, iy, iz);
+                if (ix < ex && iy < ey && iz < ez) sg |= (unsigned)(__ldg(V + ((size_t)(bi0 + ix) * g.N[1] + (bj0 + iy)) * g.N[2] + (bk0 + iz)) < 0.0) << pp;
+            }
+            X.sgn[pos] = (unsigned char)sg;
         }
-        X.pw[0][idx] = w;
+    } else {
+        for (int idx = sid; idx < ncub * GINT_CPTS; idx += GINT_SETUP_THREADS) X.pw[0][idx] = 0.0;
+    }
+    setup_sync();
+    // visit codes: which rows of which block every consumer warp works on, per listed cubelet
+    for (int idx = sid; idx < ncub * GINT_MMA_WARPS; idx += GINT_SETUP_THREADS) {
+        const int pos = idx / GINT_MMA_WARPS, w = idx - pos * GINT_MMA_WARPS;
+        const unsigned info = X.cubinfo[pos];
+        unsigned code = 0;
+#pragma unroll
+        for (int k = 0; k < GINT_WARP_BLOCKS; k++) {
+            const unsigned d = X.blk[k][w];
+            const unsigned rr = (info >> (d & 15u)) & (((d >> 4) & 1u) ? 3u : 1u);
+            const unsigned cm = (info >> (16 + ((d >> 5) & 15u))) & ((1u << ((d >> 9) & 7u)) - 1u);
+            if (cm) code |= rr << (2 * k);
+        }
+        X.vis[pos][w] = (unsigned char)code;
     }
     setup_sync();
 }
@@ -725,15 +779,16 @@ __device__ __forceinline__ Blk load_blk(const TileCtx& X, unsigned desc) {
 
 // gint_vlocal, one block on one cubelet.  pa, pb: lane addresses of the first row fragment / first column fragment; ra, rb: the rows are active.
 template <int NMAX>
-__device__ __forceinline__ void vl_visit(double (&acc)[2][4][2], int n, unsigned pa, unsigned pb, unsigned pw, bool ra, bool rb, int q) {
+__device__ __forceinline__ void vl_visit(double (&acc)[2][4][2], int n, unsigned pa, unsigned pb, int sx, int sy, bool ra, bool rb, int q) {
     double2 b[4];
 #pragma unroll
     for (int j = 0; j < 4; j++) b[j] = make_double2(0.0, 0.0);
 #pragma unroll
     for (int j = 0; j < NMAX; j++) b[j] = lds128(pb + j * GINT_FRAG_BYTES);
-    const double2 w = lds128(pw);
     double2 a0 = lds128(pa), a1 = lds128(pa + GINT_FRAG_BYTES);
-    a0.x *= w.x; a0.y *= w.y; a1.x *= w.x; a1.y *= w.y;
+    // sign of V at the lane's two points (sx, sy: 0 or 0x80000000): the orbital values carry sqrt(|V dV|)
+    a0.x = __hiloint2double(__double2hiint(a0.x) ^ sx, __double2loint(a0.x)); a0.y = __hiloint2double(__double2hiint(a0.y) ^ sy, __double2loint(a0.y));
+    a1.x = __hiloint2double(__double2hiint(a1.x) ^ sx, __double2loint(a1.x)); a1.y = __hiloint2double(__double2hiint(a1.y) ^ sy, __double2loint(a1.y));
     if (NMAX == 4 && n == 4) {
         if (ra && rb) vl_blk2<4>(acc, a0.x, a0.y, a1.x, a1.y, b, q);
         else if (ra) vl_blk1<4>(acc[0], a0.x, a0.y, b, q);
@@ -849,7 +904,6 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
             }
         }
         const int nstage = X.nstage, ncub = X.ncub;
-        const unsigned pw0 = smem_addr(&X.pw[0][0]) + lc * 16;
         DBG_T(t_tile1);
         DBG_ADD(0, t_tile1 - t_tile0);
         for (int st = 0; st < nstage; st++, gs++) {
@@ -869,20 +923,23 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
 #else
                 if (pos < ncub) {
 #endif
-                    const unsigned info = X.cubinfo[pos];
-                    const unsigned base = ring0 + s * GINT_STAGE_BYTES + qq * 2 * GINT_SLOT_MAX_BYTES;
+                    const unsigned code = X.vis[pos][warp];
+                    if (code) {
+                        const unsigned base = ring0 + s * GINT_STAGE_BYTES + qq * 2 * GINT_SLOT_MAX_BYTES;
+                        int sx = 0, sy = 0;
+                        if (VLOCAL) { const unsigned sg = (unsigned)X.sgn[pos] >> (2 * lc); sx = (int)(sg << 31); sy = (int)((sg >> 1) << 31); }
 #pragma unroll
-                    for (int k = 0; k < GINT_WARP_BLOCKS; k++) {
-                        const unsigned rr = (info >> bk[k].row()) & (bk[k].has1() ? 3u : 1u);
-                        const unsigned cm = (info >> (16 + bk[k].c0())) & ((1u << bk[k].n()) - 1u);
-                        if (rr && cm) {
-                            DBG_ADD(6, (rr == 3u ? 4 : 2) * bk[k].n());
-                            if (VLOCAL) {
-                                if (k == 0) vl_visit<4>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_v, pw0 + pos * 64, rr & 1u, rr & 2u, q);
-                                else vl_visit<3>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_v, pw0 + pos * 64, rr & 1u, rr & 2u, q);
-                            } else {
-                                if (k == 0) rho_visit<4>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_j, rr & 1u, rr & 2u, q, part[qq][0], part[qq][1]);
-                                else rho_visit<3>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_j, rr & 1u, rr & 2u, q, part[qq][0], part[qq][1]);
+                        for (int k = 0; k < GINT_WARP_BLOCKS; k++) {
+                            const unsigned rr = (code >> (2 * k)) & 3u;
+                            if (rr) {
+                                DBG_ADD(6, (rr == 3u ? 4 : 2) * bk[k].n());
+                                if (VLOCAL) {
+                                    if (k == 0) vl_visit<4>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_v, sx, sy, rr & 1u, rr & 2u, q);
+                                    else vl_visit<3>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_v, sx, sy, rr & 1u, rr & 2u, q);
+                                } else {
+                                    if (k == 0) rho_visit<4>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_j, rr & 1u, rr & 2u, q, part[qq][0], part[qq][1]);
+                                    else rho_visit<3>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_j, rr & 1u, rr & 2u, q, part[qq][0], part[qq][1]);
+                                }
                             }
                         }
                     }
@@ -925,7 +982,7 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
         DBG_ADD(5, 1);
     }
 #ifdef GINT_DBG_STATS
-    if (lane == 0) for (int i = 0; i < 8; i++) atomicAdd(&g_dbg[i], dbg_acc[i]);
+    if (lane == 0) for (int i = 0; i < 8; i++) { atomicAdd(&g_dbg[i], dbg_acc[i]); atomicAdd(&g_dbgw[warp][i], dbg_acc[i]); }
 #endif
 }
 
@@ -1067,6 +1124,10 @@ int gint_build_phi_layout(gint_ctx* c, const int* d_bgroups, size_t phi_cap_byte
     GINT_CUDA(cudaMalloc((void**)&c->d_phi, c->phi_bytes));
     c->device_bytes += c->phi_bytes;
     GINT_CUDA(cudaMalloc((void**)&c->d_queue, sizeof(int) * (c->waves.size() + 1)));
+    for (int k = 0; k < 2; k++) {
+        c->ev_wave[k].assign(2 * c->waves.size(), nullptr);
+        for (auto& e : c->ev_wave[k]) GINT_CUDA(cudaEventCreate(&e));
+    }
     return GINT_OK;
 }
 
@@ -1132,16 +1193,18 @@ static int launch_waves(gint_ctx* c, const double* in, double* out, cudaStream_t
         const unsigned nb = (unsigned)(W.b1 - W.b0);
         if (c->tab_in_smem)
             k_eval_phi<true><<<nb, GINT_EVAL_THREADS, c->smem_eval, st>>>(c->geom, W.b0, c->d_bstart, c->d_bent, c->d_gstart, c->d_goff, W.row0,
-                c->d_atom_pos, c->d_atom_species, c->d_species, c->d_tab, tab_cells, c->d_phi);
+                c->d_atom_pos, c->d_atom_species, c->d_species, c->d_tab, tab_cells, VLOCAL ? in : nullptr, c->d_phi);
         else
             k_eval_phi<false><<<nb, GINT_EVAL_THREADS, c->smem_eval, st>>>(c->geom, W.b0, c->d_bstart, c->d_bent, c->d_gstart, c->d_goff, W.row0,
-                c->d_atom_pos, c->d_atom_species, c->d_species, c->d_tab, tab_cells, c->d_phi);
+                c->d_atom_pos, c->d_atom_species, c->d_species, c->d_tab, tab_cells, VLOCAL ? in : nullptr, c->d_phi);
         GINT_CUDA(cudaGetLastError());
+        GINT_CUDA(cudaEventRecord(c->ev_wave[VLOCAL ? 0 : 1][2 * w], st));
         const int nt = (int)(W.t1 - W.t0);
         const unsigned grid = (unsigned)std::min<long long>(c->n_sm, nt);
         k_tiles<VLOCAL><<<grid, GINT_CTA_THREADS, c->smem_bytes, st>>>(c->geom, c->d_tile + W.t0, nt, c->d_queue + w, c->d_bstart, c->d_bent,
             c->d_gstart, c->d_goff, W.row0, c->d_phi, c->d_atom_species, c->d_species, c->d_crow, c->d_ckey, c->d_coff, in, out);
         GINT_CUDA(cudaGetLastError());
+        GINT_CUDA(cudaEventRecord(c->ev_wave[VLOCAL ? 0 : 1][2 * w + 1], st));
     }
     return GINT_OK;
 }

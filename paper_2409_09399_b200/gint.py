@@ -21,7 +21,7 @@ STAT_NAMES = ("n_batch", "n_batch_empty", "batch_bx", "batch_by", "batch_bz", "n
               "n_waves", "n_tiles")
 
 EXPORTS = ("gint_init", "gint_n_orb", "gint_n_pairs", "gint_get_pairs", "gint_vlocal", "gint_rho", "gint_vlocal_host",
-           "gint_rho_host", "gint_stats", "gint_kernel_times", "gint_free", "gint_last_error")
+           "gint_rho_host", "gint_stats", "gint_kernel_times", "gint_phase_times", "gint_free", "gint_last_error")
 
 
 class GintError(RuntimeError):
@@ -109,6 +109,12 @@ class Gint:
         out = (C.c_double * 2)()
         _check(lib().gint_kernel_times(self._ctx, out))
         return {"vlocal_main": float(out[0]), "rho_main": float(out[1])}
+
+    def phase_times(self) -> dict:
+        """Device seconds of the evaluation / tile kernels (summed over waves) in the last vlocal / rho call."""
+        out = (C.c_double * 4)()
+        _check(lib().gint_phase_times(self._ctx, out))
+        return {"vlocal_eval": float(out[0]), "vlocal_tiles": float(out[1]), "rho_eval": float(out[2]), "rho_tiles": float(out[3])}
 
     # ------------------------------------------------------------------ device path
     def _stream(self):
