@@ -277,8 +277,9 @@ struct alignas(16) TileCtx {
     PairEnt pair[GINT_TILE_ATOMS][GINT_TILE_ATOMS];   // canonical block of (I atom a, J atom b)
     unsigned char row_atom[2][GINT_TILE_ORB];   // orbital row -> atom slot inside the group (255 = padding)
     unsigned char row_orb[2][GINT_TILE_ORB];    // orbital row -> orbital index inside the atom
-    unsigned char vis[GINT_NCUB][16];   // per listed cubelet and consumer warp: bits 2k, 2k+1 = rows of the warp's block k to work on there (0: skip)
-    unsigned char sgn[GINT_NCUB];       // gint_vlocal: bit p = V < 0 at point p of the listed cubelet
+    unsigned short vis[GINT_NCUB + GINT_SC][16];   // per listed cubelet and consumer warp: bits 2k, 2k+1 = rows of the warp's block k to work on
+                                        // there (0: skip); bits 8..15 (gint_vlocal): bit 8 + p = V < 0 at point p of the cubelet.  Rows ncub.. are 0.
+    unsigned char sgn[GINT_NCUB];       // set-up scratch for those sign bits
     alignas(16) double pw[GINT_NCUB][GINT_CPTS];    // gint_rho: the tile's density at the listed cubelets' points (summed by the issuer warp)
 };
 struct SetupScratch {                   // private to the set-up warps
@@ -528,10 +529,15 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileCtx& 
             const unsigned d = X.blk[k][w];
             const unsigned rr = (info >> (d & 15u)) & (((d >> 4) & 1u) ? 3u : 1u);
             const unsigned cm = (info >> (16 + ((d >> 5) & 15u))) & ((1u << ((d >> 9) & 7u)) - 1u);
+#ifdef GINT_DBG_DENSE
+            if ((d >> 9) & 7u) code |= (((d >> 4) & 1u) ? 3u : 1u) << (2 * k);
+#else
             if (cm) code |= rr << (2 * k);
+#endif
         }
-        X.vis[pos][w] = (unsigned char)code;
+        X.vis[pos][w] = (unsigned short)(code | (VLOCAL ? ((unsigned)X.sgn[pos] << 8) : 0u));
     }
+    if (sid < GINT_SC * 16) X.vis[ncub + sid / 16][sid % 16] = 0;      // the consumers prefetch one stage ahead
     setup_sync();
 }
 
@@ -645,6 +651,11 @@ __device__ __forceinline__ void issuer_role(const Geom& g, TileSmem& S, double* 
 __device__ __forceinline__ double2 lds128(unsigned addr) {
     double2 v;
     asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned lds_u16(unsigned addr) {
+    unsigned short v;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr) : "memory");
     return v;
 }
 __device__ __forceinline__ double lds64(unsigned addr) {
@@ -904,6 +915,10 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
             }
         }
         const int nstage = X.nstage, ncub = X.ncub;
+        const unsigned vis0 = smem_addr(&X.vis[0][warp]);
+        unsigned cur[GINT_SC], nxt[GINT_SC];
+#pragma unroll
+        for (int qq = 0; qq < GINT_SC; qq++) cur[qq] = lds_u16(vis0 + qq * 32);
         DBG_T(t_tile1);
         DBG_ADD(0, t_tile1 - t_tile0);
         for (int st = 0; st < nstage; st++, gs++) {
@@ -914,20 +929,19 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
             DBG_ADD(1, t_w1 - t_w0);
             double part[GINT_SC][2];
 #pragma unroll
-            for (int qq = 0; qq < GINT_SC; qq++) { part[qq][0] = 0.0; part[qq][1] = 0.0; }
+            for (int qq = 0; qq < GINT_SC; qq++) { part[qq][0] = 0.0; part[qq][1] = 0.0; nxt[qq] = lds_u16(vis0 + ((st + 1) * GINT_SC + qq) * 32); }
 #pragma unroll
             for (int qq = 0; qq < GINT_SC; qq++) {
-                const int pos = st * GINT_SC + qq;
 #ifdef GINT_DBG_NO_MMA
                 if (false) {
 #else
-                if (pos < ncub) {
+                {
 #endif
-                    const unsigned code = X.vis[pos][warp];
+                    const unsigned code = cur[qq] & 63u;
                     if (code) {
                         const unsigned base = ring0 + s * GINT_STAGE_BYTES + qq * 2 * GINT_SLOT_MAX_BYTES;
                         int sx = 0, sy = 0;
-                        if (VLOCAL) { const unsigned sg = (unsigned)X.sgn[pos] >> (2 * lc); sx = (int)(sg << 31); sy = (int)((sg >> 1) << 31); }
+                        if (VLOCAL) { const unsigned sg = cur[qq] >> (8 + 2 * lc); sx = (int)(sg << 31); sy = (int)((sg >> 1) << 31); }
 #pragma unroll
                         for (int k = 0; k < GINT_WARP_BLOCKS; k++) {
                             const unsigned rr = (code >> (2 * k)) & 3u;
@@ -962,6 +976,8 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&S.empty[s]);
+#pragma unroll
+            for (int qq = 0; qq < GINT_SC; qq++) cur[qq] = nxt[qq];
             DBG_T(t_w2);
             DBG_ADD(2, t_w2 - t_w1);
         }
