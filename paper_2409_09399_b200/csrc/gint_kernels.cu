@@ -460,13 +460,16 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileCtx& 
                 if (wide != (pass == 0)) continue;
                 int best = -1;
                 for (int w = 0; w < GINT_MMA_WARPS; w++) {
-                    const bool free_slot = wide ? !(used[w] & 1) : used[w] != 7;
+                    const bool free_slot = wide ? !(used[w] & 1) : used[w] != (1 << GINT_WARP_BLOCKS) - 1;
                     if (!free_slot) continue;
                     if (best < 0 || lsm[w & 3] < lsm[best & 3] || (lsm[w & 3] == lsm[best & 3] && lw[w] < lw[best])) best = w;
                 }
-                if (best < 0) __trap();     // cannot happen: at most 28 blocks for 36 slots
+                if (best < 0) __trap();     // cannot happen: at most 28 blocks (7 of them wide) for GINT_WARP_BLOCKS * GINT_MMA_WARPS slots
                 int k = 0;
-                if (!wide) k = !(used[best] & 2) ? 1 : (!(used[best] & 4) ? 2 : 0);
+                if (!wide) {                // a narrow block prefers the slots that cannot hold a wide one
+                    k = 0;
+                    for (int kk = GINT_WARP_BLOCKS - 1; kk >= 1; kk--) if (!(used[best] & (1 << kk))) k = kk;
+                }
                 used[best] |= 1 << k; lsm[best & 3] += wgt[i]; lw[best] += wgt[i];
                 X.blk[k][best] = desc[i];
             }
