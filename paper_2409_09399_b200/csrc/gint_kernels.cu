@@ -209,7 +209,7 @@ k_eval_phi(Geom g, long long b0, const int* __restrict__ bstart, const NeighEntr
         double w0 = inside ? 1.0 : 0.0;
         if (V) {
             const int gi = i0 + ix, gj = j0 + iy, gk = k0 + iz;
-            const bool in_mesh = gi < g.N[0] && gj < g.N[1] && gk < g.N[2];
+            const bool in_mesh = ix < g.bs[0] && iy < g.bs[1] && iz < g.bs[2] && gi < g.N[0] && gj < g.N[1] && gk < g.N[2];    // a point of this batch
             w0 = (inside && in_mesh) ? sqrt(fabs(__ldg(V + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk) * g.dV)) : 0.0;
         }
         const double ux = dx * ir, uy = dy * ir, uz = dz * ir;
@@ -494,6 +494,7 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileCtx& 
             const unsigned long long el = (diag && a == bb) ? na * (na + 1) / 2 : na * nb2;       // orbital pairs
             atomx += el * ccount(Q.amask[a] & Q.amask[8 + bb]);                                     // x cubelets (8 points each)
         }
+        atomicAdd(&g_dbg[13], X.ncub == 0 ? 1ull : 0ull); atomicAdd(&g_dbg[14], X.ncub < 16 ? 1ull : 0ull); atomicAdd(&g_dbg[15], (unsigned long long)X.ncub);
         atomicAdd(&g_dbg[8], fine); atomicAdd(&g_dbg[9], atomx); atomicAdd(&g_dbg[10], dense); atomicAdd(&g_dbg[11], rowp); atomicAdd(&g_dbg[12], rowf);
     }
 #endif
