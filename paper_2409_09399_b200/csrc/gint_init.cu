@@ -257,7 +257,7 @@ __global__ void __launch_bounds__(256) k_scan_apply(const int* __restrict__ in, 
 }
 
 // out[0..n] = exclusive scan of in[0..n); block sums are scanned on the host (n/1024 values).
-static int device_excl_scan(const int* d_in, long long n, int* d_out, long long* total) {
+int gint_device_excl_scan(const int* d_in, long long n, int* d_out, long long* total) {
     int nblk = (int)((n + 1023) / 1024);
     if (nblk == 0) { int z = 0; GINT_CUDA(cudaMemcpy(d_out, &z, sizeof(int), cudaMemcpyHostToDevice)); *total = 0; return GINT_OK; }
     int* d_sums; long long* d_off;
@@ -312,7 +312,7 @@ static void free_ctx(gint_ctx* c) {
     cudaFree(c->d_poff); cudaFree(c->d_pcanon); cudaFree(c->d_pflag); cudaFree(c->d_pnA);
     cudaFree(c->d_crow); cudaFree(c->d_ckey); cudaFree(c->d_coff); cudaFree(c->d_cpub); cudaFree(c->d_cmir); cudaFree(c->d_cval);
     cudaFree(c->d_bstart); cudaFree(c->d_bent); cudaFree(c->d_tile); cudaFree(c->d_tstart); cudaFree(c->d_gstart);
-    cudaFree(c->d_goff); cudaFree(c->d_phi); cudaFree(c->d_queue);
+    cudaFree(c->d_goff); cudaFree(c->d_phi); cudaFree(c->d_queue); cudaFree(c->d_planoff); cudaFree(c->d_plan);
     cudaFree(c->d_stage_in); cudaFree(c->d_stage_out);
     for (auto& e : c->ev) if (e) cudaEventDestroy(e);
     for (auto& v : c->ev_wave) for (auto& e : v) if (e) cudaEventDestroy(e);
@@ -543,7 +543,7 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, size_t
     int rc;
     if ((rc = dev_alloc(c, &c->d_bstart, (size_t)nbt + 1))) return rc;
     long long n_ent = 0;
-    if ((rc = device_excl_scan(d_count, nbt, c->d_bstart, &n_ent))) return rc;
+    if ((rc = gint_device_excl_scan(d_count, nbt, c->d_bstart, &n_ent))) return rc;
     c->n_entries = n_ent;
     if ((rc = dev_alloc(c, &c->d_bent, (size_t)n_ent))) return rc;
     int *d_bgroups = nullptr, *d_tcount = nullptr;
@@ -558,8 +558,8 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, size_t
     k_tiles_count<<<gridT, 256>>>(nbt, d_bgroups, d_tcount);
     GINT_CUDA(cudaGetLastError());
     long long n_tiles = 0, n_groups = 0;
-    if ((rc = device_excl_scan(d_tcount, nbt, c->d_tstart, &n_tiles))) return rc;
-    if ((rc = device_excl_scan(d_bgroups, nbt, c->d_gstart, &n_groups))) return rc;
+    if ((rc = gint_device_excl_scan(d_tcount, nbt, c->d_tstart, &n_tiles))) return rc;
+    if ((rc = gint_device_excl_scan(d_bgroups, nbt, c->d_gstart, &n_groups))) return rc;
     c->n_tiles = n_tiles;
     if ((rc = dev_alloc(c, &c->d_tile, (size_t)n_tiles))) return rc;
     k_tiles_fill<<<gridT, 256>>>(nbt, d_bgroups, c->d_tstart, c->d_tile);
@@ -569,6 +569,7 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, size_t
     cudaFree(d_bgroups); cudaFree(d_tcount);
     // orbital-value ("Phi") layout: offsets of every (batch, group) slot array, waves, scratch buffer
     if ((rc = gint_build_phi_layout(c, nullptr, phi_cap))) return rc;
+    if ((rc = gint_build_plans(c))) return rc;
 
     c->padded_macs = 0; c->n_batch = 0;
     for (long long b = 0; b < nbt; b++) {

@@ -27,20 +27,21 @@
 #define GINT_MMA_WARPS 12          // warp groups 0,1,2: DMMA consumers, three per SM sub-partition; each owns up to GINT_WARP_BLOCKS blocks
                                    // of 2 row fragments x 4 (block 0) or 3 (blocks 1, 2) column fragments of the tile
 #define GINT_WARP_BLOCKS 3
-#define GINT_AUX_WARPS 4           // warp group 3: warp 12 = TMA issuer (+ rho reducer), warps 13..15 = tile set-up
-#define GINT_SETUP_THREADS 96
+#define GINT_AUX_WARPS 4           // warp group 3: warp 12 = TMA issuer (+ rho reducer), warps 13..15 idle (setmaxnreg works on whole warp groups)
 #define GINT_CTA_THREADS (32 * (GINT_MMA_WARPS + GINT_AUX_WARPS))
 #define GINT_REGS_MMA 152          // registers per thread after setmaxnreg: 384 * 152 + 128 * 56 = 65536
 #define GINT_REGS_AUX 56
 // orbital values ("Phi") in global memory: one SLOT per (atom group, active cubelet) = [orbital row][8 points] doubles,
-// rows padded to whole fragments; 64 bytes per row = the unit of all Phi offsets
+// rows padded to whole fragments, followed by one SIGN ROW (+-0.0 per point: the sign of V there; written by gint_vlocal only).
+// 64 bytes per row = the unit of all Phi offsets
 #define GINT_ROW_BYTES 64
-#define GINT_SLOT_MAX_BYTES (GINT_TILE_ORB * GINT_ROW_BYTES)   // 6656
+#define GINT_SLOT_MAX_BYTES ((GINT_TILE_ORB + 1) * GINT_ROW_BYTES)   // 6720
 // shared-memory ring of the contraction kernels: a stage = GINT_SC cubelets x (slot of group I, slot of group J)
 #define GINT_SC 2
 #define GINT_NS 6
-#define GINT_STAGE_BYTES (GINT_SC * 2 * GINT_SLOT_MAX_BYTES)   // 26624
-#define GINT_NCTX 3                // tile contexts in flight per CTA (set-up runs ahead of the TMA issuer, which runs ahead of the consumers)
+#define GINT_STAGE_BYTES (GINT_SC * 2 * GINT_SLOT_MAX_BYTES)   // 26880
+#define GINT_NCTX 4                // tile plans in flight per CTA (the issuer requests them ahead of the consumers)
+#define GINT_PLAN_THREADS 96       // k_plan_fill (gint_init)
 #define GINT_EVAL_THREADS 256      // orbital-evaluation kernel
 
 // ---- error plumbing -------------------------------------------------------------------------------
@@ -109,6 +110,36 @@ __host__ __device__ inline void image_pos(const Geom& g, const double* p, int t1
     z = fma(w, g.a[8], fma(v, g.a[5], fma(u, g.a[2], p[2])));
 }
 
+// ---- tile plans -----------------------------------------------------------------------------------
+// Everything the contraction kernels need to know about one tile = (batch, atom group I, atom group J) depends on the geometry
+// only.  gint_init writes it once per tile into a PLAN in global memory; at run time the issuer warp of a persistent CTA fetches
+// the plan of its next tile with one TMA bulk copy.  Layout: PlanHdr, then ncub + GINT_SC records PlanCub (the last GINT_SC
+// are zero: the consumers prefetch one stage ahead), padded to a multiple of 16 bytes.
+struct PairEnt { unsigned off; unsigned short sr, sc; };   // element (oa, ob) of the atom pair at off + oa*sr + ob*sc (canonical value array); off = ~0u: none
+struct alignas(16) PlanHdr {
+    int valid;                          // 0: the queue is empty, the roles leave (written by the issuer, never stored)
+    int ncub, nstage;                   // cubelets the tile walks over; ring stages of GINT_SC cubelets
+    int zero;                           // always 0: the consumers' opaque loop condition (keeps ptxas from predicating the DMMA blocks)
+    int nI, nJ, nfI, nfJ;               // atoms / fragments of the two groups
+    int RI, RJ, diag, pad0;             // orbital rows (padded to fragments); I == J
+    int i0, j0, k0, pad1;               // batch origin (mesh points)
+    int ex, ey, ez, pad2;               // batch extents (mesh points; ragged at the mesh edge)
+    unsigned long long rowI, rowJ;      // first 64-byte row of the two groups' slot arrays (numbering over the whole mesh)
+    unsigned blk[GINT_WARP_BLOCKS][GINT_MMA_WARPS];   // consumer warp w, block k: first row fragment | second row present << 4 | first column
+                                        // fragment << 5 | n column fragments << 9   (n = 0: unused).  Block 0 holds up to 4 columns, blocks 1, 2 up to 3.
+    PairEnt pair[GINT_TILE_ATOMS][GINT_TILE_ATOMS];   // canonical block of (I atom a, J atom b)
+    unsigned char row_atom[2][GINT_TILE_ORB];   // orbital row -> atom slot inside the group (255 = padding)
+    unsigned char row_orb[2][GINT_TILE_ORB];    // orbital row -> orbital index inside the atom
+};
+struct PlanCub {                        // one listed cubelet
+    unsigned short slotI, slotJ;        // its slot inside the two groups' slot arrays
+    unsigned char cub, pad[3];          // its bit number in the batch's activity masks
+    unsigned char vis[16];              // per consumer warp: bits 2k, 2k+1 = rows of the warp's block k to work on there (0: skip)
+};
+static_assert(sizeof(PlanHdr) % 16 == 0 && sizeof(PlanCub) == 24, "plan layout");
+#define GINT_PLAN_MAX_BYTES ((sizeof(PlanHdr) + (GINT_NCUB + GINT_SC + 1) * sizeof(PlanCub) + 15) & ~(size_t)15)
+__host__ __device__ inline unsigned plan_units(int ncub) { return (unsigned)((sizeof(PlanHdr) + (size_t)(ncub + GINT_SC) * sizeof(PlanCub) + 15) >> 4); }   // 16-byte units
+
 struct gint_ctx {
     int device = 0;
     Geom geom{};
@@ -148,7 +179,10 @@ struct gint_ctx {
     NeighEntry* d_bent = nullptr;    // neighbour entries sorted by (atom, shift lexicographic)
     int* d_order = nullptr;          // [n_batch_total] batch ids: non-empty first (mesh order), then empty ones
     long long n_tiles = 0;
-    int2* d_tile = nullptr;          // [n_tiles] {batch id, I | J<<8 | G<<16}: group pair (I <= J) of G groups of the batch
+    int2* d_tile = nullptr;          // [n_tiles] {batch id, I | J<<8 | G<<16}: group pair (I <= J) of G groups of the batch (freed once the plans exist)
+    unsigned* d_planoff = nullptr;   // [n_tiles+1] offsets of the tile plans in 16-byte units
+    unsigned char* d_plan = nullptr; // tile plans
+    size_t plan_bytes = 0;
     int* d_tstart = nullptr;         // [n_batch_total+1] first tile of each batch
     int* d_gstart = nullptr;         // [n_batch_total+1] first atom group of each batch (CSR into d_goff)
     unsigned long long* d_goff = nullptr; // [sum G] Phi offset (rows of 64 bytes, whole mesh) of each (batch, group) slot array
@@ -184,6 +218,8 @@ int gint_launch_alg_stats(gint_ctx* c);
 int gint_configure_kernels(gint_ctx* c);
 size_t gint_smem_needed(gint_ctx* c, size_t limit);   // also decides tab_in_smem
 int gint_build_phi_layout(gint_ctx* c, const int* d_bgroups, size_t phi_cap_bytes);   // Phi offsets of every (batch, group), waves, scratch
+int gint_build_plans(gint_ctx* c);                    // tile plans (after the Phi layout)
+int gint_device_excl_scan(const int* d_in, long long n, int* d_out, long long* total);   // gint_init.cu
 
 // Split of the n neighbour entries of a batch into G groups of consecutive entries: group k = [k*n/G, (k+1)*n/G).
 __host__ __device__ inline int group_begin(int k, int n, int G) { return (int)(((long long)k * n) / G); }

@@ -11,19 +11,18 @@
 // per (atom group, cubelet on which the group is active) = [orbital row][8 points] doubles.  The scratch holds one
 // WAVE of batches (a few GB; re-read through L2 by the tiles that follow immediately).
 //
-// Step 3 (k_vlocal_tiles / k_rho_tiles): persistent CTAs, one per SM, pull TILES = (batch, group I, group J), I <= J,
-// from a queue in batch order (tiles sharing a group run at the same time on different SMs, so their slots hit L2).
-// Per CTA three roles run decoupled through mbarriers:
-//   * set-up warps (9..11) prepare the next tiles' contexts (atom slots, canonical block of every atom pair, the list of
-//     cubelets on which both groups are active with per-cubelet fragment activity, the segment plan, V dV weights);
-//   * the issuer warp (8) streams the slots of the tile's cubelets into a shared-memory ring with TMA bulk copies
-//     (cp.async.bulk, complete_tx on the stage's mbarrier) and, in gint_rho, reduces the consumers' partial densities;
-//   * 8 consumer warps (setmaxnreg 232) keep the 104 x 104 block of Phi_I^T diag(V dV) Phi_J (gint_vlocal, Eq. 2
+// Step 3 (k_tiles<vlocal | rho>): persistent CTAs, one per SM, pull TILES = (batch, group I, group J), I <= J, from a queue
+// in batch order (tiles sharing a group run at the same time on different SMs, so their slots hit L2).  What a tile has to
+// know (atom pairs -> canonical blocks, the cubelets on which both groups are active, which warp works on which block of
+// fragments on which cubelet) depends on the geometry only: gint_init writes one PLAN per tile (k_plan_fill).  Per CTA:
+//   * the issuer warp (12) pops the queue, fetches the next tiles' plans and streams the slots of the tile's cubelets into a
+//     shared-memory ring, all with TMA bulk copies (cp.async.bulk, complete_tx on mbarriers); in gint_rho it also reduces
+//     the consumers' partial densities in fixed order and adds them to rho once per tile;
+//   * 12 consumer warps (setmaxnreg 152) keep the 104 x 104 block of Phi_I^T diag(V dV) Phi_J (gint_vlocal, Eq. 2
 //     PAPER.md:66) or of the density blocks D_IJ (gint_rho, Eq. 3) in REGISTERS as DMMA accumulators /
-//     stationary operands: the 13 x 13 fragments are cut into SEGMENTS of one row fragment x up to 7 column
-//     fragments, four per warp, dealt so that the four SM sub-partitions carry equal numbers of DMMAs.  Per cubelet a
-//     segment issues mma.sync.m8n8k4.f64 (DMMA.8x8x4) only for the (row fragment, column fragment) pairs that are
-//     both active there: one R2P sets seven predicates from the activity word, loads and DMMAs are predicated.
+//     stationary operands: the 13 x 13 fragments are cut into BLOCKS of 2 row fragments x 3..4 column fragments, up to
+//     three per warp, dealt so that the four SM sub-partitions carry equal numbers of DMMAs.  Per cubelet a block issues
+//     mma.sync.m8n8k4.f64 (DMMA.8x8x4) only if one of its rows and one of its columns are active there.
 // Only one of each mirror pair of blocks, (A,B,n) / (B,A,-n), is accumulated ("canonical half"); small streaming
 // kernels convert between the public pair-list layout and the canonical layout.
 #include "gint_internal.h"
@@ -89,7 +88,6 @@ __device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  :: "r"(dst), "l"(src), "r"(bytes), "r"(smem_addr(bar)) : "memory");
 }
-__device__ __forceinline__ void setup_sync() { asm volatile("bar.sync 1, %0;" :: "n"(GINT_SETUP_THREADS) : "memory"); }
 
 // ---------------------------------------------------------------------------------------------------
 // Step 2: orbital evaluation, once per (batch, atom, active cubelet).
@@ -103,6 +101,7 @@ struct EvalSmem {
     int row0[GINT_MAX_NB], norb[GINT_MAX_NB], grp[GINT_MAX_NB];
     int item0[GINT_MAX_NB + 1];             // prefix sums of the atoms' active cubelets
     int zitem0[GINT_MAX_NB + 1];            // prefix sums of the atoms' (group slot) pairs
+    int sitem0[GINT_MAX_GROUPS + 1];        // prefix sums of the groups' slots
     cmask gmask[GINT_MAX_GROUPS];
     u64 gbase[GINT_MAX_GROUPS];             // first row of the group's slot array in the wave's Phi scratch
     int gR[GINT_MAX_GROUPS], gfirst[GINT_MAX_GROUPS], gcnt[GINT_MAX_GROUPS], gns[GINT_MAX_GROUPS];
@@ -165,6 +164,9 @@ k_eval_phi(Geom g, long long b0, const int* __restrict__ bstart, const NeighEntr
         int a = 0, z = 0;
         for (int e = 0; e < n; e++) { S.item0[e] = a; S.zitem0[e] = z; a += ccount(S.amask[e]); z += S.gns[S.grp[e]]; }
         S.item0[n] = a; S.zitem0[n] = z;
+        int q = 0;
+        for (int k = 0; k < G; k++) { S.sitem0[k] = q; q += S.gns[k]; }
+        S.sitem0[G] = q;
     }
     __syncthreads();
     const double2* tb = TAB_SMEM ? reinterpret_cast<const double2*>(smem_raw + GINT_EVAL_TAB_OFF) : reinterpret_cast<const double2*>(tab);
@@ -222,7 +224,7 @@ k_eval_phi(Geom g, long long b0, const int* __restrict__ bstart, const NeighEntr
             yw[1] = c1 * uy; yw[2] = c1 * uz; yw[3] = c1 * ux;
             yw[4] = c2x * uy; yw[5] = c2y * uz; yw[6] = c20 * fma(3.0 * uz, uz, -1.0); yw[7] = c2x * uz; yw[8] = c22 * fma(ux, ux, -uy * uy);
         }
-        double* o0 = phi + ((S.gbase[k] + (u64)slot * S.gR[k] + S.row0[e]) << 3) + pl;
+        double* o0 = phi + ((S.gbase[k] + (u64)slot * (S.gR[k] + 1) + S.row0[e]) << 3) + pl;
         const int lpack = S.lpack[e];
 #define GINT_PUT(m) do { *o0 = R * yw[m]; o0 += 8; } while (0)
         for (int s = 0; s < nsh; s++) {
@@ -253,75 +255,80 @@ k_eval_phi(Geom g, long long b0, const int* __restrict__ bstart, const NeighEntr
         int r0 = S.row0[e], r1 = r0 + S.norb[e];
         if (act) r0 = r1;                               // an active atom's own rows were written by pass A
         if (last) r1 = S.gR[k];                         // padding rows
-        double* o0 = phi + ((S.gbase[k] + (u64)slot * S.gR[k]) << 3) + pl;
+        double* o0 = phi + ((S.gbase[k] + (u64)slot * (S.gR[k] + 1)) << 3) + pl;
         for (int rr = r0; rr < r1; rr++) o0[rr << 3] = 0.0;
+    }
+    // ---- pass C (gint_vlocal): the sign row of every slot: -0.0 where V < 0 at the point, else +0.0
+    if (V) {
+        const int n_s = S.sitem0[G];
+        for (int it = qw; it < n_s; it += GINT_EVAL_THREADS / 8) {
+            int k = 0;
+            while (S.sitem0[k + 1] <= it) k++;
+            const int slot = it - S.sitem0[k];
+            const int cl = cselect(S.gmask[k], slot);
+            int ix, iy, iz; cubelet_point(cl, pl, ix, iy, iz);
+            const int gi = i0 + ix, gj = j0 + iy, gk = k0 + iz;
+            const bool in_batch = ix < g.bs[0] && iy < g.bs[1] && iz < g.bs[2] && gi < g.N[0] && gj < g.N[1] && gk < g.N[2];
+            const bool neg = in_batch && __ldg(V + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk) < 0.0;
+            phi[((S.gbase[k] + (u64)slot * (S.gR[k] + 1) + S.gR[k]) << 3) + pl] = neg ? -0.0 : 0.0;
+        }
     }
 }
 
-// ---------------------------------------------------------------------------------------------------
-// shared memory of the contraction kernels
-struct PairEnt { unsigned off; unsigned short sr, sc; };   // element (oa, ob) of the atom pair at off + oa*sr + ob*sc; off = ~0u: none
 
-struct alignas(16) TileCtx {
-    int valid;                          // 0: the queue is empty, the roles leave
-    int ncub, nstage;                   // cubelets the tile walks over; ring stages of GINT_SC cubelets
-    int nI, nJ, nfI, nfJ, RI, RJ, diag;
-    int i0, j0, k0, ex, ey, ez;         // batch origin and extents (mesh points)
-    const double *srcI, *srcJ;          // slot arrays of the two groups
-    unsigned blk[GINT_WARP_BLOCKS][GINT_MMA_WARPS];   // consumer warp w, block k: first row fragment | second row present << 4 | first column
-                                        // fragment << 5 | n column fragments << 9   (n = 0: unused).  Block 0 holds up to 4 columns, blocks 1, 2 up to 3.
-    int zero;                           // always 0: the consumers' opaque loop condition (keeps ptxas from predicating the DMMA blocks)
-    unsigned cubinfo[GINT_NCUB];        // per listed cubelet: active row fragments of I | active column fragments of J << 16
-    unsigned short slotI[GINT_NCUB], slotJ[GINT_NCUB];     // slot of the listed cubelet inside the groups' slot arrays
-    unsigned char cub[GINT_NCUB];       // the listed cubelets (bit numbers of the batch's masks, ascending)
-    PairEnt pair[GINT_TILE_ATOMS][GINT_TILE_ATOMS];   // canonical block of (I atom a, J atom b)
-    unsigned char row_atom[2][GINT_TILE_ORB];   // orbital row -> atom slot inside the group (255 = padding)
-    unsigned char row_orb[2][GINT_TILE_ORB];    // orbital row -> orbital index inside the atom
-    unsigned short vis[GINT_NCUB + GINT_SC][16];   // per listed cubelet and consumer warp: bits 2k, 2k+1 = rows of the warp's block k to work on
-                                        // there (0: skip); bits 8..15 (gint_vlocal): bit 8 + p = V < 0 at point p of the cubelet.  Rows ncub.. are 0.
-    unsigned char sgn[GINT_NCUB];       // set-up scratch for those sign bits
-    alignas(16) double pw[GINT_NCUB][GINT_CPTS];    // gint_rho: the tile's density at the listed cubelets' points (summed by the issuer warp)
-};
-struct SetupScratch {                   // private to the set-up warps
+// ---------------------------------------------------------------------------------------------------
+// Tile plans (gint_init).  k_plan_count: plan size of every tile (one thread per tile); k_plan_fill: one CTA per tile.
+__global__ void __launch_bounds__(256) k_plan_count(long long n_tiles, const int2* __restrict__ tile, const int* __restrict__ bstart,
+                                                    const NeighEntry* __restrict__ bent, int* __restrict__ units) {
+    const long long ti = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (ti >= n_tiles) return;
+    const int2 td = tile[ti];
+    const int b = td.x, I = td.y & 255, J = (td.y >> 8) & 255, G = (td.y >> 16) & 255;
+    const int e0 = bstart[b], n = bstart[b + 1] - e0;
+    cmask mI = czero(), mJ = czero();
+    for (int e = group_begin(I, n, G); e < group_begin(I + 1, n, G); e++) { const NeighEntry en = bent[e0 + e]; mI |= cmask{en.mask[0], en.mask[1]}; }
+    for (int e = group_begin(J, n, G); e < group_begin(J + 1, n, G); e++) { const NeighEntry en = bent[e0 + e]; mJ |= cmask{en.mask[0], en.mask[1]}; }
+    units[ti] = (int)plan_units(ccount(mI & mJ));
+}
+
+struct PlanScratch {
     cmask amask[16];                    // slot s < 8: atom s of group I; slot 8 + s: atom s of group J
     cmask fmask[2][16];                 // [side][fragment]: OR of amask over the atoms with orbitals in the fragment
     int atom[16], shift[16];
     int cstart[2][GINT_TILE_ATOMS + 1]; // first orbital row of each atom inside its group
-    int tile;
+    unsigned cubinfo[GINT_NCUB];        // per listed cubelet: active row fragments of I | active column fragments of J << 16
+    unsigned char asc[GINT_NCUB];       // the cubelets on which both groups are active, ascending
+    int stride;
 };
-static_assert(GINT_SC == 2, "the density reduction of the consumers is written for two cubelets per stage");
-struct alignas(128) TileSmem {
-    unsigned char ring[GINT_NS][GINT_STAGE_BYTES];     // stage: [cubelet q][side][row][8 points]
-    TileCtx ctx[GINT_NCTX];
-    SetupScratch ss;
-    double part[GINT_NS][GINT_MMA_WARPS][GINT_SC * GINT_CPTS];   // gint_rho: per stage, the consumer warps' partial densities
-    u64 full[GINT_NS], empty[GINT_NS];             // stage filled by TMA / read by all consumer warps
-    u64 ctx_full[GINT_NCTX], ctx_free[GINT_NCTX];  // context written by the set-up warps / released by consumers and issuer
-    int hist[GINT_NS];                  // issuer: context | stage of the tile << 8 of what each ring slot holds
+struct alignas(16) PlanSmem {
+    PlanHdr H;
+    PlanCub C[GINT_NCUB + GINT_SC + 1];
+    PlanScratch Q;
 };
+#ifdef GINT_DBG_STATS
+__device__ unsigned long long g_plan_stats[8];
+extern "C" int gint_debug_plan_stats(unsigned long long* out) { return (int)cudaMemcpyFromSymbol(out, g_plan_stats, sizeof(g_plan_stats)); }
+#endif
 
-size_t gint_smem_needed(gint_ctx* c, size_t limit) {
-    c->tab_in_smem = GINT_EVAL_TAB_OFF + c->tab_bytes <= 72 * 1024 && GINT_EVAL_TAB_OFF + c->tab_bytes <= limit;   // three evaluation CTAs per SM
-    c->smem_eval = GINT_EVAL_TAB_OFF + (c->tab_in_smem ? c->tab_bytes : 0);
-    return sizeof(TileSmem) + 128;
-}
-
-// ---------------------------------------------------------------------------------------------------
-// Tile set-up by the 96 threads of warps 9..11: everything the issuer and the consumers need for one tile.
-template <bool VLOCAL>
-__device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileCtx& X, const int2 td, const int* __restrict__ bstart,
-                                           const NeighEntry* __restrict__ bent, const int* __restrict__ gstart,
-                                           const u64* __restrict__ goff, u64 wave_row0, const double* __restrict__ phi,
-                                           const int* __restrict__ atom_spec, const SpeciesDev* __restrict__ sp,
-                                           const int* __restrict__ crow, const u64* __restrict__ ckey,
-                                           const unsigned int* __restrict__ coff, const double* __restrict__ V) {
-    const int sid = threadIdx.x - 32 * (GINT_MMA_WARPS + 1), lane = threadIdx.x & 31, sw = sid >> 5;
-    SetupScratch& Q = S.ss;
+__global__ void __launch_bounds__(GINT_PLAN_THREADS)
+k_plan_fill(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
+            const int* __restrict__ gstart, const u64* __restrict__ goff, const int* __restrict__ atom_spec,
+            const SpeciesDev* __restrict__ sp, const int* __restrict__ crow, const u64* __restrict__ ckey,
+            const unsigned int* __restrict__ coff, const unsigned* __restrict__ planoff, unsigned char* __restrict__ plan) {
+    __shared__ PlanSmem P;
+    PlanHdr& X = P.H;
+    PlanScratch& Q = P.Q;
+    const int sid = threadIdx.x, lane = sid & 31, sw = sid >> 5;
+    const int2 td = tile[blockIdx.x];
     const int b = td.x, I = td.y & 255, J = (td.y >> 8) & 255, G = (td.y >> 16) & 255;
     const bool diag = I == J;
     const int e0 = bstart[b], n = bstart[b + 1] - e0;
     const int eI = group_begin(I, n, G), eJ = group_begin(J, n, G);
     const int nI = group_begin(I + 1, n, G) - eI, nJ = group_begin(J + 1, n, G) - eJ;
+    {   // the records are copied out whole: no stale bytes
+        unsigned* z = reinterpret_cast<unsigned*>(P.C);
+        for (int i = sid; i < (int)(sizeof(P.C) / 4); i += GINT_PLAN_THREADS) z[i] = 0u;
+    }
     if (sid < 16) {
         const int side = sid >> 3, a = sid & 7;
         const bool valid = a < (side ? nJ : nI);
@@ -339,7 +346,7 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileCtx& 
         Q.cstart[side][a] = inc - norb;
         if (a == 7) Q.cstart[side][8] = inc;
     }
-    setup_sync();
+    __syncthreads();
     const int totI = Q.cstart[0][GINT_TILE_ATOMS], totJ = Q.cstart[1][GINT_TILE_ATOMS];
     const int nfI = (totI + 7) >> 3, nfJ = (totJ + 7) >> 3;
     if (sid < 64) {
@@ -387,37 +394,41 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileCtx& 
             X.row_atom[sd][row] = (unsigned char)a; X.row_orb[sd][row] = (unsigned char)o;
         }
     }
-    setup_sync();
+    __syncthreads();
+    cmask mI = czero(), mJ = czero();       // union masks of the two groups (every thread)
+#pragma unroll
+    for (int a = 0; a < 8; a++) { mI |= Q.amask[a]; mJ |= Q.amask[8 + a]; }
+    const cmask U = mI & mJ;
+    const int ncub = ccount(U);
     if (sw == 0) {
-        // cubelet list: the cubelets on which both groups are active, with their slots in the two slot arrays
-        cmask mI = czero(), mJ = czero();
-        if (lane < 8) mI = Q.amask[lane]; else if (lane < 16) mJ = Q.amask[lane];
-        mI.lo = __reduce_or_sync(0xffffffffu, (unsigned)mI.lo) | ((u64)__reduce_or_sync(0xffffffffu, (unsigned)(mI.lo >> 32)) << 32);
-        mI.hi = __reduce_or_sync(0xffffffffu, (unsigned)mI.hi) | ((u64)__reduce_or_sync(0xffffffffu, (unsigned)(mI.hi >> 32)) << 32);
-        mJ.lo = __reduce_or_sync(0xffffffffu, (unsigned)mJ.lo) | ((u64)__reduce_or_sync(0xffffffffu, (unsigned)(mJ.lo >> 32)) << 32);
-        mJ.hi = __reduce_or_sync(0xffffffffu, (unsigned)mJ.hi) | ((u64)__reduce_or_sync(0xffffffffu, (unsigned)(mJ.hi >> 32)) << 32);
-        const cmask U = mI & mJ;
+        // the cubelets on which both groups are active, ascending
         const unsigned Uw[4] = {(unsigned)U.lo, (unsigned)(U.lo >> 32), (unsigned)U.hi, (unsigned)(U.hi >> 32)};
         const unsigned lt = (1u << lane) - 1u;
         int before = 0;
 #pragma unroll
         for (int wd = 0; wd < 4; wd++) {
-            if ((Uw[wd] >> lane) & 1u) {
-                const int pos = before + __popc(Uw[wd] & lt), cl = 32 * wd + lane;
-                X.cub[pos] = (unsigned char)cl;
-                X.slotI[pos] = (unsigned short)crank(mI, cl); X.slotJ[pos] = (unsigned short)crank(mJ, cl);
-            }
+            if ((Uw[wd] >> lane) & 1u) Q.asc[before + __popc(Uw[wd] & lt)] = (unsigned char)(32 * wd + lane);
             before += __popc(Uw[wd]);
         }
-        if (lane == 0) { X.ncub = before; X.nstage = (before + GINT_SC - 1) / GINT_SC; }
     } else if (sid == 32) {
         const int bz = b % g.nb[2], by = (b / g.nb[2]) % g.nb[1], bx = b / (g.nb[2] * g.nb[1]);
         X.i0 = bx * g.bs[0]; X.j0 = by * g.bs[1]; X.k0 = bz * g.bs[2];
         X.ex = min(g.bs[0], g.N[0] - X.i0); X.ey = min(g.bs[1], g.N[1] - X.j0); X.ez = min(g.bs[2], g.N[2] - X.k0);
         X.nI = nI; X.nJ = nJ; X.nfI = nfI; X.nfJ = nfJ; X.RI = 8 * nfI; X.RJ = 8 * nfJ; X.diag = diag;
-        X.srcI = phi + ((goff[gstart[b] + I] - wave_row0) << 3);
-        X.srcJ = phi + ((goff[gstart[b] + J] - wave_row0) << 3);
-        X.valid = 1; X.zero = 0;
+        X.pad0 = X.pad1 = X.pad2 = 0;
+        X.rowI = goff[gstart[b] + I]; X.rowJ = goff[gstart[b] + J];
+        X.valid = 1; X.zero = 0; X.ncub = ncub; X.nstage = (ncub + GINT_SC - 1) / GINT_SC;
+        // The list is walked with a stride coprime to its length (about 0.62 of it): any window of a few consecutive entries then
+        // samples the whole batch, so the work of the consumer warps (whose blocks are active on different parts of the batch)
+        // stays balanced inside the few ring stages they may drift apart.
+        int s = 1;
+#ifndef GINT_PLAN_NO_SCRAMBLE
+        if (ncub > 2) {
+            s = max(1, (ncub * 618) / 1000);
+            for (;; s++) { int x = s, y = ncub; while (y) { const int t = x % y; x = y; y = t; } if (x == 1) break; }
+        }
+#endif
+        Q.stride = s;
     } else if (sid == 64) {
         // Block plan.  The 13 x 13 fragments of the tile are cut into blocks of two adjacent row fragments x 3 or 4 adjacent column
         // fragments (neighbours are sorted by falling activity, so the fragments of a block have similar activity masks).  A block is
@@ -435,15 +446,15 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileCtx& 
             const cmask rm = has1 ? (Q.fmask[0][r0] | Q.fmask[0][r0 + 1]) : Q.fmask[0][r0];
             int c0 = 0;
             for (int gi = 0; gi < ng; gi++) {
-                const int n = ng == 1 ? nfJ : ((gi == 0 && nfJ % 3 == 1) ? 4 : min(3, nfJ - c0));
-                if (c0 + n > cf0) {                    // the block holds a fragment on or above the diagonal
+                const int nn = ng == 1 ? nfJ : ((gi == 0 && nfJ % 3 == 1) ? 4 : min(3, nfJ - c0));
+                if (c0 + nn > cf0) {                    // the block holds a fragment on or above the diagonal
                     cmask cm = czero();
-                    for (int j = 0; j < n; j++) cm |= Q.fmask[1][c0 + j];
-                    desc[np] = (unsigned)r0 | ((unsigned)has1 << 4) | ((unsigned)c0 << 5) | ((unsigned)n << 9);
-                    wgt[np] = ccount(rm & cm) * n * (has1 ? 2 : 1);
+                    for (int j = 0; j < nn; j++) cm |= Q.fmask[1][c0 + j];
+                    desc[np] = (unsigned)r0 | ((unsigned)has1 << 4) | ((unsigned)c0 << 5) | ((unsigned)nn << 9);
+                    wgt[np] = ccount(rm & cm) * nn * (has1 ? 2 : 1);
                     np++;
                 }
-                c0 += n;
+                c0 += nn;
             }
         }
         for (int i = 1; i < np; i++) {      // insertion sort by falling weight
@@ -474,59 +485,23 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileCtx& 
                 X.blk[k][best] = desc[i];
             }
     }
-    setup_sync();
-#ifdef GINT_DBG_STATS
-    if (VLOCAL && sid == 1) {
-        // DMMAs per tile at several granularities of skipping (debug statistics)
-        unsigned long long fine = 0, atomx = 0, dense = 0, rowp = 0, rowf = 0;
-        cmask mJ = czero();
-        for (int cc = 0; cc < nfJ; cc++) mJ |= Q.fmask[1][cc];
-        for (int r = 0; r < nfI; r++) {
-            const int cf = diag ? (Q.cstart[1][X.row_atom[0][8 * r]] >> 3) : 0;
-            for (int cc = cf; cc < nfJ; cc++) fine += 2ull * ccount(Q.fmask[0][r] & Q.fmask[1][cc]);
-            dense += 2ull * (nfJ - cf) * X.ncub;
-            rowf += 2ull * (nfJ - cf) * ccount(Q.fmask[0][r] & mJ);
-            const cmask rp = Q.fmask[0][r & ~1] | Q.fmask[0][min(r | 1, nfI - 1)];
-            rowp += 2ull * (nfJ - cf) * ccount(rp & mJ);
-        }
-        for (int a = 0; a < nI; a++) for (int bb = (diag ? a : 0); bb < nJ; bb++) {
-            const unsigned long long na = Q.cstart[0][a + 1] - Q.cstart[0][a], nb2 = Q.cstart[1][bb + 1] - Q.cstart[1][bb];
-            const unsigned long long el = (diag && a == bb) ? na * (na + 1) / 2 : na * nb2;       // orbital pairs
-            atomx += el * ccount(Q.amask[a] & Q.amask[8 + bb]);                                     // x cubelets (8 points each)
-        }
-        atomicAdd(&g_dbg[13], X.ncub == 0 ? 1ull : 0ull); atomicAdd(&g_dbg[14], X.ncub < 16 ? 1ull : 0ull); atomicAdd(&g_dbg[15], (unsigned long long)X.ncub);
-        atomicAdd(&g_dbg[8], fine); atomicAdd(&g_dbg[9], atomx); atomicAdd(&g_dbg[10], dense); atomicAdd(&g_dbg[11], rowp); atomicAdd(&g_dbg[12], rowf);
-    }
-#endif
-    const int ncub = X.ncub;
-    const int bi0 = X.i0, bj0 = X.j0, bk0 = X.k0, ex = X.ex, ey = X.ey, ez = X.ez;
-    // per listed cubelet: which fragments are active, and the points' weights
-    for (int pos = sid; pos < ncub; pos += GINT_SETUP_THREADS) {
-        const int cl = X.cub[pos];
+    __syncthreads();
+    // the listed cubelets in walking order, their slots and which fragments are active there
+    for (int pos = sid; pos < ncub; pos += GINT_PLAN_THREADS) {
+        const int cl = Q.asc[(int)(((long long)pos * Q.stride) % ncub)];
+        PlanCub& c = P.C[pos];
+        c.cub = (unsigned char)cl;
+        c.slotI = (unsigned short)crank(mI, cl); c.slotJ = (unsigned short)crank(mJ, cl);
         unsigned info = 0;
         for (int f = 0; f < nfI; f++) info |= (unsigned)cbit(Q.fmask[0][f], cl) << f;
         for (int f = 0; f < nfJ; f++) info |= (unsigned)cbit(Q.fmask[1][f], cl) << (16 + f);
-        X.cubinfo[pos] = info;
+        Q.cubinfo[pos] = info;
     }
-    if (VLOCAL) {
-        for (int pos = sid; pos < ncub; pos += GINT_SETUP_THREADS) {
-            const int cl = X.cub[pos];
-            unsigned sg = 0;
-#pragma unroll
-            for (int pp = 0; pp < GINT_CPTS; pp++) {
-                int ix, iy, iz; cubelet_point(cl, pp, ix, iy, iz);
-                if (ix < ex && iy < ey && iz < ez) sg |= (unsigned)(__ldg(V + ((size_t)(bi0 + ix) * g.N[1] + (bj0 + iy)) * g.N[2] + (bk0 + iz)) < 0.0) << pp;
-            }
-            X.sgn[pos] = (unsigned char)sg;
-        }
-    } else {
-        for (int idx = sid; idx < ncub * GINT_CPTS; idx += GINT_SETUP_THREADS) X.pw[0][idx] = 0.0;
-    }
-    setup_sync();
+    __syncthreads();
     // visit codes: which rows of which block every consumer warp works on, per listed cubelet
-    for (int idx = sid; idx < ncub * GINT_MMA_WARPS; idx += GINT_SETUP_THREADS) {
+    for (int idx = sid; idx < ncub * GINT_MMA_WARPS; idx += GINT_PLAN_THREADS) {
         const int pos = idx / GINT_MMA_WARPS, w = idx - pos * GINT_MMA_WARPS;
-        const unsigned info = X.cubinfo[pos];
+        const unsigned info = Q.cubinfo[pos];
         unsigned code = 0;
 #pragma unroll
         for (int k = 0; k < GINT_WARP_BLOCKS; k++) {
@@ -539,59 +514,85 @@ __device__ __forceinline__ void tile_setup(const Geom& g, TileSmem& S, TileCtx& 
             if (cm) code |= rr << (2 * k);
 #endif
         }
-        X.vis[pos][w] = (unsigned short)(code | (VLOCAL ? ((unsigned)X.sgn[pos] << 8) : 0u));
+        P.C[pos].vis[w] = (unsigned char)code;
     }
-    if (sid < GINT_SC * 16) X.vis[ncub + sid / 16][sid % 16] = 0;      // the consumers prefetch one stage ahead
-    setup_sync();
-}
-
-template <bool VLOCAL>
-__device__ __forceinline__ void setup_role(const Geom& g, TileSmem& S, const int2* __restrict__ tile, int n_tiles, int* __restrict__ queue,
-                                           const int* __restrict__ bstart, const NeighEntry* __restrict__ bent, const int* __restrict__ gstart,
-                                           const u64* __restrict__ goff, u64 wave_row0, const double* __restrict__ phi,
-                                           const int* __restrict__ atom_spec, const SpeciesDev* __restrict__ sp,
-                                           const int* __restrict__ crow, const u64* __restrict__ ckey,
-                                           const unsigned int* __restrict__ coff, const double* __restrict__ V) {
-    const int sid = threadIdx.x - 32 * (GINT_MMA_WARPS + 1);
-    for (int t = 0;; t++) {
-        const int c = t % GINT_NCTX;
-        if (t >= GINT_NCTX) mbar_wait(&S.ctx_free[c], ((t / GINT_NCTX) - 1) & 1);
-        if (sid == 0) S.ss.tile = atomicAdd(queue, 1);
-        setup_sync();
-        const int ti = S.ss.tile;
-        if (ti >= n_tiles) {
-            if (sid == 0) { S.ctx[c].valid = 0; mbar_arrive(&S.ctx_full[c]); }
-            return;
+    __syncthreads();
+#ifdef GINT_DBG_STATS
+    if (sid == 1) {
+        // DMMAs per tile at several granularities of skipping (debug statistics)
+        unsigned long long fine = 0, atomx = 0, dense = 0, exec = 0;
+        for (int r = 0; r < nfI; r++) {
+            const int cf = diag ? (Q.cstart[1][X.row_atom[0][8 * r]] >> 3) : 0;
+            for (int cc = cf; cc < nfJ; cc++) fine += 2ull * ccount(Q.fmask[0][r] & Q.fmask[1][cc]);
+            dense += 2ull * (nfJ - cf) * ncub;
         }
-        tile_setup<VLOCAL>(g, S, S.ctx[c], tile[ti], bstart, bent, gstart, goff, wave_row0, phi, atom_spec, sp, crow, ckey, coff, V);
-        if (sid == 0) mbar_arrive(&S.ctx_full[c]);
+        for (int a = 0; a < nI; a++) for (int bb = (diag ? a : 0); bb < nJ; bb++) {
+            const unsigned long long na = Q.cstart[0][a + 1] - Q.cstart[0][a], nb2 = Q.cstart[1][bb + 1] - Q.cstart[1][bb];
+            const unsigned long long el = (diag && a == bb) ? na * (na + 1) / 2 : na * nb2;       // orbital pairs
+            atomx += el * ccount(Q.amask[a] & Q.amask[8 + bb]);                                     // x cubelets (8 points each)
+        }
+        for (int pos = 0; pos < ncub; pos++) for (int w = 0; w < GINT_MMA_WARPS; w++) for (int k = 0; k < GINT_WARP_BLOCKS; k++) {
+            const unsigned rr = (P.C[pos].vis[w] >> (2 * k)) & 3u;
+            if (rr) exec += (rr == 3u ? 4ull : 2ull) * ((X.blk[k][w] >> 9) & 7u);
+        }
+        atomicAdd(&g_plan_stats[0], fine); atomicAdd(&g_plan_stats[1], atomx); atomicAdd(&g_plan_stats[2], dense); atomicAdd(&g_plan_stats[3], exec);
+        atomicAdd(&g_plan_stats[4], (unsigned long long)ncub); atomicAdd(&g_plan_stats[5], 1ull);
     }
+#endif
+    // copy out
+    const unsigned o0 = planoff[blockIdx.x], o1 = planoff[blockIdx.x + 1];
+    const uint4* src = reinterpret_cast<const uint4*>(&P);
+    uint4* dst = reinterpret_cast<uint4*>(plan + (size_t)o0 * 16);
+    for (unsigned i = sid; i < o1 - o0; i += GINT_PLAN_THREADS) dst[i] = src[i];
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Issuer warp: streams the tile's slots into the ring; in gint_rho it also retires the stages: sums the consumer
-// warps' partial densities in fixed order into the tile's density, which it adds to rho when the tile is complete
-// (one red.global.add.f64 per mesh point per tile).
+// shared memory of the contraction kernels
+static_assert(GINT_SC == 2, "the density reduction of the consumers is written for two cubelets per stage");
+struct alignas(128) TileSmem {
+    unsigned char ring[GINT_NS][GINT_STAGE_BYTES];     // stage: [cubelet q][side][row][8 points]
+    alignas(16) unsigned char plan[GINT_NCTX][GINT_PLAN_MAX_BYTES];    // PlanHdr + PlanCub[]
+    alignas(16) double pw[GINT_NCTX][GINT_NCUB][GINT_CPTS];            // gint_rho: the tile's density at the listed cubelets' points (summed by the issuer warp)
+    double part[GINT_NS][GINT_MMA_WARPS][GINT_SC * GINT_CPTS];         // gint_rho: per stage, the consumer warps' partial densities
+    u64 full[GINT_NS], empty[GINT_NS];             // stage filled by TMA / read by all consumer warps
+    u64 ctx_full[GINT_NCTX], ctx_free[GINT_NCTX];  // plan arrived / released by consumers and issuer
+    int hist[GINT_NS];                  // issuer: context | stage of the tile << 8 of what each ring slot holds
+};
+__device__ __forceinline__ const PlanHdr& plan_hdr(const TileSmem& S, int c) { return *reinterpret_cast<const PlanHdr*>(S.plan[c]); }
+__device__ __forceinline__ const PlanCub* plan_cub(const TileSmem& S, int c) { return reinterpret_cast<const PlanCub*>(S.plan[c] + sizeof(PlanHdr)); }
+
+size_t gint_smem_needed(gint_ctx* c, size_t limit) {
+    c->tab_in_smem = GINT_EVAL_TAB_OFF + c->tab_bytes <= 72 * 1024 && GINT_EVAL_TAB_OFF + c->tab_bytes <= limit;   // three evaluation CTAs per SM
+    c->smem_eval = GINT_EVAL_TAB_OFF + (c->tab_in_smem ? c->tab_bytes : 0);
+    return sizeof(TileSmem) + 128;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Issuer warp: pops the tile queue, fetches plans, streams the tile's slots into the ring; in gint_rho it also retires the
+// stages: sums the consumer warps' partial densities in fixed order into the tile's density, which it adds to rho when the
+// tile is complete (one red.global.add.f64 per mesh point per tile).
 template <bool VLOCAL>
 __device__ __forceinline__ void retire_stage(const Geom& g, TileSmem& S, int gr, double* __restrict__ rho) {
     const int lane = threadIdx.x & 31, s = gr % GINT_NS;
     mbar_wait(&S.empty[s], (gr / GINT_NS) & 1);
     if (VLOCAL) return;
     const int h = S.hist[s], c = h & 255, st = h >> 8;
-    TileCtx& X = S.ctx[c];
+    const PlanHdr& X = plan_hdr(S, c);
+    double* pw = &S.pw[c][0][0];
     const int ncs = min(GINT_SC, X.ncub - st * GINT_SC);
     if (lane < ncs * GINT_CPTS) {
         double v = 0.0;
 #pragma unroll
         for (int w = 0; w < GINT_MMA_WARPS; w++) v += S.part[s][w][lane];
-        X.pw[0][st * GINT_SC * GINT_CPTS + lane] += v;
+        pw[st * GINT_SC * GINT_CPTS + lane] = v;        // every listed cubelet belongs to exactly one stage
     }
     if (st == X.nstage - 1) {
         __syncwarp();
+        const PlanCub* C = plan_cub(S, c);
         const int npt = X.ncub * GINT_CPTS;
         for (int idx = lane; idx < npt; idx += 32) {
-            const double v = X.pw[0][idx];
-            int ix, iy, iz; cubelet_point(X.cub[idx >> 3], idx & 7, ix, iy, iz);
+            const double v = pw[idx];
+            int ix, iy, iz; cubelet_point(C[idx >> 3].cub, idx & 7, ix, iy, iz);
             if (v != 0.0 && ix < X.ex && iy < X.ey && iz < X.ez)
                 atomicAdd(rho + ((size_t)(X.i0 + ix) * g.N[1] + (X.j0 + iy)) * g.N[2] + (X.k0 + iz), v);
         }
@@ -601,27 +602,55 @@ __device__ __forceinline__ void retire_stage(const Geom& g, TileSmem& S, int gr,
 }
 
 template <bool VLOCAL>
-__device__ __forceinline__ void issuer_role(const Geom& g, TileSmem& S, double* __restrict__ rho) {
+__device__ __forceinline__ void issuer_role(const Geom& g, TileSmem& S, const unsigned char* __restrict__ plan, const unsigned* __restrict__ planoff,
+                                            int n_tiles, int* __restrict__ queue, const double* __restrict__ phi, u64 wave_row0, double* __restrict__ rho) {
     const int lane = threadIdx.x & 31;
     int gi = 0, gr = 0;                 // stages issued / retired
-    int tile_end[GINT_NCTX];
+    int tile_end[GINT_NCTX];            // gi at the end of the tile that used the context last
 #pragma unroll
     for (int c = 0; c < GINT_NCTX; c++) tile_end[c] = 0;
+    int requested = 0;                  // plans requested so far
+    bool drained = false;               // the queue has run out
+    // request the plan of the next tile into context requested % GINT_NCTX
+    auto request = [&]() {
+        const int t = requested, c = t % GINT_NCTX;
+        if (t >= GINT_NCTX) {
+            // the context's previous tile must be over: all its stages retired (gint_rho flushes its density then), consumers gone
+            if (!VLOCAL) {
+                int te = 0;
+#pragma unroll
+                for (int k = 0; k < GINT_NCTX; k++) if (k == c) te = tile_end[k];
+                while (gr < te) { retire_stage<VLOCAL>(g, S, gr, rho); gr++; }
+            }
+            mbar_wait(&S.ctx_free[c], ((t / GINT_NCTX) - 1) & 1);
+        }
+        int ti = 0;
+        if (lane == 0) ti = atomicAdd(queue, 1);
+        ti = __shfl_sync(0xffffffffu, ti, 0);
+        if (ti >= n_tiles) {
+            if (lane == 0) { reinterpret_cast<PlanHdr*>(S.plan[c])->valid = 0; mbar_arrive(&S.ctx_full[c]); }
+            drained = true;
+        } else if (lane == 0) {
+            const unsigned o0 = __ldg(planoff + ti), o1 = __ldg(planoff + ti + 1);
+            mbar_expect_tx(&S.ctx_full[c], (o1 - o0) * 16u);
+            bulk_g2s(smem_addr(S.plan[c]), plan + (size_t)o0 * 16, (o1 - o0) * 16u, &S.ctx_full[c]);
+        }
+        requested++;
+    };
+    for (int k = 0; k < GINT_NCTX - 2 && !drained; k++) request();
     for (int t = 0;; t++) {
         const int c = t % GINT_NCTX;
-        // the set-up warps can only rebuild this context when its previous tile is retired
-        if (!VLOCAL) {
-            int te = 0;
-#pragma unroll
-            for (int k = 0; k < GINT_NCTX; k++) if (k == c) te = tile_end[k];
-            while (gr < te) { retire_stage<VLOCAL>(g, S, gr, rho); gr++; }
-        }
+        if (!drained && requested < t + GINT_NCTX - 1) request();    // into the context of tile t - 2, which the consumers have left or are about to (tile t - 1 still has stages in the ring)
         mbar_wait(&S.ctx_full[c], (t / GINT_NCTX) & 1);
-        TileCtx& X = S.ctx[c];
+        const PlanHdr& X = plan_hdr(S, c);
         if (!X.valid) break;
+        const PlanCub* C = plan_cub(S, c);
         const int nstage = X.nstage, ncub = X.ncub;
-        const unsigned bI = (unsigned)X.RI * GINT_ROW_BYTES, bJ = X.diag ? 0u : (unsigned)X.RJ * GINT_ROW_BYTES;
-        const double *srcI = X.srcI, *srcJ = X.srcJ;
+        const unsigned strI = (unsigned)(X.RI + 1) * GINT_ROW_BYTES, strJ = (unsigned)(X.RJ + 1) * GINT_ROW_BYTES;     // slot strides
+        const unsigned bI = VLOCAL ? strI : strI - GINT_ROW_BYTES;                 // gint_vlocal also needs the sign row of side I
+        const unsigned bJ = X.diag ? 0u : strJ - GINT_ROW_BYTES;
+        const unsigned char* srcI = reinterpret_cast<const unsigned char*>(phi) + (X.rowI - wave_row0) * GINT_ROW_BYTES;
+        const unsigned char* srcJ = reinterpret_cast<const unsigned char*>(phi) + (X.rowJ - wave_row0) * GINT_ROW_BYTES;
         for (int st = 0; st < nstage; st++, gi++) {
             const int s = gi % GINT_NS;
             while (gi - gr >= GINT_NS) { retire_stage<VLOCAL>(g, S, gr, rho); gr++; }
@@ -635,10 +664,10 @@ __device__ __forceinline__ void issuer_role(const Geom& g, TileSmem& S, double* 
             __syncwarp();
             if (lane < ncs) {
 #endif
-                const int pos = st * GINT_SC + lane;
+                const PlanCub& pc = C[st * GINT_SC + lane];
                 const unsigned dst = smem_addr(&S.ring[s][lane * 2 * GINT_SLOT_MAX_BYTES]);
-                bulk_g2s(dst, reinterpret_cast<const unsigned char*>(srcI) + (size_t)X.slotI[pos] * bI, bI, &S.full[s]);
-                if (bJ) bulk_g2s(dst + GINT_SLOT_MAX_BYTES, reinterpret_cast<const unsigned char*>(srcJ) + (size_t)X.slotJ[pos] * bJ, bJ, &S.full[s]);
+                bulk_g2s(dst, srcI + (size_t)pc.slotI * strI, bI, &S.full[s]);
+                if (bJ) bulk_g2s(dst + GINT_SLOT_MAX_BYTES, srcJ + (size_t)pc.slotJ * strJ, bJ, &S.full[s]);
             }
         }
 #pragma unroll
@@ -649,6 +678,7 @@ __device__ __forceinline__ void issuer_role(const Geom& g, TileSmem& S, double* 
 }
 
 // ---------------------------------------------------------------------------------------------------
+// ---------------------------------------------------------------------------------------------------
 // Consumers.  DMMA.8x8x4 fragment layouts (mma.sync.m8n8k4.f64): A[m = lane / 4][k = lane % 4], B[k = lane % 4][n = lane / 4],
 // C[m = lane / 4][n = 2 (lane % 4) + {0, 1}].  A slot row holds the 8 points of a cubelet; the two k-steps of a cubelet
 // take points {0,2,4,6} and {1,3,5,7}, so that one 128-bit load fetches a lane's operands of both steps.
@@ -657,9 +687,9 @@ __device__ __forceinline__ double2 lds128(unsigned addr) {
     asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory");
     return v;
 }
-__device__ __forceinline__ unsigned lds_u16(unsigned addr) {
-    unsigned short v;
-    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr) : "memory");
+__device__ __forceinline__ unsigned lds_u8(unsigned addr) {
+    unsigned v;
+    asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
     return v;
 }
 __device__ __forceinline__ double lds64(unsigned addr) {
@@ -779,13 +809,13 @@ __device__ __forceinline__ void rho_blk1(const double (&d)[4][2], const double (
 #define GINT_FRAG_BYTES (8 * GINT_ROW_BYTES)
 struct Blk {
     unsigned oa, ob;                 // byte offsets of the first row fragment (side I) and of the first column fragment (side J) inside a cubelet of a stage
-    unsigned d;                      // descriptor (TileCtx::blk)
+    unsigned d;                      // descriptor (PlanHdr::blk)
     __device__ __forceinline__ int row() const { return d & 15; }
     __device__ __forceinline__ bool has1() const { return (d >> 4) & 1u; }
     __device__ __forceinline__ int c0() const { return (d >> 5) & 15; }
     __device__ __forceinline__ int n() const { return (d >> 9) & 7; }
 };
-__device__ __forceinline__ Blk load_blk(const TileCtx& X, unsigned desc) {
+__device__ __forceinline__ Blk load_blk(const PlanHdr& X, unsigned desc) {
     Blk s; s.d = desc;
     s.oa = (unsigned)(s.row() * GINT_FRAG_BYTES);
     s.ob = (unsigned)((X.diag ? 0 : GINT_SLOT_MAX_BYTES) + s.c0() * GINT_FRAG_BYTES);
@@ -842,7 +872,7 @@ __device__ __forceinline__ void rho_visit(const double (&d)[2][4][2], int n, uns
 }
 
 // stationary operands of a row fragment (gint_rho): d[j][h] = Dh[orbital row 8 row + lr of I][orbital column 8 (c0 + j) + 4 h + lc of J]
-__device__ __forceinline__ void load_drow(const TileCtx& X, int rowf, int c0, int n, const double* __restrict__ Dh, double (&d)[4][2]) {
+__device__ __forceinline__ void load_drow(const PlanHdr& X, int rowf, int c0, int n, const double* __restrict__ Dh, double (&d)[4][2]) {
     const int lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
     const int row = 8 * rowf + lr;
     const int a = row < GINT_TILE_ORB ? X.row_atom[0][row] : 255, oa = row < GINT_TILE_ORB ? X.row_orb[0][row] : 0;
@@ -864,7 +894,7 @@ __device__ __forceinline__ void load_drow(const TileCtx& X, int rowf, int c0, in
 }
 // flush of a row fragment's accumulators (gint_vlocal): element (row, col) -> atom pair (a, b), orbitals (oa, ob) -> canonical block
 // (transposed if the canonical key is (b, a)).  Exact zeros (fragments never touched, atoms that do not overlap inside this batch) are skipped.
-__device__ __forceinline__ void flush_row(const TileCtx& X, int rowf, int c0, int n, const double (&acc)[4][2], double* __restrict__ Hc) {
+__device__ __forceinline__ void flush_row(const PlanHdr& X, int rowf, int c0, int n, const double (&acc)[4][2], double* __restrict__ Hc) {
     const int lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
     const int row = 8 * rowf + lr;
     const int a = X.row_atom[0][row], oa = X.row_orb[0][row];
@@ -900,7 +930,7 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
         const int c = t % GINT_NCTX;
         DBG_T(t_ctx0);
         mbar_wait(&S.ctx_full[c], (t / GINT_NCTX) & 1);
-        const TileCtx& X = S.ctx[c];
+        const PlanHdr& X = plan_hdr(S, c);
         if (!X.valid) break;
         DBG_T(t_tile0);
         DBG_ADD(7, t_tile0 - t_ctx0);
@@ -918,11 +948,12 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
                 load_drow(X, bk[k].row() + 1, bk[k].c0(), bk[k].has1() ? bk[k].n() : 0, Dh, acc[k][1]);
             }
         }
-        const int nstage = X.nstage, ncub = X.ncub;
-        const unsigned vis0 = smem_addr(&X.vis[0][warp]);
+        const int nstage = X.nstage;
+        const unsigned vis0 = smem_addr(&plan_cub(S, c)[0].vis[warp]);
+        const unsigned sgn_off = (unsigned)X.RI * GINT_ROW_BYTES + lc * 16;    // gint_vlocal: the lane's two points in the sign row of slot I
         unsigned cur[GINT_SC], nxt[GINT_SC];
 #pragma unroll
-        for (int qq = 0; qq < GINT_SC; qq++) cur[qq] = lds_u16(vis0 + qq * 32);
+        for (int qq = 0; qq < GINT_SC; qq++) cur[qq] = lds_u8(vis0 + qq * (unsigned)sizeof(PlanCub));
         DBG_T(t_tile1);
         DBG_ADD(0, t_tile1 - t_tile0);
         for (int st = 0; st < nstage; st++, gs++) {
@@ -933,7 +964,7 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
             DBG_ADD(1, t_w1 - t_w0);
             double part[GINT_SC][2];
 #pragma unroll
-            for (int qq = 0; qq < GINT_SC; qq++) { part[qq][0] = 0.0; part[qq][1] = 0.0; nxt[qq] = lds_u16(vis0 + ((st + 1) * GINT_SC + qq) * 32); }
+            for (int qq = 0; qq < GINT_SC; qq++) { part[qq][0] = 0.0; part[qq][1] = 0.0; nxt[qq] = lds_u8(vis0 + ((st + 1) * GINT_SC + qq) * (unsigned)sizeof(PlanCub)); }
 #pragma unroll
             for (int qq = 0; qq < GINT_SC; qq++) {
 #ifdef GINT_DBG_NO_MMA
@@ -941,11 +972,11 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
 #else
                 {
 #endif
-                    const unsigned code = cur[qq] & 63u;
+                    const unsigned code = cur[qq];
                     if (code) {
                         const unsigned base = ring0 + s * GINT_STAGE_BYTES + qq * 2 * GINT_SLOT_MAX_BYTES;
                         int sx = 0, sy = 0;
-                        if (VLOCAL) { const unsigned sg = cur[qq] >> (8 + 2 * lc); sx = (int)(sg << 31); sy = (int)((sg >> 1) << 31); }
+                        if (VLOCAL) { const double2 sg = lds128(base + sgn_off); sx = __double2hiint(sg.x); sy = __double2hiint(sg.y); }
 #pragma unroll
                         for (int k = 0; k < GINT_WARP_BLOCKS; k++) {
                             const unsigned rr = (code >> (2 * k)) & 3u;
@@ -1010,11 +1041,8 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
 // gint_vlocal / gint_rho main kernels (north_star step 3): persistent, one CTA per SM.
 template <bool VLOCAL>
 __global__ void __launch_bounds__(GINT_CTA_THREADS, 1)
-k_tiles(Geom g, const int2* __restrict__ tile, int n_tiles, int* __restrict__ queue, const int* __restrict__ bstart,
-        const NeighEntry* __restrict__ bent, const int* __restrict__ gstart, const u64* __restrict__ goff, u64 wave_row0,
-        const double* __restrict__ phi, const int* __restrict__ atom_spec, const SpeciesDev* __restrict__ sp,
-        const int* __restrict__ crow, const u64* __restrict__ ckey, const unsigned int* __restrict__ coff,
-        const double* __restrict__ in /* V or Dh */, double* __restrict__ out /* Hc or rho */) {
+k_tiles(Geom g, const unsigned char* __restrict__ plan, const unsigned* __restrict__ planoff /* of the wave's first tile */, int n_tiles,
+        int* __restrict__ queue, u64 wave_row0, const double* __restrict__ phi, const double* __restrict__ Dh, double* __restrict__ out /* Hc or rho */) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     TileSmem& S = *reinterpret_cast<TileSmem*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~(uintptr_t)127);
     const int warp = threadIdx.x >> 5;
@@ -1026,11 +1054,10 @@ k_tiles(Geom g, const int2* __restrict__ tile, int n_tiles, int* __restrict__ qu
     __syncthreads();
     if (warp < GINT_MMA_WARPS) {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(GINT_REGS_MMA));
-        consumer_role<VLOCAL>(S, in, out);
+        consumer_role<VLOCAL>(S, Dh, out);
     } else {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(GINT_REGS_AUX));
-        if (warp == GINT_MMA_WARPS) issuer_role<VLOCAL>(g, S, out);
-        else setup_role<VLOCAL>(g, S, tile, n_tiles, queue, bstart, bent, gstart, goff, wave_row0, phi, atom_spec, sp, crow, ckey, coff, in);
+        if (warp == GINT_MMA_WARPS) issuer_role<VLOCAL>(g, S, plan, planoff, n_tiles, queue, phi, wave_row0, out);
     }
 }
 
@@ -1079,7 +1106,7 @@ __global__ void __launch_bounds__(256) k_sym_D(long long n_canon, const long lon
 
 // ---------------------------------------------------------------------------------------------------
 // Phi layout (gint_init): rows of every (batch, group) slot array = (cubelets on which the group is active) x (orbital rows
-// padded to whole fragments).  One thread per batch.
+// padded to whole fragments + the sign row).  One thread per batch.
 __global__ void __launch_bounds__(128) k_phi_rows(long long n_batch_total, const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
                                                   const int* __restrict__ gstart, const int* __restrict__ atom_spec,
                                                   const SpeciesDev* __restrict__ sp, unsigned* __restrict__ grows) {
@@ -1094,7 +1121,7 @@ __global__ void __launch_bounds__(128) k_phi_rows(long long n_batch_total, const
             m |= cmask{en.mask[0], en.mask[1]};
             rows += sp[atom_spec[en.atom]].norb;
         }
-        grows[gstart[b] + k] = (unsigned)(ccount(m) * ((rows + 7) & ~7));
+        grows[gstart[b] + k] = (unsigned)(ccount(m) * (((rows + 7) & ~7) + 1));       // + the sign row
     }
 }
 
@@ -1148,6 +1175,32 @@ int gint_build_phi_layout(gint_ctx* c, const int* d_bgroups, size_t phi_cap_byte
         c->ev_wave[k].assign(2 * c->waves.size(), nullptr);
         for (auto& e : c->ev_wave[k]) GINT_CUDA(cudaEventCreate(&e));
     }
+    return GINT_OK;
+}
+
+// Tile plans: sizes, offsets, contents.  The tile list itself is not needed afterwards.
+int gint_build_plans(gint_ctx* c) {
+    const long long nt = c->n_tiles;
+    int* d_units = nullptr;
+    GINT_CUDA(cudaMalloc(&d_units, sizeof(int) * (size_t)(nt ? nt : 1)));
+    GINT_CUDA(cudaMalloc((void**)&c->d_planoff, sizeof(unsigned) * (size_t)(nt + 1)));
+    c->device_bytes += sizeof(unsigned) * (size_t)(nt + 1);
+    if (nt > 0) k_plan_count<<<(unsigned)((nt + 255) / 256), 256>>>(nt, c->d_tile, c->d_bstart, c->d_bent, d_units);
+    GINT_CUDA(cudaGetLastError());
+    long long total = 0;
+    int rc = gint_device_excl_scan(d_units, nt, reinterpret_cast<int*>(c->d_planoff), &total);
+    cudaFree(d_units);
+    if (rc) return rc;
+    c->plan_bytes = (size_t)total * 16;
+    GINT_CUDA(cudaMalloc((void**)&c->d_plan, c->plan_bytes ? c->plan_bytes : 16));
+    c->device_bytes += c->plan_bytes;
+    if (nt > 0)
+        k_plan_fill<<<(unsigned)nt, GINT_PLAN_THREADS>>>(c->geom, c->d_tile, c->d_bstart, c->d_bent, c->d_gstart, c->d_goff, c->d_atom_species,
+                                                          c->d_species, c->d_crow, c->d_ckey, c->d_coff, c->d_planoff, c->d_plan);
+    GINT_CUDA(cudaGetLastError());
+    GINT_CUDA(cudaDeviceSynchronize());
+    cudaFree(c->d_tile); c->d_tile = nullptr;
+    c->device_bytes -= sizeof(int2) * (size_t)(nt ? nt : 1);
     return GINT_OK;
 }
 
@@ -1221,8 +1274,8 @@ static int launch_waves(gint_ctx* c, const double* in, double* out, cudaStream_t
         GINT_CUDA(cudaEventRecord(c->ev_wave[VLOCAL ? 0 : 1][2 * w], st));
         const int nt = (int)(W.t1 - W.t0);
         const unsigned grid = (unsigned)std::min<long long>(c->n_sm, nt);
-        k_tiles<VLOCAL><<<grid, GINT_CTA_THREADS, c->smem_bytes, st>>>(c->geom, c->d_tile + W.t0, nt, c->d_queue + w, c->d_bstart, c->d_bent,
-            c->d_gstart, c->d_goff, W.row0, c->d_phi, c->d_atom_species, c->d_species, c->d_crow, c->d_ckey, c->d_coff, in, out);
+        k_tiles<VLOCAL><<<grid, GINT_CTA_THREADS, c->smem_bytes, st>>>(c->geom, c->d_plan, c->d_planoff + W.t0, nt, c->d_queue + w, W.row0, c->d_phi,
+                                                                       VLOCAL ? nullptr : in, out);
         GINT_CUDA(cudaGetLastError());
         GINT_CUDA(cudaEventRecord(c->ev_wave[VLOCAL ? 0 : 1][2 * w + 1], st));
     }
