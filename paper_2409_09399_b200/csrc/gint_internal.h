@@ -38,7 +38,9 @@
 #define GINT_SLOT_MAX_BYTES ((GINT_TILE_ORB + 1) * GINT_ROW_BYTES)   // 6720
 // shared-memory ring of the contraction kernels: a stage = GINT_SC cubelets x (slot of group I, slot of group J)
 #define GINT_SC 2
+#ifndef GINT_NS
 #define GINT_NS 6
+#endif
 #define GINT_STAGE_BYTES (GINT_SC * 2 * GINT_SLOT_MAX_BYTES)   // 26880
 #define GINT_NCTX 4                // tile plans in flight per CTA (the issuer requests them ahead of the consumers)
 #define GINT_PLAN_THREADS 96       // k_plan_fill (gint_init)

@@ -306,7 +306,7 @@ struct alignas(16) PlanSmem {
     PlanScratch Q;
 };
 #ifdef GINT_DBG_STATS
-__device__ unsigned long long g_plan_stats[8];
+__device__ unsigned long long g_plan_stats[16];
 extern "C" int gint_debug_plan_stats(unsigned long long* out) { return (int)cudaMemcpyFromSymbol(out, g_plan_stats, sizeof(g_plan_stats)); }
 #endif
 
@@ -418,14 +418,16 @@ k_plan_fill(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstar
         X.pad0 = X.pad1 = X.pad2 = 0;
         X.rowI = goff[gstart[b] + I]; X.rowJ = goff[gstart[b] + J];
         X.valid = 1; X.zero = 0; X.ncub = ncub; X.nstage = (ncub + GINT_SC - 1) / GINT_SC;
-        // The list is walked with a stride coprime to its length (about 0.62 of it): any window of a few consecutive entries then
-        // samples the whole batch, so the work of the consumer warps (whose blocks are active on different parts of the batch)
-        // stays balanced inside the few ring stages they may drift apart.
+        // A ring stage holds two neighbours of the ascending list (mostly neighbours along a3: similar activity, gint_rho visits a
+        // stage as a whole).  The pairs are walked with a stride coprime to their number (about 0.62 of it): any window of a few
+        // consecutive stages then samples the whole batch, so the work of the consumer warps (whose blocks are active on different
+        // parts of the batch) stays balanced inside the few ring stages they may drift apart.  An odd last cubelet comes last.
         int s = 1;
 #ifndef GINT_PLAN_NO_SCRAMBLE
-        if (ncub > 2) {
-            s = max(1, (ncub * 618) / 1000);
-            for (;; s++) { int x = s, y = ncub; while (y) { const int t = x % y; x = y; y = t; } if (x == 1) break; }
+        const int npair = ncub / GINT_SC;
+        if (npair > 2) {
+            s = max(1, (npair * 618) / 1000);
+            for (;; s++) { int x = s, y = npair; while (y) { const int t = x % y; x = y; y = t; } if (x == 1) break; }
         }
 #endif
         Q.stride = s;
@@ -488,7 +490,8 @@ k_plan_fill(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstar
     __syncthreads();
     // the listed cubelets in walking order, their slots and which fragments are active there
     for (int pos = sid; pos < ncub; pos += GINT_PLAN_THREADS) {
-        const int cl = Q.asc[(int)(((long long)pos * Q.stride) % ncub)];
+        const int npair = ncub / GINT_SC;
+        const int cl = pos < GINT_SC * npair ? Q.asc[GINT_SC * (int)(((long long)(pos / GINT_SC) * Q.stride) % npair) + pos % GINT_SC] : Q.asc[pos];
         PlanCub& c = P.C[pos];
         c.cub = (unsigned char)cl;
         c.slotI = (unsigned short)crank(mI, cl); c.slotJ = (unsigned short)crank(mJ, cl);
@@ -535,6 +538,46 @@ k_plan_fill(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstar
             const unsigned rr = (P.C[pos].vis[w] >> (2 * k)) & 3u;
             if (rr) exec += (rr == 3u ? 4ull : 2ull) * ((X.blk[k][w] >> 9) & 7u);
         }
+        // what-if: a visit covers GR consecutive cubelets of the ascending list (rows / columns active on any of them)
+        unsigned long long execg[2] = {0, 0}, visg[3] = {0, 0, 0};
+        for (int gi = 0; gi < 3; gi++) {
+            const int GR = gi == 0 ? 1 : (gi == 1 ? 2 : 4);
+            for (int p0 = 0; p0 < ncub; p0 += GR) {
+                unsigned info = 0; int cnt = 0;
+                for (int u = 0; u < GR && p0 + u < ncub; u++) {
+                    const int cl = Q.asc[p0 + u]; cnt++;
+                    for (int f = 0; f < nfI; f++) info |= (unsigned)cbit(Q.fmask[0][f], cl) << f;
+                    for (int f = 0; f < nfJ; f++) info |= (unsigned)cbit(Q.fmask[1][f], cl) << (16 + f);
+                }
+                for (int w = 0; w < GINT_MMA_WARPS; w++) for (int k = 0; k < GINT_WARP_BLOCKS; k++) {
+                    const unsigned d = X.blk[k][w];
+                    if (!((d >> 9) & 7u)) continue;
+                    const unsigned rr = (info >> (d & 15u)) & (((d >> 4) & 1u) ? 3u : 1u);
+                    const unsigned cm = (info >> (16 + ((d >> 5) & 15u))) & ((1u << ((d >> 9) & 7u)) - 1u);
+                    if (rr && cm) { visg[gi]++; if (gi) execg[gi - 1] += (rr == 3u ? 4ull : 2ull) * ((d >> 9) & 7u) * cnt; }
+                }
+            }
+        }
+        // balance of the four SM sub-partitions (consumer warp w runs on w % 4): per window of GINT_NS stages, max / mean of their DMMA counts
+        {
+            unsigned long long sum_max = 0, sum_all = 0, tot[4] = {0, 0, 0, 0}, win[4] = {0, 0, 0, 0};
+            for (int pos = 0; pos < ncub; pos++) {
+                for (int w = 0; w < GINT_MMA_WARPS; w++) for (int k = 0; k < GINT_WARP_BLOCKS; k++) {
+                    const unsigned rr = (P.C[pos].vis[w] >> (2 * k)) & 3u;
+                    if (rr) { const unsigned long long v = (rr == 3u ? 4ull : 2ull) * ((X.blk[k][w] >> 9) & 7u); win[w & 3] += v; tot[w & 3] += v; }
+                }
+                if ((pos + 1) % (GINT_NS * GINT_SC) == 0 || pos == ncub - 1) {
+                    unsigned long long m = 0;
+                    for (int q4 = 0; q4 < 4; q4++) { m = win[q4] > m ? win[q4] : m; sum_all += win[q4]; win[q4] = 0; }
+                    sum_max += 4 * m;
+                }
+            }
+            unsigned long long mt = 0;
+            for (int q4 = 0; q4 < 4; q4++) mt = tot[q4] > mt ? tot[q4] : mt;
+            atomicAdd(&g_plan_stats[11], sum_max); atomicAdd(&g_plan_stats[12], sum_all); atomicAdd(&g_plan_stats[13], 4 * mt);
+        }
+        atomicAdd(&g_plan_stats[6], execg[0]); atomicAdd(&g_plan_stats[7], execg[1]);
+        atomicAdd(&g_plan_stats[8], visg[0]); atomicAdd(&g_plan_stats[9], visg[1]); atomicAdd(&g_plan_stats[10], visg[2]);
         atomicAdd(&g_plan_stats[0], fine); atomicAdd(&g_plan_stats[1], atomx); atomicAdd(&g_plan_stats[2], dense); atomicAdd(&g_plan_stats[3], exec);
         atomicAdd(&g_plan_stats[4], (unsigned long long)ncub); atomicAdd(&g_plan_stats[5], 1ull);
     }
@@ -753,58 +796,6 @@ __device__ __forceinline__ void vl_blk1(double (&c)[4][2], double ax, double ay,
             : "d"(ax), "d"(ay), "d"(b[0].x), "d"(b[0].y), "d"(b[1].x), "d"(b[1].y), "d"(b[2].x), "d"(b[2].y), "r"(q));
     }
 }
-// gint_rho block, both rows: y_r += sum_j D[r][j] b_j (two chains, interleaved).  d[r][j][h]: stationary A operands, bx/by[j]: the two k-steps of column j.
-template <int N>
-__device__ __forceinline__ void rho_blk2(const double (&d)[2][4][2], const double (&bx)[4], const double (&by)[4], int q, double (&y0)[2], double (&y1)[2]) {
-    if (N == 4) {
-        asm volatile(
-            "{\n\t.reg .pred pq;\n\tsetp.ne.s32 pq, %28, 0;\n\tL_%=:\n\t"
-            GINT_DMMA("%0", "%1", "%4", "%20") GINT_DMMA("%2", "%3", "%12", "%20") GINT_DMMA("%0", "%1", "%5", "%24") GINT_DMMA("%2", "%3", "%13", "%24")
-            GINT_DMMA("%0", "%1", "%6", "%21") GINT_DMMA("%2", "%3", "%14", "%21") GINT_DMMA("%0", "%1", "%7", "%25") GINT_DMMA("%2", "%3", "%15", "%25")
-            GINT_DMMA("%0", "%1", "%8", "%22") GINT_DMMA("%2", "%3", "%16", "%22") GINT_DMMA("%0", "%1", "%9", "%26") GINT_DMMA("%2", "%3", "%17", "%26")
-            GINT_DMMA("%0", "%1", "%10", "%23") GINT_DMMA("%2", "%3", "%18", "%23") GINT_DMMA("%0", "%1", "%11", "%27") GINT_DMMA("%2", "%3", "%19", "%27")
-            "@pq bra.uni L_%=;\n\t}"
-            : "+d"(y0[0]), "+d"(y0[1]), "+d"(y1[0]), "+d"(y1[1])
-            : "d"(d[0][0][0]), "d"(d[0][0][1]), "d"(d[0][1][0]), "d"(d[0][1][1]), "d"(d[0][2][0]), "d"(d[0][2][1]), "d"(d[0][3][0]), "d"(d[0][3][1]),
-              "d"(d[1][0][0]), "d"(d[1][0][1]), "d"(d[1][1][0]), "d"(d[1][1][1]), "d"(d[1][2][0]), "d"(d[1][2][1]), "d"(d[1][3][0]), "d"(d[1][3][1]),
-              "d"(bx[0]), "d"(bx[1]), "d"(bx[2]), "d"(bx[3]), "d"(by[0]), "d"(by[1]), "d"(by[2]), "d"(by[3]), "r"(q));
-    } else {
-        asm volatile(
-            "{\n\t.reg .pred pq;\n\tsetp.ne.s32 pq, %22, 0;\n\tL_%=:\n\t"
-            GINT_DMMA("%0", "%1", "%4", "%16") GINT_DMMA("%2", "%3", "%10", "%16") GINT_DMMA("%0", "%1", "%5", "%19") GINT_DMMA("%2", "%3", "%11", "%19")
-            GINT_DMMA("%0", "%1", "%6", "%17") GINT_DMMA("%2", "%3", "%12", "%17") GINT_DMMA("%0", "%1", "%7", "%20") GINT_DMMA("%2", "%3", "%13", "%20")
-            GINT_DMMA("%0", "%1", "%8", "%18") GINT_DMMA("%2", "%3", "%14", "%18") GINT_DMMA("%0", "%1", "%9", "%21") GINT_DMMA("%2", "%3", "%15", "%21")
-            "@pq bra.uni L_%=;\n\t}"
-            : "+d"(y0[0]), "+d"(y0[1]), "+d"(y1[0]), "+d"(y1[1])
-            : "d"(d[0][0][0]), "d"(d[0][0][1]), "d"(d[0][1][0]), "d"(d[0][1][1]), "d"(d[0][2][0]), "d"(d[0][2][1]),
-              "d"(d[1][0][0]), "d"(d[1][0][1]), "d"(d[1][1][0]), "d"(d[1][1][1]), "d"(d[1][2][0]), "d"(d[1][2][1]),
-              "d"(bx[0]), "d"(bx[1]), "d"(bx[2]), "d"(by[0]), "d"(by[1]), "d"(by[2]), "r"(q));
-    }
-}
-// one row of a block: two chains (the x and the y k-steps), summed by the caller
-template <int N>
-__device__ __forceinline__ void rho_blk1(const double (&d)[4][2], const double (&bx)[4], const double (&by)[4], int q, double (&ya)[2], double (&yb)[2]) {
-    if (N == 4) {
-        asm volatile(
-            "{\n\t.reg .pred pq;\n\tsetp.ne.s32 pq, %20, 0;\n\tL_%=:\n\t"
-            GINT_DMMA("%0", "%1", "%4", "%12") GINT_DMMA("%2", "%3", "%5", "%16") GINT_DMMA("%0", "%1", "%6", "%13") GINT_DMMA("%2", "%3", "%7", "%17")
-            GINT_DMMA("%0", "%1", "%8", "%14") GINT_DMMA("%2", "%3", "%9", "%18") GINT_DMMA("%0", "%1", "%10", "%15") GINT_DMMA("%2", "%3", "%11", "%19")
-            "@pq bra.uni L_%=;\n\t}"
-            : "+d"(ya[0]), "+d"(ya[1]), "+d"(yb[0]), "+d"(yb[1])
-            : "d"(d[0][0]), "d"(d[0][1]), "d"(d[1][0]), "d"(d[1][1]), "d"(d[2][0]), "d"(d[2][1]), "d"(d[3][0]), "d"(d[3][1]),
-              "d"(bx[0]), "d"(bx[1]), "d"(bx[2]), "d"(bx[3]), "d"(by[0]), "d"(by[1]), "d"(by[2]), "d"(by[3]), "r"(q));
-    } else {
-        asm volatile(
-            "{\n\t.reg .pred pq;\n\tsetp.ne.s32 pq, %16, 0;\n\tL_%=:\n\t"
-            GINT_DMMA("%0", "%1", "%4", "%10") GINT_DMMA("%2", "%3", "%5", "%13") GINT_DMMA("%0", "%1", "%6", "%11") GINT_DMMA("%2", "%3", "%7", "%14")
-            GINT_DMMA("%0", "%1", "%8", "%12") GINT_DMMA("%2", "%3", "%9", "%15")
-            "@pq bra.uni L_%=;\n\t}"
-            : "+d"(ya[0]), "+d"(ya[1]), "+d"(yb[0]), "+d"(yb[1])
-            : "d"(d[0][0]), "d"(d[0][1]), "d"(d[1][0]), "d"(d[1][1]), "d"(d[2][0]), "d"(d[2][1]),
-              "d"(bx[0]), "d"(bx[1]), "d"(bx[2]), "d"(by[0]), "d"(by[1]), "d"(by[2]), "r"(q));
-    }
-}
-
 // Blocks of a consumer warp.
 #define GINT_FRAG_BYTES (8 * GINT_ROW_BYTES)
 struct Blk {
@@ -844,33 +835,93 @@ __device__ __forceinline__ void vl_visit(double (&acc)[2][4][2], int n, unsigned
         else vl_blk1<3>(acc[1], a1.x, a1.y, b, q);
     }
 }
-// gint_rho, one block on one cubelet: Y_r = sum_j D[row r][column j] Phi_J[column j] (8 orbitals of I x 8 points), then
-// rho_g += sum_i Phi_I[i][g] Y_r[i][g].  pj: lane address of Phi_J[8 c0 + lane % 4][point lane / 4]; pi: of Phi_I[8 row + lane / 4][points 2 (lane % 4), + 1].
-template <int NMAX>
-__device__ __forceinline__ void rho_visit(const double (&d)[2][4][2], int n, unsigned pi, unsigned pj, bool ra, bool rb, int q, double& r0, double& r1) {
-    double bx[4], by[4];
-#pragma unroll
-    for (int j = 0; j < 4; j++) { bx[j] = 0.0; by[j] = 0.0; }
-#pragma unroll
-    for (int j = 0; j < NMAX; j++) { bx[j] = lds64(pj + j * GINT_FRAG_BYTES); by[j] = lds64(pj + j * GINT_FRAG_BYTES + 4 * GINT_ROW_BYTES); }
-#pragma unroll
-    for (int j = 1; j < 3; j++) if (j >= n) { bx[j] = 0.0; by[j] = 0.0; }      // a narrower block: D is zero there, the operand must be finite
-    const double2 f0 = lds128(pi), f1 = lds128(pi + GINT_FRAG_BYTES);
-    double y0[2] = {0.0, 0.0}, y1[2] = {0.0, 0.0};
-    const bool wide = NMAX == 4 && n == 4;
-    if (ra && rb) {
-        if (wide) rho_blk2<4>(d, bx, by, q, y0, y1); else rho_blk2<3>(d, bx, by, q, y0, y1);
-        r0 = fma(y0[0], f0.x, r0); r1 = fma(y0[1], f0.y, r1);
-        r0 = fma(y1[0], f1.x, r0); r1 = fma(y1[1], f1.y, r1);
-    } else if (ra) {        // an inactive row fragment of a slot may hold anything: its Phi_I values must not be touched
-        if (wide) rho_blk1<4>(d[0], bx, by, q, y0, y1); else rho_blk1<3>(d[0], bx, by, q, y0, y1);
-        r0 = fma(y0[0] + y1[0], f0.x, r0); r1 = fma(y0[1] + y1[1], f0.y, r1);
+// gint_rho, one block on one ring stage (two cubelets): Y_qr = sum_j D[row r][column j] Phi_J[column j] at the 8 points of cubelet q
+// (8 orbitals of I x 8 points), four accumulator chains (two with one row); the operands of Phi_J are loaded inside the block, so
+// that ptxas schedules them among the DMMAs.  d[r][j][h]: stationary A operands (k-step h of column j); pj0, pj1: lane addresses of
+// Phi_J[8 c0 + lane % 4][point lane / 4] in the two cubelets; y[q][r][e]: C fragments (orbital row lane / 4, points 2 (lane % 4) + e).
+template <int R, int N>
+__device__ __forceinline__ void rho_stage_blk(const double (&d)[2][4][2], unsigned pj0, unsigned pj1, int q, double (&y)[2][2][2]) {
+    if (R == 2 && N == 4) {
+        asm volatile(
+            "{\n\t.reg .pred pq;\n\t.reg .f64 z;\n\t.reg .f64 b<16>;\n\tsetp.ne.s32 pq, %26, 0;\n\tmov.f64 z, 0d0000000000000000;\n\tL_%=:\n\t"
+            "ld.shared.f64 b0, [%24+0];\n\tld.shared.f64 b1, [%24+256];\n\tld.shared.f64 b2, [%24+512];\n\tld.shared.f64 b3, [%24+768];\n\tld.shared.f64 b4, [%24+1024];\n\tld.shared.f64 b5, [%24+1280];\n\tld.shared.f64 b6, [%24+1536];\n\tld.shared.f64 b7, [%24+1792];\n\tld.shared.f64 b8, [%25+0];\n\tld.shared.f64 b9, [%25+256];\n\tld.shared.f64 b10, [%25+512];\n\tld.shared.f64 b11, [%25+768];\n\tld.shared.f64 b12, [%25+1024];\n\tld.shared.f64 b13, [%25+1280];\n\tld.shared.f64 b14, [%25+1536];\n\tld.shared.f64 b15, [%25+1792];\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%8},{b0},{z,z};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%16},{b0},{z,z};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{%8},{b8},{z,z};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{%16},{b8},{z,z};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%9},{b1},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%17},{b1},{%2,%3};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{%9},{b9},{%4,%5};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{%17},{b9},{%6,%7};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%10},{b2},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%18},{b2},{%2,%3};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{%10},{b10},{%4,%5};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{%18},{b10},{%6,%7};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%11},{b3},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%19},{b3},{%2,%3};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{%11},{b11},{%4,%5};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{%19},{b11},{%6,%7};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%12},{b4},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%20},{b4},{%2,%3};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{%12},{b12},{%4,%5};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{%20},{b12},{%6,%7};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%13},{b5},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%21},{b5},{%2,%3};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{%13},{b13},{%4,%5};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{%21},{b13},{%6,%7};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%14},{b6},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%22},{b6},{%2,%3};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{%14},{b14},{%4,%5};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{%22},{b14},{%6,%7};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%15},{b7},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%23},{b7},{%2,%3};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{%15},{b15},{%4,%5};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{%23},{b15},{%6,%7};\n\t"
+            "@pq bra.uni L_%=;\n\t}"
+            : "=d"(y[0][0][0]), "=d"(y[0][0][1]), "=d"(y[0][1][0]), "=d"(y[0][1][1]), "=d"(y[1][0][0]), "=d"(y[1][0][1]), "=d"(y[1][1][0]), "=d"(y[1][1][1])
+            : "d"(d[0][0][0]), "d"(d[0][0][1]), "d"(d[0][1][0]), "d"(d[0][1][1]), "d"(d[0][2][0]), "d"(d[0][2][1]), "d"(d[0][3][0]), "d"(d[0][3][1]), "d"(d[1][0][0]), "d"(d[1][0][1]), "d"(d[1][1][0]), "d"(d[1][1][1]), "d"(d[1][2][0]), "d"(d[1][2][1]), "d"(d[1][3][0]), "d"(d[1][3][1]), "r"(pj0), "r"(pj1), "r"(q));
+    } else if (R == 2) {
+        asm volatile(
+            "{\n\t.reg .pred pq;\n\t.reg .f64 z;\n\t.reg .f64 b<12>;\n\tsetp.ne.s32 pq, %22, 0;\n\tmov.f64 z, 0d0000000000000000;\n\tL_%=:\n\t"
+            "ld.shared.f64 b0, [%20+0];\n\tld.shared.f64 b1, [%20+256];\n\tld.shared.f64 b2, [%20+512];\n\tld.shared.f64 b3, [%20+768];\n\tld.shared.f64 b4, [%20+1024];\n\tld.shared.f64 b5, [%20+1280];\n\tld.shared.f64 b6, [%21+0];\n\tld.shared.f64 b7, [%21+256];\n\tld.shared.f64 b8, [%21+512];\n\tld.shared.f64 b9, [%21+768];\n\tld.shared.f64 b10, [%21+1024];\n\tld.shared.f64 b11, [%21+1280];\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%8},{b0},{z,z};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%14},{b0},{z,z};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{%8},{b6},{z,z};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{%14},{b6},{z,z};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%9},{b1},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%15},{b1},{%2,%3};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{%9},{b7},{%4,%5};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{%15},{b7},{%6,%7};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%10},{b2},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%16},{b2},{%2,%3};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{%10},{b8},{%4,%5};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{%16},{b8},{%6,%7};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%11},{b3},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%17},{b3},{%2,%3};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{%11},{b9},{%4,%5};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{%17},{b9},{%6,%7};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%12},{b4},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%18},{b4},{%2,%3};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{%12},{b10},{%4,%5};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{%18},{b10},{%6,%7};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%13},{b5},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%19},{b5},{%2,%3};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%4,%5},{%13},{b11},{%4,%5};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%6,%7},{%19},{b11},{%6,%7};\n\t"
+            "@pq bra.uni L_%=;\n\t}"
+            : "=d"(y[0][0][0]), "=d"(y[0][0][1]), "=d"(y[0][1][0]), "=d"(y[0][1][1]), "=d"(y[1][0][0]), "=d"(y[1][0][1]), "=d"(y[1][1][0]), "=d"(y[1][1][1])
+            : "d"(d[0][0][0]), "d"(d[0][0][1]), "d"(d[0][1][0]), "d"(d[0][1][1]), "d"(d[0][2][0]), "d"(d[0][2][1]), "d"(d[1][0][0]), "d"(d[1][0][1]), "d"(d[1][1][0]), "d"(d[1][1][1]), "d"(d[1][2][0]), "d"(d[1][2][1]), "r"(pj0), "r"(pj1), "r"(q));
+    } else if (N == 4) {
+        asm volatile(
+            "{\n\t.reg .pred pq;\n\t.reg .f64 z;\n\t.reg .f64 b<16>;\n\tsetp.ne.s32 pq, %14, 0;\n\tmov.f64 z, 0d0000000000000000;\n\tL_%=:\n\t"
+            "ld.shared.f64 b0, [%12+0];\n\tld.shared.f64 b1, [%12+256];\n\tld.shared.f64 b2, [%12+512];\n\tld.shared.f64 b3, [%12+768];\n\tld.shared.f64 b4, [%12+1024];\n\tld.shared.f64 b5, [%12+1280];\n\tld.shared.f64 b6, [%12+1536];\n\tld.shared.f64 b7, [%12+1792];\n\tld.shared.f64 b8, [%13+0];\n\tld.shared.f64 b9, [%13+256];\n\tld.shared.f64 b10, [%13+512];\n\tld.shared.f64 b11, [%13+768];\n\tld.shared.f64 b12, [%13+1024];\n\tld.shared.f64 b13, [%13+1280];\n\tld.shared.f64 b14, [%13+1536];\n\tld.shared.f64 b15, [%13+1792];\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%4},{b0},{z,z};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%4},{b8},{z,z};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%5},{b1},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%5},{b9},{%2,%3};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%6},{b2},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%6},{b10},{%2,%3};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%7},{b3},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%7},{b11},{%2,%3};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%8},{b4},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%8},{b12},{%2,%3};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%9},{b5},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%9},{b13},{%2,%3};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%10},{b6},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%10},{b14},{%2,%3};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%11},{b7},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%11},{b15},{%2,%3};\n\t"
+            "@pq bra.uni L_%=;\n\t}"
+            : "=d"(y[0][0][0]), "=d"(y[0][0][1]), "=d"(y[1][0][0]), "=d"(y[1][0][1])
+            : "d"(d[0][0][0]), "d"(d[0][0][1]), "d"(d[0][1][0]), "d"(d[0][1][1]), "d"(d[0][2][0]), "d"(d[0][2][1]), "d"(d[0][3][0]), "d"(d[0][3][1]), "r"(pj0), "r"(pj1), "r"(q));
     } else {
-        if (wide) rho_blk1<4>(d[1], bx, by, q, y0, y1); else rho_blk1<3>(d[1], bx, by, q, y0, y1);
-        r0 = fma(y0[0] + y1[0], f1.x, r0); r1 = fma(y0[1] + y1[1], f1.y, r1);
+        asm volatile(
+            "{\n\t.reg .pred pq;\n\t.reg .f64 z;\n\t.reg .f64 b<12>;\n\tsetp.ne.s32 pq, %12, 0;\n\tmov.f64 z, 0d0000000000000000;\n\tL_%=:\n\t"
+            "ld.shared.f64 b0, [%10+0];\n\tld.shared.f64 b1, [%10+256];\n\tld.shared.f64 b2, [%10+512];\n\tld.shared.f64 b3, [%10+768];\n\tld.shared.f64 b4, [%10+1024];\n\tld.shared.f64 b5, [%10+1280];\n\tld.shared.f64 b6, [%11+0];\n\tld.shared.f64 b7, [%11+256];\n\tld.shared.f64 b8, [%11+512];\n\tld.shared.f64 b9, [%11+768];\n\tld.shared.f64 b10, [%11+1024];\n\tld.shared.f64 b11, [%11+1280];\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%4},{b0},{z,z};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%4},{b6},{z,z};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%5},{b1},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%5},{b7},{%2,%3};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%6},{b2},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%6},{b8},{%2,%3};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%7},{b3},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%7},{b9},{%2,%3};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%8},{b4},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%8},{b10},{%2,%3};\n\t"
+            "mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%9},{b5},{%0,%1};\n\tmma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%2,%3},{%9},{b11},{%2,%3};\n\t"
+            "@pq bra.uni L_%=;\n\t}"
+            : "=d"(y[0][0][0]), "=d"(y[0][0][1]), "=d"(y[1][0][0]), "=d"(y[1][0][1])
+            : "d"(d[0][0][0]), "d"(d[0][0][1]), "d"(d[0][1][0]), "d"(d[0][1][1]), "d"(d[0][2][0]), "d"(d[0][2][1]), "r"(pj0), "r"(pj1), "r"(q));
     }
 }
-
+// One block on one stage, then rho_g += sum_i Phi_I[i][g] Y[i][g] (the sum over the 8 orbital rows of a fragment = over lane / 4 is
+// taken once per stage by the caller).  pi: lane address of Phi_I[8 row + lane / 4][points 2 (lane % 4), + 1] in cubelet 0.
+// Columns beyond the block's n hold D = 0 and whatever the ring holds there (always finite: the ring starts zeroed and only ever
+// receives orbital values), likewise the second row of a single-row block.
+template <int NMAX>
+__device__ __forceinline__ void rho_stage_issue(const double (&d)[2][4][2], int n, bool has1, unsigned pj, int q, double (&y)[2][2][2]) {
+    const bool wide = NMAX == 4 && n == 4;
+    const unsigned pj1 = pj + 2 * GINT_SLOT_MAX_BYTES;
+    if (has1) {
+        if (wide) rho_stage_blk<2, 4>(d, pj, pj1, q, y); else rho_stage_blk<2, 3>(d, pj, pj1, q, y);
+    } else {
+        y[0][1][0] = 0.0; y[0][1][1] = 0.0; y[1][1][0] = 0.0; y[1][1][1] = 0.0;
+        if (wide) rho_stage_blk<1, 4>(d, pj, pj1, q, y); else rho_stage_blk<1, 3>(d, pj, pj1, q, y);
+    }
+}
+__device__ __forceinline__ void rho_stage_retire(const double (&y)[2][2][2], unsigned pi, double (&part)[GINT_SC][2]) {
+    const unsigned pi1 = pi + 2 * GINT_SLOT_MAX_BYTES;
+    const double2 f00 = lds128(pi), f01 = lds128(pi + GINT_FRAG_BYTES), f10 = lds128(pi1), f11 = lds128(pi1 + GINT_FRAG_BYTES);
+    part[0][0] = fma(y[0][0][0], f00.x, part[0][0]); part[0][1] = fma(y[0][0][1], f00.y, part[0][1]);
+    part[1][0] = fma(y[1][0][0], f10.x, part[1][0]); part[1][1] = fma(y[1][0][1], f10.y, part[1][1]);
+    part[0][0] = fma(y[0][1][0], f01.x, part[0][0]); part[0][1] = fma(y[0][1][1], f01.y, part[0][1]);
+    part[1][0] = fma(y[1][1][0], f11.x, part[1][0]); part[1][1] = fma(y[1][1][1], f11.y, part[1][1]);
+}
 // stationary operands of a row fragment (gint_rho): d[j][h] = Dh[orbital row 8 row + lr of I][orbital column 8 (c0 + j) + 4 h + lc of J]
 __device__ __forceinline__ void load_drow(const PlanHdr& X, int rowf, int c0, int n, const double* __restrict__ Dh, double (&d)[4][2]) {
     const int lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
@@ -965,35 +1016,45 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
             double part[GINT_SC][2];
 #pragma unroll
             for (int qq = 0; qq < GINT_SC; qq++) { part[qq][0] = 0.0; part[qq][1] = 0.0; nxt[qq] = lds_u8(vis0 + ((st + 1) * GINT_SC + qq) * (unsigned)sizeof(PlanCub)); }
+#ifndef GINT_DBG_NO_MMA
+            if (VLOCAL) {
 #pragma unroll
-            for (int qq = 0; qq < GINT_SC; qq++) {
-#ifdef GINT_DBG_NO_MMA
-                if (false) {
-#else
-                {
-#endif
+                for (int qq = 0; qq < GINT_SC; qq++) {
                     const unsigned code = cur[qq];
                     if (code) {
                         const unsigned base = ring0 + s * GINT_STAGE_BYTES + qq * 2 * GINT_SLOT_MAX_BYTES;
-                        int sx = 0, sy = 0;
-                        if (VLOCAL) { const double2 sg = lds128(base + sgn_off); sx = __double2hiint(sg.x); sy = __double2hiint(sg.y); }
+                        const double2 sg = lds128(base + sgn_off);
+                        const int sx = __double2hiint(sg.x), sy = __double2hiint(sg.y);
 #pragma unroll
                         for (int k = 0; k < GINT_WARP_BLOCKS; k++) {
                             const unsigned rr = (code >> (2 * k)) & 3u;
                             if (rr) {
                                 DBG_ADD(6, (rr == 3u ? 4 : 2) * bk[k].n());
-                                if (VLOCAL) {
-                                    if (k == 0) vl_visit<4>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_v, sx, sy, rr & 1u, rr & 2u, q);
-                                    else vl_visit<3>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_v, sx, sy, rr & 1u, rr & 2u, q);
-                                } else {
-                                    if (k == 0) rho_visit<4>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_j, rr & 1u, rr & 2u, q, part[qq][0], part[qq][1]);
-                                    else rho_visit<3>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_j, rr & 1u, rr & 2u, q, part[qq][0], part[qq][1]);
-                                }
+                                if (k == 0) vl_visit<4>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_v, sx, sy, rr & 1u, rr & 2u, q);
+                                else vl_visit<3>(acc[k], bk[k].n(), base + bk[k].oa + lane_v, base + bk[k].ob + lane_v, sx, sy, rr & 1u, rr & 2u, q);
                             }
                         }
                     }
                 }
+            } else {
+                // a block is worked on the whole stage if one of its rows and one of its columns are active on one of the two cubelets
+                const unsigned code = cur[0] | cur[GINT_SC - 1];
+                const unsigned base = ring0 + s * GINT_STAGE_BYTES;
+                double y[2][2][2];
+                unsigned pend = 0;              // lane address of the Phi_I rows of the block whose Y is still to be used (0: none)
+#pragma unroll
+                for (int k = 0; k < GINT_WARP_BLOCKS; k++) {
+                    if ((code >> (2 * k)) & 3u) {
+                        DBG_ADD(6, (bk[k].has1() ? 8 : 4) * bk[k].n());
+                        if (pend) rho_stage_retire(y, pend, part);
+                        if (k == 0) rho_stage_issue<4>(acc[k], bk[k].n(), bk[k].has1(), base + bk[k].ob + lane_j, q, y);
+                        else rho_stage_issue<3>(acc[k], bk[k].n(), bk[k].has1(), base + bk[k].ob + lane_j, q, y);
+                        pend = base + bk[k].oa + lane_v;
+                    }
+                }
+                if (pend) rho_stage_retire(y, pend, part);
             }
+#endif
             if (!VLOCAL) {
                 // part[q][e]: point 2 lc + e of cubelet q, partial over the lane's orbital row lr -> sum over lr (lane bits 2..4)
                 const bool hi = lane & 16, mid = lane & 8;
@@ -1051,6 +1112,8 @@ k_tiles(Geom g, const unsigned char* __restrict__ plan, const unsigned* __restri
         for (int c = 0; c < GINT_NCTX; c++) { mbar_init(&S.ctx_full[c], 1); mbar_init(&S.ctx_free[c], GINT_MMA_WARPS + 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    // the ring starts zeroed: the consumers may read rows of a stage that no copy has written yet (multiplied by zeros: must be finite)
+    for (unsigned i = threadIdx.x; i < sizeof(S.ring) / 16; i += GINT_CTA_THREADS) reinterpret_cast<uint4*>(&S.ring[0][0])[i] = make_uint4(0u, 0u, 0u, 0u);
     __syncthreads();
     if (warp < GINT_MMA_WARPS) {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(GINT_REGS_MMA));
