@@ -39,7 +39,7 @@
 // shared-memory ring of the contraction kernels: a stage = GINT_SC cubelets x (slot of group I, slot of group J)
 #define GINT_SC 2
 #ifndef GINT_NS
-#define GINT_NS 6
+#define GINT_NS 7
 #endif
 #define GINT_STAGE_BYTES (GINT_SC * 2 * GINT_SLOT_MAX_BYTES)   // 26880
 #define GINT_NCTX 4                // tile plans in flight per CTA (the issuer requests them ahead of the consumers)

@@ -83,6 +83,15 @@ __device__ __forceinline__ void mbar_wait(u64* bar, int parity) {
     asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
                  :: "r"(smem_addr(bar)), "r"(parity) : "memory");
 }
+// the same on 32-bit shared-memory addresses (the hot loops keep them in registers: a generic pointer costs 64-bit arithmetic)
+__device__ __forceinline__ void mbar_arrive_s(unsigned bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_s(unsigned bar, unsigned parity) {
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
+                 :: "r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void sts64(unsigned addr, double v) { asm volatile("st.shared.f64 [%0], %1;" :: "r"(addr), "d"(v) : "memory"); }
 // TMA bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP.S.G)
 __device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, u64* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -111,7 +120,7 @@ struct EvalSmem {
 // gint_vlocal (V != nullptr) stores sqrt(|V dV|) phi: the contraction Phi_I^T diag(V dV) Phi_J then needs no FP64 multiply, only
 // the sign of V at the point, which the consumers apply to one operand with an integer XOR (an FP64 multiply queues behind the
 // other warps' DMMAs in the shared FP64 pipe).  Points outside the mesh (ragged edge batches) get weight 0.
-template <bool TAB_SMEM>
+template <bool TAB_SMEM, bool VL>
 __global__ void __launch_bounds__(GINT_EVAL_THREADS)
 k_eval_phi(Geom g, long long b0, const int* __restrict__ bstart, const NeighEntry* __restrict__ bent,
            const int* __restrict__ gstart, const u64* __restrict__ goff, u64 wave_row0,
@@ -209,7 +218,7 @@ k_eval_phi(Geom g, long long b0, const int* __restrict__ bstart, const NeighEntr
         if (tiny) ir = 0.0;
         // lanes outside the sphere run the same instructions on a clamped radius and store zeros
         double w0 = inside ? 1.0 : 0.0;
-        if (V) {
+        if (VL) {
             const int gi = i0 + ix, gj = j0 + iy, gk = k0 + iz;
             const bool in_mesh = ix < g.bs[0] && iy < g.bs[1] && iz < g.bs[2] && gi < g.N[0] && gj < g.N[1] && gk < g.N[2];    // a point of this batch
             w0 = (inside && in_mesh) ? sqrt(fabs(__ldg(V + ((size_t)gi * g.N[1] + gj) * g.N[2] + gk) * g.dV)) : 0.0;
@@ -224,9 +233,13 @@ k_eval_phi(Geom g, long long b0, const int* __restrict__ bstart, const NeighEntr
             yw[1] = c1 * uy; yw[2] = c1 * uz; yw[3] = c1 * ux;
             yw[4] = c2x * uy; yw[5] = c2y * uz; yw[6] = c20 * fma(3.0 * uz, uz, -1.0); yw[7] = c2x * uz; yw[8] = c22 * fma(ux, ux, -uy * uy);
         }
-        double* o0 = phi + ((S.gbase[k] + (u64)slot * (S.gR[k] + 1) + S.row0[e]) << 3) + pl;
+        // SWIZZLE (gint_rho): point p of slot row r sits at position p ^ (4 * ((r >> 1) & 1)) of the row's 64 bytes.  The B operands of gint_rho
+        // (64-bit loads, a half warp = 4 consecutive rows x 4 points) would otherwise hit every bank twice (rows r and r + 2).
+        double* o0 = phi + ((S.gbase[k] + (u64)slot * (S.gR[k] + 1) + S.row0[e]) << 3);
+        int orow = S.row0[e];
         const int lpack = S.lpack[e];
-#define GINT_PUT(m) do { *o0 = R * yw[m]; o0 += 8; } while (0)
+        const int swz = VL ? 0 : 2;     // gint_rho only (gint_vlocal reads its slots with conflict-free 128-bit loads as they are)
+#define GINT_PUT(m) do { o0[pl ^ ((orow & swz) << 1)] = R * yw[m]; o0 += 8; orow++; } while (0)
         for (int s = 0; s < nsh; s++) {
             const double2 c0 = row[s], c1 = row[nsh + s];
             const double R = fma(am, c0.x, fma(bb, c1.x, fma(a3, c0.y, b3 * c1.y)));
@@ -259,7 +272,7 @@ k_eval_phi(Geom g, long long b0, const int* __restrict__ bstart, const NeighEntr
         for (int rr = r0; rr < r1; rr++) o0[rr << 3] = 0.0;
     }
     // ---- pass C (gint_vlocal): the sign row of every slot: -0.0 where V < 0 at the point, else +0.0
-    if (V) {
+    if (VL) {
         const int n_s = S.sitem0[G];
         for (int it = qw; it < n_s; it += GINT_EVAL_THREADS / 8) {
             int k = 0;
@@ -595,7 +608,6 @@ static_assert(GINT_SC == 2, "the density reduction of the consumers is written f
 struct alignas(128) TileSmem {
     unsigned char ring[GINT_NS][GINT_STAGE_BYTES];     // stage: [cubelet q][side][row][8 points]
     alignas(16) unsigned char plan[GINT_NCTX][GINT_PLAN_MAX_BYTES];    // PlanHdr + PlanCub[]
-    alignas(16) double pw[GINT_NCTX][GINT_NCUB][GINT_CPTS];            // gint_rho: the tile's density at the listed cubelets' points (summed by the issuer warp)
     double part[GINT_NS][GINT_MMA_WARPS][GINT_SC * GINT_CPTS];         // gint_rho: per stage, the consumer warps' partial densities
     u64 full[GINT_NS], empty[GINT_NS];             // stage filled by TMA / read by all consumer warps
     u64 ctx_full[GINT_NCTX], ctx_free[GINT_NCTX];  // plan arrived / released by consumers and issuer
@@ -621,24 +633,19 @@ __device__ __forceinline__ void retire_stage(const Geom& g, TileSmem& S, int gr,
     if (VLOCAL) return;
     const int h = S.hist[s], c = h & 255, st = h >> 8;
     const PlanHdr& X = plan_hdr(S, c);
-    double* pw = &S.pw[c][0][0];
     const int ncs = min(GINT_SC, X.ncub - st * GINT_SC);
     if (lane < ncs * GINT_CPTS) {
-        double v = 0.0;
+        // four chains: the adds queue behind the consumers' DMMAs in the FP64 pipe of this warp's SM sub-partition
+        double v[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
-        for (int w = 0; w < GINT_MMA_WARPS; w++) v += S.part[s][w][lane];
-        pw[st * GINT_SC * GINT_CPTS + lane] = v;        // every listed cubelet belongs to exactly one stage
+        for (int w = 0; w < GINT_MMA_WARPS; w++) v[w & 3] += S.part[s][w][lane];
+        const double sum = (v[0] + v[1]) + (v[2] + v[3]);
+        // every listed cubelet belongs to exactly one stage of the tile: one add per mesh point per tile
+        int ix, iy, iz; cubelet_point(plan_cub(S, c)[st * GINT_SC + (lane >> 3)].cub, lane & 7, ix, iy, iz);
+        if (sum != 0.0 && ix < X.ex && iy < X.ey && iz < X.ez)
+            atomicAdd(rho + ((size_t)(X.i0 + ix) * g.N[1] + (X.j0 + iy)) * g.N[2] + (X.k0 + iz), sum);
     }
     if (st == X.nstage - 1) {
-        __syncwarp();
-        const PlanCub* C = plan_cub(S, c);
-        const int npt = X.ncub * GINT_CPTS;
-        for (int idx = lane; idx < npt; idx += 32) {
-            const double v = pw[idx];
-            int ix, iy, iz; cubelet_point(C[idx >> 3].cub, idx & 7, ix, iy, iz);
-            if (v != 0.0 && ix < X.ex && iy < X.ey && iz < X.ez)
-                atomicAdd(rho + ((size_t)(X.i0 + ix) * g.N[1] + (X.j0 + iy)) * g.N[2] + (X.k0 + iz), v);
-        }
         __syncwarp();
         if (lane == 0) mbar_arrive(&S.ctx_free[c]);
     }
@@ -971,9 +978,14 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, lr = lane >> 2, lc = lane & 3;
     const unsigned ring0 = smem_addr(&S.ring[0][0]);
     // lane parts of the operand addresses
-    const unsigned lane_v = lr * GINT_ROW_BYTES + lc * 16;                 // row lr of a fragment, points 2 lc, 2 lc + 1
-    const unsigned lane_j = lc * GINT_ROW_BYTES + lr * 8;                  // gint_rho B operand: row lc of the k-step, point lr
-    int gs = 0;                                                            // ring stages consumed
+    // (gint_rho: with the swizzle of the slot rows, see k_eval_phi; fragments start at multiples of 8 rows)
+    const unsigned lane_v = lr * GINT_ROW_BYTES + ((VLOCAL ? lc : (lc ^ (lr & 2))) * 16);  // row lr of a fragment, points 2 lc, 2 lc + 1
+    const unsigned lane_j = lc * GINT_ROW_BYTES + ((lr ^ ((lc & 2) << 1)) * 8);            // gint_rho B operand: row lc of the k-step, point lr
+    // ring position of the next stage: slot, parity of its full barrier, and the slot's addresses (all 32-bit shared addresses)
+    unsigned rs = 0, rph = 0;
+    const unsigned full0 = smem_addr(&S.full[0]), empty0 = smem_addr(&S.empty[0]);
+    // gint_rho: where the lane's reduced partial density of a stage goes (see the butterfly below)
+    const unsigned part0 = smem_addr(&S.part[0][warp][((lane >> 4) & 1) * GINT_CPTS + 2 * lc + ((lane >> 3) & 1)]);
 #ifdef GINT_DBG_STATS
     unsigned long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 #endif
@@ -1007,15 +1019,20 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
         for (int qq = 0; qq < GINT_SC; qq++) cur[qq] = lds_u8(vis0 + qq * (unsigned)sizeof(PlanCub));
         DBG_T(t_tile1);
         DBG_ADD(0, t_tile1 - t_tile0);
-        for (int st = 0; st < nstage; st++, gs++) {
-            const int s = gs % GINT_NS;
+        unsigned visp = vis0 + GINT_SC * (unsigned)sizeof(PlanCub);           // visit codes of the next stage
+        for (int st = 0; st < nstage; st++) {
+            const unsigned s = rs;
             DBG_T(t_w0);
-            mbar_wait(&S.full[s], (gs / GINT_NS) & 1);
+            mbar_wait_s(full0 + 8 * s, rph);
             DBG_T(t_w1);
             DBG_ADD(1, t_w1 - t_w0);
             double part[GINT_SC][2];
 #pragma unroll
-            for (int qq = 0; qq < GINT_SC; qq++) { part[qq][0] = 0.0; part[qq][1] = 0.0; nxt[qq] = lds_u8(vis0 + ((st + 1) * GINT_SC + qq) * (unsigned)sizeof(PlanCub)); }
+            for (int qq = 0; qq < GINT_SC; qq++) { part[qq][0] = 0.0; part[qq][1] = 0.0; nxt[qq] = lds_u8(visp + qq * (unsigned)sizeof(PlanCub)); }
+            visp += GINT_SC * (unsigned)sizeof(PlanCub);
+#ifdef GINT_DBG_WARPS
+            if (warp < GINT_DBG_WARPS)        // developer switch: only the first warps work (serial time of a warp without competition for the pipe)
+#endif
 #ifndef GINT_DBG_NO_MMA
             if (VLOCAL) {
 #pragma unroll
@@ -1068,10 +1085,11 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
                 double r1 = keep + __shfl_xor_sync(0xffffffffu, send, 8);
                 r1 += __shfl_xor_sync(0xffffffffu, r1, 4);
                 // the lane holds cubelet (lane >> 4) & 1, point 2 lc + ((lane >> 3) & 1)
-                if (!(lane & 4)) S.part[s][warp][((lane >> 4) & 1) * GINT_CPTS + 2 * lc + ((lane >> 3) & 1)] = r1;
+                if (!(lane & 4)) sts64(part0 + s * (unsigned)sizeof(S.part[0]), r1);
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(&S.empty[s]);
+            if (lane == 0) mbar_arrive_s(empty0 + 8 * s);
+            if (++rs == GINT_NS) { rs = 0; rph ^= 1u; }
 #pragma unroll
             for (int qq = 0; qq < GINT_SC; qq++) cur[qq] = nxt[qq];
             DBG_T(t_w2);
@@ -1312,8 +1330,10 @@ int gint_configure_kernels(gint_ctx* c) {
     const int lim = (int)prop.sharedMemPerBlockOptin;
     GINT_CUDA(cudaFuncSetAttribute(k_tiles<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim));
     GINT_CUDA(cudaFuncSetAttribute(k_tiles<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim));
-    GINT_CUDA(cudaFuncSetAttribute(k_eval_phi<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim));
-    GINT_CUDA(cudaFuncSetAttribute(k_eval_phi<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim));
+    GINT_CUDA(cudaFuncSetAttribute(k_eval_phi<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim));
+    GINT_CUDA(cudaFuncSetAttribute(k_eval_phi<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim));
+    GINT_CUDA(cudaFuncSetAttribute(k_eval_phi<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim));
+    GINT_CUDA(cudaFuncSetAttribute(k_eval_phi<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim));
     c->n_sm = prop.multiProcessorCount;
     return GINT_OK;
 }
@@ -1328,10 +1348,10 @@ static int launch_waves(gint_ctx* c, const double* in, double* out, cudaStream_t
         const gint_ctx::Wave& W = c->waves[w];
         const unsigned nb = (unsigned)(W.b1 - W.b0);
         if (c->tab_in_smem)
-            k_eval_phi<true><<<nb, GINT_EVAL_THREADS, c->smem_eval, st>>>(c->geom, W.b0, c->d_bstart, c->d_bent, c->d_gstart, c->d_goff, W.row0,
+            k_eval_phi<true, VLOCAL><<<nb, GINT_EVAL_THREADS, c->smem_eval, st>>>(c->geom, W.b0, c->d_bstart, c->d_bent, c->d_gstart, c->d_goff, W.row0,
                 c->d_atom_pos, c->d_atom_species, c->d_species, c->d_tab, tab_cells, VLOCAL ? in : nullptr, c->d_phi);
         else
-            k_eval_phi<false><<<nb, GINT_EVAL_THREADS, c->smem_eval, st>>>(c->geom, W.b0, c->d_bstart, c->d_bent, c->d_gstart, c->d_goff, W.row0,
+            k_eval_phi<false, VLOCAL><<<nb, GINT_EVAL_THREADS, c->smem_eval, st>>>(c->geom, W.b0, c->d_bstart, c->d_bent, c->d_gstart, c->d_goff, W.row0,
                 c->d_atom_pos, c->d_atom_species, c->d_species, c->d_tab, tab_cells, VLOCAL ? in : nullptr, c->d_phi);
         GINT_CUDA(cudaGetLastError());
         GINT_CUDA(cudaEventRecord(c->ev_wave[VLOCAL ? 0 : 1][2 * w], st));
