@@ -37,18 +37,50 @@ def alg_flops(st: dict) -> float:
     return float(st["alg_sum_n2"] + st["alg_sum_n"]) + float(st["alg_sum_n"]) + EVAL_FLOP_PER_INCIDENCE * st["alg_incidence"]
 
 
-def ncu_traffic(cfg: int, kernel: str):
-    """DRAM bytes (read + write) of one launch of `kernel` from the committed ncu capture (profiles/r1h_traffic.csv), or None."""
-    path = os.path.join(ROOT, "profiles", "r1h_traffic.csv")
+TRAFFIC_CSV = os.path.join("profiles", "r2_traffic.csv")
+
+
+def csrc_digest() -> str:
+    """sha256 over the kernel sources: the committed ncu capture names the digest it was taken on."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2409_09399_b200", "csrc")
+    for name in sorted(os.listdir(d)):
+        with open(os.path.join(d, name), "rb") as f:
+            h.update(name.encode()); h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(cfg: int, call: str):
+    """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum, summed over the kernels of one `call` = "vlocal_main" or
+    "rho_main", all waves) from the committed ncu capture profiles/r2_traffic.csv, with a note.  The capture names the digest of
+    the kernel sources it was taken on: when csrc/ has changed since, the figure is STALE and is not reported."""
+    path = os.path.join(ROOT, TRAFFIC_CSV)
     try:
         with open(path) as f:
-            for ln in f.read().splitlines()[1:]:
-                c, k, rd, wr = ln.split(",")[:4]
-                if int(c) == cfg and k == kernel:
-                    return int(rd) + int(wr)
+            lines = [ln for ln in f.read().splitlines() if ln and not ln.startswith("#")]
+        for ln in lines[1:]:
+            c, k, rd, wr, digest = [x.strip() for x in ln.split(",")[:5]]
+            if int(c) == cfg and k == call:
+                if digest != csrc_digest():
+                    print(f"bench.py: {TRAFFIC_CSV} was captured on csrc digest {digest}, the tree is at {csrc_digest()}: "
+                          "roofline.traffic not reported (re-capture with ncu)", file=sys.stderr)
+                    return None, f"stale capture (csrc digest {digest} != {csrc_digest()})"
+                return int(rd) + int(wr), f"{TRAFFIC_CSV}, csrc digest {digest}"
     except (OSError, ValueError):
         pass
-    return None
+    return None, "no capture for this config"
+
+
+def cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as f:
+            for ln in f:
+                if ln.startswith("model name"):
+                    return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 def max_over_ranks(values, device, world: int):
@@ -138,7 +170,7 @@ def oracle_sample(w, V, D, plist, budget_s: float = 20.0):
     t0 = time.perf_counter(); O.vlocal(w, V, plist, sel=np.arange(p0, p0 + np_s, dtype=np.int64)); t_v = time.perf_counter() - t0
     t0 = time.perf_counter(); O.rho(w, D, plist, sel=(np.arange(g0, g0 + ng_s, dtype=np.int64) % npts)); t_r = time.perf_counter() - t0
     t_step = t_v * npairs / np_s + t_r * npts / ng_s          # extrapolated full-mesh step
-    info = {"kind": "oracle", "cores": O.threads(),
+    info = {"kind": "oracle", "cores": O.threads(), "cpu": cpu_model(),
             "sample": f"vlocal: {np_s} of {npairs} pair keys in {t_v:.2f} s; rho: {ng_s} of {npts} mesh points in {t_r:.2f} s; "
                       f"scaled to the full mesh (vlocal {t_v * npairs / np_s:.1f} s + rho {t_r * npts / ng_s:.1f} s per step)"}
     return npts / t_step, info
@@ -160,7 +192,7 @@ def run_reference(args):
         v, info = oracle_sample(w, V, D, plist, budget_s=budget)
         if s >= args.warmup:
             vals.append(v)
-    value = float(np.mean(vals))
+    value = float(np.median(vals))
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": "mesh points/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * w.n_points / value,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -183,7 +215,11 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--batch", default="", help="override grid-batch shape, e.g. 8,8,8")
+    ap.add_argument("--csrc-digest", action="store_true", help="print the digest of the kernel sources (for profiles/r2_traffic.csv) and exit")
     args = ap.parse_args()
+    if args.csrc_digest:
+        print(csrc_digest())
+        return 0
     if args.impl == "reference":
         return run_reference(args)
 
@@ -198,7 +234,10 @@ def main():
     dev = torch.device("cuda", local)
 
     from paper_2409_09399_b200 import workloads as W
-    from paper_2409_09399_b200.gint import Gint, batch_flag
+    from paper_2409_09399_b200.gint import Gint, batch_flag, fp64_peak
+
+    # same-run FP64 peak: DMMA / DFMA micro-benchmark of the library, in this process, before the timed region
+    peak_measured = fp64_peak(local)
 
     t0 = time.perf_counter()
     w = W.make_workload(args.cfg)
@@ -250,7 +289,7 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     t_v = np.array([ev[s][0].elapsed_time(ev[s][1]) for s in range(args.steps)]) * 1e-3
     t_r = np.array([ev[s][1].elapsed_time(ev[s][2]) for s in range(args.steps)]) * 1e-3
-    t_step = float((t_v + t_r).mean())
+    t_step = float(np.median(t_v + t_r))          # median over the steps
     # identity P4: sum_g V rho dV == <D, H> -- a full-size consistency check of the two kernels
     dV = abs(np.linalg.det(w.cell)) / npts
     lhs = float((V_d * rho_d).sum().item() * dV); rhs = float((D_d * H_d).sum().item())
@@ -286,6 +325,7 @@ def main():
             cpu = {"value": val, "unit": "mesh points/s", **info}
         dom = "vlocal_main" if kt["vlocal_main"] >= kt["rho_main"] else "rho_main"
         achieved = F_alg / kt[dom] / 1e12
+        traffic, traffic_note = ncu_traffic(args.cfg, dom)
         # context: the same kernel against the HBM roofline (measured copy bandwidth of this pool's B200s, MEASURED_PEAKS.json;
         # 6650 GB/s is the profiling guide's fallback).  Algorithmic bytes: V + canonical H (vlocal) / canonical D + rho (rho).
         try:
@@ -304,15 +344,20 @@ def main():
                        "batch": [st["batch_bx"], st["batch_by"], st["batch_bz"]],
                        "l2": "inputs larger than L2" if flush is None else "L2 flushed between steps",
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
-            "vlocal_points_per_s": npts / float(t_v.mean()), "rho_points_per_s": npts / float(t_r.mean()),
-            "ms_vlocal": 1e3 * float(t_v.mean()), "ms_rho": 1e3 * float(t_r.mean()), "init_s": t_init,
-            "alg_flop_per_call": F_alg, "alg_tflops_vlocal": F_alg / float(t_v.mean()) / 1e12,
-            "alg_tflops_rho": F_alg / float(t_r.mean()) / 1e12,
+            "vlocal_points_per_s": npts / float(np.median(t_v)), "rho_points_per_s": npts / float(np.median(t_r)),
+            "ms_vlocal": 1e3 * float(np.median(t_v)), "ms_rho": 1e3 * float(np.median(t_r)), "init_s": t_init,
+            "alg_flop_per_call": F_alg, "alg_tflops_vlocal": F_alg / float(np.median(t_v)) / 1e12,
+            "alg_tflops_rho": F_alg / float(np.median(t_r)) / 1e12,
+            "roofline_frac_vlocal": F_alg / kt["vlocal_main"] / 1e12 / FP64_PEAK_TFLOPS,
+            "roofline_frac_rho": F_alg / kt["rho_main"] / 1e12 / FP64_PEAK_TFLOPS,
             "identity_P4_rel": p4,
             "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                         "frac": achieved / FP64_PEAK_TFLOPS, "traffic": ncu_traffic(args.cfg, dom),
-                         "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1h_final_kernels.md)",
-                         "peak_source": "148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md; DMMA micro-benchmark reaches 37.1)",
+                         "frac": achieved / FP64_PEAK_TFLOPS, "traffic": traffic,
+                         "traffic_unit": "bytes per call: dram__bytes_read.sum + dram__bytes_write.sum over the call's kernels (k_eval_phi + k_tiles, all waves)",
+                         "traffic_source": traffic_note,
+                         "kernels": "k_eval_phi + k_tiles<%s> over all waves of one call (CUDA events inside the library)" % ("vlocal" if dom == "vlocal_main" else "rho"),
+                         "peak_source": "stated: 148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESIGN.md 6); peak_measured = gint_fp64_peak in this process",
+                         "peak_measured": peak_measured,
                          "kernel_ms": {k: 1e3 * v for k, v in kt.items()},
                          "hbm_context": {"achieved": hbm_achieved, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_achieved / hbm_peak,
                                          "peak_source": hbm_src, "algorithmic_bytes": alg_bytes}},

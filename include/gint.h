@@ -149,6 +149,15 @@ int gint_kernel_times(gint_ctx* ctx, double out[2]);
  * last gint_vlocal call, out[2] / out[3] = of the last gint_rho call; -1 when that call has not been made yet. */
 int gint_phase_times(gint_ctx* ctx, double out[4]);
 
+/* FP64 peak of the device, measured now (the roofline denominator's cross-check): a register-only micro-benchmark
+ * on all SMs, 16 warps per SM, timed with CUDA events on the default stream of `device`.
+ *   out[0]  DMMA.8x8x4 (mma.sync.m8n8k4.f64, the instruction of the contraction kernels), TFLOP/s (2 flop per multiply-add)
+ *   out[1]  DFMA (fma.rn.f64), TFLOP/s
+ *   out[2]  SM clock during the DMMA run, MHz (clock64 ticks / elapsed time)
+ *   out[3]  number of SMs
+ * Synchronises the device.  GINT_ERR_CUDA without a usable device. */
+int gint_fp64_peak(int device, double out[4]);
+
 int gint_free(gint_ctx* ctx);
 
 const char* gint_last_error(void);

@@ -316,6 +316,8 @@ static void free_ctx(gint_ctx* c) {
     cudaFree(c->d_stage_in); cudaFree(c->d_stage_out);
     for (auto& e : c->ev) if (e) cudaEventDestroy(e);
     for (auto& v : c->ev_wave) for (auto& e : v) if (e) cudaEventDestroy(e);
+    for (auto& e : c->ev_copy) if (e) cudaEventDestroy(e);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     delete c;
 }
 
@@ -585,11 +587,9 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, size_t
 }
 
 // ---------------------------------------------------------------------------------------------------
-extern "C" int gint_init(gint_ctx** out, int n_species, const int* n_shell, const int* shell_l, const double* rcut, double dr,
-                         const int* n_knot, const double* tab_y, const double* tab_y2, int n_atoms, const int* atom_species,
-                         const double* atom_pos, const double cell[9], const int mesh[3], int device, unsigned long long flags) {
-    if (!out) GINT_FAIL(GINT_ERR_INVALID_ARG, "out is NULL");
-    *out = nullptr;
+static int gint_init_impl(gint_ctx** out, gint_ctx*& c, int n_species, const int* n_shell, const int* shell_l, const double* rcut, double dr,
+                          const int* n_knot, const double* tab_y, const double* tab_y2, int n_atoms, const int* atom_species,
+                          const double* atom_pos, const double cell[9], const int mesh[3], int device, unsigned long long flags) {
     if (!n_shell || !shell_l || !rcut || !n_knot || !tab_y || !tab_y2 || !cell || !mesh) GINT_FAIL(GINT_ERR_INVALID_ARG, "NULL array argument");
     if (n_species < 1) GINT_FAIL(GINT_ERR_INVALID_ARG, "n_species = %d", n_species);
     if (n_atoms < 0 || (n_atoms > 0 && (!atom_species || !atom_pos))) GINT_FAIL(GINT_ERR_INVALID_ARG, "bad atom arrays");
@@ -611,7 +611,7 @@ extern "C" int gint_init(gint_ctx** out, int n_species, const int* n_shell, cons
     GINT_CUDA(cudaGetDeviceProperties(&prop, device));
     if (prop.major < 10) GINT_FAIL(GINT_ERR_UNSUPPORTED, "device %s is sm_%d%d; libgint is built for sm_100a only", prop.name, prop.major, prop.minor);
 
-    gint_ctx* c = new (std::nothrow) gint_ctx();
+    c = new (std::nothrow) gint_ctx();
     if (!c) GINT_FAIL(GINT_ERR_OUT_OF_MEMORY, "host allocation failed");
     c->device = device;
     Geom& g = c->geom;
@@ -627,11 +627,11 @@ extern "C" int gint_init(gint_ctx** out, int n_species, const int* n_shell, cons
     c->h_atom_pos.assign(atom_pos, atom_pos + 3 * (size_t)n_atoms);
 
     int rc = build_basis(c, n_species, n_shell, shell_l, rcut, dr, n_knot, tab_y, tab_y2);
-    if (rc) { free_ctx(c); return rc; }
+    if (rc) { return rc; }
     c->n_orb_total = 0;
     for (int a = 0; a < n_atoms; a++) c->n_orb_total += c->h_species[atom_species[a]].norb;
-    if ((rc = dev_upload(c, &c->d_atom_pos, c->h_atom_pos)) || (rc = dev_upload(c, &c->d_atom_species, c->h_atom_species))) { free_ctx(c); return rc; }
-    if ((rc = build_pairs(c))) { free_ctx(c); return rc; }
+    if ((rc = dev_upload(c, &c->d_atom_pos, c->h_atom_pos)) || (rc = dev_upload(c, &c->d_atom_species, c->h_atom_species))) { return rc; }
+    if ((rc = build_pairs(c))) { return rc; }
 
     const size_t smem_limit = prop.sharedMemPerBlockOptin;
     // scratch for the orbital values of one wave of batches: at most 16 GiB and a quarter of the free device memory
@@ -643,26 +643,53 @@ extern "C" int gint_init(gint_ctx** out, int n_species, const int* n_shell, cons
     bool fits = false;
     if (fx || fy || fz) {
         const int bs[3] = {fx ? fx : 8, fy ? fy : 8, fz ? fz : 8};
-        if ((rc = build_batches(c, bs, smem_limit, phi_cap, &fits))) { free_ctx(c); return rc; }
-        if (!fits) { free_ctx(c); GINT_FAIL(GINT_ERR_UNSUPPORTED, "requested batch %dx%dx%d needs more shared memory than %zu bytes (or > %d neighbours)", bs[0], bs[1], bs[2], smem_limit, GINT_MAX_NB); }
+        if ((rc = build_batches(c, bs, smem_limit, phi_cap, &fits))) { return rc; }
+        if (!fits) { GINT_FAIL(GINT_ERR_UNSUPPORTED, "requested batch %dx%dx%d needs more shared memory than %zu bytes (or > %d neighbours)", bs[0], bs[1], bs[2], smem_limit, GINT_MAX_NB); }
     } else {
         static const int shapes[][3] = {{8, 8, GINT_MAX_BSZ}, {8, 8, 8}, {4, 4, 8}, {4, 4, 4}, {2, 2, 4}, {1, 1, 4}, {1, 1, 1}};
         for (auto& s : shapes) {
-            if ((rc = build_batches(c, s, smem_limit, phi_cap, &fits))) { free_ctx(c); return rc; }
+            if ((rc = build_batches(c, s, smem_limit, phi_cap, &fits))) { return rc; }
             if (fits) break;
         }
-        if (!fits) { free_ctx(c); GINT_FAIL(GINT_ERR_UNSUPPORTED, "even a 1-point batch does not fit: too many overlapping atoms"); }
+        if (!fits) { GINT_FAIL(GINT_ERR_UNSUPPORTED, "even a 1-point batch does not fit: too many overlapping atoms"); }
     }
     c->smem_bytes = gint_smem_needed(c, smem_limit);
-    if ((rc = gint_configure_kernels(c))) { free_ctx(c); return rc; }
-    for (auto& e : c->ev) if (cudaEventCreate(&e) != cudaSuccess) { free_ctx(c); GINT_FAIL(GINT_ERR_CUDA, "cudaEventCreate failed"); }
-    if (cudaDeviceSynchronize() != cudaSuccess) { free_ctx(c); GINT_FAIL(GINT_ERR_CUDA, "gint_init: device error %s", cudaGetErrorString(cudaGetLastError())); }
+    if ((rc = gint_configure_kernels(c))) { return rc; }
+    for (auto& e : c->ev) if (cudaEventCreate(&e) != cudaSuccess) { GINT_FAIL(GINT_ERR_CUDA, "cudaEventCreate failed"); }
+    if (cudaDeviceSynchronize() != cudaSuccess) { GINT_FAIL(GINT_ERR_CUDA, "gint_init: device error %s", cudaGetErrorString(cudaGetLastError())); }
     *out = c;
     return GINT_OK;
 }
 
+// The C boundary: nothing is thrown across it (std::vector of up to 2e9 keys can run out of host memory), every failure frees what
+// was built so far, and the caller's current device is restored.
+extern "C" int gint_init(gint_ctx** out, int n_species, const int* n_shell, const int* shell_l, const double* rcut, double dr,
+                         const int* n_knot, const double* tab_y, const double* tab_y2, int n_atoms, const int* atom_species,
+                         const double* atom_pos, const double cell[9], const int mesh[3], int device, unsigned long long flags) {
+    if (!out) GINT_FAIL(GINT_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    DeviceGuard guard;
+    gint_ctx* c = nullptr;
+    int rc;
+    try {
+        rc = gint_init_impl(out, c, n_species, n_shell, shell_l, rcut, dr, n_knot, tab_y, tab_y2, n_atoms, atom_species, atom_pos, cell, mesh, device, flags);
+    } catch (const std::bad_alloc&) {
+        gint_set_error("gint_init: out of host memory");
+        rc = GINT_ERR_OUT_OF_MEMORY;
+    } catch (...) {
+        gint_set_error("gint_init: unexpected exception");
+        rc = GINT_ERR_BAD_STATE;
+    }
+    if (rc != GINT_OK) {
+        if (c) { cudaDeviceSynchronize(); free_ctx(c); }
+        *out = nullptr;
+    }
+    return rc;
+}
+
 extern "C" int gint_free(gint_ctx* ctx) {
     if (!ctx) GINT_FAIL(GINT_ERR_BAD_STATE, "NULL context");
+    DeviceGuard guard;
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
     free_ctx(ctx);
@@ -756,14 +783,15 @@ static int ensure_stage(gint_ctx* c, double** p, size_t* have, size_t want) {
 extern "C" int gint_vlocal_host(gint_ctx* c, const double* V_host, double* H_host, void* stream) {
     if (!c) GINT_FAIL(GINT_ERR_BAD_STATE, "NULL context");
     if (!V_host || !H_host) GINT_FAIL(GINT_ERR_INVALID_ARG, "NULL buffer");
+    DeviceGuard guard;
     cudaStream_t st = (cudaStream_t)stream;
     GINT_CUDA(cudaSetDevice(c->device));
     const size_t npts = (size_t)c->geom.N[0] * c->geom.N[1] * c->geom.N[2];
     int rc;
     if ((rc = ensure_stage(c, &c->d_stage_in, &c->stage_in_n, std::max(npts, (size_t)c->n_values)))) return rc;
     if ((rc = ensure_stage(c, &c->d_stage_out, &c->stage_out_n, std::max(npts, (size_t)c->n_values)))) return rc;
-    GINT_CUDA(cudaMemcpyAsync(c->d_stage_in, V_host, sizeof(double) * npts, cudaMemcpyHostToDevice, st));
-    if ((rc = gint_launch_vlocal(c, c->d_stage_in, c->d_stage_out, st))) return rc;
+    // V goes up in chunks on the copy stream, ahead of the waves that read it
+    if ((rc = gint_launch_vlocal(c, c->d_stage_in, c->d_stage_out, st, V_host))) return rc;
     GINT_CUDA(cudaMemcpyAsync(H_host, c->d_stage_out, sizeof(double) * (size_t)c->n_values, cudaMemcpyDeviceToHost, st));
     GINT_CUDA(cudaStreamSynchronize(st));
     return GINT_OK;
@@ -771,6 +799,7 @@ extern "C" int gint_vlocal_host(gint_ctx* c, const double* V_host, double* H_hos
 extern "C" int gint_rho_host(gint_ctx* c, const double* D_host, double* rho_host, void* stream) {
     if (!c) GINT_FAIL(GINT_ERR_BAD_STATE, "NULL context");
     if (!D_host || !rho_host) GINT_FAIL(GINT_ERR_INVALID_ARG, "NULL buffer");
+    DeviceGuard guard;
     cudaStream_t st = (cudaStream_t)stream;
     GINT_CUDA(cudaSetDevice(c->device));
     const size_t npts = (size_t)c->geom.N[0] * c->geom.N[1] * c->geom.N[2];
@@ -778,8 +807,8 @@ extern "C" int gint_rho_host(gint_ctx* c, const double* D_host, double* rho_host
     if ((rc = ensure_stage(c, &c->d_stage_in, &c->stage_in_n, std::max(npts, (size_t)c->n_values)))) return rc;
     if ((rc = ensure_stage(c, &c->d_stage_out, &c->stage_out_n, std::max(npts, (size_t)c->n_values)))) return rc;
     GINT_CUDA(cudaMemcpyAsync(c->d_stage_in, D_host, sizeof(double) * (size_t)c->n_values, cudaMemcpyHostToDevice, st));
-    if ((rc = gint_launch_rho(c, c->d_stage_in, c->d_stage_out, st))) return rc;
-    GINT_CUDA(cudaMemcpyAsync(rho_host, c->d_stage_out, sizeof(double) * npts, cudaMemcpyDeviceToHost, st));
+    // rho comes down in chunks on the copy stream, each behind the wave that completes it
+    if ((rc = gint_launch_rho(c, c->d_stage_in, c->d_stage_out, st, rho_host))) return rc;
     GINT_CUDA(cudaStreamSynchronize(st));
     return GINT_OK;
 }
@@ -787,11 +816,13 @@ extern "C" int gint_vlocal(gint_ctx* c, const double* V_dev, double* H_dev, void
     if (!c) GINT_FAIL(GINT_ERR_BAD_STATE, "NULL context");
     if (!V_dev || (!H_dev && c->n_values)) GINT_FAIL(GINT_ERR_INVALID_ARG, "NULL device pointer");
     if (((uintptr_t)V_dev | (uintptr_t)H_dev) & 7) GINT_FAIL(GINT_ERR_INVALID_ARG, "device pointers must be 8-byte aligned");
+    DeviceGuard guard;
     return gint_launch_vlocal(c, V_dev, H_dev, (cudaStream_t)stream);
 }
 extern "C" int gint_rho(gint_ctx* c, const double* D_dev, double* rho_dev, void* stream) {
     if (!c) GINT_FAIL(GINT_ERR_BAD_STATE, "NULL context");
     if ((!D_dev && c->n_values) || !rho_dev) GINT_FAIL(GINT_ERR_INVALID_ARG, "NULL device pointer");
     if (((uintptr_t)D_dev | (uintptr_t)rho_dev) & 7) GINT_FAIL(GINT_ERR_INVALID_ARG, "device pointers must be 8-byte aligned");
+    DeviceGuard guard;
     return gint_launch_rho(c, D_dev, rho_dev, (cudaStream_t)stream);
 }

@@ -53,6 +53,13 @@ void gint_set_error(const char* fmt, ...);
     gint_set_error("%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
     return e_ == cudaErrorMemoryAllocation ? GINT_ERR_OUT_OF_MEMORY : GINT_ERR_CUDA; } } while (0)
 
+// The entry points run on the context's device and give the caller's current device back on return.
+struct DeviceGuard {
+    int prev = -1;
+    DeviceGuard() { if (cudaGetDevice(&prev) != cudaSuccess) prev = -1; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 // ---- device-side descriptions ---------------------------------------------------------------------
 struct SpeciesDev {
     double rc;                      // cutoff radius
@@ -208,14 +215,18 @@ struct gint_ctx {
     bool timed[2] = {false, false};
     // per-wave events (gint_phase_times): [call][2 * wave] after the evaluation kernel, [call][2 * wave + 1] after the tile kernel
     std::vector<cudaEvent_t> ev_wave[2];
-    // host-path staging
+    // host-path staging; the copies run on a stream of their own, chunk by chunk beside the waves
     double* d_stage_in = nullptr; size_t stage_in_n = 0;
     double* d_stage_out = nullptr; size_t stage_out_n = 0;
+    cudaStream_t copy_stream = nullptr;
+    std::vector<cudaEvent_t> ev_copy;  // [waves + 1]
 };
 
 // implemented in gint_kernels.cu
-int gint_launch_vlocal(gint_ctx* c, const double* V, double* H, cudaStream_t st);
-int gint_launch_rho(gint_ctx* c, const double* D, double* rho, cudaStream_t st);
+// V_host / rho_host (optional): the host buffer behind V (gint_vlocal) or in front of rho (gint_rho); the copies then run in chunks,
+// one per wave, on the context's copy stream beside the kernels
+int gint_launch_vlocal(gint_ctx* c, const double* V, double* H, cudaStream_t st, const double* V_host = nullptr);
+int gint_launch_rho(gint_ctx* c, const double* D, double* rho, cudaStream_t st, double* rho_host = nullptr);
 int gint_launch_alg_stats(gint_ctx* c);
 int gint_configure_kernels(gint_ctx* c);
 size_t gint_smem_needed(gint_ctx* c, size_t limit);   // also decides tab_in_smem

@@ -1252,6 +1252,10 @@ int gint_build_phi_layout(gint_ctx* c, const int* d_bgroups, size_t phi_cap_byte
     GINT_CUDA(cudaMalloc((void**)&c->d_phi, c->phi_bytes));
     c->device_bytes += c->phi_bytes;
     GINT_CUDA(cudaMalloc((void**)&c->d_queue, sizeof(int) * (c->waves.size() + 1)));
+    if (!c->copy_stream) GINT_CUDA(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    for (auto& e : c->ev_copy) if (e) cudaEventDestroy(e);
+    c->ev_copy.assign(c->waves.size() + 1, nullptr);
+    for (auto& e : c->ev_copy) GINT_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     for (int k = 0; k < 2; k++) {
         c->ev_wave[k].assign(2 * c->waves.size(), nullptr);
         for (auto& e : c->ev_wave[k]) GINT_CUDA(cudaEventCreate(&e));
@@ -1338,15 +1342,47 @@ int gint_configure_kernels(gint_ctx* c) {
     return GINT_OK;
 }
 
-// one wave: evaluate the orbital values of its batches, then contract its tiles
+// Mesh planes (index along a1) below which every point belongs to a batch before batch b (batches are numbered a1-major).
+static long long planes_before(const gint_ctx* c, long long b) {
+    const Geom& g = c->geom;
+    const long long per_plane = (long long)g.nb[1] * g.nb[2];
+    return std::min<long long>((b / per_plane) * g.bs[0], g.N[0]);
+}
+// ... and the planes that hold the points of all batches before b (the plane of batch b - 1 included)
+static long long planes_through(const gint_ctx* c, long long b) {
+    const Geom& g = c->geom;
+    const long long per_plane = (long long)g.nb[1] * g.nb[2];
+    return b <= 0 ? 0 : std::min<long long>(((b - 1) / per_plane + 1) * g.bs[0], g.N[0]);
+}
+
+// one wave: evaluate the orbital values of its batches, then contract its tiles.
+// Host path (h_in / h_out != nullptr): gint_vlocal copies the planes of V a wave needs on the copy stream, all waves ahead of the
+// kernels; gint_rho copies the planes of rho a wave has completed back while the next wave runs.
 template <bool VLOCAL>
-static int launch_waves(gint_ctx* c, const double* in, double* out, cudaStream_t st) {
+static int launch_waves(gint_ctx* c, const double* in, double* out, cudaStream_t st, const double* h_in, double* h_out) {
     if (c->waves.empty()) return GINT_OK;
     GINT_CUDA(cudaMemsetAsync(c->d_queue, 0, sizeof(int) * c->waves.size(), st));
     const int tab_cells = (int)(c->tab_bytes / 16);
-    for (size_t w = 0; w < c->waves.size(); w++) {
+    const size_t plane = (size_t)c->geom.N[1] * c->geom.N[2];
+    const size_t nw = c->waves.size();
+    cudaStream_t cs = c->copy_stream;
+    if (VLOCAL && h_in) {
+        // the copy stream starts where the caller's stream stands, then runs ahead
+        GINT_CUDA(cudaEventRecord(c->ev_copy[nw], st));
+        GINT_CUDA(cudaStreamWaitEvent(cs, c->ev_copy[nw], 0));
+        long long done = 0;
+        for (size_t w = 0; w < nw; w++) {
+            const long long upto = w + 1 == nw ? c->geom.N[0] : planes_through(c, c->waves[w].b1);
+            if (upto > done) GINT_CUDA(cudaMemcpyAsync(const_cast<double*>(in) + done * plane, h_in + done * plane, sizeof(double) * (upto - done) * plane, cudaMemcpyHostToDevice, cs));
+            done = std::max(done, upto);
+            GINT_CUDA(cudaEventRecord(c->ev_copy[w], cs));
+        }
+    }
+    long long copied = 0;
+    for (size_t w = 0; w < nw; w++) {
         const gint_ctx::Wave& W = c->waves[w];
         const unsigned nb = (unsigned)(W.b1 - W.b0);
+        if (VLOCAL && h_in) GINT_CUDA(cudaStreamWaitEvent(st, c->ev_copy[w], 0));
         if (c->tab_in_smem)
             k_eval_phi<true, VLOCAL><<<nb, GINT_EVAL_THREADS, c->smem_eval, st>>>(c->geom, W.b0, c->d_bstart, c->d_bent, c->d_gstart, c->d_goff, W.row0,
                 c->d_atom_pos, c->d_atom_species, c->d_species, c->d_tab, tab_cells, VLOCAL ? in : nullptr, c->d_phi);
@@ -1361,35 +1397,53 @@ static int launch_waves(gint_ctx* c, const double* in, double* out, cudaStream_t
                                                                        VLOCAL ? nullptr : in, out);
         GINT_CUDA(cudaGetLastError());
         GINT_CUDA(cudaEventRecord(c->ev_wave[VLOCAL ? 0 : 1][2 * w + 1], st));
+        if (!VLOCAL && h_out) {
+            // the planes no later wave adds to
+            const long long upto = w + 1 == nw ? c->geom.N[0] : planes_before(c, c->waves[w + 1].b0);
+            GINT_CUDA(cudaEventRecord(c->ev_copy[w], st));
+            GINT_CUDA(cudaStreamWaitEvent(cs, c->ev_copy[w], 0));
+            if (upto > copied) GINT_CUDA(cudaMemcpyAsync(h_out + copied * plane, out + copied * plane, sizeof(double) * (upto - copied) * plane, cudaMemcpyDeviceToHost, cs));
+            copied = std::max(copied, upto);
+        }
+    }
+    if (!VLOCAL && h_out) {         // the caller's stream ends behind the last copy
+        GINT_CUDA(cudaEventRecord(c->ev_copy[nw], cs));
+        GINT_CUDA(cudaStreamWaitEvent(st, c->ev_copy[nw], 0));
     }
     return GINT_OK;
 }
 
-int gint_launch_vlocal(gint_ctx* c, const double* V, double* H, cudaStream_t st) {
+int gint_launch_vlocal(gint_ctx* c, const double* V, double* H, cudaStream_t st, const double* V_host) {
     GINT_CUDA(cudaSetDevice(c->device));
+    const size_t npts = (size_t)c->geom.N[0] * c->geom.N[1] * c->geom.N[2];
     if (c->n_values == 0) return GINT_OK;
     GINT_CUDA(cudaMemsetAsync(c->d_cval, 0, sizeof(double) * (size_t)c->n_cvalues, st));
     if (c->n_tiles > 0) {
         GINT_CUDA(cudaEventRecord(c->ev[0], st));
-        int rc = launch_waves<true>(c, V, c->d_cval, st);
+        int rc = launch_waves<true>(c, V, c->d_cval, st, V_host, nullptr);
         if (rc) return rc;
         GINT_CUDA(cudaEventRecord(c->ev[1], st));
         c->timed[0] = true;
+    } else if (V_host) {
+        GINT_CUDA(cudaMemcpyAsync(const_cast<double*>(V), V_host, sizeof(double) * npts, cudaMemcpyHostToDevice, st));
     }
     k_expand_H<<<(unsigned)((c->n_pairs + 7) / 8), 256, 0, st>>>(c->n_pairs, c->d_poff, c->d_pcanon, c->d_pflag, c->d_pnA, c->d_coff, c->d_cval, H);
     GINT_CUDA(cudaGetLastError());
     return GINT_OK;
 }
 
-int gint_launch_rho(gint_ctx* c, const double* D, double* rho, cudaStream_t st) {
+int gint_launch_rho(gint_ctx* c, const double* D, double* rho, cudaStream_t st, double* rho_host) {
     GINT_CUDA(cudaSetDevice(c->device));
     const size_t npts = (size_t)c->geom.N[0] * c->geom.N[1] * c->geom.N[2];
     GINT_CUDA(cudaMemsetAsync(rho, 0, sizeof(double) * npts, st));
-    if (c->n_tiles == 0) return GINT_OK;
+    if (c->n_tiles == 0) {
+        if (rho_host) GINT_CUDA(cudaMemcpyAsync(rho_host, rho, sizeof(double) * npts, cudaMemcpyDeviceToHost, st));
+        return GINT_OK;
+    }
     k_sym_D<<<(unsigned)((c->n_canon + 7) / 8), 256, 0, st>>>(c->n_canon, c->d_poff, c->d_cpub, c->d_cmir, c->d_pnA, c->d_coff, D, c->d_cval);
     GINT_CUDA(cudaGetLastError());
     GINT_CUDA(cudaEventRecord(c->ev[2], st));
-    int rc = launch_waves<false>(c, c->d_cval, rho, st);
+    int rc = launch_waves<false>(c, c->d_cval, rho, st, nullptr, rho_host);
     if (rc) return rc;
     GINT_CUDA(cudaEventRecord(c->ev[3], st));
     c->timed[1] = true;
@@ -1410,5 +1464,75 @@ int gint_launch_alg_stats(gint_ctx* c) {
     GINT_CUDA(cudaFree(d_out));
     for (int i = 0; i < 4; i++) c->alg[i] = (long long)h[i];
     c->have_alg = true;
+    return GINT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// FP64 peak micro-benchmark (gint_fp64_peak): registers only, 4 warps per SM sub-partition, 4 independent chains per warp.
+template <bool MMA>
+__global__ void __launch_bounds__(512) k_fp64_peak(int iters, double seed, double* __restrict__ sink, long long* __restrict__ ticks) {
+    double c[4][2], f[16];
+    const double a = seed + 1e-9 * threadIdx.x, b = 1.0 - seed;
+    for (int i = 0; i < 4; i++) { c[i][0] = 0.0; c[i][1] = 0.0; }
+    for (int i = 0; i < 16; i++) f[i] = a * i;
+    const long long t0 = clock64();
+    for (int it = 0; it < iters; it++) {
+        if (MMA) {
+#pragma unroll
+            for (int r = 0; r < 4; r++)
+#pragma unroll
+                for (int i = 0; i < 4; i++)
+                    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};" : "+d"(c[i][0]), "+d"(c[i][1]) : "d"(a), "d"(b));
+        } else {
+#pragma unroll
+            for (int r = 0; r < 8; r++)
+#pragma unroll
+                for (int i = 0; i < 16; i++) f[i] = fma(f[i], a, b);
+        }
+    }
+    const long long t1 = clock64();
+    double s = 0.0;
+    for (int i = 0; i < 4; i++) s += c[i][0] + c[i][1];
+    for (int i = 0; i < 16; i++) s += f[i];
+    if (s == 0.123456789) sink[0] = s;          // never true: keeps the loops alive
+    if (blockIdx.x == 0 && threadIdx.x == 0) ticks[0] = t1 - t0;
+}
+
+extern "C" int gint_fp64_peak(int device, double out[4]) {
+    if (!out) GINT_FAIL(GINT_ERR_INVALID_ARG, "out is NULL");
+    DeviceGuard guard;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) GINT_FAIL(GINT_ERR_CUDA, "no usable CUDA device %d", device);
+    GINT_CUDA(cudaSetDevice(device));
+    cudaDeviceProp prop;
+    GINT_CUDA(cudaGetDeviceProperties(&prop, device));
+    const int nsm = prop.multiProcessorCount;
+    double* d_sink = nullptr; long long* d_ticks = nullptr;
+    GINT_CUDA(cudaMalloc(&d_sink, sizeof(double)));
+    GINT_CUDA(cudaMalloc(&d_ticks, sizeof(long long)));
+    cudaEvent_t e0, e1;
+    GINT_CUDA(cudaEventCreate(&e0)); GINT_CUDA(cudaEventCreate(&e1));
+    const int iters = 20000;
+    for (int mode = 0; mode < 2; mode++) {
+        float ms = 0.f;
+        for (int rep = 0; rep < 2; rep++) {         // the first run warms up
+            cudaEventRecord(e0, 0);
+            if (mode == 0) k_fp64_peak<true><<<nsm, 512>>>(iters, 0.25, d_sink, d_ticks);
+            else k_fp64_peak<false><<<nsm, 512>>>(iters, 0.25, d_sink, d_ticks);
+            cudaEventRecord(e1, 0);
+            if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d_sink); cudaFree(d_ticks); GINT_FAIL(GINT_ERR_CUDA, "gint_fp64_peak: %s", cudaGetErrorString(cudaGetLastError())); }
+            cudaEventElapsedTime(&ms, e0, e1);
+        }
+        // per warp and iteration: 16 DMMAs of 8 x 8 x 4 multiply-adds / 128 fma instructions of 32 lanes
+        const double fma_count = (double)nsm * 16.0 * iters * (mode == 0 ? 16.0 * 256.0 : 128.0 * 32.0);
+        out[mode] = 2.0 * fma_count / (ms * 1e-3) / 1e12;
+        if (mode == 0) {
+            long long ticks = 0;
+            cudaMemcpy(&ticks, d_ticks, sizeof(ticks), cudaMemcpyDeviceToHost);
+            out[2] = (double)ticks / (ms * 1e-3) / 1e6;
+        }
+    }
+    out[3] = nsm;
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_sink); cudaFree(d_ticks);
     return GINT_OK;
 }

@@ -21,7 +21,7 @@ STAT_NAMES = ("n_batch", "n_batch_empty", "batch_bx", "batch_by", "batch_bz", "n
               "n_waves", "n_tiles")
 
 EXPORTS = ("gint_init", "gint_n_orb", "gint_n_pairs", "gint_get_pairs", "gint_vlocal", "gint_rho", "gint_vlocal_host",
-           "gint_rho_host", "gint_stats", "gint_kernel_times", "gint_phase_times", "gint_free", "gint_last_error")
+           "gint_rho_host", "gint_stats", "gint_kernel_times", "gint_phase_times", "gint_fp64_peak", "gint_free", "gint_last_error")
 
 
 class GintError(RuntimeError):
@@ -53,6 +53,13 @@ def _ip(a):
 
 def _dp(a):
     return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def fp64_peak(device: int = 0) -> dict:
+    """gint_fp64_peak: DMMA / DFMA TFLOP/s of the device measured now, with the SM clock seen during the run."""
+    out = (C.c_double * 4)()
+    _check(lib().gint_fp64_peak(C.c_int(device), out))
+    return {"dmma_tflops": float(out[0]), "dfma_tflops": float(out[1]), "sm_mhz": float(out[2]), "n_sm": int(out[3])}
 
 
 def batch_flag(bx: int, by: int, bz: int) -> int:

@@ -13,7 +13,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def _declared():
     src = open(os.path.join(ROOT, "include", "gint.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(gint_[a-z_]+)\s*\(", src)) - {"gint_ctx"})
+    return sorted(set(re.findall(r"\b(gint_[a-z0-9_]+)\s*\(", src)) - {"gint_ctx"})
 
 
 def test_header_declares_the_north_star_calls():

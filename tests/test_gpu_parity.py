@@ -146,18 +146,75 @@ def test_empty_and_single_atom(torch_cuda):
 # ---------------------------------------------------------------------------------------------------------------
 # Full-size configurations in the launch configuration bench.py times: sampled outputs the oracle computes one by one
 # (selected pair keys / mesh points are still the exact definition for those outputs), plus identity P4, which holds
-# at any size and ties the two kernels together.
+# at any size and ties the two kernels together.  The samples are STRATIFIED: besides uniform draws they hold the places
+# where a wrong activity-mask bit or a dropped (batch, atom, cubelet) item would live -- whole ragged last batches along
+# every axis, the mesh faces (periodic wrap), whole batches of the most crowded regions (most neighbours, most atom
+# groups), and pair keys of every kind: on-site, nearest neighbours, pairs at the rim of the cutoff (atoms in different
+# groups of a batch, few common cubelets), keys across the cell boundary (R != 0).
+def _box_points(w, lo, hi):
+    """Flat indices of the mesh points lo <= (i, j, k) < hi (clipped to the mesh)."""
+    N = [int(x) for x in w.mesh]
+    r = [np.arange(max(0, lo[d]), min(N[d], hi[d]), dtype=np.int64) for d in range(3)]
+    return ((r[0][:, None, None] * N[1] + r[1][None, :, None]) * N[2] + r[2][None, None, :]).ravel()
+
+
+def _stratified_points(w, st, rng, n_uniform):
+    from scipy.spatial import cKDTree
+    N = np.array([int(x) for x in w.mesh]); bs = np.array([st["batch_bx"], st["batch_by"], st["batch_bz"]]); nb = -(-N // bs)
+    parts = [rng.integers(0, w.n_points, n_uniform)]
+    # whole last batches along each axis (ragged when bs does not divide N), two per axis
+    for ax in range(3):
+        for _ in range(2):
+            b = rng.integers(0, nb); b[ax] = nb[ax] - 1
+            parts.append(_box_points(w, b * bs, (b + 1) * bs))
+    # the six mesh faces
+    for ax in range(3):
+        for side in (0, N[ax] - 1):
+            ijk = np.stack([rng.integers(0, N[d], 1500) for d in range(3)], axis=1); ijk[:, ax] = side
+            parts.append((ijk[:, 0] * N[1] + ijk[:, 1]) * N[2] + ijk[:, 2])
+    # whole batches of the most crowded regions: most atom images within rc + half the batch diagonal of the batch centre
+    step = w.cell / N[:, None]
+    img = np.concatenate([w.atom_pos + np.array(n) @ w.cell for n in np.ndindex(3, 3, 3)]) - np.array([1, 1, 1]) @ w.cell
+    tree = cKDTree(img)
+    cand = np.stack([rng.integers(0, nb[d], 4000) for d in range(3)], axis=1)
+    centres = ((cand + 0.5) * bs) @ step
+    reach = float(w.basis.rcut.max()) + 0.5 * float(np.linalg.norm(bs @ step))
+    cnt = np.array([len(x) for x in tree.query_ball_point(centres, reach)])
+    for b in cand[np.argsort(-cnt)[:2]]:
+        parts.append(_box_points(w, b * bs, (b + 1) * bs))
+    return np.unique(np.concatenate(parts)).astype(np.int64)
+
+
+def _stratified_keys(w, plist, rng, n_uniform):
+    A, B, R, off = plist
+    d = np.linalg.norm(w.atom_pos[B] + R @ w.cell - w.atom_pos[A], axis=1)
+    rim = w.basis.rcut[w.atom_species[A]] + w.basis.rcut[w.atom_species[B]]
+    strata = [np.flatnonzero((A == B) & (np.abs(R).sum(1) == 0)),          # on-site
+              np.flatnonzero((d > 0) & (d < 3.0)),                             # nearest neighbours
+              np.flatnonzero(d > 0.9 * rim),                                   # rim of the cutoff
+              np.flatnonzero((d > 0.45 * rim) & (d < 0.55 * rim)),             # middle
+              np.flatnonzero(np.abs(R).sum(1) != 0)]                           # across the cell boundary
+    parts = [rng.integers(0, len(A), n_uniform)]
+    for s in strata:
+        if len(s):
+            parts.append(rng.choice(s, size=min(len(s), max(8, n_uniform // 5)), replace=False))
+    return np.unique(np.concatenate(parts)).astype(np.int64)
+
+
 def _sampled_parity(torch, cfg, n_keys, n_pts):
     w = W.make_workload(cfg)
     plist = O.pairs(w)
     g = _gint(w)
     _check_pairs(g, plist)
+    st = g.stats()
     V = W.make_potential(w)
     D = W.make_density_blocks(w, *plist)
     A, B, R, off = plist
     rng = np.random.default_rng([2409, 9399, cfg, 77])
-    keys = np.unique(np.concatenate([rng.integers(0, len(A), n_keys), np.flatnonzero((A == B) & (np.abs(R).sum(1) == 0))[:8]])).astype(np.int64)
-    pts = np.unique(rng.integers(0, w.n_points, n_pts)).astype(np.int64)
+    keys = _stratified_keys(w, plist, rng, n_keys)
+    pts = _stratified_points(w, st, rng, n_pts)
+    assert len(keys) >= n_keys // 2 and len(pts) >= n_pts // 2
+    assert np.any(np.abs(R[keys]).sum(1) != 0) or not np.any(np.abs(R).sum(1) != 0)
     V_d, D_d = torch.from_numpy(V).cuda(), torch.from_numpy(D).cuda()
     H_d, rho_d = g.vlocal(V_d), g.rho(D_d)
     H, rho = H_d.cpu().numpy(), rho_d.cpu().numpy()
@@ -169,24 +226,112 @@ def _sampled_parity(torch, cfg, n_keys, n_pts):
     er = float(np.max(np.abs(rho[pts] - rho_or[pts]))) / rmax
     dV = abs(np.linalg.det(w.cell)) / w.n_points
     lhs = float((V_d * rho_d).sum().item() * dV); rhs = float((D_d * H_d).sum().item())
+    # run-to-run: accumulation into H and rho is by floating-point atomics (order not fixed): equal to rounding, not bitwise
+    H2, rho2 = g.vlocal(V_d), g.rho(D_d)
+    rep_H = float((H2 - H_d).abs().max().item()) / Hmax; rep_r = float((rho2 - rho_d).abs().max().item()) / rmax
+    # a pin that does not go through the oracle: V == 1 gives the overlap matrix, whose on-site blocks have a closed form
+    S = g.vlocal(torch.ones_like(V_d)).cpu().numpy()
     g.close()
+    E = _onsite_overlap_closed_form(w)
+    onsite = np.flatnonzero((A == B) & (np.abs(R).sum(1) == 0))
+    eS = max(float(np.max(np.abs(S[off[k]:off[k + 1]].reshape(E.shape) - E))) for k in onsite)
     assert eH <= TOL, f"cfg{cfg} H parity on {len(keys)} sampled keys {eH:.3e}"
     assert er <= TOL, f"cfg{cfg} rho parity on {len(pts)} sampled points {er:.3e}"
     assert abs(lhs - rhs) <= 1e-11 * abs(lhs), f"cfg{cfg} identity P4 {abs(lhs - rhs) / abs(lhs):.3e}"
+    assert rep_H <= 1e-13 and rep_r <= 1e-13, f"cfg{cfg} repeatability {rep_H:.3e} {rep_r:.3e}"
+    assert eS <= 1e-8, f"cfg{cfg} on-site overlap blocks against the closed form {eS:.3e}"
+
+
+def _onsite_overlap_closed_form(w):
+    """S_(A,A,0) = delta_ll' delta_mm' int R_s R_s' r^2 dr for the one-species 2s2p1d basis of the five configs (reading R6:
+    r^l exp(-alpha r^2) (1 - (r/rc)^2)^3, normalised), by adaptive quadrature.  rc = 7: 0.859485228247 (s), 0.815140222328 (p)."""
+    from scipy.integrate import quad
+    rc = float(w.basis.rcut[0])
+    alpha = {0: (0.60, 0.20), 1: (0.50, 0.18)}
+
+    def f(r, l, a, b):
+        return r ** (2 * l + 2) * np.exp(-(a + b) * r * r) * (1 - (r / rc) ** 2) ** 6
+
+    E = np.eye(13)
+    for l, (a1, a2) in alpha.items():
+        n1 = quad(f, 0, rc, args=(l, a1, a1), epsabs=1e-15, epsrel=1e-13)[0]
+        n2 = quad(f, 0, rc, args=(l, a2, a2), epsabs=1e-15, epsrel=1e-13)[0]
+        v = quad(f, 0, rc, args=(l, a1, a2), epsabs=1e-15, epsrel=1e-13)[0] / np.sqrt(n1 * n2)
+        if l == 0:
+            E[0, 1] = E[1, 0] = v
+        else:
+            for m in range(3):
+                E[2 + m, 5 + m] = E[5 + m, 2 + m] = v
+    return E
 
 
 def test_cfg2_bulk_sampled(torch_cuda):
     """512-atom bulk diamond: up to 7 atom groups per batch (28 tiles), the largest dense contractions."""
-    _sampled_parity(torch_cuda, 2, 96, 4000)
+    _sampled_parity(torch_cuda, 2, 400, 20000)
 
 
 def test_cfg3_tbg_sampled(torch_cuda):
-    _sampled_parity(torch_cuda, 3, 128, 6000)
+    _sampled_parity(torch_cuda, 3, 600, 50000)
 
 
 def test_cfg4_tbg_headline_sampled(torch_cuda):
     """The headline workload (10,444 atoms, 1.76e8 points) exactly as bench.py launches it."""
-    _sampled_parity(torch_cuda, 4, 96, 4000)
+    _sampled_parity(torch_cuda, 4, 1000, 100000)
+
+
+def test_repeatability_and_two_live_contexts(torch_cuda):
+    """Two contexts alive at once on one device (different shared-memory needs: the big-table path leaves the radial table out of
+    shared memory), calls interleaved; and the same call twice gives the same result to rounding."""
+    torch = torch_cuda
+    w0 = W.make_workload(0)
+    pl0 = O.pairs(w0)
+    g0 = _gint(w0)
+    V0 = torch.from_numpy(W.make_potential(w0)).cuda(); D0 = torch.from_numpy(W.make_density_blocks(w0, *pl0)).cuda()
+    H_a, r_a = g0.vlocal(V0).clone(), g0.rho(D0).clone()
+    bs = [W.make_basis(9.0, shells=((0, 0.5 + 0.1 * k), (0, 0.2), (1, 0.45), (1, 0.2), (2, 0.35))) for k in range(3)]
+    basis = W.Basis(3, np.array([5, 5, 5], np.int32), np.concatenate([b.shell_l for b in bs]), np.array([9.0, 9.0, 9.0]), W.DR,
+                    np.concatenate([b.n_knot for b in bs]), np.concatenate([b.tab_y for b in bs]), np.concatenate([b.tab_y2 for b in bs]))
+    w1 = W.Workload("big-table", 95, np.diag([22.0, 21.0, 20.0]), np.array([24, 24, 24], np.int32), np.array([0, 1, 2], np.int32),
+                    np.array([[3.0, 4.0, 5.0], [9.5, 6.0, 8.0], [15.0, 14.0, 12.0]]), basis)
+    g1 = _gint(w1)                              # second live context with another kernel configuration
+    assert g1.stats()["tab_in_smem"] == 0 and g0.stats()["tab_in_smem"] == 1
+    pl1 = O.pairs(w1)
+    V1 = np.random.default_rng(5).standard_normal(w1.n_points)
+    H1 = g1.vlocal(torch.from_numpy(V1).cuda()).cpu().numpy()
+    H_b, r_b = g0.vlocal(V0), g0.rho(D0)        # the first context still works, and repeats itself
+    assert float((H_b - H_a).abs().max() / H_a.abs().max()) <= 1e-13
+    assert float((r_b - r_a).abs().max() / r_a.abs().max()) <= 1e-13
+    assert _rel(H1, O.vlocal(w1, V1, pl1)) <= TOL
+    assert _rel(H_b.cpu().numpy(), O.vlocal(w0, V0.cpu().numpy(), pl0)) <= TOL
+    g1.close(); g0.close()
+
+
+def test_many_orbitals_per_atom(torch_cuda):
+    """A species with 31 orbitals (3s 3p 2d... here s,s,s,p,p,p,d,d,d + s: 3 + 9 + 15 + ... <= 32) in a dense cell: eight atoms
+    exceed the 104 orbitals of a tile group, so gint_init must cut the batch neighbours into more groups than ceil(n / 8), row
+    fragments straddle atoms unevenly and groups hold fewer than eight atoms."""
+    torch = torch_cuda
+    big = W.make_basis(4.5, shells=((0, 0.8), (0, 0.4), (0, 0.2), (1, 0.7), (1, 0.35), (1, 0.2), (2, 0.6), (2, 0.3), (2, 0.2), (0, 0.12)))
+    small = W.make_basis(4.0, shells=((0, 0.5), (1, 0.4)))
+    assert int(sum(2 * l + 1 for l in big.shell_l)) == 28
+    basis = W.Basis(2, np.array([len(big.shell_l), len(small.shell_l)], np.int32), np.concatenate([big.shell_l, small.shell_l]),
+                    np.array([4.5, 4.0]), W.DR, np.concatenate([big.n_knot, small.n_knot]),
+                    np.concatenate([big.tab_y, small.tab_y]), np.concatenate([big.tab_y2, small.tab_y2]))
+    rng = np.random.default_rng(31)
+    cell = np.array([[6.0, 0.0, 0.0], [0.5, 5.5, 0.0], [0.0, 0.3, 6.5]])
+    pos = rng.uniform(0, 1, (14, 3)) @ cell
+    species = np.array([0, 0, 1, 0, 1, 0, 0, 1, 0, 0, 1, 0, 0, 1], np.int32)
+    w = W.Workload("many-orbitals", 96, cell, np.array([20, 18, 22], np.int32), species, pos, basis)
+    plist = O.pairs(w)
+    g = _gint(w)
+    _check_pairs(g, plist)
+    V = rng.standard_normal(w.n_points)
+    D = rng.standard_normal(int(plist[3][-1]))
+    H = g.vlocal(torch.from_numpy(V).cuda()).cpu().numpy()
+    rho = g.rho(torch.from_numpy(D).cuda()).cpu().numpy()
+    g.close()
+    assert _rel(H, O.vlocal(w, V, plist)) <= TOL
+    assert _rel(rho, O.rho(w, D, plist)) <= TOL
 
 
 def test_unsupported_batch_edge(torch_cuda):
