@@ -389,3 +389,165 @@ int oracle_rho(int n_species, const int *n_shell, const int *shell_l, const doub
     free(bstart); free(blist); free(fill); free(img); free(row); basis_free(&bs);
     return bad ? -2 : 0;
 }
+
+/* =====================================================================================
+ * Pulay force and stress of the local-potential energy (Eq. 4 and Eq. 5; orbital gradients PAPER.md:163).
+ *
+ * Reading R15: with E = sum_keys <D_key, H_key> = dV sum_g V_g rho_g (identity P4), at FIXED V (values per mesh index),
+ * D and dV,
+ *   F_C^a      = - dE / d tau_C^a
+ *              = dV sum_{r in all space} V(r) sum_i  d_a phi_{C i}(r - tau_C)  Psi_{C i}(r),
+ *   Psi_{C i}(r) = sum_{keys (C,B,n)} sum_j ( D_(C,B,n)[i][j] + D_(B,C,-n)[j][i] ) phi_{B j}(r - tau_B - R_n)
+ * (moving atom C changes phi_C in every key it heads and, through the mirror key, every key it ends; d phi(r - tau)/d tau = - grad phi),
+ *   sigma^{ab} = - (1/Omega) dE / d eps_ab   under r -> (1 + eps) r of atoms AND mesh points
+ *              = - (1/Omega) sum_C dV sum_r V(r) sum_i d_a phi_{C i} Psi_{C i} (r - tau_C)^b .
+ * Eq. 4 prints a factor 1/Omega for the force as well: dropped (a force is an energy derivative, the factor belongs to Eq. 5);
+ * Eq. 5 prints tau^b: read as the position of the atom relative to the integration point (the only translation-invariant reading).
+ *
+ * Orbital gradient: phi = R(r) Y(u), u = d / r, Y = c P_l(u) with P_l a homogeneous polynomial of degree l
+ * (3 z^2 - 1 == 2 z^2 - x^2 - y^2 on the unit sphere):
+ *   grad phi = (R' - l R / r) u Y + (R / r) c grad_u P_l(u),
+ *   R'(r) = [ (y_{i+1} - y_i) - (3 a^2 - 1) y''_i dr^2/6 + (3 b^2 - 1) y''_{i+1} dr^2/6 ] / dr   (derivative of the spline of R5).
+ * At |d| < 1e-12 the direction is undefined: grad phi = 0 for l = 0 and l = 2, and c_1 R'(0) e_m for l = 1 (the limit of R / r).
+ * Pins (tests/test_oracle_pins.py): central finite differences of E through oracle_vlocal (atoms displaced; cell strained),
+ * an independent brute force with scipy's spline derivative on a skew two-species cell, sum of forces under a rigid shift.
+ * sel == NULL: all atoms, sigma is written; else only the forces of atoms sel[0..n_sel) are written and sigma is left alone. */
+static double radial_d1(const basis_t *bs, int species, int shell, double r) {
+    int n = bs->n_knot[species] - 1;
+    const double *y  = bs->tab_y  + bs->tab_off[bs->shell_off[species] + shell];
+    const double *y2 = bs->tab_y2 + bs->tab_off[bs->shell_off[species] + shell];
+    double x = r / bs->dr;
+    int i = (int)floor(x);
+    if (i > n - 1) i = n - 1;
+    if (i < 0) i = 0;
+    double b = x - (double)i, a = 1.0 - b;
+    return (y[i + 1] - y[i]) / bs->dr
+         + (-(3.0 * a * a - 1.0) * y2[i] + (3.0 * b * b - 1.0) * y2[i + 1]) * bs->dr / 6.0;
+}
+
+/* values out[norb] and gradients grad[norb][3]; returns 1 if inside the sphere */
+static int dphi_eval(const basis_t *bs, int species, const double d[3], double *out, double *grad) {
+    const double PI = 3.14159265358979323846;
+    int no = bs->norb[species];
+    double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    if (!(r < bs->rcut[species])) { for (int k = 0; k < no; k++) { out[k] = 0.0; grad[3 * k] = grad[3 * k + 1] = grad[3 * k + 2] = 0.0; } return 0; }
+    phi_eval(bs, species, d, out);
+    int tiny = (r < 1e-12);
+    double u[3] = { 0, 0, 0 };
+    if (!tiny) { u[0] = d[0] / r; u[1] = d[1] / r; u[2] = d[2] / r; }
+    double x = u[0], y = u[1], z = u[2];
+    int o = 0, nsh = bs->n_shell[species];
+    for (int s = 0; s < nsh; s++) {
+        int l = bs->shell_l[bs->shell_off[species] + s];
+        double R = radial(bs, species, s, r), R1 = radial_d1(bs, species, s, r);
+        int nm = 2 * l + 1;
+        double c[5], P[5], gP[5][3];
+        if (l == 0) {
+            c[0] = 0.5 / sqrt(PI); P[0] = 1.0; gP[0][0] = gP[0][1] = gP[0][2] = 0.0;
+        } else if (l == 1) {
+            double c1 = sqrt(3.0 / (4.0 * PI));
+            for (int m = 0; m < 3; m++) { c[m] = c1; gP[m][0] = gP[m][1] = gP[m][2] = 0.0; }
+            P[0] = y; gP[0][1] = 1.0;  P[1] = z; gP[1][2] = 1.0;  P[2] = x; gP[2][0] = 1.0;
+        } else {
+            double c2 = sqrt(15.0 / (4.0 * PI));
+            c[0] = c2; P[0] = x * y;  gP[0][0] = y; gP[0][1] = x; gP[0][2] = 0.0;
+            c[1] = c2; P[1] = y * z;  gP[1][0] = 0.0; gP[1][1] = z; gP[1][2] = y;
+            c[2] = sqrt(5.0 / (16.0 * PI)); P[2] = 2.0 * z * z - x * x - y * y; gP[2][0] = -2.0 * x; gP[2][1] = -2.0 * y; gP[2][2] = 4.0 * z;
+            c[3] = c2; P[3] = x * z;  gP[3][0] = z; gP[3][1] = 0.0; gP[3][2] = x;
+            c[4] = 0.5 * c2; P[4] = x * x - y * y; gP[4][0] = 2.0 * x; gP[4][1] = -2.0 * y; gP[4][2] = 0.0;
+        }
+        for (int m = 0; m < nm; m++, o++) {
+            for (int a = 0; a < 3; a++) {
+                if (tiny) grad[3 * o + a] = (l == 1) ? c[m] * R1 * gP[m][a] : 0.0;
+                else grad[3 * o + a] = (R1 - l * R / r) * u[a] * c[m] * P[m] + (R / r) * c[m] * gP[m][a];
+            }
+        }
+    }
+    return 1;
+}
+
+/* single-point orbital gradient, exported for the pins */
+int oracle_dphi(int n_species, const int *n_shell, const int *shell_l, const double *rcut, double dr,
+                const int *n_knot, const double *tab_y, const double *tab_y2,
+                int species, const double d[3], double *out, double *grad)
+{
+    basis_t bs = { n_species, n_shell, shell_l, rcut, dr, n_knot, tab_y, tab_y2, 0, 0, 0 };
+    if (basis_setup(&bs)) return -1;
+    int in = dphi_eval(&bs, species, d, out, grad);
+    basis_free(&bs);
+    return in;
+}
+
+int oracle_force_stress(int n_species, const int *n_shell, const int *shell_l, const double *rcut, double dr,
+                        const int *n_knot, const double *tab_y, const double *tab_y2,
+                        int n_atoms, const int *atom_species, const double *atom_pos, const double cell[9], const int mesh[3],
+                        const double *V, const double *D, long long n_pairs, const int *pA, const int *pB, const int *pR, const long long *offset,
+                        double *F, double *sigma, long long n_sel, const long long *sel)
+{
+    basis_t bs = { n_species, n_shell, shell_l, rcut, dr, n_knot, tab_y, tab_y2, 0, 0, 0 };
+    if (basis_setup(&bs)) return -1;
+    double inv[9], h[3]; inv3(cell, inv); heights(inv, h);
+    const int N1 = mesh[0], N2 = mesh[1], N3 = mesh[2];
+    const double Omega = det3(cell), dV = Omega / ((double)N1 * N2 * N3);
+    long long *row = (long long *)malloc(sizeof(long long) * (n_atoms + 1));
+    { long long p = 0; for (int A = 0; A <= n_atoms; A++) { while (p < n_pairs && pA[p] < A) p++; row[A] = p; } }
+    long long ntask = sel ? n_sel : n_atoms;
+    double sg[9] = { 0, 0, 0, 0, 0, 0, 0, 0, 0 };
+    int bad = 0;
+#pragma omp parallel for schedule(dynamic, 1) reduction(| : bad) reduction(+ : sg[:9])
+    for (long long q = 0; q < ntask; q++) {
+        int C = sel ? (int)sel[q] : (int)q, sC = atom_species[C], nC = bs.norb[sC];
+        const double *tC = atom_pos + 3 * C;
+        double fC[3]; to_frac(inv, tC, fC);
+        double rcC = rcut[sC];
+        long long lo[3], hi[3]; const int NN[3] = { N1, N2, N3 };
+        for (int i = 0; i < 3; i++) {
+            lo[i] = (long long)floor((fC[i] - rcC / h[i]) * NN[i]) - 1;
+            hi[i] = (long long)ceil((fC[i] + rcC / h[i]) * NN[i]) + 1;
+        }
+        /* mirror key (B, C, -n) of every key (C, B, n) of row C */
+        long long nk = row[C + 1] - row[C];
+        long long *mir = (long long *)malloc(sizeof(long long) * (nk > 0 ? nk : 1));
+        for (long long k = 0; k < nk; k++) {
+            long long p = row[C] + k; int mn[3] = { -pR[3 * p], -pR[3 * p + 1], -pR[3 * p + 2] };
+            mir[k] = find_pair(row, pB, pR, pB[p], C, mn);
+            if (mir[k] < 0) bad |= 1;
+        }
+        double Fc[3] = { 0, 0, 0 };
+        double pc[ORACLE_MAX_ORB], gc[3 * ORACLE_MAX_ORB], pb[ORACLE_MAX_ORB], psi[ORACLE_MAX_ORB];
+        for (long long i = lo[0]; i <= hi[0] && !bad; i++)
+        for (long long j = lo[1]; j <= hi[1]; j++)
+        for (long long k = lo[2]; k <= hi[2]; k++) {
+            double u = (double)i / N1, v = (double)j / N2, w = (double)k / N3;
+            double r[3] = { u * cell[0] + v * cell[3] + w * cell[6], u * cell[1] + v * cell[4] + w * cell[7], u * cell[2] + v * cell[5] + w * cell[8] };
+            double dC[3] = { r[0] - tC[0], r[1] - tC[1], r[2] - tC[2] };
+            if (!dphi_eval(&bs, sC, dC, pc, gc)) continue;
+            for (int m = 0; m < nC; m++) psi[m] = 0.0;
+            for (long long kk = 0; kk < nk; kk++) {
+                long long p = row[C] + kk; int B = pB[p], sB = atom_species[B], nB = bs.norb[sB];
+                double R[3]; lattice(cell, pR[3 * p], pR[3 * p + 1], pR[3 * p + 2], R);
+                double dB[3] = { r[0] - atom_pos[3 * B] - R[0], r[1] - atom_pos[3 * B + 1] - R[1], r[2] - atom_pos[3 * B + 2] - R[2] };
+                if (!phi_eval(&bs, sB, dB, pb)) continue;
+                const double *Dp = D + offset[p], *Dm = D + offset[mir[kk]];      /* nC x nB  and  nB x nC */
+                for (int mu = 0; mu < nC; mu++) {
+                    double t = 0.0;
+                    for (int nu = 0; nu < nB; nu++) t += (Dp[mu * nB + nu] + Dm[nu * nC + mu]) * pb[nu];
+                    psi[mu] += t;
+                }
+            }
+            double Vg = V[(imod(i, N1) * N2 + imod(j, N2)) * N3 + imod(k, N3)];
+            for (int a = 0; a < 3; a++) {
+                double s = 0.0;
+                for (int mu = 0; mu < nC; mu++) s += gc[3 * mu + a] * psi[mu];
+                s *= Vg * dV;
+                Fc[a] += s;
+                for (int b = 0; b < 3; b++) sg[3 * a + b] -= s * dC[b] / Omega;
+            }
+        }
+        F[3 * C] = Fc[0]; F[3 * C + 1] = Fc[1]; F[3 * C + 2] = Fc[2];
+        free(mir);
+    }
+    if (!sel && sigma) for (int k = 0; k < 9; k++) sigma[k] = sg[k];
+    free(row); basis_free(&bs);
+    return bad ? -2 : 0;
+}

@@ -123,3 +123,32 @@ def rho(w, D, plist, sel=None, out=None) -> np.ndarray:
                           _p(out, C.c_double), nsel, selp)
     assert rc == 0, rc
     return out
+
+
+def dphi(basis, species: int, d):
+    """(values[norb], gradients[norb, 3]) of the orbitals of `species` at displacement d."""
+    out = np.zeros(basis.norb[species]); grad = np.zeros((basis.norb[species], 3))
+    d = np.ascontiguousarray(d, np.float64)
+    rc = lib().oracle_dphi(*_basis_args(basis), C.c_int(species), _p(d, C.c_double), _p(out, C.c_double), _p(grad, C.c_double))
+    assert rc >= 0
+    return out, grad
+
+
+def force_stress(w, V, D, plist, sel=None):
+    """Pulay force F[n_atoms, 3] and stress sigma[3, 3] of the local-potential energy (Eq. 4 / Eq. 5, reading R15).
+    sel: only the forces of these atoms (other rows stay zero; sigma is None)."""
+    A, B, R, off = plist
+    V = np.ascontiguousarray(V, np.float64); D = np.ascontiguousarray(D, np.float64)
+    assert V.size == w.n_points and D.size == off[-1]
+    F = np.zeros((w.n_atoms, 3)); sigma = np.zeros((3, 3))
+    keep, geo = _common(w)
+    if sel is None:
+        nsel, selp = C.c_longlong(0), None
+    else:
+        sel = np.ascontiguousarray(sel, np.int64); nsel, selp = C.c_longlong(len(sel)), _p(sel, C.c_longlong)
+    Rc = np.ascontiguousarray(R, np.int32)
+    rc = lib().oracle_force_stress(*_basis_args(w.basis), *geo, _p(V, C.c_double), _p(D, C.c_double), C.c_longlong(len(A)),
+                                   _p(A, C.c_int), _p(B, C.c_int), _p(Rc, C.c_int), _p(off, C.c_longlong),
+                                   _p(F, C.c_double), _p(sigma, C.c_double), nsel, selp)
+    assert rc == 0, rc
+    return F, (sigma if sel is None else None)

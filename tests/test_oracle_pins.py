@@ -477,3 +477,116 @@ def test_table2_tbg_family():
     assert abs(np.linalg.norm(w4.cell[0]) / bohr - np.linalg.norm(np.array(rows[3][1:4], float))) < 2e-3 * 125.7
     d = cKDTree(w4.atom_pos).query(w4.atom_pos, k=2)[0][:, 1]
     assert abs(d.min() - 4.65 / np.sqrt(3)) < 1e-9            # no overlapping atoms: shortest bond = a/sqrt(3)
+
+
+# ----------------------------------------------------------------------------- P10 Pulay force and stress (Eq. 4, Eq. 5; reading R15)
+def _energy(w, V, D, pl):
+    """E = <D, H> (= dV sum_g V_g rho_g, identity P4) through the oracle's H."""
+    return float(D @ O.vlocal(w, V, pl))
+
+
+def test_P10_orbital_gradient_is_the_derivative_of_phi(skew2):
+    """oracle_dphi against central differences (Richardson, O(h^4)) of oracle_phi and of the scipy-based brute_phi."""
+    w = skew2["w"]
+    rng = np.random.default_rng(41)
+    h = 2e-3
+    for sp in (0, 1):
+        for _ in range(25):
+            d = rng.normal(size=3) * 1.1
+            val, grad = O.dphi(w.basis, sp, d)
+            assert np.array_equal(val, O.phi(w.basis, sp, d))
+            for a in range(3):
+                e = np.zeros(3); e[a] = 1.0
+                for f in (lambda x: O.phi(w.basis, sp, x), lambda x: brute_phi(w.basis, sp, x)):
+                    fd = (8.0 * (f(d + 0.5 * h * e) - f(d - 0.5 * h * e)) - (f(d + h * e) - f(d - h * e))) / (6.0 * h)
+                    assert np.abs(grad[:, a] - fd).max() <= 2e-8 * max(1.0, np.abs(grad).max()), (sp, d, a)
+    # outside the sphere everything vanishes; at the nucleus only the p orbitals have a gradient (c_1 R'(0) e_m, m = y, z, x)
+    val, grad = O.dphi(w.basis, 0, np.array([0.0, 0.0, 3.0]))
+    assert not val.any() and not grad.any()
+    val, grad = O.dphi(w.basis, 0, np.zeros(3))
+    assert not grad[0].any() and not grad[4:].any()
+    p = grad[1:4]                                       # rows: p_y, p_z, p_x
+    assert abs(p[0, 1]) > 0.1 and p[0, 1] == p[1, 2] == p[2, 0] and np.count_nonzero(p) == 3
+    eps = 1e-6
+    assert abs(O.phi(w.basis, 0, np.array([0.0, eps, 0.0]))[1] / eps - p[0, 1]) <= 1e-6 * abs(p[0, 1])
+
+
+def test_P10_force_is_minus_dE_dtau(cfg0):
+    """F_C = -dE/dtau_C at fixed V, D, by central differences of E = <D, H> through oracle_vlocal (which P1..P9 pin)."""
+    w, pl, V, D = cfg0["w"], cfg0["pl"], cfg0["V"], cfg0["D"]
+    rng = np.random.default_rng(42)
+    D = D + 0.3 * rng.standard_normal(D.size)           # no symmetry of D assumed
+    F, sigma = O.force_stress(w, V, D, pl)
+    Fsel, none = O.force_stress(w, V, D, pl, sel=np.array([5, 2]))
+    assert none is None and np.array_equal(Fsel[[2, 5]], F[[2, 5]]) and not Fsel[[0, 1, 3, 4, 6, 7]].any()
+    scale = np.abs(F).max()
+    assert scale > 1e-3
+    h = 1e-4
+    for C, a in ((0, 0), (3, 1), (6, 2), (5, 0)):
+        Ep = []
+        for sgn in (+1, -1):
+            pos = w.atom_pos.copy(); pos[C, a] += sgn * h
+            Ep.append(_energy(W.Workload(w.name, w.cfg, w.cell, w.mesh, w.atom_species, pos, w.basis), V, D, pl))
+        fd = -(Ep[0] - Ep[1]) / (2 * h)
+        assert abs(F[C, a] - fd) <= 1e-6 * scale, (C, a, F[C, a], fd)
+
+
+def test_P10_stress_is_minus_dE_deps_over_volume(skew2):
+    """sigma^{ab} = -(1/Omega) dE/d eps_ab at fixed V (per mesh index), D and dV, under r -> (1 + eps) r of atoms and mesh points.
+    The oracle's E carries dV = det(cell) / N, which the strain also changes: that part, delta_ab E, is taken out."""
+    w = skew2["w"]
+    pl = O.pairs(w)
+    rng = np.random.default_rng(43)
+    V = rng.normal(size=w.n_points); D = rng.normal(size=int(pl[3][-1]))
+    F, sigma = O.force_stress(w, V, D, pl)
+    Omega = abs(np.linalg.det(w.cell))
+    E0 = _energy(w, V, D, pl)
+    h = 1e-5
+    for a in range(3):
+        for b in range(3):
+            Ep = []
+            for sgn in (+1, -1):
+                S = np.eye(3); S[a, b] += sgn * h              # r'_a = r_a + eps_ab r_b  (row vectors: r' = r S^T)
+                ws = W.Workload(w.name, w.cfg, w.cell @ S.T, w.mesh, w.atom_species, w.atom_pos @ S.T, w.basis)
+                Ep.append(_energy(ws, V, D, pl))
+            dE = (Ep[0] - Ep[1]) / (2 * h) - (E0 if a == b else 0.0)
+            assert abs(sigma[a, b] + dE / Omega) <= 2e-6 * np.abs(sigma).max(), (a, b, sigma[a, b], -dE / Omega)
+
+
+def test_P10_brute_force_force_and_stress(skew2):
+    """Independent restatement on the skew two-species cell: scipy splines and harmonics, orbital gradients by Richardson
+    differences of brute_phi, plain loops over keys, images and mesh points."""
+    w, Phi, keys = skew2["w"], skew2["Phi"], skew2["keys"]
+    pl = O.pairs(w)
+    off = pl[3]
+    no = np.array(w.basis.norb)[w.atom_species]
+    rng = np.random.default_rng(44)
+    V = rng.normal(size=w.n_points); D = rng.normal(size=int(off[-1]))
+    F, sigma = O.force_stress(w, V, D, pl)
+    index = {k: p for p, k in enumerate(keys)}
+    pts = mesh_points(w)
+    h = 2e-3
+    Fref = np.zeros((w.n_atoms, 3)); sref = np.zeros((3, 3))
+    Omega = abs(np.linalg.det(w.cell))
+    for (C, t), pc in Phi.items():
+        sp = int(w.atom_species[C])
+        d = pts - w.atom_pos[C] - np.array(t) @ w.cell
+        psi = np.zeros((w.n_points, no[C]))
+        for (C2, B, n1, n2, n3), p in index.items():
+            if C2 != C:
+                continue
+            pb = Phi.get((B, (t[0] + n1, t[1] + n2, t[2] + n3)))
+            if pb is None:
+                continue
+            q = index[(B, C, -n1, -n2, -n3)]
+            Dsym = D[off[p]:off[p + 1]].reshape(no[C], no[B]) + D[off[q]:off[q + 1]].reshape(no[B], no[C]).T
+            psi += pb @ Dsym.T
+        for a in range(3):
+            e = np.zeros(3); e[a] = 1.0
+            g = (8.0 * (brute_phi(w.basis, sp, d + 0.5 * h * e) - brute_phi(w.basis, sp, d - 0.5 * h * e))
+                 - (brute_phi(w.basis, sp, d + h * e) - brute_phi(w.basis, sp, d - h * e))) / (6.0 * h)
+            s = dV(w) * V * (g * psi).sum(1)
+            Fref[C, a] += s.sum()
+            sref[a] -= (s[:, None] * d).sum(0) / Omega
+    assert np.abs(F - Fref).max() <= 1e-7 * np.abs(Fref).max(), np.abs(F - Fref).max() / np.abs(Fref).max()
+    assert np.abs(sigma - sref).max() <= 1e-7 * np.abs(sref).max()
