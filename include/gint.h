@@ -104,6 +104,26 @@ int gint_vlocal(gint_ctx* ctx, const double* V_dev, double* H_dev, void* cuda_st
  */
 int gint_rho(gint_ctx* ctx, const double* D_dev, double* rho_dev, void* cuda_stream);
 
+/* Eq. 4 and Eq. 5: Pulay force and stress of the local-potential energy E = <D, H> = dV sum_g V_g rho_g, at fixed V
+ * (per mesh index), D and dV (reading R15 of DESIGN.md; orbital gradients: spline derivative and gradient of the real harmonics,
+ * PAPER.md:163):
+ *   F_C^a      = -dE/dtau_C^a      = dV sum_g V_g sum_t grad_a phi_(C,t)(r_g) . Psi_(C,t)(r_g),
+ *   Psi_(C,t)  = sum over atom images (B,t') non-zero at r_g of ( D_(C,B,t'-t) + D_(B,C,t-t')^T ) phi_(B,t')(r_g),
+ *   sigma^{ab} = -(1/Omega) dE/d eps_ab = -(1/Omega) sum_(C,t) dV sum_g V_g ( grad_a phi . Psi ) (r_g - tau_C - t)^b
+ * (the factor 1/Omega that Eq. 4 prints for the force is dropped; tau^b of Eq. 5 is read relative to the integration point).
+ * No symmetry of D is assumed.
+ *   V_dev     device, N1*N2*N3 doubles                                 -- read
+ *   D_dev     device, n_values doubles in pair-list layout             -- read
+ *   F_dev     device, 3 * n_atoms doubles, [atom][x, y, z]             -- OVERWRITTEN
+ *   sigma_dev device, 9 doubles [a][b], or NULL (stress not wanted)    -- OVERWRITTEN
+ * Enqueued on `cuda_stream`, no synchronisation.  The first call allocates a context-owned copy of D in the pair-list layout
+ * (8 * n_values bytes; GINT_ERR_OUT_OF_MEMORY if that fails).  GINT_ERR_UNSUPPORTED: more than 2^32 matrix elements, or a
+ * grid batch whose orbitals do not fit the kernel's shared memory (about 800 orbitals per batch). */
+int gint_force_stress(gint_ctx* ctx, const double* V_dev, const double* D_dev, double* F_dev, double* sigma_dev, void* cuda_stream);
+
+/* Device duration (seconds) of the kernels of the LAST gint_force_stress call (CUDA events on the caller's stream); -1 before it. */
+int gint_force_time(gint_ctx* ctx, double* seconds);
+
 /* Host-buffer convenience forms (the end-to-end path timed by bench.py's "e2e"): copy the input from host
  * memory (pinned or pageable) to context-owned device buffers, run the device path, copy the result back to
  * host memory and synchronise the stream before returning. */

@@ -313,7 +313,8 @@ static void free_ctx(gint_ctx* c) {
     cudaFree(c->d_crow); cudaFree(c->d_ckey); cudaFree(c->d_coff); cudaFree(c->d_cpub); cudaFree(c->d_cmir); cudaFree(c->d_cval);
     cudaFree(c->d_bstart); cudaFree(c->d_bent); cudaFree(c->d_tile); cudaFree(c->d_tstart); cudaFree(c->d_gstart);
     cudaFree(c->d_goff); cudaFree(c->d_phi); cudaFree(c->d_queue); cudaFree(c->d_planoff); cudaFree(c->d_plan);
-    cudaFree(c->d_stage_in); cudaFree(c->d_stage_out);
+    cudaFree(c->d_stage_in); cudaFree(c->d_stage_out); cudaFree(c->d_dfull);
+    for (auto& e : c->ev_force) if (e) cudaEventDestroy(e);
     for (auto& e : c->ev) if (e) cudaEventDestroy(e);
     for (auto& v : c->ev_wave) for (auto& e : v) if (e) cudaEventDestroy(e);
     for (auto& e : c->ev_copy) if (e) cudaEventDestroy(e);
@@ -656,6 +657,7 @@ static int gint_init_impl(gint_ctx** out, gint_ctx*& c, int n_species, const int
     c->smem_bytes = gint_smem_needed(c, smem_limit);
     if ((rc = gint_configure_kernels(c))) { return rc; }
     for (auto& e : c->ev) if (cudaEventCreate(&e) != cudaSuccess) { GINT_FAIL(GINT_ERR_CUDA, "cudaEventCreate failed"); }
+    for (auto& e : c->ev_force) if (cudaEventCreate(&e) != cudaSuccess) { GINT_FAIL(GINT_ERR_CUDA, "cudaEventCreate failed"); }
     if (cudaDeviceSynchronize() != cudaSuccess) { GINT_FAIL(GINT_ERR_CUDA, "gint_init: device error %s", cudaGetErrorString(cudaGetLastError())); }
     *out = c;
     return GINT_OK;
@@ -825,4 +827,27 @@ extern "C" int gint_rho(gint_ctx* c, const double* D_dev, double* rho_dev, void*
     if (((uintptr_t)D_dev | (uintptr_t)rho_dev) & 7) GINT_FAIL(GINT_ERR_INVALID_ARG, "device pointers must be 8-byte aligned");
     DeviceGuard guard;
     return gint_launch_rho(c, D_dev, rho_dev, (cudaStream_t)stream);
+}
+
+// ---- Pulay force and stress (Eq. 4, Eq. 5) ------------------------------------------------------------------
+extern "C" int gint_force_stress(gint_ctx* c, const double* V_dev, const double* D_dev, double* F_dev, double* sigma_dev, void* stream) {
+    if (!c) GINT_FAIL(GINT_ERR_BAD_STATE, "NULL context");
+    if (!V_dev || (!D_dev && c->n_values) || (!F_dev && c->n_atoms)) GINT_FAIL(GINT_ERR_INVALID_ARG, "NULL device pointer");
+    if (((uintptr_t)V_dev | (uintptr_t)D_dev | (uintptr_t)F_dev | (uintptr_t)sigma_dev) & 7) GINT_FAIL(GINT_ERR_INVALID_ARG, "device pointers must be 8-byte aligned");
+    DeviceGuard guard;
+    return gint_launch_force(c, V_dev, D_dev, F_dev, sigma_dev, (cudaStream_t)stream);
+}
+extern "C" int gint_force_time(gint_ctx* ctx, double* seconds) {
+    if (!ctx) GINT_FAIL(GINT_ERR_BAD_STATE, "NULL context");
+    if (!seconds) GINT_FAIL(GINT_ERR_INVALID_ARG, "NULL output");
+    DeviceGuard guard;
+    GINT_CUDA(cudaSetDevice(ctx->device));
+    *seconds = -1.0;
+    if (ctx->timed_force) {
+        GINT_CUDA(cudaEventSynchronize(ctx->ev_force[1]));
+        float ms = 0.f;
+        GINT_CUDA(cudaEventElapsedTime(&ms, ctx->ev_force[0], ctx->ev_force[1]));
+        *seconds = 1e-3 * ms;
+    }
+    return GINT_OK;
 }

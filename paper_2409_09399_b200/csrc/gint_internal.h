@@ -186,7 +186,6 @@ struct gint_ctx {
     long long n_batch_total = 0, n_batch = 0, n_batch_empty = 0, n_entries = 0;
     int* d_bstart = nullptr;         // [n_batch_total+1] CSR into d_bent
     NeighEntry* d_bent = nullptr;    // neighbour entries sorted by (atom, shift lexicographic)
-    int* d_order = nullptr;          // [n_batch_total] batch ids: non-empty first (mesh order), then empty ones
     long long n_tiles = 0;
     int2* d_tile = nullptr;          // [n_tiles] {batch id, I | J<<8 | G<<16}: group pair (I <= J) of G groups of the batch (freed once the plans exist)
     unsigned* d_planoff = nullptr;   // [n_tiles+1] offsets of the tile plans in 16-byte units
@@ -219,6 +218,10 @@ struct gint_ctx {
     double* d_stage_in = nullptr; size_t stage_in_n = 0;
     double* d_stage_out = nullptr; size_t stage_out_n = 0;
     cudaStream_t copy_stream = nullptr;
+    // gint_force_stress: full-layout copy of D + mirror^T (allocated by the first call), events around its kernels
+    double* d_dfull = nullptr;
+    cudaEvent_t ev_force[2] = {nullptr, nullptr};
+    bool timed_force = false;
     std::vector<cudaEvent_t> ev_copy;  // [waves + 1]
 };
 
@@ -228,6 +231,8 @@ struct gint_ctx {
 int gint_launch_vlocal(gint_ctx* c, const double* V, double* H, cudaStream_t st, const double* V_host = nullptr);
 int gint_launch_rho(gint_ctx* c, const double* D, double* rho, cudaStream_t st, double* rho_host = nullptr);
 int gint_launch_alg_stats(gint_ctx* c);
+int gint_launch_force(gint_ctx* c, const double* V, const double* D, double* F, double* sigma, cudaStream_t st);   // gint_force.cu
+size_t gint_force_smem(const gint_ctx* c);
 int gint_configure_kernels(gint_ctx* c);
 size_t gint_smem_needed(gint_ctx* c, size_t limit);   // also decides tab_in_smem
 int gint_build_phi_layout(gint_ctx* c, const int* d_bgroups, size_t phi_cap_bytes);   // Phi offsets of every (batch, group), waves, scratch

@@ -21,7 +21,8 @@ STAT_NAMES = ("n_batch", "n_batch_empty", "batch_bx", "batch_by", "batch_bz", "n
               "n_waves", "n_tiles")
 
 EXPORTS = ("gint_init", "gint_n_orb", "gint_n_pairs", "gint_get_pairs", "gint_vlocal", "gint_rho", "gint_vlocal_host",
-           "gint_rho_host", "gint_stats", "gint_kernel_times", "gint_phase_times", "gint_fp64_peak", "gint_free", "gint_last_error")
+           "gint_rho_host", "gint_force_stress", "gint_force_time", "gint_stats", "gint_kernel_times", "gint_phase_times", "gint_fp64_peak",
+           "gint_free", "gint_last_error")
 
 
 class GintError(RuntimeError):
@@ -87,6 +88,7 @@ class Gint:
                            C.c_double(float(basis.dr)), _ip(n_knot), _dp(tab_y), _dp(tab_y2), C.c_int(sp.size), _ip(sp),
                            _dp(pos), _dp(cell), _ip(mesh), C.c_int(device), C.c_ulonglong(flags)))
         self.device = device
+        self.n_atoms = int(sp.size)
         self.mesh = tuple(int(m) for m in mesh)
         self.n_points = int(np.prod(np.asarray(self.mesh, np.int64)))
         n_pairs, n_values, n_orb = C.c_longlong(), C.c_longlong(), C.c_longlong()
@@ -153,6 +155,22 @@ class Gint:
         self._dev_check(out, self.n_points, "rho")
         _check(lib().gint_rho(self._ctx, C.c_void_p(D.data_ptr()), C.c_void_p(out.data_ptr()), self._stream()))
         return out
+
+    def force_stress(self, V, D, stress: bool = True):
+        """Eq. 4 / Eq. 5: V (device, n_points), D values (device, n_values) -> (F [n_atoms, 3], sigma [3, 3] or None), device tensors."""
+        import torch
+        self._dev_check(V, self.n_points, "V")
+        self._dev_check(D, self.n_values, "D")
+        F = torch.empty((self.n_atoms, 3), dtype=torch.float64, device=V.device)
+        sigma = torch.empty((3, 3), dtype=torch.float64, device=V.device) if stress else None
+        _check(lib().gint_force_stress(self._ctx, C.c_void_p(V.data_ptr()), C.c_void_p(D.data_ptr()), C.c_void_p(F.data_ptr()),
+                                       C.c_void_p(sigma.data_ptr()) if stress else None, self._stream()))
+        return F, sigma
+
+    def force_time(self) -> float:
+        out = C.c_double()
+        _check(lib().gint_force_time(self._ctx, C.byref(out)))
+        return float(out.value)
 
     # ------------------------------------------------------------------ host-buffer path (end to end)
     @staticmethod

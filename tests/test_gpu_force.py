@@ -1,0 +1,105 @@
+"""GPU parity of gint_force_stress (Eq. 4 / Eq. 5; reading R15) against the CPU oracle, through the C ABI.
+Bar: max|dF| / max|F| <= 1e-10 and max|dsigma| / max|sigma| <= 1e-10 (the north_star tolerance of H and rho, carried over)."""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2409_09399_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+def _run(torch, w, V, D, flags=0, stress=True):
+    from paper_2409_09399_b200.gint import Gint
+    g = Gint.from_workload(w, flags=flags)
+    F, sigma = g.force_stress(torch.from_numpy(V).cuda(), torch.from_numpy(D).cuda(), stress=stress)
+    F2, sigma2 = g.force_stress(torch.from_numpy(V).cuda(), torch.from_numpy(D).cuda(), stress=stress)
+    t = g.force_time()
+    g.close()
+    assert t > 0
+    F, F2 = F.cpu().numpy(), F2.cpu().numpy()
+    assert np.abs(F2 - F).max() <= 1e-13 * np.abs(F).max()          # repeatable to rounding (floating-point atomics)
+    return F, (sigma.cpu().numpy() if stress else None)
+
+
+def _rel(a, b):
+    return float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
+
+
+@pytest.mark.parametrize("shape", [None, (3, 3, 5), (8, 8, 8), (1, 1, 1)])
+def test_cfg0_force_and_stress(torch_cuda, shape):
+    """8-atom diamond: atoms sit on mesh points (the nucleus rule of the gradient), periodic images, ragged batch shapes."""
+    from paper_2409_09399_b200.gint import batch_flag
+    w = W.make_workload(0)
+    pl = O.pairs(w)
+    V = W.make_potential(w)
+    D = W.make_density_blocks(w, *pl) + 0.3 * np.random.default_rng(8).standard_normal(int(pl[3][-1]))    # no symmetry of D assumed
+    F, sigma = _run(torch_cuda, w, V, D, flags=batch_flag(*shape) if shape else 0)
+    F_or, s_or = O.force_stress(w, V, D, pl)
+    assert _rel(F, F_or) <= TOL and _rel(sigma, s_or) <= TOL
+
+
+def test_cfg1_graphene_force_and_stress(torch_cuda):
+    w = W.make_workload(1)
+    pl = O.pairs(w)
+    V = W.make_potential(w)
+    D = W.make_density_blocks(w, *pl)
+    F, sigma = _run(torch_cuda, w, V, D)
+    F_or, s_or = O.force_stress(w, V, D, pl)
+    assert _rel(F, F_or) <= TOL and _rel(sigma, s_or) <= TOL
+
+
+def test_skew_two_species_force_and_stress(torch_cuda):
+    b1 = W.make_basis(4.0, shells=((0, 0.7), (1, 0.5), (2, 0.45)))
+    b2 = W.make_basis(3.0, shells=((0, 0.9), (0, 0.3), (1, 0.6)))
+    basis = W.Basis(2, np.array([3, 3], np.int32), np.concatenate([b1.shell_l, b2.shell_l]),
+                    np.array([4.0, 3.0]), W.DR, np.concatenate([b1.n_knot, b2.n_knot]),
+                    np.concatenate([b1.tab_y, b2.tab_y]), np.concatenate([b1.tab_y2, b2.tab_y2]))
+    cell = np.array([[5.0, 0.3, 0.0], [1.7, 4.6, 0.2], [0.4, -0.5, 5.5]])
+    pos = np.array([[0.1, 0.2, 0.3], [2.5, 2.0, 1.0], [7.9, -1.0, 6.0], [3.3, 3.9, 4.4]])
+    w = W.Workload("skew", 90, cell, np.array([17, 19, 23], np.int32), np.array([0, 1, 1, 0], np.int32), pos, basis)
+    pl = O.pairs(w)
+    rng = np.random.default_rng(12)
+    V = rng.standard_normal(w.n_points); D = rng.standard_normal(int(pl[3][-1]))
+    F, sigma = _run(torch_cuda, w, V, D)
+    F_or, s_or = O.force_stress(w, V, D, pl)
+    assert _rel(F, F_or) <= TOL and _rel(sigma, s_or) <= TOL
+    # no stress wanted: same forces
+    F_only, none = _run(torch_cuda, w, V, D, stress=False)
+    assert none is None and np.abs(F_only - F).max() <= 1e-13 * np.abs(F).max()
+
+
+def _sampled_forces(torch, cfg, n_atoms):
+    """Full-size workload: the forces of a stratified sample of atoms (first, last, random; the oracle computes any atom alone)."""
+    w = W.make_workload(cfg)
+    pl = O.pairs(w)
+    V = W.make_potential(w)
+    D = W.make_density_blocks(w, *pl)
+    rng = np.random.default_rng([2409, 9399, cfg, 78])
+    sel = np.unique(np.concatenate([[0, w.n_atoms - 1], rng.integers(0, w.n_atoms, n_atoms)])).astype(np.int64)
+    F, _ = _run(torch, w, V, D, stress=False)
+    F_or, _ = O.force_stress(w, V, D, pl, sel=sel)
+    err = float(np.abs(F[sel] - F_or[sel]).max() / np.abs(F).max())
+    assert err <= TOL, f"cfg{cfg} force parity on {len(sel)} atoms {err:.3e}"
+    # (no net-force check: V carries seeded noise per mesh point, so E is not invariant under a rigid shift of the atoms)
+
+
+def test_cfg2_bulk_sampled_forces(torch_cuda):
+    _sampled_forces(torch_cuda, 2, 24)
+
+
+def test_cfg3_tbg_sampled_forces(torch_cuda):
+    _sampled_forces(torch_cuda, 3, 48)
+
+
+def test_cfg4_tbg_headline_sampled_forces(torch_cuda):
+    _sampled_forces(torch_cuda, 4, 48)
