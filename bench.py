@@ -214,6 +214,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-force", action="store_true", help="skip the (separately reported) gint_force_stress timing")
     ap.add_argument("--batch", default="", help="override grid-batch shape, e.g. 8,8,8")
     ap.add_argument("--csrc-digest", action="store_true", help="print the digest of the kernel sources (for profiles/r2_traffic.csv) and exit")
     args = ap.parse_args()
@@ -234,7 +235,7 @@ def main():
     dev = torch.device("cuda", local)
 
     from paper_2409_09399_b200 import workloads as W
-    from paper_2409_09399_b200.gint import Gint, batch_flag, fp64_peak
+    from paper_2409_09399_b200.gint import FLAG_TUNE, Gint, batch_flag, fp64_peak
 
     # same-run FP64 peak: DMMA / DFMA micro-benchmark of the library, in this process, before the timed region
     peak_measured = fp64_peak(local)
@@ -242,7 +243,8 @@ def main():
     t0 = time.perf_counter()
     w = W.make_workload(args.cfg)
     V = W.make_potential(w)
-    flags = batch_flag(*(int(x) for x in args.batch.split(","))) if args.batch else 0
+    # default: the library's init-time batch-shape tuner; --batch fixes the shape instead
+    flags = batch_flag(*(int(x) for x in args.batch.split(","))) if args.batch else FLAG_TUNE
     t1 = time.perf_counter()
     g = Gint.from_workload(w, device=local, flags=flags)
     torch.cuda.synchronize()
@@ -298,6 +300,16 @@ def main():
     # ---- per-kernel durations of the dominant kernels (CUDA events inside the library around the main kernel)
     kt = g.kernel_times()                     # seconds, last call of each: {"vlocal_main": .., "rho_main": ..}
 
+    # ---- Pulay force + stress (Eq. 4 / Eq. 5): reported beside the step, not part of `value`
+    force = None
+    if not args.no_force:
+        g.force_stress(V_d, D_d); torch.cuda.synchronize()
+        tf = []
+        for _ in range(2):
+            g.force_stress(V_d, D_d); torch.cuda.synchronize(); tf.append(g.force_time())
+        force = {"ms": 1e3 * float(np.median(tf)), "points_per_s": npts / float(np.median(tf)),
+                 "what": "gint_force_stress: forces of all atoms and the 3x3 stress in one call (k_sym_full + k_force_batch)"}
+
     # ---- end to end through the host-buffer entry points (pinned host memory, H2D + D2H every step)
     e2e = None
     if not args.no_e2e:
@@ -342,6 +354,7 @@ def main():
             "config": {"workload": w.name, "cfg": args.cfg, "mesh": [int(m) for m in w.mesh], "atoms": int(w.n_atoms),
                        "orbitals": int(g.n_orb), "pair_blocks": int(g.n_pairs),
                        "batch": [st["batch_bx"], st["batch_by"], st["batch_bz"]],
+                       "batch_tuner": {"seconds": st["tune_us"] / 1e6, "tried_ns_per_point": {f"{a}x{b}x{c}": t for a, b, c, t in g.tune_report()}},
                        "l2": "inputs larger than L2" if flush is None else "L2 flushed between steps",
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
             "vlocal_points_per_s": npts / float(np.median(t_v)), "rho_points_per_s": npts / float(np.median(t_r)),
@@ -368,6 +381,8 @@ def main():
         if e2e:
             line["e2e"] = {"value": world * npts / e2e["t"], "unit": "mesh points/s", "h2d_bytes_per_step": e2e["h2d"],
                            "d2h_bytes_per_step": e2e["d2h"], "ms_per_step": 1e3 * e2e["t"]}
+        if force:
+            line["force_stress"] = force
         if cpu:
             line["cpu_baseline"] = cpu
         print(json.dumps(line))

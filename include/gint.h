@@ -44,6 +44,10 @@ typedef enum gint_status {
 /* flags of gint_init: three 8-bit fields override the grid-batch edge lengths (mesh points) along a1,a2,a3: 1..8, 1..8, 1..16;
  * 0 = choose automatically: 8x8x16 points, or the largest smaller shape whose batches have at most 96 neighbouring atom
  * images (PAPER.md:165 uses batches of 27..1000 points; Table 3 sweeps 125..512).  A larger edge is GINT_ERR_UNSUPPORTED. */
+/* GINT_FLAG_TUNE (with no batch-edge field set): gint_init times gint_vlocal + gint_rho for several grid-batch shapes on a slab of the
+ * mesh of fixed size and keeps the fastest (the paper's online auto-tuning; there over GEMM tile sizes, here over
+ * the grid-batch shape, the parameter its Table 3 sweeps by hand).  gint_tune_report tells what was tried. */
+#define GINT_FLAG_TUNE (1ull << 32)
 #define GINT_FLAG_BATCH(bx, by, bz) ((unsigned long long)(bx) | ((unsigned long long)(by) << 8) | ((unsigned long long)(bz) << 16))
 
 /*
@@ -155,9 +159,14 @@ enum {
     GINT_STAT_PHI_SCRATCH_BYTES = 21, /* size of the context's orbital-value scratch buffer (one wave)      */
     GINT_STAT_N_WAVES = 22,       /* waves (evaluate + contract launches) per call                          */
     GINT_STAT_N_TILES = 23,       /* (batch, group pair) tiles per call                                     */
-    GINT_N_STATS = 24
+    GINT_STAT_TUNE_US = 24,       /* microseconds gint_init spent in the batch-shape tuner (0: not asked for) */
+    GINT_N_STATS = 25
 };
 int gint_stats(gint_ctx* ctx, long long* out);
+
+/* What the batch-shape tuner tried: up to max_rows rows of out[4] = {bx, by, bz, nanoseconds per mesh point of gint_vlocal + gint_rho
+ * on the tuning slab, or -1 if the shape did not fit}; *n_rows = rows written (0 when gint_init ran without GINT_FLAG_TUNE). */
+int gint_tune_report(const gint_ctx* ctx, int max_rows, double* out, int* n_rows);
 
 /* Device durations (seconds) of the dominant kernels in the LAST gint_vlocal / gint_rho call on this context,
  * measured with CUDA events recorded on the caller's stream immediately before and after the kernel.

@@ -7,6 +7,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <chrono>
 
 #include "gint_internal.h"
 
@@ -464,13 +465,30 @@ static int build_pairs(gint_ctx* c) {
     return GINT_OK;
 }
 
+// Frees what build_batches built (the tuner builds several batch shapes in turn).
+static void release_batches(gint_ctx* c) {
+    cudaDeviceSynchronize();
+    cudaFree(c->d_bstart); cudaFree(c->d_bent); cudaFree(c->d_tile); cudaFree(c->d_tstart); cudaFree(c->d_gstart);
+    cudaFree(c->d_goff); cudaFree(c->d_phi); cudaFree(c->d_queue); cudaFree(c->d_planoff); cudaFree(c->d_plan);
+    c->d_bstart = nullptr; c->d_bent = nullptr; c->d_tile = nullptr; c->d_tstart = nullptr; c->d_gstart = nullptr;
+    c->d_goff = nullptr; c->d_phi = nullptr; c->d_queue = nullptr; c->d_planoff = nullptr; c->d_plan = nullptr;
+    for (auto& v : c->ev_wave) { for (auto& e : v) if (e) cudaEventDestroy(e); v.clear(); }
+    for (auto& e : c->ev_copy) if (e) cudaEventDestroy(e);
+    c->ev_copy.clear();
+    c->waves.clear();
+    c->device_bytes = c->device_bytes_base;
+    c->have_alg = false;
+}
+
 // ---- step a2: grid batches and their neighbour lists ------------------------------------------------------
 // Tries one batch shape: fills geom.bs/nb/K/LD/max_cols/max_nb and the CSR neighbour table.  Returns
 // GINT_ERR_UNSUPPORTED (without message) when the orbital tile of the largest batch does not fit in `smem_limit`.
-static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, size_t phi_cap, bool* fits) {
+// crop_planes > 0 (the batch-shape tuner): only the batches of the first crop_planes batch planes along a1 are built.
+static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, size_t phi_cap, bool* fits, int crop_planes = 0) {
     Geom& g = c->geom;
     *fits = false;
     for (int i = 0; i < 3; i++) { g.bs[i] = std::min(bs[i], g.N[i]); g.nb[i] = (g.N[i] + g.bs[i] - 1) / g.bs[i]; }
+    if (crop_planes > 0) g.nb[0] = std::min(g.nb[0], crop_planes);
     g.K = g.bs[0] * g.bs[1] * g.bs[2];
     for (int i = 0; i < 3; i++) if (bs[i] < 1 || bs[i] > (i == 2 ? GINT_MAX_BSZ : GINT_MAX_BS)) GINT_FAIL(GINT_ERR_UNSUPPORTED, "batch edge %d (1..%d supported)", bs[i], i == 2 ? GINT_MAX_BSZ : GINT_MAX_BS);
     const long long nbt = (long long)g.nb[0] * g.nb[1] * g.nb[2];
@@ -640,10 +658,66 @@ static int gint_init_impl(gint_ctx** out, gint_ctx*& c, int n_species, const int
     GINT_CUDA(cudaMemGetInfo(&mem_free, &mem_total));
     size_t phi_cap = std::min<size_t>((size_t)16 << 30, mem_free / 4);
     if (const char* e = getenv("GINT_PHI_CAP_MB")) { const long long mb = atoll(e); if (mb > 0) phi_cap = (size_t)mb << 20; }   // developer knob (tests use it to force several waves)
+    for (auto& e : c->ev) if (cudaEventCreate(&e) != cudaSuccess) { GINT_FAIL(GINT_ERR_CUDA, "cudaEventCreate failed"); }
+    for (auto& e : c->ev_force) if (cudaEventCreate(&e) != cudaSuccess) { GINT_FAIL(GINT_ERR_CUDA, "cudaEventCreate failed"); }
     const int fx = (int)(flags & 255), fy = (int)((flags >> 8) & 255), fz = (int)((flags >> 16) & 255);
+    c->device_bytes_base = c->device_bytes;
     bool fits = false;
-    if (fx || fy || fz) {
-        const int bs[3] = {fx ? fx : 8, fy ? fy : 8, fz ? fz : 8};
+    int tuned[3] = {0, 0, 0};
+    if ((flags & GINT_FLAG_TUNE) && !(fx || fy || fz) && n_atoms > 0) {
+        // Online tuning of the grid-batch shape (kernels of several tile sizes are tried at start-up on a task of fixed
+        // size, "no more than two seconds"): every candidate shape is built for a slab of the mesh (about GINT_TUNE_BATCHES batches,
+        // whole batch planes along a1), gint_vlocal + gint_rho run on it twice with V = 1, D = 1, and the shape with the least time per
+        // covered mesh plane is kept.
+        static const int cand[][3] = {{8, 8, 16}, {8, 8, 8}, {4, 8, 16}, {4, 4, 16}, {4, 4, 8}};
+        const auto t_begin = std::chrono::steady_clock::now();
+        const size_t npts = (size_t)mesh[0] * mesh[1] * mesh[2];
+        double *d_V = nullptr, *d_rho = nullptr, *d_D = nullptr, *d_H = nullptr;
+        GINT_CUDA(cudaMalloc(&d_V, sizeof(double) * npts)); GINT_CUDA(cudaMalloc(&d_rho, sizeof(double) * npts));
+        GINT_CUDA(cudaMalloc(&d_D, sizeof(double) * (size_t)std::max<long long>(c->n_values, 1))); GINT_CUDA(cudaMalloc(&d_H, sizeof(double) * (size_t)std::max<long long>(c->n_values, 1)));
+        {   // 1.0 everywhere (an exact zero would be skipped by the flush of gint_vlocal)
+            std::vector<double> ones(1 << 20, 1.0);
+            for (size_t o = 0; o < npts; o += ones.size()) GINT_CUDA(cudaMemcpy(d_V + o, ones.data(), sizeof(double) * std::min(ones.size(), npts - o), cudaMemcpyHostToDevice));
+            for (size_t o = 0; o < (size_t)c->n_values; o += ones.size()) GINT_CUDA(cudaMemcpy(d_D + o, ones.data(), sizeof(double) * std::min(ones.size(), (size_t)c->n_values - o), cudaMemcpyHostToDevice));
+        }
+        cudaEvent_t e0, e1;
+        GINT_CUDA(cudaEventCreate(&e0)); GINT_CUDA(cudaEventCreate(&e1));
+        double best = 0.0;
+        c->tune.clear();
+        for (auto& s : cand) {
+            const int nby = (mesh[1] + std::min(s[1], mesh[1]) - 1) / std::min(s[1], mesh[1]), nbz = (mesh[2] + std::min(s[2], mesh[2]) - 1) / std::min(s[2], mesh[2]);
+            // the same slab of the mesh for every candidate: the planes that GINT_TUNE_BATCHES batches of the largest shape cover
+            const int planes16 = std::max(2, (int)((GINT_TUNE_BATCHES + (long long)((mesh[1] + 7) / 8) * ((mesh[2] + 15) / 16) - 1) / ((long long)((mesh[1] + 7) / 8) * ((mesh[2] + 15) / 16))));
+            const int crop = std::max(1, planes16 * 8 / std::min(s[0], mesh[0]));
+            (void)nby; (void)nbz;
+            if ((rc = build_batches(c, s, smem_limit, phi_cap, &fits, crop))) { cudaFree(d_V); cudaFree(d_rho); cudaFree(d_D); cudaFree(d_H); return rc; }
+            gint_ctx::TuneResult tr; tr.bs[0] = s[0]; tr.bs[1] = s[1]; tr.bs[2] = s[2]; tr.ns_per_point = -1.0;
+            if (fits && c->n_tiles > 0) {
+                c->smem_bytes = gint_smem_needed(c, smem_limit);
+                if ((rc = gint_configure_kernels(c))) return rc;
+                float ms = 0.f;
+                for (int rep = 0; rep < 2; rep++) {
+                    cudaEventRecord(e0, 0);
+                    if ((rc = gint_launch_vlocal(c, d_V, d_H, 0)) || (rc = gint_launch_rho(c, d_D, d_rho, 0))) return rc;
+                    cudaEventRecord(e1, 0);
+                    if (cudaEventSynchronize(e1) != cudaSuccess) GINT_FAIL(GINT_ERR_CUDA, "tuner: %s", cudaGetErrorString(cudaGetLastError()));
+                    cudaEventElapsedTime(&ms, e0, e1);
+                }
+                const double pts = (double)std::min(mesh[0], c->geom.nb[0] * c->geom.bs[0]) * mesh[1] * mesh[2];
+                tr.ns_per_point = 1e6 * ms / pts;
+                if (best == 0.0 || tr.ns_per_point < best) { best = tr.ns_per_point; tuned[0] = s[0]; tuned[1] = s[1]; tuned[2] = s[2]; }
+            }
+            c->tune.push_back(tr);
+            if (fits) release_batches(c);
+            c->timed[0] = c->timed[1] = false;
+        }
+        cudaEventDestroy(e0); cudaEventDestroy(e1);
+        cudaFree(d_V); cudaFree(d_rho); cudaFree(d_D); cudaFree(d_H);
+        c->tune_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
+        fits = false;
+    }
+    if (fx || fy || fz || tuned[0]) {
+        const int bs[3] = {tuned[0] ? tuned[0] : (fx ? fx : 8), tuned[0] ? tuned[1] : (fy ? fy : 8), tuned[0] ? tuned[2] : (fz ? fz : 8)};
         if ((rc = build_batches(c, bs, smem_limit, phi_cap, &fits))) { return rc; }
         if (!fits) { GINT_FAIL(GINT_ERR_UNSUPPORTED, "requested batch %dx%dx%d needs more shared memory than %zu bytes (or > %d neighbours)", bs[0], bs[1], bs[2], smem_limit, GINT_MAX_NB); }
     } else {
@@ -656,8 +730,6 @@ static int gint_init_impl(gint_ctx** out, gint_ctx*& c, int n_species, const int
     }
     c->smem_bytes = gint_smem_needed(c, smem_limit);
     if ((rc = gint_configure_kernels(c))) { return rc; }
-    for (auto& e : c->ev) if (cudaEventCreate(&e) != cudaSuccess) { GINT_FAIL(GINT_ERR_CUDA, "cudaEventCreate failed"); }
-    for (auto& e : c->ev_force) if (cudaEventCreate(&e) != cudaSuccess) { GINT_FAIL(GINT_ERR_CUDA, "cudaEventCreate failed"); }
     if (cudaDeviceSynchronize() != cudaSuccess) { GINT_FAIL(GINT_ERR_CUDA, "gint_init: device error %s", cudaGetErrorString(cudaGetLastError())); }
     *out = c;
     return GINT_OK;
@@ -735,6 +807,7 @@ extern "C" int gint_stats(gint_ctx* ctx, long long* out) {
     out[GINT_STAT_SMEM_EVAL] = (long long)ctx->smem_eval; out[GINT_STAT_TAB_IN_SMEM] = ctx->tab_in_smem ? 1 : 0;
     out[GINT_STAT_PHI_BYTES] = (long long)(ctx->phi_rows_total * GINT_ROW_BYTES); out[GINT_STAT_PHI_SCRATCH_BYTES] = (long long)ctx->phi_bytes;
     out[GINT_STAT_N_WAVES] = (long long)ctx->waves.size(); out[GINT_STAT_N_TILES] = ctx->n_tiles;
+    out[GINT_STAT_TUNE_US] = (long long)(1e6 * ctx->tune_seconds);
     return GINT_OK;
 }
 
@@ -849,5 +922,18 @@ extern "C" int gint_force_time(gint_ctx* ctx, double* seconds) {
         GINT_CUDA(cudaEventElapsedTime(&ms, ctx->ev_force[0], ctx->ev_force[1]));
         *seconds = 1e-3 * ms;
     }
+    return GINT_OK;
+}
+
+extern "C" int gint_tune_report(const gint_ctx* ctx, int max_rows, double* out, int* n_rows) {
+    if (!ctx) GINT_FAIL(GINT_ERR_BAD_STATE, "NULL context");
+    if (!out || !n_rows || max_rows < 0) GINT_FAIL(GINT_ERR_INVALID_ARG, "bad output arguments");
+    int n = 0;
+    for (const auto& t : ctx->tune) {
+        if (n >= max_rows) break;
+        out[4 * n] = t.bs[0]; out[4 * n + 1] = t.bs[1]; out[4 * n + 2] = t.bs[2]; out[4 * n + 3] = t.ns_per_point;
+        n++;
+    }
+    *n_rows = n;
     return GINT_OK;
 }

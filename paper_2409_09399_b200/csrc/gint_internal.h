@@ -45,6 +45,7 @@
 #define GINT_NCTX 4                // tile plans in flight per CTA (the issuer requests them ahead of the consumers)
 #define GINT_PLAN_THREADS 96       // k_plan_fill (gint_init)
 #define GINT_EVAL_THREADS 256      // orbital-evaluation kernel
+#define GINT_TUNE_BATCHES 4096     // batches (of the largest shape) in the slab the batch-shape tuner times
 
 // ---- error plumbing -------------------------------------------------------------------------------
 void gint_set_error(const char* fmt, ...);
@@ -206,6 +207,11 @@ struct gint_ctx {
     size_t smem_bytes = 0;           // contraction kernels
     size_t smem_eval = 0;            // evaluation kernel
     size_t device_bytes = 0;
+    size_t device_bytes_base = 0;    // before the batch structures (the tuner builds and frees several of them)
+    // batch-shape tuner (GINT_FLAG_TUNE): what was tried
+    struct TuneResult { int bs[3]; double ns_per_point; };
+    std::vector<TuneResult> tune;
+    double tune_seconds = 0.0;
     // lazily computed statistics
     bool have_alg = false;
     long long alg[4] = {0, 0, 0, 0};

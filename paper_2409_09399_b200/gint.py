@@ -18,10 +18,10 @@ _lib = None
 STAT_NAMES = ("n_batch", "n_batch_empty", "batch_bx", "batch_by", "batch_bz", "neigh_entries", "max_nb", "max_cols",
               "padded_macs", "n_canon", "alg_incidence", "alg_sum_n", "alg_sum_n2", "nonempty_points", "smem_bytes",
               "device_bytes", "launches_vlocal", "launches_rho", "smem_eval", "tab_in_smem", "phi_bytes", "phi_scratch_bytes",
-              "n_waves", "n_tiles")
+              "n_waves", "n_tiles", "tune_us")
 
 EXPORTS = ("gint_init", "gint_n_orb", "gint_n_pairs", "gint_get_pairs", "gint_vlocal", "gint_rho", "gint_vlocal_host",
-           "gint_rho_host", "gint_force_stress", "gint_force_time", "gint_stats", "gint_kernel_times", "gint_phase_times", "gint_fp64_peak",
+           "gint_rho_host", "gint_force_stress", "gint_force_time", "gint_tune_report", "gint_stats", "gint_kernel_times", "gint_phase_times", "gint_fp64_peak",
            "gint_free", "gint_last_error")
 
 
@@ -61,6 +61,9 @@ def fp64_peak(device: int = 0) -> dict:
     out = (C.c_double * 4)()
     _check(lib().gint_fp64_peak(C.c_int(device), out))
     return {"dmma_tflops": float(out[0]), "dfma_tflops": float(out[1]), "sm_mhz": float(out[2]), "n_sm": int(out[3])}
+
+
+FLAG_TUNE = 1 << 32       # gint_init times several grid-batch shapes and keeps the fastest
 
 
 def batch_flag(bx: int, by: int, bz: int) -> int:
@@ -112,6 +115,12 @@ class Gint:
         out = np.zeros(len(STAT_NAMES), np.int64)
         _check(lib().gint_stats(self._ctx, out.ctypes.data_as(C.POINTER(C.c_longlong))))
         return dict(zip(STAT_NAMES, (int(x) for x in out)))
+
+    def tune_report(self) -> list:
+        """[(bx, by, bz, ns per mesh point or -1)] of the batch shapes the tuner tried (empty without FLAG_TUNE)."""
+        out = (C.c_double * 64)(); n = C.c_int()
+        _check(lib().gint_tune_report(self._ctx, C.c_int(16), out, C.byref(n)))
+        return [(int(out[4 * i]), int(out[4 * i + 1]), int(out[4 * i + 2]), float(out[4 * i + 3])) for i in range(n.value)]
 
     def kernel_times(self) -> dict:
         """Device seconds of the main contraction kernels in the last vlocal / rho call (CUDA events in the library)."""

@@ -334,6 +334,26 @@ def test_many_orbitals_per_atom(torch_cuda):
     assert _rel(rho, O.rho(w, D, plist)) <= TOL
 
 
+def test_batch_shape_tuner(torch_cuda):
+    """GINT_FLAG_TUNE (the paper's online auto-tuning): gint_init times the candidate batch shapes on a slab of the
+    mesh, keeps the fastest, reports what it tried -- and the context it returns is exact."""
+    from paper_2409_09399_b200.gint import FLAG_TUNE
+    st = _full_parity(torch_cuda, W.make_workload(1), flags=FLAG_TUNE)
+    from paper_2409_09399_b200.gint import Gint
+    g = Gint.from_workload(W.make_workload(1), flags=FLAG_TUNE)
+    rep = g.tune_report()
+    st = g.stats()
+    g.close()
+    tried = [r for r in rep if r[3] > 0]
+    assert len(rep) >= 3 and len(tried) >= 2 and 0 < st["tune_us"] < 2_000_000          # "no more than two seconds"
+    best = min(tried, key=lambda r: r[3])
+    assert (st["batch_bx"], st["batch_by"], st["batch_bz"]) == best[:3]
+    # without the flag nothing is tuned
+    g = Gint.from_workload(W.make_workload(0))
+    assert g.tune_report() == [] and g.stats()["tune_us"] == 0
+    g.close()
+
+
 def test_unsupported_batch_edge(torch_cuda):
     from paper_2409_09399_b200.gint import GintError, batch_flag
     with pytest.raises(GintError, match="batch edge"):
