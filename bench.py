@@ -210,7 +210,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--cfg", type=int, default=4, help="BASELINE.json configs[i]; 4 = TBG 10,444 atoms (headline)")
+    ap.add_argument("--cfg", type=int, default=4, help="BASELINE.json configs[i]; 4 = TBG 10,444 atoms (headline); 5 = mixed-species bilayer (SURVEY 8f NEXT-4)")
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")

@@ -169,7 +169,7 @@ def graphene(n: int, a: float = 4.65, c: float = 20.0):
     return np.array([n * a1, n * a2, [0.0, 0.0, c]]), np.array(pos)
 
 
-def twisted_bilayer(i: int, a: float = 4.65, d: float = 6.33, c: float = 25.0):
+def twisted_bilayer(i: int, a: float = 4.65, d: float = 6.33, c: float = 25.0, labels: bool = False):
     """Commensurate TBG, N = 4(3i^2+3i+1) atoms, cos(theta) = (3i^2+3i+1/2)/(3i^2+3i+1).
 
     Layer lattice a1 = a(1,0), a2 = a(1/2, sqrt3/2), basis {0, (a1+a2)/3}; supercell
@@ -189,8 +189,9 @@ def twisted_bilayer(i: int, a: float = 4.65, d: float = 6.33, c: float = 25.0):
     P, Q = np.meshgrid(rng, rng, indexing="ij")
     base = P.reshape(-1, 1) * a1 + Q.reshape(-1, 1) * a2
     pts = np.vstack([base, base + (a1 + a2) / 3.0])
-    out = []
-    for R, z in ((np.eye(2), c / 2.0 - d / 2.0), (Rm, c / 2.0 + d / 2.0)):
+    sub = np.r_[np.zeros(len(base), np.int32), np.ones(len(base), np.int32)]      # sublattice of every site
+    out, lab = [], []
+    for layer, (R, z) in enumerate(((np.eye(2), c / 2.0 - d / 2.0), (Rm, c / 2.0 + d / 2.0))):
         Pr = pts @ R.T
         f = np.round(Pr @ Minv, 9)
         keep = np.all((f >= -1e-9) & (f < 1 - 1e-9), axis=1)
@@ -198,9 +199,12 @@ def twisted_bilayer(i: int, a: float = 4.65, d: float = 6.33, c: float = 25.0):
         order = np.lexsort((Pk[:, 1], Pk[:, 0]))       # deterministic atom order
         Pk = Pk[order]
         out.append(np.c_[Pk, np.full(len(Pk), z)])
+        lab.append(2 * layer + sub[keep][order])
     cell = np.array([[T1[0], T1[1], 0.0], [T2[0], T2[1], 0.0], [0.0, 0.0, c]])
     pos = np.vstack(out)
     assert len(pos) == 4 * (3 * i * i + 3 * i + 1)
+    if labels:
+        return cell, pos, np.concatenate(lab)          # 2 * layer + sublattice
     return cell, pos
 
 
@@ -208,8 +212,27 @@ def _mesh_for(cell, h=0.2):
     return np.array([int(round(np.linalg.norm(cell[k]) / h)) for k in range(3)], dtype=np.int32)
 
 
+def concat_bases(parts) -> Basis:
+    """One Basis of several species from one-species bases (tables concatenated in species order)."""
+    return Basis(len(parts), np.array([len(b.shell_l) for b in parts], np.int32), np.concatenate([b.shell_l for b in parts]),
+                 np.array([float(b.rcut[0]) for b in parts]), DR, np.concatenate([b.n_knot for b in parts]),
+                 np.concatenate([b.tab_y for b in parts]), np.concatenate([b.tab_y2 for b in parts]),
+                 norm=sum((list(b.norm) for b in parts), []))
+
+
 def make_workload(cfg: int) -> Workload:
-    """The five BASELINE.json configs."""
+    """The five BASELINE.json configs (0..4), and 5: a MIXED-SPECIES bilayer ("m, n = orbitals per atom 1...30",
+    PAPER.md:165): the geometry of cfg3 with layer 1 of species 0 (2s2p1d, 13 orbitals, rc 7) and layer 2 of two species by
+    sublattice, species 1 (2s2p, 8 orbitals, rc 8) and species 2 (2s2p2d, 18 orbitals, rc 6) -- three radial tables of different
+    lengths, orbital rows that do not line up with the 8-row fragments, cutoff spheres of three sizes."""
+    if cfg == 5:
+        cell, pos, lab = twisted_bilayer(9, labels=True)
+        species = np.where(lab < 2, 0, lab - 1).astype(np.int32)
+        basis = concat_bases([make_basis(7.0),
+                              make_basis(8.0, shells=((0, 0.45), (0, 0.15), (1, 0.40), (1, 0.14))),
+                              make_basis(6.0, shells=((0, 0.75), (0, 0.28), (1, 0.60), (1, 0.22), (2, 0.50), (2, 0.25)))])
+        return Workload("cfg5 mixed-species bilayer i=9 (1084 atoms, 13/8/18 orbitals)", 5, np.ascontiguousarray(cell, np.float64),
+                        _mesh_for(cell), species, np.ascontiguousarray(pos, np.float64), basis)
     if cfg == 0:
         cell, pos = diamond(1)
         mesh, rc, name = np.array([24, 24, 24], np.int32), 5.0, "cfg0 diamond-8"
@@ -308,7 +331,8 @@ def make_density_blocks(w: Workload, pA, pB, pR, offset, scale_len2: float = 20.
     pA = np.asarray(pA); pB = np.asarray(pB); pR = np.asarray(pR).reshape(-1, 3)
     offset = np.asarray(offset, np.int64)
     norb = w.basis.norb
-    assert len(set(norb)) == 1, "make_density_blocks: uniform orbital count per atom only"
+    if len(set(norb)) != 1:
+        return _make_density_blocks_mixed(w, pA, pB, pR, offset, scale_len2)
     no = norb[0]
     npairs = len(pA)
     assert offset[-1] == npairs * no * no
@@ -330,3 +354,25 @@ def make_density_blocks(w: Workload, pA, pB, pR, offset, scale_len2: float = 20.
         selfm = mir[q] == q
         D[mir[q][~selfm]] = np.transpose(g[~selfm], (0, 2, 1))
     return np.ascontiguousarray(D.reshape(-1))
+
+
+def _make_density_blocks_mixed(w: Workload, pA, pB, pR, offset, scale_len2: float) -> np.ndarray:
+    """The same recipe for species with different orbital counts: the canonical key (A, B, R) gets N(0,1) entries times
+    exp(-d^2/scale_len2) (symmetrised when it is its own mirror), the mirror key the transpose; one block at a time."""
+    no = np.asarray(w.basis.norb)[w.atom_species]
+    r0, r1, r2 = pR[:, 0], pR[:, 1], pR[:, 2]
+    lex_ge0 = (r0 > 0) | ((r0 == 0) & ((r1 > 0) | ((r1 == 0) & (r2 >= 0))))
+    canon = (pA < pB) | ((pA == pB) & lex_ge0)
+    mir = mirror_index(pA, pB, pR)
+    d = np.linalg.norm(w.atom_pos[pB] + pR @ w.cell - w.atom_pos[pA], axis=1)
+    rng = np.random.default_rng([*SEED, w.cfg, 1])
+    D = np.zeros(int(offset[-1]))
+    for q in np.nonzero(canon)[0]:
+        nA, nB = int(no[pA[q]]), int(no[pB[q]])
+        g = rng.standard_normal((nA, nB)) * np.exp(-d[q] ** 2 / scale_len2)
+        if mir[q] == q:
+            g = np.triu(g) + np.triu(g, 1).T
+        D[offset[q]:offset[q + 1]] = g.ravel()
+        if mir[q] != q:
+            D[offset[mir[q]]:offset[mir[q] + 1]] = g.T.ravel()
+    return D

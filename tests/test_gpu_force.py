@@ -101,5 +101,9 @@ def test_cfg3_tbg_sampled_forces(torch_cuda):
     _sampled_forces(torch_cuda, 3, 48)
 
 
+def test_cfg5_mixed_species_sampled_forces(torch_cuda):
+    _sampled_forces(torch_cuda, 5, 48)
+
+
 def test_cfg4_tbg_headline_sampled_forces(torch_cuda):
     _sampled_forces(torch_cuda, 4, 48)

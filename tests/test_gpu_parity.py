@@ -232,9 +232,16 @@ def _sampled_parity(torch, cfg, n_keys, n_pts):
     # a pin that does not go through the oracle: V == 1 gives the overlap matrix, whose on-site blocks have a closed form
     S = g.vlocal(torch.ones_like(V_d)).cpu().numpy()
     g.close()
-    E = _onsite_overlap_closed_form(w)
-    onsite = np.flatnonzero((A == B) & (np.abs(R).sum(1) == 0))
-    eS = max(float(np.max(np.abs(S[off[k]:off[k + 1]].reshape(E.shape) - E))) for k in onsite)
+    eS = 0.0
+    if w.basis.n_species == 1:
+        E = _onsite_overlap_closed_form(w)
+        onsite = np.flatnonzero((A == B) & (np.abs(R).sum(1) == 0))
+        eS = max(float(np.max(np.abs(S[off[k]:off[k + 1]].reshape(E.shape) - E))) for k in onsite)
+    else:       # several species: orthonormality of every on-site block (real harmonics, normalised radial functions of one l differ)
+        no = np.asarray(w.basis.norb)[w.atom_species]
+        for k in np.flatnonzero((A == B) & (np.abs(R).sum(1) == 0))[::37]:
+            blk = S[off[k]:off[k + 1]].reshape(no[A[k]], no[A[k]])
+            eS = max(eS, float(np.max(np.abs(np.diag(blk) - 1.0))), float(np.max(np.abs(blk - blk.T))))
     assert eH <= TOL, f"cfg{cfg} H parity on {len(keys)} sampled keys {eH:.3e}"
     assert er <= TOL, f"cfg{cfg} rho parity on {len(pts)} sampled points {er:.3e}"
     assert abs(lhs - rhs) <= 1e-11 * abs(lhs), f"cfg{cfg} identity P4 {abs(lhs - rhs) / abs(lhs):.3e}"
@@ -277,6 +284,11 @@ def test_cfg3_tbg_sampled(torch_cuda):
 def test_cfg4_tbg_headline_sampled(torch_cuda):
     """The headline workload (10,444 atoms, 1.76e8 points) exactly as bench.py launches it."""
     _sampled_parity(torch_cuda, 4, 1000, 100000)
+
+
+def test_cfg5_mixed_species_sampled(torch_cuda):
+    """Mixed-species bilayer (13 / 8 / 18 orbitals per atom, rc 7 / 8 / 6, three radial tables): SURVEY 8f NEXT-4."""
+    _sampled_parity(torch_cuda, 5, 600, 50000)
 
 
 def test_repeatability_and_two_live_contexts(torch_cuda):
