@@ -27,7 +27,7 @@
 #define GINT_MMA_WARPS 12          // warp groups 0,1,2: DMMA consumers, three per SM sub-partition; each owns up to GINT_WARP_BLOCKS blocks
                                    // of 2 row fragments x 4 (block 0) or 3 (blocks 1, 2) column fragments of the tile
 #define GINT_WARP_BLOCKS 3
-#define GINT_AUX_WARPS 4           // warp group 3: warp 12 = TMA issuer (+ rho reducer), warps 13..15 idle (setmaxnreg works on whole warp groups)
+#define GINT_AUX_WARPS 4           // warp group 3: warp 12 = TMA issuer, warps 13, 14 = reducers of gint_rho, warp 15 idle (setmaxnreg works on whole warp groups)
 #define GINT_CTA_THREADS (32 * (GINT_MMA_WARPS + GINT_AUX_WARPS))
 #define GINT_REGS_MMA 152          // registers per thread after setmaxnreg: 384 * 152 + 128 * 56 = 65536
 #define GINT_REGS_AUX 56

@@ -605,13 +605,23 @@ k_plan_fill(Geom g, const int2* __restrict__ tile, const int* __restrict__ bstar
 // ---------------------------------------------------------------------------------------------------
 // shared memory of the contraction kernels
 static_assert(GINT_SC == 2, "the density reduction of the consumers is written for two cubelets per stage");
+// gint_rho runs a ring of GINT_NS - 1 stages; the memory of the last stage holds GINT_NRED buffers of the consumers' LANE partial
+// densities of a stage, [consumer warp][lane][cubelet of the stage, point 2 (lane % 4) + e] (partial over the lane's orbital row):
+// the sum over the 8 rows of a fragment and over the warps is taken by the reducer warps (13, 14) of the issuer's warp group, which
+// also add the stage's 16 densities to rho -- the consumers' stage ends with two stores behind its last DMMAs.
+#define GINT_NRED 2                 // reducer warps
+#ifndef GINT_NBUF
+#define GINT_NBUF 4                 // buffers of lane partial densities (a consumer may run this many stages ahead of the reducers)
+#endif
+#define GINT_LPART_BYTES (GINT_MMA_WARPS * 32 * GINT_SC * 2 * 8)
+#define GINT_RHO_RSV ((GINT_NBUF * GINT_LPART_BYTES + GINT_STAGE_BYTES - 1) / GINT_STAGE_BYTES)     // ring stages given up for them
+static_assert(GINT_NBUF % GINT_NRED == 0, "a buffer always goes to the same reducer");
 struct alignas(128) TileSmem {
     unsigned char ring[GINT_NS][GINT_STAGE_BYTES];     // stage: [cubelet q][side][row][8 points]
     alignas(16) unsigned char plan[GINT_NCTX][GINT_PLAN_MAX_BYTES];    // PlanHdr + PlanCub[]
-    double part[GINT_NS][GINT_MMA_WARPS][GINT_SC * GINT_CPTS];         // gint_rho: per stage, the consumer warps' partial densities
     u64 full[GINT_NS], empty[GINT_NS];             // stage filled by TMA / read by all consumer warps
-    u64 ctx_full[GINT_NCTX], ctx_free[GINT_NCTX];  // plan arrived / released by consumers and issuer
-    int hist[GINT_NS];                  // issuer: context | stage of the tile << 8 of what each ring slot holds
+    u64 ctx_full[GINT_NCTX], ctx_free[GINT_NCTX];  // plan arrived / released by consumers, issuer and (gint_rho) reducers
+    u64 lfull[GINT_NBUF], lempty[GINT_NBUF];       // gint_rho: a buffer of lane partial densities written by all consumers / read by its reducer
 };
 __device__ __forceinline__ const PlanHdr& plan_hdr(const TileSmem& S, int c) { return *reinterpret_cast<const PlanHdr*>(S.plan[c]); }
 __device__ __forceinline__ const PlanCub* plan_cub(const TileSmem& S, int c) { return reinterpret_cast<const PlanCub*>(S.plan[c] + sizeof(PlanHdr)); }
@@ -623,29 +633,51 @@ size_t gint_smem_needed(gint_ctx* c, size_t limit) {
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Issuer warp: pops the tile queue, fetches plans, streams the tile's slots into the ring; in gint_rho it also retires the
-// stages: sums the consumer warps' partial densities in fixed order into the tile's density, which it adds to rho when the
-// tile is complete (one red.global.add.f64 per mesh point per tile).
-template <bool VLOCAL>
-__device__ __forceinline__ void retire_stage(const Geom& g, TileSmem& S, int gr, double* __restrict__ rho) {
-    const int lane = threadIdx.x & 31, s = gr % GINT_NS;
-    mbar_wait(&S.empty[s], (gr / GINT_NS) & 1);
-    if (VLOCAL) return;
-    const int h = S.hist[s], c = h & 255, st = h >> 8;
-    const PlanHdr& X = plan_hdr(S, c);
-    const int ncs = min(GINT_SC, X.ncub - st * GINT_SC);
-    if (lane < ncs * GINT_CPTS) {
-        // four chains: the adds queue behind the consumers' DMMAs in the FP64 pipe of this warp's SM sub-partition
-        double v[4] = {0.0, 0.0, 0.0, 0.0};
+// Issuer warp: pops the tile queue, fetches plans, streams the tile's slots into the ring (NSK stages).
+template <int NSK>
+__device__ __forceinline__ void retire_stage(TileSmem& S, int gr) {
+    mbar_wait(&S.empty[gr % NSK], (gr / NSK) & 1);
+}
+
+// Reducer warp `id` of gint_rho (stages id, id + GINT_NRED, ... of the CTA's stage sequence): sums the lane partial densities of a
+// stage in fixed order and adds the 16 densities to rho (every listed cubelet belongs to exactly one stage of its tile: one
+// red.global.add.f64 per mesh point per tile).
+__device__ __forceinline__ void reducer_role(const Geom& g, TileSmem& S, int id, double* __restrict__ rho) {
+    const int lane = threadIdx.x & 31;
+    const int pt = lane & 15, half = lane >> 4, q = pt >> 3, p = pt & 7;
+    // lane partial (warp w, lane 4 lr + lc)[2 q + e] with lc = p / 2, e = p % 2
+    const double* lp0 = reinterpret_cast<const double*>(&S.ring[GINT_NS - GINT_RHO_RSV][0]) + (size_t)(p >> 1) * 4 + 2 * q + (p & 1);
+    int g0 = 0;
+    for (int t = 0;; t++) {
+        const int c = t % GINT_NCTX;
+        mbar_wait(&S.ctx_full[c], (t / GINT_NCTX) & 1);
+        const PlanHdr& X = plan_hdr(S, c);
+        if (!X.valid) break;
+        const PlanCub* C = plan_cub(S, c);
+        const int nstage = X.nstage;
+        for (int st = 0; st < nstage; st++) {
+            const int gs = g0 + st;
+            if (gs % GINT_NRED != id) continue;
+            const int lb = gs % GINT_NBUF;
+            const double* lp = lp0 + (size_t)lb * (GINT_LPART_BYTES / 8);
+            mbar_wait(&S.lfull[lb], (gs / GINT_NBUF) & 1);
+            double v[4] = {0.0, 0.0, 0.0, 0.0};         // four chains: the adds queue behind the consumers' DMMAs in the FP64 pipe
 #pragma unroll
-        for (int w = 0; w < GINT_MMA_WARPS; w++) v[w & 3] += S.part[s][w][lane];
-        const double sum = (v[0] + v[1]) + (v[2] + v[3]);
-        // every listed cubelet belongs to exactly one stage of the tile: one add per mesh point per tile
-        int ix, iy, iz; cubelet_point(plan_cub(S, c)[st * GINT_SC + (lane >> 3)].cub, lane & 7, ix, iy, iz);
-        if (sum != 0.0 && ix < X.ex && iy < X.ey && iz < X.ez)
-            atomicAdd(rho + ((size_t)(X.i0 + ix) * g.N[1] + (X.j0 + iy)) * g.N[2] + (X.k0 + iz), sum);
-    }
-    if (st == X.nstage - 1) {
+            for (int w = 0; w < GINT_MMA_WARPS / 2; w++)
+#pragma unroll
+                for (int lr = 0; lr < 8; lr++) v[lr & 3] += lp[((size_t)(half * (GINT_MMA_WARPS / 2) + w) * 32 + lr * 4) * 4];
+            double sum = (v[0] + v[1]) + (v[2] + v[3]);
+            sum += __shfl_xor_sync(0xffffffffu, sum, 16);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&S.lempty[lb]);
+            const int ncs = min(GINT_SC, X.ncub - st * GINT_SC);
+            if (half == 0 && q < ncs) {
+                int ix, iy, iz; cubelet_point(C[st * GINT_SC + q].cub, p, ix, iy, iz);
+                if (sum != 0.0 && ix < X.ex && iy < X.ey && iz < X.ez)
+                    atomicAdd(rho + ((size_t)(X.i0 + ix) * g.N[1] + (X.j0 + iy)) * g.N[2] + (X.k0 + iz), sum);
+            }
+        }
+        g0 += nstage;
         __syncwarp();
         if (lane == 0) mbar_arrive(&S.ctx_free[c]);
     }
@@ -655,23 +687,15 @@ template <bool VLOCAL>
 __device__ __forceinline__ void issuer_role(const Geom& g, TileSmem& S, const unsigned char* __restrict__ plan, const unsigned* __restrict__ planoff,
                                             int n_tiles, int* __restrict__ queue, const double* __restrict__ phi, u64 wave_row0, double* __restrict__ rho) {
     const int lane = threadIdx.x & 31;
+    constexpr int NSK = VLOCAL ? GINT_NS : GINT_NS - GINT_RHO_RSV;     // gint_rho: the last stages' memory holds the lane partial densities
     int gi = 0, gr = 0;                 // stages issued / retired
-    int tile_end[GINT_NCTX];            // gi at the end of the tile that used the context last
-#pragma unroll
-    for (int c = 0; c < GINT_NCTX; c++) tile_end[c] = 0;
     int requested = 0;                  // plans requested so far
     bool drained = false;               // the queue has run out
     // request the plan of the next tile into context requested % GINT_NCTX
     auto request = [&]() {
         const int t = requested, c = t % GINT_NCTX;
         if (t >= GINT_NCTX) {
-            // the context's previous tile must be over: all its stages retired (gint_rho flushes its density then), consumers gone
-            if (!VLOCAL) {
-                int te = 0;
-#pragma unroll
-                for (int k = 0; k < GINT_NCTX; k++) if (k == c) te = tile_end[k];
-                while (gr < te) { retire_stage<VLOCAL>(g, S, gr, rho); gr++; }
-            }
+            // the context's previous tile must be over: consumers, issuer (and the reducers of gint_rho) have left it
             mbar_wait(&S.ctx_free[c], ((t / GINT_NCTX) - 1) & 1);
         }
         int ti = 0;
@@ -702,15 +726,15 @@ __device__ __forceinline__ void issuer_role(const Geom& g, TileSmem& S, const un
         const unsigned char* srcI = reinterpret_cast<const unsigned char*>(phi) + (X.rowI - wave_row0) * GINT_ROW_BYTES;
         const unsigned char* srcJ = reinterpret_cast<const unsigned char*>(phi) + (X.rowJ - wave_row0) * GINT_ROW_BYTES;
         for (int st = 0; st < nstage; st++, gi++) {
-            const int s = gi % GINT_NS;
-            while (gi - gr >= GINT_NS) { retire_stage<VLOCAL>(g, S, gr, rho); gr++; }
+            const int s = gi % NSK;
+            while (gi - gr >= NSK) { retire_stage<NSK>(S, gr); gr++; }
             const int ncs = min(GINT_SC, ncub - st * GINT_SC);
 #ifdef GINT_DBG_NO_TMA
-            if (lane == 0) { mbar_arrive(&S.full[s]); S.hist[s] = c | (st << 8); }
+            if (lane == 0) mbar_arrive(&S.full[s]);
             __syncwarp();
             if (false) {
 #else
-            if (lane == 0) { mbar_expect_tx(&S.full[s], (unsigned)ncs * (bI + bJ)); S.hist[s] = c | (st << 8); }
+            if (lane == 0) mbar_expect_tx(&S.full[s], (unsigned)ncs * (bI + bJ));
             __syncwarp();
             if (lane < ncs) {
 #endif
@@ -720,11 +744,10 @@ __device__ __forceinline__ void issuer_role(const Geom& g, TileSmem& S, const un
                 if (bJ) bulk_g2s(dst + GINT_SLOT_MAX_BYTES, srcJ + (size_t)pc.slotJ * strJ, bJ, &S.full[s]);
             }
         }
-#pragma unroll
-        for (int k = 0; k < GINT_NCTX; k++) if (k == c) tile_end[k] = gi;
-        if (nstage == 0 || VLOCAL) { __syncwarp(); if (lane == 0) mbar_arrive(&S.ctx_free[c]); }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&S.ctx_free[c]);          // the issuer is done with the plan
     }
-    while (gr < gi) { retire_stage<VLOCAL>(g, S, gr, rho); gr++; }
+    while (gr < gi) { retire_stage<NSK>(S, gr); gr++; }
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -982,10 +1005,13 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
     const unsigned lane_v = lr * GINT_ROW_BYTES + ((VLOCAL ? lc : (lc ^ (lr & 2))) * 16);  // row lr of a fragment, points 2 lc, 2 lc + 1
     const unsigned lane_j = lc * GINT_ROW_BYTES + ((lr ^ ((lc & 2) << 1)) * 8);            // gint_rho B operand: row lc of the k-step, point lr
     // ring position of the next stage: slot, parity of its full barrier, and the slot's addresses (all 32-bit shared addresses)
+    constexpr unsigned NSK = VLOCAL ? GINT_NS : GINT_NS - GINT_RHO_RSV;
     unsigned rs = 0, rph = 0;
+    int gsl = 0;                                                           // gint_rho: stages done (selects the lane-partial buffer)
     const unsigned full0 = smem_addr(&S.full[0]), empty0 = smem_addr(&S.empty[0]);
     // gint_rho: where the lane's reduced partial density of a stage goes (see the butterfly below)
-    const unsigned part0 = smem_addr(&S.part[0][warp][((lane >> 4) & 1) * GINT_CPTS + 2 * lc + ((lane >> 3) & 1)]);
+    const unsigned lpart0 = smem_addr(&S.ring[GINT_NS - GINT_RHO_RSV][0]) + (unsigned)(warp * 32 + lane) * (GINT_SC * 2 * 8);
+    const unsigned lfull0 = smem_addr(&S.lfull[0]), lempty0 = smem_addr(&S.lempty[0]);
 #ifdef GINT_DBG_STATS
     unsigned long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 #endif
@@ -1073,23 +1099,22 @@ __device__ __forceinline__ void consumer_role(TileSmem& S, const double* __restr
             }
 #endif
             if (!VLOCAL) {
-                // part[q][e]: point 2 lc + e of cubelet q, partial over the lane's orbital row lr -> sum over lr (lane bits 2..4)
-                const bool hi = lane & 16, mid = lane & 8;
-                double r2[2];
-#pragma unroll
-                for (int e = 0; e < 2; e++) {
-                    const double keep = hi ? part[GINT_SC - 1][e] : part[0][e], send = hi ? part[0][e] : part[GINT_SC - 1][e];
-                    r2[e] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-                }
-                const double keep = mid ? r2[1] : r2[0], send = mid ? r2[0] : r2[1];
-                double r1 = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-                r1 += __shfl_xor_sync(0xffffffffu, r1, 4);
-                // the lane holds cubelet (lane >> 4) & 1, point 2 lc + ((lane >> 3) & 1)
-                if (!(lane & 4)) sts64(part0 + s * (unsigned)sizeof(S.part[0]), r1);
+                // part[q][e]: point 2 lc + e of cubelet q, partial over the lane's orbital row: handed to a reducer warp as it is
+                const unsigned lb = (unsigned)gsl % GINT_NBUF;
+                DBG_T(t_l0);
+                if (gsl >= GINT_NBUF) mbar_wait_s(lempty0 + 8 * lb, (unsigned)((gsl / GINT_NBUF) - 1) & 1u);
+                DBG_T(t_l1);
+                DBG_ADD(3, t_l1 - t_l0);
+                const unsigned dst = lpart0 + lb * GINT_LPART_BYTES;
+                asm volatile("st.shared.v2.f64 [%0], {%1, %2};" :: "r"(dst), "d"(part[0][0]), "d"(part[0][1]) : "memory");
+                asm volatile("st.shared.v2.f64 [%0], {%1, %2};" :: "r"(dst + 16), "d"(part[GINT_SC - 1][0]), "d"(part[GINT_SC - 1][1]) : "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive_s(lfull0 + 8 * lb);
+                gsl++;
             }
             __syncwarp();
             if (lane == 0) mbar_arrive_s(empty0 + 8 * s);
-            if (++rs == GINT_NS) { rs = 0; rph ^= 1u; }
+            if (++rs == NSK) { rs = 0; rph ^= 1u; }
 #pragma unroll
             for (int qq = 0; qq < GINT_SC; qq++) cur[qq] = nxt[qq];
             DBG_T(t_w2);
@@ -1127,7 +1152,8 @@ k_tiles(Geom g, const unsigned char* __restrict__ plan, const unsigned* __restri
     const int warp = threadIdx.x >> 5;
     if (threadIdx.x == 0) {
         for (int s = 0; s < GINT_NS; s++) { mbar_init(&S.full[s], 1); mbar_init(&S.empty[s], GINT_MMA_WARPS); }
-        for (int c = 0; c < GINT_NCTX; c++) { mbar_init(&S.ctx_full[c], 1); mbar_init(&S.ctx_free[c], GINT_MMA_WARPS + 1); }
+        for (int c = 0; c < GINT_NCTX; c++) { mbar_init(&S.ctx_full[c], 1); mbar_init(&S.ctx_free[c], GINT_MMA_WARPS + 1 + (VLOCAL ? 0 : GINT_NRED)); }
+        for (int k = 0; k < GINT_NBUF; k++) { mbar_init(&S.lfull[k], GINT_MMA_WARPS); mbar_init(&S.lempty[k], 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     // the ring starts zeroed: the consumers may read rows of a stage that no copy has written yet (multiplied by zeros: must be finite)
@@ -1139,6 +1165,7 @@ k_tiles(Geom g, const unsigned char* __restrict__ plan, const unsigned* __restri
     } else {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" :: "n"(GINT_REGS_AUX));
         if (warp == GINT_MMA_WARPS) issuer_role<VLOCAL>(g, S, plan, planoff, n_tiles, queue, phi, wave_row0, out);
+        else if (!VLOCAL && warp - GINT_MMA_WARPS - 1 < GINT_NRED) reducer_role(g, S, warp - GINT_MMA_WARPS - 1, out);
     }
 }
 
