@@ -190,19 +190,21 @@ k_force_batch(Geom g, const int* __restrict__ bstart, const NeighEntry* __restri
         for (int rr = tid; rr < nrows; rr += GINT_FORCE_THREADS) {
             int lo = 0, hi = nact - 1;
             while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (S.arow[mid] <= rr) lo = mid; else hi = mid - 1; }
-            const int a = S.act[lo], i = rr - S.arow[lo];
+            const int a = S.act[lo], i = rr - S.arow[lo], nA = S.ent[a].norb;
             double acc[8];
 #pragma unroll
             for (int p = 0; p < 8; p++) acc[p] = 0.0;
             for (int kb = 0; kb < nact; kb++) {
                 const int bb = S.act[kb];
-                const unsigned off = pairp[a * n + bb];
+                // Dfull_(a,b)[i][j] is read as Dfull_(b,a)[j][i] (the full-layout copy is symmetric: Dfull_q = Dfull_p^T for mirror keys):
+                // the threads of a warp hold consecutive rows i, so that their loads fall into a few sectors instead of one each
+                const unsigned off = pairp[bb * n + a];
                 if (off == 0xffffffffu) continue;
                 const int nB = S.ent[bb].norb;
-                const double* drow = Dfull + off + (size_t)i * nB;
+                const double* dcol = Dfull + off + i;
                 const double2* pr = reinterpret_cast<const double2*>(phi + (size_t)S.ent[bb].row0 * 8);
                 for (int j = 0; j < nB; j++) {
-                    const double d = __ldg(drow + j);
+                    const double d = __ldg(dcol + (size_t)j * nA);
                     const double2 f0 = pr[4 * j], f1 = pr[4 * j + 1], f2 = pr[4 * j + 2], f3 = pr[4 * j + 3];
                     acc[0] = fma(d, f0.x, acc[0]); acc[1] = fma(d, f0.y, acc[1]); acc[2] = fma(d, f1.x, acc[2]); acc[3] = fma(d, f1.y, acc[3]);
                     acc[4] = fma(d, f2.x, acc[4]); acc[5] = fma(d, f2.y, acc[5]); acc[6] = fma(d, f3.x, acc[6]); acc[7] = fma(d, f3.y, acc[7]);

@@ -24,13 +24,21 @@
 #define GINT_TILE_ORB 104          // orbitals per group = 13 fragments of 8 (8 atoms x 13 orbitals exactly)
 #define GINT_TILE_FRAG 13
 #define GINT_SEG_COLS 7            // column fragments of one segment
+#ifndef GINT_MMA_WARPS
 #define GINT_MMA_WARPS 12          // warp groups 0,1,2: DMMA consumers, three per SM sub-partition; each owns up to GINT_WARP_BLOCKS blocks
+#endif
                                    // of 2 row fragments x 4 (block 0) or 3 (blocks 1, 2) column fragments of the tile
+#ifndef GINT_WARP_BLOCKS
 #define GINT_WARP_BLOCKS 3
+#endif
 #define GINT_AUX_WARPS 4           // warp group 3: warp 12 = TMA issuer, warps 13, 14 = reducers of gint_rho, warp 15 idle (setmaxnreg works on whole warp groups)
 #define GINT_CTA_THREADS (32 * (GINT_MMA_WARPS + GINT_AUX_WARPS))
+#ifndef GINT_REGS_MMA
 #define GINT_REGS_MMA 152          // registers per thread after setmaxnreg: 384 * 152 + 128 * 56 = 65536
+#endif
+#ifndef GINT_REGS_AUX
 #define GINT_REGS_AUX 56
+#endif
 // orbital values ("Phi") in global memory: one SLOT per (atom group, active cubelet) = [orbital row][8 points] doubles,
 // rows padded to whole fragments, followed by one SIGN ROW (+-0.0 per point: the sign of V there; written by gint_vlocal only).
 // 64 bytes per row = the unit of all Phi offsets
