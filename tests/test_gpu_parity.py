@@ -117,6 +117,31 @@ def test_host_entry_points(torch_cuda):
     assert _rel(rho.numpy(), O.rho(w, D, plist)) <= TOL
 
 
+def test_many_waves_and_chunked_host_copies(torch_cuda, monkeypatch):
+    """A small orbital-value scratch (developer knob GINT_PHI_CAP_MB) cuts cfg1 into many waves, as the headline workload is cut into
+    20: the device path, and the host entry points whose copies of V / rho run in per-wave chunks on a copy stream beside the kernels,
+    must give the same exact results (also with a batch shape whose planes do not line up with the waves)."""
+    from paper_2409_09399_b200.gint import batch_flag
+    torch = torch_cuda
+    w = W.make_workload(1)
+    plist = O.pairs(w)
+    V = W.make_potential(w)
+    D = W.make_density_blocks(w, *plist)
+    H_or, rho_or = O.vlocal(w, V, plist), O.rho(w, D, plist)
+    monkeypatch.setenv("GINT_PHI_CAP_MB", "24")
+    for flags in (0, batch_flag(3, 8, 16)):
+        g = _gint(w, flags)
+        assert g.stats()["n_waves"] >= 8
+        H = g.vlocal(torch.from_numpy(V).cuda()).cpu().numpy()
+        rho = g.rho(torch.from_numpy(D).cuda()).cpu().numpy()
+        H_h = torch.empty(g.n_values, dtype=torch.float64).pin_memory(); rho_h = torch.full((g.n_points,), np.nan, dtype=torch.float64).pin_memory()
+        g.vlocal_host(torch.from_numpy(V).pin_memory(), H_h)
+        g.rho_host(torch.from_numpy(D).pin_memory(), rho_h)
+        g.close()
+        assert _rel(H, H_or) <= TOL and _rel(rho, rho_or) <= TOL
+        assert _rel(H_h.numpy(), H_or) <= TOL and _rel(rho_h.numpy(), rho_or) <= TOL
+
+
 def test_empty_and_single_atom(torch_cuda):
     torch = torch_cuda
     basis = W.make_basis(5.0)
