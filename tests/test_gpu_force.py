@@ -107,3 +107,34 @@ def test_cfg5_mixed_species_sampled_forces(torch_cuda):
 
 def test_cfg4_tbg_headline_sampled_forces(torch_cuda):
     _sampled_forces(torch_cuda, 4, 48)
+
+
+def test_force_many_orbitals_and_crowded_batches(torch_cuda):
+    """A 28-orbital species beside a 4-orbital one (rows of an atom longer than a warp's share; blocks of unequal shape), and the dense
+    diamond cell with rc = 8.5 whose batches hold up to 96 atom images: the force kernel's shared memory grows with the orbitals of a
+    batch -- either it fits and the result is exact, or the call fails loudly with GINT_ERR_UNSUPPORTED (never a wrong result)."""
+    from paper_2409_09399_b200.gint import GintError
+    torch = torch_cuda
+    big = W.make_basis(4.5, shells=((0, 0.8), (0, 0.4), (0, 0.2), (1, 0.7), (1, 0.35), (1, 0.2), (2, 0.6), (2, 0.3), (2, 0.2), (0, 0.12)))
+    small = W.make_basis(4.0, shells=((0, 0.5), (1, 0.4)))
+    basis = W.concat_bases([big, small])
+    rng = np.random.default_rng(31)
+    cell = np.array([[6.0, 0.0, 0.0], [0.5, 5.5, 0.0], [0.0, 0.3, 6.5]])
+    pos = rng.uniform(0, 1, (14, 3)) @ cell
+    species = np.array([0, 0, 1, 0, 1, 0, 0, 1, 0, 0, 1, 0, 0, 1], np.int32)
+    w = W.Workload("many-orbitals", 96, cell, np.array([20, 18, 22], np.int32), species, pos, basis)
+    w0 = W.make_workload(0)
+    wd = W.Workload("dense", 94, w0.cell, np.array([16, 16, 16], np.int32), w0.atom_species, w0.atom_pos, W.make_basis(8.5))
+    ran = 0
+    for wl in (w, wd):
+        pl = O.pairs(wl)
+        V = rng.standard_normal(wl.n_points); D = rng.standard_normal(int(pl[3][-1]))
+        try:
+            F, sigma = _run(torch, wl, V, D)
+        except GintError as e:
+            assert "shared memory" in str(e) or "-2" in str(e)
+            continue
+        F_or, s_or = O.force_stress(wl, V, D, pl)
+        assert _rel(F, F_or) <= TOL and _rel(sigma, s_or) <= TOL
+        ran += 1
+    assert ran >= 1
