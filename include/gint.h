@@ -125,6 +125,30 @@ int gint_rho(gint_ctx* ctx, const double* D_dev, double* rho_dev, void* cuda_str
  * grid batch whose orbitals do not fit the kernel's shared memory (about 800 orbitals per batch). */
 int gint_force_stress(gint_ctx* ctx, const double* V_dev, const double* D_dev, double* F_dev, double* sigma_dev, void* cuda_stream);
 
+/*
+ * gint_force_stress_static -- gint_force_stress for callers that cannot allocate device memory.
+ *
+ * Who needs it: a host code that gave the whole GPU to its own memory arena at start-up (so a cudaMalloc inside a library fails),
+ * a process confined to a fixed MPS / MIG memory slice, or a relaxation loop that cannot tolerate the device-wide stall a
+ * cudaMalloc / cudaFree may cause while its other streams are running.  gint_force_stress does one such allocation (its
+ * 8 * n_values-byte symmetrised copy of D, on the first call); this variant keeps that copy in a fixed array that is part of the
+ * library's own device image instead, and calls no cudaMalloc, cudaFree or other allocating routine.
+ *
+ * Same arguments, same result (to rounding: the floating-point atomics add in a different order from call to call) and same
+ * errors as gint_force_stress, plus:
+ *   - GINT_ERR_UNSUPPORTED when n_values (gint_n_pairs) exceeds GINT_STATIC_SCRATCH_DOUBLES; nothing is enqueued then.
+ *     1,048,576 doubles = 8 MiB: enough for the 8-atom diamond and 72-atom graphene cells of the test suite (0.17 M / 0.82 M
+ *     elements), not for the twisted-bilayer cells.  The array costs that much memory on every GPU that loads libgint.so, used or not.
+ *   - The first call on a device looks up the array's device address and raises the kernel's shared-memory limit.  Make that first
+ *     call outside any stream capture; later calls only enqueue two memsets, two kernels and two event records.
+ *   - One array per device serves all contexts, streams and threads and keeps what the last call left in it.  The call rewrites the
+ *     part it reads, so stale contents are harmless, but two calls that may overlap on the GPU race on it: put them on one stream
+ *     (or order them with events).  gint_force_stress has its own per-context copy and may run beside this one.
+ * gint_force_time reports this call's kernels as well.
+ */
+#define GINT_STATIC_SCRATCH_DOUBLES (1 << 20)
+int gint_force_stress_static(gint_ctx* ctx, const double* V_dev, const double* D_dev, double* F_dev, double* sigma_dev, void* cuda_stream);
+
 /* Device duration (seconds) of the kernels of the LAST gint_force_stress call (CUDA events on the caller's stream); -1 before it. */
 int gint_force_time(gint_ctx* ctx, double* seconds);
 

@@ -18,6 +18,8 @@
 // The batch adds 3 doubles per neighbouring atom and 9 for the stress with red.global.add.f64.
 #include "gint_internal.h"
 
+#include <mutex>
+
 typedef unsigned long long u64;
 namespace {
 
@@ -336,6 +338,79 @@ int gint_launch_force(gint_ctx* c, const double* V, const double* D, double* F, 
     const double omega = c->geom.dV * (double)c->geom.N[0] * c->geom.N[1] * c->geom.N[2];
     k_force_batch<<<(unsigned)c->n_batch_total, GINT_FORCE_THREADS, smem, st>>>(c->geom, c->d_bstart, c->d_bent, c->d_atom_pos, c->d_atom_species,
         c->d_species, c->d_tab, c->d_crow, c->d_ckey, c->d_cpub, c->d_cmir, c->d_poff, V, c->d_dfull, 1.0 / omega, F, sigma);
+    GINT_CUDA(cudaGetLastError());
+    GINT_CUDA(cudaEventRecord(c->ev_force[1], st));
+    c->timed_force = true;
+    return GINT_OK;
+}
+
+// ================================================================================================================================
+// gint_force_stress_static -- the same two kernels as gint_force_stress, for callers that must not allocate device memory.
+//
+// gint_force_stress needs one piece of scratch: Dfull = D + mirror^T in the pair-list layout (8 * n_values bytes), which it obtains
+// with cudaMalloc on its first call.  Some callers cannot afford that call: a DFT driver that handed the whole device to its own
+// arena at start-up (a cudaMalloc then fails although "its" memory is free), a job inside a fixed-size MPS / MIG memory slice, or an
+// ionic-step loop that must not hit cudaMalloc's device-wide synchronisation while other streams are busy.  For them the scratch
+// lives in the library image itself: the array below is part of libgint.so's device data, so every GPU on which the library's
+// module gets loaded holds these GINT_STATIC_SCRATCH_DOUBLES * 8 bytes = 8 MiB until the process exits, whether or not this entry
+// point is ever called.  That is why the limit is small; systems beyond it use gint_force_stress.
+//
+// The array is shared by every context and every call on a device, and nothing serialises them: two calls that can run at the same
+// time on the GPU (two streams, two contexts, two host threads) overwrite each other's Dfull.  Order such calls on one stream.
+// Nothing in it has to start at zero: k_sym_full writes every element of [0, n_values) before k_force_batch reads any of them, so
+// the previous call's contents (another geometry's, perhaps) are never seen.  F and sigma, the outputs, are cleared as usual.
+static __device__ __align__(256) double g_dfull_static[GINT_STATIC_SCRATCH_DOUBLES];
+
+namespace {
+// Per-device set-up, done by the first call on that device: in host code `g_dfull_static` names a host-side shadow of the symbol,
+// not device memory, so the address the kernels get has to come from cudaGetSymbolAddress (asked with that device current).
+struct StaticSetup { bool done = false; double* dfull = nullptr; int smem_optin = 0; };
+constexpr int kMaxDevices = 64;
+StaticSetup g_static_setup[kMaxDevices];
+std::mutex g_static_mutex;
+
+int static_setup(int device, const StaticSetup** out) {
+    if (device < 0 || device >= kMaxDevices) GINT_FAIL(GINT_ERR_UNSUPPORTED, "gint_force_stress_static: device ordinal %d (supported: 0..%d)", device, kMaxDevices - 1);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticSetup& s = g_static_setup[device];
+    if (!s.done) {
+        GINT_CUDA(cudaSetDevice(device));
+        void* p = nullptr;
+        GINT_CUDA(cudaGetSymbolAddress(&p, g_dfull_static));
+        if (!p || ((uintptr_t)p & 255)) GINT_FAIL(GINT_ERR_CUDA, "gint_force_stress_static: bad address %p for the static scratch", p);
+        GINT_CUDA(cudaDeviceGetAttribute(&s.smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device));
+        GINT_CUDA(cudaFuncSetAttribute(k_force_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, s.smem_optin));
+        s.dfull = static_cast<double*>(p);
+        s.done = true;
+    }
+    *out = &s;
+    return GINT_OK;
+}
+}  // namespace
+
+extern "C" int gint_force_stress_static(gint_ctx* c, const double* V_dev, const double* D_dev, double* F_dev, double* sigma_dev, void* stream) {
+    if (!c) GINT_FAIL(GINT_ERR_BAD_STATE, "NULL context");
+    if (!V_dev || (!D_dev && c->n_values) || (!F_dev && c->n_atoms)) GINT_FAIL(GINT_ERR_INVALID_ARG, "NULL device pointer");
+    if (((uintptr_t)V_dev | (uintptr_t)D_dev | (uintptr_t)F_dev | (uintptr_t)sigma_dev) & 7) GINT_FAIL(GINT_ERR_INVALID_ARG, "device pointers must be 8-byte aligned");
+    if (c->n_values > (long long)GINT_STATIC_SCRATCH_DOUBLES)
+        GINT_FAIL(GINT_ERR_UNSUPPORTED, "gint_force_stress_static: the pair list holds %lld matrix elements, the static scratch %lld "
+                  "(GINT_STATIC_SCRATCH_DOUBLES); use gint_force_stress, which allocates its own", c->n_values, (long long)GINT_STATIC_SCRATCH_DOUBLES);
+    DeviceGuard guard;
+    const StaticSetup* s = nullptr;
+    if (int rc = static_setup(c->device, &s)) return rc;
+    GINT_CUDA(cudaSetDevice(c->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    GINT_CUDA(cudaMemsetAsync(F_dev, 0, sizeof(double) * 3 * (size_t)c->n_atoms, st));
+    if (sigma_dev) GINT_CUDA(cudaMemsetAsync(sigma_dev, 0, sizeof(double) * 9, st));
+    if (c->n_batch == 0 || c->n_values == 0) return GINT_OK;
+    const size_t smem = gint_force_smem(c);
+    if (smem > (size_t)s->smem_optin) GINT_FAIL(GINT_ERR_UNSUPPORTED, "gint_force_stress_static: a batch of %d orbitals needs %zu bytes of shared memory", c->geom.max_cols, smem);
+    GINT_CUDA(cudaEventRecord(c->ev_force[0], st));
+    k_sym_full<<<(unsigned)((c->n_pairs + 7) / 8), 256, 0, st>>>(c->n_pairs, c->d_poff, c->d_pcanon, c->d_pflag, c->d_cpub, c->d_cmir, c->d_pnA, D_dev, s->dfull);
+    GINT_CUDA(cudaGetLastError());
+    const double omega = c->geom.dV * (double)c->geom.N[0] * c->geom.N[1] * c->geom.N[2];
+    k_force_batch<<<(unsigned)c->n_batch_total, GINT_FORCE_THREADS, smem, st>>>(c->geom, c->d_bstart, c->d_bent, c->d_atom_pos, c->d_atom_species,
+        c->d_species, c->d_tab, c->d_crow, c->d_ckey, c->d_cpub, c->d_cmir, c->d_poff, V_dev, s->dfull, 1.0 / omega, F_dev, sigma_dev);
     GINT_CUDA(cudaGetLastError());
     GINT_CUDA(cudaEventRecord(c->ev_force[1], st));
     c->timed_force = true;

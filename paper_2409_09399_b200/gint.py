@@ -21,8 +21,11 @@ STAT_NAMES = ("n_batch", "n_batch_empty", "batch_bx", "batch_by", "batch_bz", "n
               "n_waves", "n_tiles", "tune_us")
 
 EXPORTS = ("gint_init", "gint_n_orb", "gint_n_pairs", "gint_get_pairs", "gint_vlocal", "gint_rho", "gint_vlocal_host",
-           "gint_rho_host", "gint_force_stress", "gint_force_time", "gint_tune_report", "gint_stats", "gint_kernel_times", "gint_phase_times", "gint_fp64_peak",
+           "gint_rho_host", "gint_force_stress", "gint_force_stress_static", "gint_force_time", "gint_tune_report", "gint_stats", "gint_kernel_times", "gint_phase_times", "gint_fp64_peak",
            "gint_free", "gint_last_error")
+
+
+STATIC_SCRATCH_DOUBLES = 1 << 20      # GINT_STATIC_SCRATCH_DOUBLES of include/gint.h
 
 
 class GintError(RuntimeError):
@@ -174,6 +177,20 @@ class Gint:
         sigma = torch.empty((3, 3), dtype=torch.float64, device=V.device) if stress else None
         _check(lib().gint_force_stress(self._ctx, C.c_void_p(V.data_ptr()), C.c_void_p(D.data_ptr()), C.c_void_p(F.data_ptr()),
                                        C.c_void_p(sigma.data_ptr()) if stress else None, self._stream()))
+        return F, sigma
+
+    def force_stress_static(self, V, D, stress: bool = True):
+        """gint_force_stress_static: the same F and sigma as force_stress(), for users who cannot let the library allocate device memory
+        (all memory held by their own pool, a fixed MPS / MIG slice, no tolerance for cudaMalloc's device-wide stall).  The library's
+        only scratch, the symmetrised copy of D, then sits in a fixed 8 MiB array inside libgint.so: n_values <= STATIC_SCRATCH_DOUBLES
+        or GintError.  F and sigma are still torch tensors created here -- pass-through callers of the C ABI bring their own."""
+        import torch
+        self._dev_check(V, self.n_points, "V")
+        self._dev_check(D, self.n_values, "D")
+        F = torch.empty((self.n_atoms, 3), dtype=torch.float64, device=V.device)
+        sigma = torch.empty((3, 3), dtype=torch.float64, device=V.device) if stress else None
+        _check(lib().gint_force_stress_static(self._ctx, C.c_void_p(V.data_ptr()), C.c_void_p(D.data_ptr()), C.c_void_p(F.data_ptr()),
+                                              C.c_void_p(sigma.data_ptr()) if stress else None, self._stream()))
         return F, sigma
 
     def force_time(self) -> float:
