@@ -45,9 +45,18 @@ typedef enum gint_status {
  * 0 = choose automatically: 8x8x16 points, or the largest smaller shape whose batches have at most 96 neighbouring atom
  * images (PAPER.md:165 uses batches of 27..1000 points; Table 3 sweeps 125..512).  A larger edge is GINT_ERR_UNSUPPORTED. */
 /* GINT_FLAG_TUNE (with no batch-edge field set): gint_init times gint_vlocal + gint_rho for several grid-batch shapes on a slab of the
- * mesh of fixed size and keeps the fastest (the paper's online auto-tuning; there over GEMM tile sizes, here over
- * the grid-batch shape, the parameter its Table 3 sweeps by hand).  gint_tune_report tells what was tried. */
+ * mesh of fixed size (the paper's online auto-tuning; there over GEMM tile sizes, here over the grid-batch shape,
+ * the parameter its Table 3 sweeps by hand).  Each shape's time is the least of three runs after a warm-up run.  The default
+ * 8x8x16 is kept unless the fastest other shape beats it by more than 2 %, so that timing noise does not flip the choice (and with
+ * it memory use and summation order) from run to run.  A shape that cannot be built or run is skipped (reported as -1); if the
+ * tuner's own buffers (two slabs of the mesh, 2 * n_values doubles) cannot be allocated, gint_init goes on untuned instead of failing.
+ * gint_tune_report tells what was tried. */
 #define GINT_FLAG_TUNE (1ull << 32)
+/* GINT_FLAG_PHI_CAP_MB(mb), mb = 1..1048575: upper bound, in MiB, of the context's orbital-value scratch (the buffer one "wave" of grid
+ * batches is evaluated into before it is contracted; GINT_STAT_PHI_SCRATCH_BYTES, GINT_STAT_N_WAVES).  0 = automatic: the smaller of
+ * 16 GiB and a quarter of the device memory free at gint_init.  A smaller cap trades memory for more, shorter waves; a batch shape
+ * whose single largest batch exceeds the cap counts as "does not fit" and the next smaller shape is tried. */
+#define GINT_FLAG_PHI_CAP_MB(mb) (((unsigned long long)(mb) & 0xfffffull) << 40)
 #define GINT_FLAG_BATCH(bx, by, bz) ((unsigned long long)(bx) | ((unsigned long long)(by) << 8) | ((unsigned long long)(bz) << 16))
 
 /*
@@ -192,10 +201,12 @@ int gint_stats(gint_ctx* ctx, long long* out);
  * on the tuning slab, or -1 if the shape did not fit}; *n_rows = rows written (0 when gint_init ran without GINT_FLAG_TUNE). */
 int gint_tune_report(const gint_ctx* ctx, int max_rows, double* out, int* n_rows);
 
-/* Device durations (seconds) of the dominant kernels in the LAST gint_vlocal / gint_rho call on this context,
- * measured with CUDA events recorded on the caller's stream immediately before and after the kernel.
- * Synchronises on those events.  out[0] = vlocal contraction kernel, out[1] = rho contraction kernel; an entry
- * is -1 when that call has not been made yet. */
+/* Device durations (seconds) of the LAST gint_vlocal / gint_rho call on this context, between two CUDA events recorded on the
+ * caller's stream: one before the first wave's orbital-evaluation kernel, one after the last wave's tile-contraction kernel.  The
+ * span therefore covers the evaluation and contraction kernels of every wave and, for the *_host forms, the time the stream waits
+ * for a wave's chunk of V to arrive; it leaves out the clearing memset, the symmetrisation of D (gint_rho) and the expansion of the
+ * canonical blocks into H (gint_vlocal).  Synchronises on those events.  out[0] = gint_vlocal, out[1] = gint_rho; an entry is -1 when
+ * that call has not been made yet. */
 int gint_kernel_times(gint_ctx* ctx, double out[2]);
 
 /* The same, split by kernel: out[0] / out[1] = orbital-evaluation kernels / tile-contraction kernels (summed over the waves) of the

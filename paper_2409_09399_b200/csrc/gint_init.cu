@@ -257,23 +257,41 @@ __global__ void __launch_bounds__(256) k_scan_apply(const int* __restrict__ in, 
     if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 255) out[n] = (int)o;
 }
 
+// Device temporaries of the init passes: released on every way out of the scope, the early returns of GINT_CUDA / GINT_FAIL included.
+template <class T> struct DevTmp {
+    T* p = nullptr;
+    DevTmp() = default;
+    DevTmp(const DevTmp&) = delete;
+    DevTmp& operator=(const DevTmp&) = delete;
+    ~DevTmp() { reset(); }
+    cudaError_t alloc(size_t n) { reset(); return cudaMalloc((void**)&p, sizeof(T) * (n ? n : 1)); }
+    void reset() { if (p) { cudaFree(p); p = nullptr; } }
+    operator T*() const { return p; }
+};
+struct EventTmp {
+    cudaEvent_t e = nullptr;
+    ~EventTmp() { if (e) cudaEventDestroy(e); }
+    cudaError_t create() { return cudaEventCreate(&e); }
+    operator cudaEvent_t() const { return e; }
+};
+
 // out[0..n] = exclusive scan of in[0..n); block sums are scanned on the host (n/1024 values).
 int gint_device_excl_scan(const int* d_in, long long n, int* d_out, long long* total) {
     int nblk = (int)((n + 1023) / 1024);
     if (nblk == 0) { int z = 0; GINT_CUDA(cudaMemcpy(d_out, &z, sizeof(int), cudaMemcpyHostToDevice)); *total = 0; return GINT_OK; }
-    int* d_sums; long long* d_off;
-    GINT_CUDA(cudaMalloc(&d_sums, sizeof(int) * nblk));
-    GINT_CUDA(cudaMalloc(&d_off, sizeof(long long) * nblk));
+    DevTmp<int> d_sums; DevTmp<long long> d_off;
+    GINT_CUDA(d_sums.alloc(nblk));
+    GINT_CUDA(d_off.alloc(nblk));
     k_scan_block_sums<<<nblk, 256>>>(d_in, n, d_sums);
     std::vector<int> hs(nblk); std::vector<long long> ho(nblk);
     GINT_CUDA(cudaMemcpy(hs.data(), d_sums, sizeof(int) * nblk, cudaMemcpyDeviceToHost));
     long long acc = 0;
     for (int i = 0; i < nblk; i++) { ho[i] = acc; acc += hs[i]; }
-    if (acc > 2000000000LL) { cudaFree(d_sums); cudaFree(d_off); GINT_FAIL(GINT_ERR_UNSUPPORTED, "neighbour table has %lld entries (> 2e9)", acc); }
+    if (acc > 2000000000LL) GINT_FAIL(GINT_ERR_UNSUPPORTED, "neighbour table has %lld entries (> 2e9)", acc);
     GINT_CUDA(cudaMemcpy(d_off, ho.data(), sizeof(long long) * nblk, cudaMemcpyHostToDevice));
     k_scan_apply<<<nblk, 256>>>(d_in, n, d_off, d_out);
     GINT_CUDA(cudaGetLastError());
-    GINT_CUDA(cudaFree(d_sums)); GINT_CUDA(cudaFree(d_off));
+    GINT_CUDA(cudaDeviceSynchronize());     // the temporaries go out of scope here
     *total = acc;
     return GINT_OK;
 }
@@ -373,7 +391,7 @@ static int build_basis(gint_ctx* c, int n_species, const int* n_shell, const int
 static int build_pairs(gint_ctx* c) {
     const int n = c->n_atoms;
     Geom& g = c->geom;
-    int* d_cnt; GINT_CUDA(cudaMalloc(&d_cnt, sizeof(int) * (n ? n : 1)));
+    DevTmp<int> d_cnt; GINT_CUDA(d_cnt.alloc(n));
     if (n > 0) k_pairs<false><<<n, 256>>>(g, n, c->d_atom_pos, c->d_atom_species, c->d_species, d_cnt, nullptr, nullptr, nullptr);
     GINT_CUDA(cudaGetLastError());
     std::vector<int> cnt(n);
@@ -382,10 +400,10 @@ static int build_pairs(gint_ctx* c) {
     for (int i = 0; i < n; i++) rs[i + 1] = rs[i] + cnt[i];
     const long long np = rs[n];
     if (np > 2000000000LL) GINT_FAIL(GINT_ERR_UNSUPPORTED, "%lld pair keys (> 2e9)", np);
-    long long* d_rs; int *d_pB, *d_pR;
-    GINT_CUDA(cudaMalloc(&d_rs, sizeof(long long) * (n + 1)));
-    GINT_CUDA(cudaMalloc(&d_pB, sizeof(int) * (np ? np : 1)));
-    GINT_CUDA(cudaMalloc(&d_pR, sizeof(int) * 3 * (np ? np : 1)));
+    DevTmp<long long> d_rs; DevTmp<int> d_pB, d_pR;
+    GINT_CUDA(d_rs.alloc(n + 1));
+    GINT_CUDA(d_pB.alloc(np));
+    GINT_CUDA(d_pR.alloc(3 * np));
     GINT_CUDA(cudaMemcpy(d_rs, rs.data(), sizeof(long long) * (n + 1), cudaMemcpyHostToDevice));
     if (n > 0) k_pairs<true><<<n, 256>>>(g, n, c->d_atom_pos, c->d_atom_species, c->d_species, d_cnt, d_rs, d_pB, d_pR);
     GINT_CUDA(cudaGetLastError());
@@ -395,7 +413,7 @@ static int build_pairs(gint_ctx* c) {
         GINT_CUDA(cudaMemcpy(c->h_pB.data(), d_pB, sizeof(int) * np, cudaMemcpyDeviceToHost));
         GINT_CUDA(cudaMemcpy(c->h_pR.data(), d_pR, sizeof(int) * 3 * np, cudaMemcpyDeviceToHost));
     }
-    cudaFree(d_cnt); cudaFree(d_rs); cudaFree(d_pB); cudaFree(d_pR);
+    d_cnt.reset(); d_rs.reset(); d_pB.reset(); d_pR.reset();
 
     // host bookkeeping: offsets, canonical half, mirror map (integer work on ~1e6 keys)
     int m = 0;
@@ -521,8 +539,8 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, size_t
         }
     }
     const int n_img = (int)img.size();
-    ImageDev* d_img = nullptr;
-    GINT_CUDA(cudaMalloc(&d_img, sizeof(ImageDev) * (n_img ? n_img : 1)));
+    DevTmp<ImageDev> d_img;
+    GINT_CUDA(d_img.alloc(n_img));
     if (n_img) GINT_CUDA(cudaMemcpy(d_img, img.data(), sizeof(ImageDev) * n_img, cudaMemcpyHostToDevice));
 
     // stage A: coarse cells of about 16 x 16 x 8 points
@@ -530,23 +548,22 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, size_t
     const int nc[3] = {(g.nb[0] + cb[0] - 1) / cb[0], (g.nb[1] + cb[1] - 1) / cb[1], (g.nb[2] + cb[2] - 1) / cb[2]};
     const long long ncell = (long long)nc[0] * nc[1] * nc[2];
     int cap = 256;
-    int *d_cand = nullptr, *d_ccount = nullptr;
-    GINT_CUDA(cudaMalloc(&d_ccount, sizeof(int) * ncell));
+    DevTmp<int> d_cand, d_ccount;
+    GINT_CUDA(d_ccount.alloc(ncell));
     for (;;) {
-        GINT_CUDA(cudaMalloc(&d_cand, sizeof(int) * ncell * cap));
+        GINT_CUDA(d_cand.alloc((size_t)ncell * cap));
         k_coarse_candidates<<<(unsigned)ncell, 256>>>(g, cb[0], cb[1], cb[2], nc[0], nc[1], nc[2], n_img, d_img, cap, d_cand, d_ccount);
         GINT_CUDA(cudaGetLastError());
         std::vector<int> cc(ncell);
         GINT_CUDA(cudaMemcpy(cc.data(), d_ccount, sizeof(int) * ncell, cudaMemcpyDeviceToHost));
         int mx = 0; for (long long i = 0; i < ncell; i++) mx = std::max(mx, cc[i]);
         if (mx <= cap) break;
-        cudaFree(d_cand); d_cand = nullptr;
         cap = ((mx + 63) / 64) * 64;
     }
     // stage B: count, scan, fill
-    int *d_count = nullptr, *d_cols = nullptr;
-    GINT_CUDA(cudaMalloc(&d_count, sizeof(int) * nbt));
-    GINT_CUDA(cudaMalloc(&d_cols, sizeof(int) * nbt));
+    DevTmp<int> d_count, d_cols;
+    GINT_CUDA(d_count.alloc(nbt));
+    GINT_CUDA(d_cols.alloc(nbt));
     const unsigned gridB = (unsigned)((nbt + 7) / 8);
     k_batch_neighbours<false><<<gridB, 256>>>(g, cb[0], cb[1], cb[2], nc[1], nc[2], d_img, cap, d_cand, d_ccount, nbt, d_count, d_cols,
                                               c->d_species, c->d_atom_species, nullptr, nullptr, nullptr);
@@ -558,7 +575,7 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, size_t
     for (long long b = 0; b < nbt; b++) { max_nb = std::max(max_nb, count[b]); max_cols = std::max(max_cols, cols[b]); }
     g.max_nb = std::max(max_nb, 1); g.max_cols = std::max(max_cols, 1);
     const bool ok = max_nb <= GINT_MAX_NB && gint_smem_needed(c, smem_limit) <= smem_limit;     // else: try a smaller batch shape
-    if (!ok) { cudaFree(d_img); cudaFree(d_cand); cudaFree(d_ccount); cudaFree(d_count); cudaFree(d_cols); return GINT_OK; }
+    if (!ok) return GINT_OK;
     *fits = true;
 
     int rc;
@@ -567,9 +584,9 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, size_t
     if ((rc = gint_device_excl_scan(d_count, nbt, c->d_bstart, &n_ent))) return rc;
     c->n_entries = n_ent;
     if ((rc = dev_alloc(c, &c->d_bent, (size_t)n_ent))) return rc;
-    int *d_bgroups = nullptr, *d_tcount = nullptr;
-    GINT_CUDA(cudaMalloc(&d_bgroups, sizeof(int) * nbt));
-    GINT_CUDA(cudaMalloc(&d_tcount, sizeof(int) * nbt));
+    DevTmp<int> d_bgroups, d_tcount;
+    GINT_CUDA(d_bgroups.alloc(nbt));
+    GINT_CUDA(d_tcount.alloc(nbt));
     if ((rc = dev_alloc(c, &c->d_tstart, (size_t)nbt + 1))) return rc;
     if ((rc = dev_alloc(c, &c->d_gstart, (size_t)nbt + 1))) return rc;
     k_batch_neighbours<true><<<gridB, 256>>>(g, cb[0], cb[1], cb[2], nc[1], nc[2], d_img, cap, d_cand, d_ccount, nbt, d_count, d_cols,
@@ -586,10 +603,16 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, size_t
     k_tiles_fill<<<gridT, 256>>>(nbt, d_bgroups, c->d_tstart, c->d_tile);
     GINT_CUDA(cudaGetLastError());
     GINT_CUDA(cudaDeviceSynchronize());
-    cudaFree(d_img); cudaFree(d_cand); cudaFree(d_ccount); cudaFree(d_count); cudaFree(d_cols);
-    cudaFree(d_bgroups); cudaFree(d_tcount);
+    d_img.reset(); d_cand.reset(); d_ccount.reset(); d_count.reset(); d_cols.reset();
+    d_bgroups.reset(); d_tcount.reset();
     // orbital-value ("Phi") layout: offsets of every (batch, group) slot array, waves, scratch buffer
-    if ((rc = gint_build_phi_layout(c, nullptr, phi_cap))) return rc;
+    bool batch_too_big = false;
+    if ((rc = gint_build_phi_layout(c, nullptr, phi_cap, &batch_too_big))) {
+        if (!batch_too_big) return rc;
+        release_batches(c);          // one batch alone overflows the scratch: this shape does not fit, a smaller one may
+        *fits = false;
+        return GINT_OK;
+    }
     if ((rc = gint_build_plans(c))) return rc;
 
     c->padded_macs = 0; c->n_batch = 0;
@@ -653,11 +676,11 @@ static int gint_init_impl(gint_ctx** out, gint_ctx*& c, int n_species, const int
     if ((rc = build_pairs(c))) { return rc; }
 
     const size_t smem_limit = prop.sharedMemPerBlockOptin;
-    // scratch for the orbital values of one wave of batches: at most 16 GiB and a quarter of the free device memory
+    // scratch for the orbital values of one wave of batches: at most 16 GiB and a quarter of the free device memory, or what the caller asks for
     size_t mem_free = 0, mem_total = 0;
     GINT_CUDA(cudaMemGetInfo(&mem_free, &mem_total));
     size_t phi_cap = std::min<size_t>((size_t)16 << 30, mem_free / 4);
-    if (const char* e = getenv("GINT_PHI_CAP_MB")) { const long long mb = atoll(e); if (mb > 0) phi_cap = (size_t)mb << 20; }   // developer knob (tests use it to force several waves)
+    if (const unsigned long long mb = (flags >> 40) & 0xfffffull) phi_cap = (size_t)mb << 20;   // GINT_FLAG_PHI_CAP_MB
     for (auto& e : c->ev) if (cudaEventCreate(&e) != cudaSuccess) { GINT_FAIL(GINT_ERR_CUDA, "cudaEventCreate failed"); }
     for (auto& e : c->ev_force) if (cudaEventCreate(&e) != cudaSuccess) { GINT_FAIL(GINT_ERR_CUDA, "cudaEventCreate failed"); }
     const int fx = (int)(flags & 255), fy = (int)((flags >> 8) & 255), fz = (int)((flags >> 16) & 255);
@@ -669,55 +692,80 @@ static int gint_init_impl(gint_ctx** out, gint_ctx*& c, int n_species, const int
         // size, "no more than two seconds"): every candidate shape is built for a slab of the mesh (about GINT_TUNE_BATCHES batches,
         // whole batch planes along a1), gint_vlocal + gint_rho run on it twice with V = 1, D = 1, and the shape with the least time per
         // covered mesh plane is kept.
+        // The first candidate is the untuned default; another shape replaces it only if it wins by GINT_TUNE_MARGIN (the shapes
+        // often lie within 1 % of each other, and the choice also fixes memory, plan size and the order of summation: it should not
+        // flip from run to run on timing noise).  Each candidate's time is the least of GINT_TUNE_REPS runs after one warm-up run.
+        // A candidate that cannot be built or run is recorded with -1 and skipped; if the tuning buffers themselves cannot be
+        // allocated, init goes on untuned.
         static const int cand[][3] = {{8, 8, 16}, {8, 8, 8}, {4, 8, 16}, {4, 4, 16}, {4, 4, 8}};
         const auto t_begin = std::chrono::steady_clock::now();
-        const size_t npts = (size_t)mesh[0] * mesh[1] * mesh[2];
-        double *d_V = nullptr, *d_rho = nullptr, *d_D = nullptr, *d_H = nullptr;
-        GINT_CUDA(cudaMalloc(&d_V, sizeof(double) * npts)); GINT_CUDA(cudaMalloc(&d_rho, sizeof(double) * npts));
-        GINT_CUDA(cudaMalloc(&d_D, sizeof(double) * (size_t)std::max<long long>(c->n_values, 1))); GINT_CUDA(cudaMalloc(&d_H, sizeof(double) * (size_t)std::max<long long>(c->n_values, 1)));
-        {   // 1.0 everywhere (an exact zero would be skipped by the flush of gint_vlocal)
+        const size_t plane = (size_t)mesh[1] * mesh[2];
+        // the same slab of the mesh for every candidate: the planes that GINT_TUNE_BATCHES batches of the largest shape cover
+        const long long per_plane16 = (long long)((mesh[1] + 7) / 8) * ((mesh[2] + 15) / 16);
+        const int planes16 = std::max(2, (int)((GINT_TUNE_BATCHES + per_plane16 - 1) / per_plane16));
+        int crop[sizeof(cand) / sizeof(cand[0])], slab = 0;
+        for (size_t k = 0; k < sizeof(cand) / sizeof(cand[0]); k++) {
+            const int bs0 = std::min(cand[k][0], mesh[0]);
+            crop[k] = std::max(1, planes16 * 8 / bs0);
+            slab = std::max(slab, std::min(mesh[0], crop[k] * bs0));
+        }
+        DevTmp<double> d_V, d_rho, d_D, d_H;
+        EventTmp e0, e1;
+        const size_t nval = (size_t)std::max<long long>(c->n_values, 1);
+        c->tune.clear();
+        bool have_buffers = d_V.alloc(slab * plane) == cudaSuccess && d_rho.alloc(slab * plane) == cudaSuccess && d_D.alloc(nval) == cudaSuccess &&
+                            d_H.alloc(nval) == cudaSuccess && e0.create() == cudaSuccess && e1.create() == cudaSuccess;
+        if (!have_buffers) cudaGetLastError();      // out of memory for the tuner is not an error of gint_init
+        if (have_buffers) {   // 1.0 everywhere (an exact zero would be skipped by the flush of gint_vlocal)
             std::vector<double> ones(1 << 20, 1.0);
-            for (size_t o = 0; o < npts; o += ones.size()) GINT_CUDA(cudaMemcpy(d_V + o, ones.data(), sizeof(double) * std::min(ones.size(), npts - o), cudaMemcpyHostToDevice));
+            for (size_t o = 0; o < slab * plane; o += ones.size()) GINT_CUDA(cudaMemcpy(d_V + o, ones.data(), sizeof(double) * std::min(ones.size(), slab * plane - o), cudaMemcpyHostToDevice));
             for (size_t o = 0; o < (size_t)c->n_values; o += ones.size()) GINT_CUDA(cudaMemcpy(d_D + o, ones.data(), sizeof(double) * std::min(ones.size(), (size_t)c->n_values - o), cudaMemcpyHostToDevice));
         }
-        cudaEvent_t e0, e1;
-        GINT_CUDA(cudaEventCreate(&e0)); GINT_CUDA(cudaEventCreate(&e1));
-        double best = 0.0;
-        c->tune.clear();
-        for (auto& s : cand) {
-            const int nby = (mesh[1] + std::min(s[1], mesh[1]) - 1) / std::min(s[1], mesh[1]), nbz = (mesh[2] + std::min(s[2], mesh[2]) - 1) / std::min(s[2], mesh[2]);
-            // the same slab of the mesh for every candidate: the planes that GINT_TUNE_BATCHES batches of the largest shape cover
-            const int planes16 = std::max(2, (int)((GINT_TUNE_BATCHES + (long long)((mesh[1] + 7) / 8) * ((mesh[2] + 15) / 16) - 1) / ((long long)((mesh[1] + 7) / 8) * ((mesh[2] + 15) / 16))));
-            const int crop = std::max(1, planes16 * 8 / std::min(s[0], mesh[0]));
-            (void)nby; (void)nbz;
-            if ((rc = build_batches(c, s, smem_limit, phi_cap, &fits, crop))) { cudaFree(d_V); cudaFree(d_rho); cudaFree(d_D); cudaFree(d_H); return rc; }
+        for (size_t k = 0; have_buffers && k < sizeof(cand) / sizeof(cand[0]); k++) {
+            const int* s = cand[k];
             gint_ctx::TuneResult tr; tr.bs[0] = s[0]; tr.bs[1] = s[1]; tr.bs[2] = s[2]; tr.ns_per_point = -1.0;
-            if (fits && c->n_tiles > 0) {
+            c->rho_planes = slab;                   // gint_rho clears only the slab while tuning
+            int trc = build_batches(c, s, smem_limit, phi_cap, &fits, crop[k]);
+            if (trc == GINT_OK && fits && c->n_tiles > 0) {
                 c->smem_bytes = gint_smem_needed(c, smem_limit);
-                if ((rc = gint_configure_kernels(c))) return rc;
-                float ms = 0.f;
-                for (int rep = 0; rep < 2; rep++) {
+                trc = gint_configure_kernels(c);
+                float ms_best = -1.f;
+                for (int rep = 0; trc == GINT_OK && rep < 1 + GINT_TUNE_REPS; rep++) {
                     cudaEventRecord(e0, 0);
-                    if ((rc = gint_launch_vlocal(c, d_V, d_H, 0)) || (rc = gint_launch_rho(c, d_D, d_rho, 0))) return rc;
+                    if ((trc = gint_launch_vlocal(c, d_V, d_H, 0)) || (trc = gint_launch_rho(c, d_D, d_rho, 0))) break;
                     cudaEventRecord(e1, 0);
-                    if (cudaEventSynchronize(e1) != cudaSuccess) GINT_FAIL(GINT_ERR_CUDA, "tuner: %s", cudaGetErrorString(cudaGetLastError()));
-                    cudaEventElapsedTime(&ms, e0, e1);
+                    float ms = 0.f;
+                    if (cudaEventSynchronize(e1) != cudaSuccess || cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess) { trc = GINT_ERR_CUDA; break; }
+                    if (rep > 0 && (ms_best < 0.f || ms < ms_best)) ms_best = ms;
                 }
-                const double pts = (double)std::min(mesh[0], c->geom.nb[0] * c->geom.bs[0]) * mesh[1] * mesh[2];
-                tr.ns_per_point = 1e6 * ms / pts;
-                if (best == 0.0 || tr.ns_per_point < best) { best = tr.ns_per_point; tuned[0] = s[0]; tuned[1] = s[1]; tuned[2] = s[2]; }
+                if (trc == GINT_OK && ms_best >= 0.f)
+                    tr.ns_per_point = 1e6 * ms_best / ((double)std::min(mesh[0], c->geom.nb[0] * c->geom.bs[0]) * mesh[1] * mesh[2]);
+            }
+            if (trc != GINT_OK) {
+                // a sticky device error cannot be skipped; anything else (out of memory, unsupported shape) only drops this candidate
+                cudaGetLastError();
+                if (cudaDeviceSynchronize() != cudaSuccess) { c->rho_planes = 0; GINT_FAIL(GINT_ERR_CUDA, "tuner: %s", cudaGetErrorString(cudaGetLastError())); }
             }
             c->tune.push_back(tr);
-            if (fits) release_batches(c);
+            release_batches(c);
             c->timed[0] = c->timed[1] = false;
         }
-        cudaEventDestroy(e0); cudaEventDestroy(e1);
-        cudaFree(d_V); cudaFree(d_rho); cudaFree(d_D); cudaFree(d_H);
+        c->rho_planes = 0;
+        {   // the default (first row) stays unless the fastest other shape beats it by the margin
+            int kb = -1;
+            for (size_t k = 1; k < c->tune.size(); k++) if (c->tune[k].ns_per_point > 0 && (kb < 0 || c->tune[k].ns_per_point < c->tune[kb].ns_per_point)) kb = (int)k;
+            const double t_default = c->tune.empty() ? -1.0 : c->tune[0].ns_per_point;
+            if (t_default > 0 && !(kb >= 0 && c->tune[kb].ns_per_point < t_default * (1.0 - GINT_TUNE_MARGIN))) kb = 0;
+            if (kb >= 0) { tuned[0] = c->tune[kb].bs[0]; tuned[1] = c->tune[kb].bs[1]; tuned[2] = c->tune[kb].bs[2]; }
+        }
         c->tune_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
         fits = false;
     }
-    if (fx || fy || fz || tuned[0]) {
-        const int bs[3] = {tuned[0] ? tuned[0] : (fx ? fx : 8), tuned[0] ? tuned[1] : (fy ? fy : 8), tuned[0] ? tuned[2] : (fz ? fz : 8)};
+    // the tuned shape was timed on a slab; should the whole mesh not fit it, the untuned ladder below takes over
+    if (tuned[0] && (rc = build_batches(c, tuned, smem_limit, phi_cap, &fits))) { return rc; }
+    if (fits) {
+    } else if (fx || fy || fz) {
+        const int bs[3] = {fx ? fx : 8, fy ? fy : 8, fz ? fz : 8};
         if ((rc = build_batches(c, bs, smem_limit, phi_cap, &fits))) { return rc; }
         if (!fits) { GINT_FAIL(GINT_ERR_UNSUPPORTED, "requested batch %dx%dx%d needs more shared memory than %zu bytes (or > %d neighbours)", bs[0], bs[1], bs[2], smem_limit, GINT_MAX_NB); }
     } else {
@@ -794,6 +842,7 @@ extern "C" int gint_get_pairs(const gint_ctx* ctx, int* A, int* B, int* R3, long
 extern "C" int gint_stats(gint_ctx* ctx, long long* out) {
     if (!ctx) GINT_FAIL(GINT_ERR_BAD_STATE, "NULL context");
     if (!out) GINT_FAIL(GINT_ERR_INVALID_ARG, "NULL output");
+    DeviceGuard guard;
     if (!ctx->have_alg) { int rc = gint_launch_alg_stats(ctx); if (rc) return rc; }
     const Geom& g = ctx->geom;
     out[GINT_STAT_N_BATCH] = ctx->n_batch; out[GINT_STAT_N_BATCH_EMPTY] = ctx->n_batch_empty;
@@ -814,6 +863,7 @@ extern "C" int gint_stats(gint_ctx* ctx, long long* out) {
 extern "C" int gint_kernel_times(gint_ctx* ctx, double out[2]) {
     if (!ctx) GINT_FAIL(GINT_ERR_BAD_STATE, "NULL context");
     if (!out) GINT_FAIL(GINT_ERR_INVALID_ARG, "NULL output");
+    DeviceGuard guard;
     GINT_CUDA(cudaSetDevice(ctx->device));
     for (int k = 0; k < 2; k++) {
         out[k] = -1.0;
@@ -829,6 +879,7 @@ extern "C" int gint_kernel_times(gint_ctx* ctx, double out[2]) {
 extern "C" int gint_phase_times(gint_ctx* ctx, double out[4]) {
     if (!ctx) GINT_FAIL(GINT_ERR_BAD_STATE, "NULL context");
     if (!out) GINT_FAIL(GINT_ERR_INVALID_ARG, "NULL output");
+    DeviceGuard guard;
     GINT_CUDA(cudaSetDevice(ctx->device));
     for (int k = 0; k < 2; k++) {
         out[2 * k] = out[2 * k + 1] = -1.0;

@@ -54,6 +54,8 @@
 #define GINT_PLAN_THREADS 96       // k_plan_fill (gint_init)
 #define GINT_EVAL_THREADS 256      // orbital-evaluation kernel
 #define GINT_TUNE_BATCHES 4096     // batches (of the largest shape) in the slab the batch-shape tuner times
+#define GINT_TUNE_REPS 3            // timed runs per candidate shape (after one warm-up run); the least time counts
+#define GINT_TUNE_MARGIN 0.02      // a shape replaces the default 8 x 8 x 16 only if it is this much faster (fraction)
 
 // ---- error plumbing -------------------------------------------------------------------------------
 void gint_set_error(const char* fmt, ...);
@@ -232,6 +234,7 @@ struct gint_ctx {
     double* d_stage_in = nullptr; size_t stage_in_n = 0;
     double* d_stage_out = nullptr; size_t stage_out_n = 0;
     cudaStream_t copy_stream = nullptr;
+    int rho_planes = 0;              // > 0 (batch-shape tuner only): gint_rho clears just the first rho_planes mesh planes along a1
     // gint_force_stress: full-layout copy of D + mirror^T (allocated by the first call), events around its kernels
     double* d_dfull = nullptr;
     cudaEvent_t ev_force[2] = {nullptr, nullptr};
@@ -249,7 +252,7 @@ int gint_launch_force(gint_ctx* c, const double* V, const double* D, double* F, 
 size_t gint_force_smem(const gint_ctx* c);
 int gint_configure_kernels(gint_ctx* c);
 size_t gint_smem_needed(gint_ctx* c, size_t limit);   // also decides tab_in_smem
-int gint_build_phi_layout(gint_ctx* c, const int* d_bgroups, size_t phi_cap_bytes);   // Phi offsets of every (batch, group), waves, scratch
+int gint_build_phi_layout(gint_ctx* c, const int* d_bgroups, size_t phi_cap_bytes, bool* batch_too_big);   // Phi offsets of every (batch, group), waves, scratch
 int gint_build_plans(gint_ctx* c);                    // tile plans (after the Phi layout)
 int gint_device_excl_scan(const int* d_in, long long n, int* d_out, long long* total);   // gint_init.cu
 

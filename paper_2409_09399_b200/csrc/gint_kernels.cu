@@ -702,7 +702,11 @@ __device__ __forceinline__ void issuer_role(const Geom& g, TileSmem& S, const un
         if (lane == 0) ti = atomicAdd(queue, 1);
         ti = __shfl_sync(0xffffffffu, ti, 0);
         if (ti >= n_tiles) {
-            if (lane == 0) { reinterpret_cast<PlanHdr*>(S.plan[c])->valid = 0; mbar_arrive(&S.ctx_full[c]); }
+            if (lane == 0) {
+                reinterpret_cast<PlanHdr*>(S.plan[c])->valid = 0;              // a generic store into a buffer the bulk copies also write
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                mbar_arrive(&S.ctx_full[c]);
+            }
             drained = true;
         } else if (lane == 0) {
             const unsigned o0 = __ldg(planoff + ti), o1 = __ldg(planoff + ti + 1);
@@ -1158,6 +1162,8 @@ k_tiles(Geom g, const unsigned char* __restrict__ plan, const unsigned* __restri
     }
     // the ring starts zeroed: the consumers may read rows of a stage that no copy has written yet (multiplied by zeros: must be finite)
     for (unsigned i = threadIdx.x; i < sizeof(S.ring) / 16; i += GINT_CTA_THREADS) reinterpret_cast<uint4*>(&S.ring[0][0])[i] = make_uint4(0u, 0u, 0u, 0u);
+    // generic-proxy stores above, async-proxy (cp.async.bulk) writes to the same bytes later: order the two proxies
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
     if (warp < GINT_MMA_WARPS) {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" :: "n"(GINT_REGS_MMA));
@@ -1233,8 +1239,9 @@ __global__ void __launch_bounds__(128) k_phi_rows(long long n_batch_total, const
     }
 }
 
-int gint_build_phi_layout(gint_ctx* c, const int* d_bgroups, size_t phi_cap_bytes) {
+int gint_build_phi_layout(gint_ctx* c, const int* d_bgroups, size_t phi_cap_bytes, bool* batch_too_big) {
     (void)d_bgroups;
+    *batch_too_big = false;
     const long long nbt = c->n_batch_total;
     std::vector<int> gs(nbt + 1);
     GINT_CUDA(cudaMemcpy(gs.data(), c->d_gstart, sizeof(int) * (nbt + 1), cudaMemcpyDeviceToHost));
@@ -1263,7 +1270,7 @@ int gint_build_phi_layout(gint_ctx* c, const int* d_bgroups, size_t phi_cap_byte
         unsigned long long rows = 0;
         while (b < nbt) {
             const unsigned long long br = goff[gs[b + 1]] - goff[gs[b]];
-            if (br > cap_rows) GINT_FAIL(GINT_ERR_OUT_OF_MEMORY, "orbital values of one batch (%llu bytes) exceed the scratch buffer", br * GINT_ROW_BYTES);
+            if (br > cap_rows) { *batch_too_big = true; GINT_FAIL(GINT_ERR_OUT_OF_MEMORY, "orbital values of one batch (%llu bytes) exceed the scratch buffer (%zu bytes)", br * GINT_ROW_BYTES, phi_cap_bytes); }
             if (rows + br > cap_rows) break;
             rows += br; b++;
         }
@@ -1461,7 +1468,7 @@ int gint_launch_vlocal(gint_ctx* c, const double* V, double* H, cudaStream_t st,
 
 int gint_launch_rho(gint_ctx* c, const double* D, double* rho, cudaStream_t st, double* rho_host) {
     GINT_CUDA(cudaSetDevice(c->device));
-    const size_t npts = (size_t)c->geom.N[0] * c->geom.N[1] * c->geom.N[2];
+    const size_t npts = (size_t)(c->rho_planes > 0 ? std::min(c->rho_planes, c->geom.N[0]) : c->geom.N[0]) * c->geom.N[1] * c->geom.N[2];
     GINT_CUDA(cudaMemsetAsync(rho, 0, sizeof(double) * npts, st));
     if (c->n_tiles == 0) {
         if (rho_host) GINT_CUDA(cudaMemcpyAsync(rho_host, rho, sizeof(double) * npts, cudaMemcpyDeviceToHost, st));

@@ -66,11 +66,18 @@ def fp64_peak(device: int = 0) -> dict:
     return {"dmma_tflops": float(out[0]), "dfma_tflops": float(out[1]), "sm_mhz": float(out[2]), "n_sm": int(out[3])}
 
 
-FLAG_TUNE = 1 << 32       # gint_init times several grid-batch shapes and keeps the fastest
+FLAG_TUNE = 1 << 32       # gint_init times several grid-batch shapes; the default stays unless another is > 2 % faster
 
 
 def batch_flag(bx: int, by: int, bz: int) -> int:
     return bx | (by << 8) | (bz << 16)
+
+
+def phi_cap_flag(mib: int) -> int:
+    """GINT_FLAG_PHI_CAP_MB: upper bound (MiB) of the context's orbital-value scratch; 0 = automatic."""
+    if not 0 <= mib < (1 << 20):
+        raise ValueError("phi_cap_flag: 0..1048575 MiB")
+    return mib << 40
 
 
 class Gint:

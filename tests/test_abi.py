@@ -60,3 +60,8 @@ def test_batch_flag_packing():
     from paper_2409_09399_b200.gint import batch_flag
     assert batch_flag(8, 4, 2) == 8 | (4 << 8) | (2 << 16)
     assert np.int64(batch_flag(1, 1, 1)) == 0x010101
+    # the fields of the flags word do not overlap (include/gint.h): batch edges 0..23, GINT_FLAG_TUNE bit 32, scratch cap bits 40..59
+    from paper_2409_09399_b200.gint import FLAG_TUNE, phi_cap_flag
+    assert phi_cap_flag(24) == 24 << 40 and phi_cap_flag((1 << 20) - 1) & (FLAG_TUNE | 0xffffff) == 0
+    src = open(os.path.join(ROOT, "include", "gint.h")).read()
+    assert "#define GINT_FLAG_TUNE (1ull << 32)" in src and "0xfffffull) << 40)" in src
