@@ -78,18 +78,20 @@ def test_skew_two_species_force_and_stress(torch_cuda):
     assert none is None and np.abs(F_only - F).max() <= 1e-13 * np.abs(F).max()
 
 
-def _sampled_forces(torch, cfg, n_atoms):
-    """Full-size workload: the forces of a stratified sample of atoms (first, last, random; the oracle computes any atom alone)."""
+def _sampled_forces(torch, cfg, n_atoms, flag_sets=(0,)):
+    """Full-size workload: the forces of a stratified sample of atoms (first, last, random; the oracle computes any atom alone), from
+    the library initialised with each entry of flag_sets (default batch shape, GINT_FLAG_TUNE as bench.py passes it, a forced shape)."""
     w = W.make_workload(cfg)
     pl = O.pairs(w)
     V = W.make_potential(w)
     D = W.make_density_blocks(w, *pl)
     rng = np.random.default_rng([2409, 9399, cfg, 78])
     sel = np.unique(np.concatenate([[0, w.n_atoms - 1], rng.integers(0, w.n_atoms, n_atoms)])).astype(np.int64)
-    F, _ = _run(torch, w, V, D, stress=False)
+    Fs = [_run(torch, w, V, D, flags=flags, stress=False)[0] for flags in flag_sets]
     F_or, _ = O.force_stress(w, V, D, pl, sel=sel)
-    err = float(np.abs(F[sel] - F_or[sel]).max() / np.abs(F).max())
-    assert err <= TOL, f"cfg{cfg} force parity on {len(sel)} atoms {err:.3e}"
+    for flags, F in zip(flag_sets, Fs):
+        err = float(np.abs(F[sel] - F_or[sel]).max() / np.abs(F).max())
+        assert err <= TOL, f"cfg{cfg} flags={flags:#x} force parity on {len(sel)} atoms {err:.3e}"
     # (no net-force check: V carries seeded noise per mesh point, so E is not invariant under a rigid shift of the atoms)
 
 
@@ -106,7 +108,31 @@ def test_cfg5_mixed_species_sampled_forces(torch_cuda):
 
 
 def test_cfg4_tbg_headline_sampled_forces(torch_cuda):
-    _sampled_forces(torch_cuda, 4, 48)
+    """As bench.py initialises the headline workload (GINT_FLAG_TUNE), and with the 4x8x16 shape forced."""
+    from paper_2409_09399_b200.gint import FLAG_TUNE, batch_flag
+    _sampled_forces(torch_cuda, 4, 48, flag_sets=(FLAG_TUNE, batch_flag(4, 8, 16)))
+
+
+def test_dense_multi_group_cell_force_and_all_nine_stress_components(torch_cuda):
+    """64-atom bulk diamond (2 x 2 x 2 cells, rc 7, mesh 67^3: ragged last batches on every axis): the largest dense cell whose full
+    stress the oracle can afford.  Its batches hold several groups of atoms, so the stress (Eq. 5) crosses group
+    boundaries and batch tails here, not only on the few-atom cells; D carries no mirror symmetry.  Two batch shapes."""
+    from paper_2409_09399_b200.gint import Gint, batch_flag
+    cell, pos = W.diamond(2)
+    w = W.Workload("diamond 2x2x2 (64 atoms), rc 7", 97, np.ascontiguousarray(cell), W._mesh_for(cell), np.zeros(len(pos), np.int32),
+                   np.ascontiguousarray(pos), W.make_basis(7.0))
+    pl = O.pairs(w)
+    V = W.make_potential(w)
+    D = W.make_density_blocks(w, *pl) + 0.3 * np.random.default_rng(14).standard_normal(int(pl[3][-1]))
+    g = Gint.from_workload(w)
+    st = g.stats()
+    g.close()
+    assert st["max_nb"] > 8, "the cell is meant to need several atom groups per batch"
+    F_or, s_or = O.force_stress(w, V, D, pl)
+    assert np.abs(s_or).min() > 1e-4 * np.abs(s_or).max()          # all nine components carry signal
+    for flags in (0, batch_flag(4, 8, 16)):
+        F, sigma = _run(torch_cuda, w, V, D, flags=flags)
+        assert _rel(F, F_or) <= TOL and _rel(sigma, s_or) <= TOL, f"flags={flags:#x}"
 
 
 def test_force_many_orbitals_and_crowded_batches(torch_cuda):
@@ -125,7 +151,7 @@ def test_force_many_orbitals_and_crowded_batches(torch_cuda):
     w = W.Workload("many-orbitals", 96, cell, np.array([20, 18, 22], np.int32), species, pos, basis)
     w0 = W.make_workload(0)
     wd = W.Workload("dense", 94, w0.cell, np.array([16, 16, 16], np.int32), w0.atom_species, w0.atom_pos, W.make_basis(8.5))
-    ran = 0
+    ran = []
     for wl in (w, wd):
         pl = O.pairs(wl)
         V = rng.standard_normal(wl.n_points); D = rng.standard_normal(int(pl[3][-1]))
@@ -136,5 +162,6 @@ def test_force_many_orbitals_and_crowded_batches(torch_cuda):
             continue
         F_or, s_or = O.force_stress(wl, V, D, pl)
         assert _rel(F, F_or) <= TOL and _rel(sigma, s_or) <= TOL
-        ran += 1
-    assert ran >= 1
+        ran.append(wl.name)
+    print("gint_force_stress ran on:", ran)
+    assert len(ran) >= 1

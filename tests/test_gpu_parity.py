@@ -117,20 +117,19 @@ def test_host_entry_points(torch_cuda):
     assert _rel(rho.numpy(), O.rho(w, D, plist)) <= TOL
 
 
-def test_many_waves_and_chunked_host_copies(torch_cuda, monkeypatch):
-    """A small orbital-value scratch (developer knob GINT_PHI_CAP_MB) cuts cfg1 into many waves, as the headline workload is cut into
+def test_many_waves_and_chunked_host_copies(torch_cuda):
+    """A small orbital-value scratch (GINT_FLAG_PHI_CAP_MB of gint_init) cuts cfg1 into many waves, as the headline workload is cut into
     20: the device path, and the host entry points whose copies of V / rho run in per-wave chunks on a copy stream beside the kernels,
     must give the same exact results (also with a batch shape whose planes do not line up with the waves)."""
-    from paper_2409_09399_b200.gint import batch_flag
+    from paper_2409_09399_b200.gint import batch_flag, phi_cap_flag
     torch = torch_cuda
     w = W.make_workload(1)
     plist = O.pairs(w)
     V = W.make_potential(w)
     D = W.make_density_blocks(w, *plist)
     H_or, rho_or = O.vlocal(w, V, plist), O.rho(w, D, plist)
-    monkeypatch.setenv("GINT_PHI_CAP_MB", "24")
     for flags in (0, batch_flag(3, 8, 16)):
-        g = _gint(w, flags)
+        g = _gint(w, flags | phi_cap_flag(24))
         assert g.stats()["n_waves"] >= 8
         H = g.vlocal(torch.from_numpy(V).cuda()).cpu().numpy()
         rho = g.rho(torch.from_numpy(D).cuda()).cpu().numpy()
@@ -226,52 +225,70 @@ def _stratified_keys(w, plist, rng, n_uniform):
     return np.unique(np.concatenate(parts)).astype(np.int64)
 
 
-def _sampled_parity(torch, cfg, n_keys, n_pts):
+def _sampled_parity(torch, cfg, n_keys, n_pts, flag_sets=(0,), seed_extra=None):
+    """One oracle evaluation, compared with the library run once per entry of flag_sets (gint_init flags: the default batch shape,
+    GINT_FLAG_TUNE as bench.py passes it, a forced shape).  The sampled mesh points are the union of the stratified samples of every
+    batch shape that ran.  seed_extra: break the symmetry of D (reading R9: no symmetry assumed)."""
     w = W.make_workload(cfg)
     plist = O.pairs(w)
-    g = _gint(w)
-    _check_pairs(g, plist)
-    st = g.stats()
     V = W.make_potential(w)
     D = W.make_density_blocks(w, *plist)
+    if seed_extra is not None:
+        D = D + 0.3 * np.random.default_rng(seed_extra).standard_normal(D.size)
     A, B, R, off = plist
     rng = np.random.default_rng([2409, 9399, cfg, 77])
     keys = _stratified_keys(w, plist, rng, n_keys)
-    pts = _stratified_points(w, st, rng, n_pts)
-    assert len(keys) >= n_keys // 2 and len(pts) >= n_pts // 2
+    assert len(keys) >= n_keys // 2
     assert np.any(np.abs(R[keys]).sum(1) != 0) or not np.any(np.abs(R).sum(1) != 0)
-    V_d, D_d = torch.from_numpy(V).cuda(), torch.from_numpy(D).cuda()
-    H_d, rho_d = g.vlocal(V_d), g.rho(D_d)
-    H, rho = H_d.cpu().numpy(), rho_d.cpu().numpy()
+    dV = abs(np.linalg.det(w.cell)) / w.n_points
+    E = _onsite_overlap_closed_form(w) if w.basis.n_species == 1 else None
+    onsite = np.flatnonzero((A == B) & (np.abs(R).sum(1) == 0))
+    runs, pts_parts = [], []
+    for flags in flag_sets:
+        g = _gint(w, flags)
+        _check_pairs(g, plist)
+        st = g.stats()
+        st["n_pairs"] = len(A)                      # the oracle's list, just checked key by key against the library's
+        pts_parts.append(_stratified_points(w, st, rng, n_pts))
+        V_d, D_d = torch.from_numpy(V).cuda(), torch.from_numpy(D).cuda()
+        H_d, rho_d = g.vlocal(V_d), g.rho(D_d)
+        lhs = float((V_d * rho_d).sum().item() * dV); rhs = float((D_d * H_d).sum().item())
+        Hmax, rmax = float(H_d.abs().max().item()), float(rho_d.abs().max().item())
+        # run-to-run: accumulation into H and rho is by floating-point atomics (order not fixed): equal to rounding, not bitwise
+        H2, rho2 = g.vlocal(V_d), g.rho(D_d)
+        rep_H = float((H2 - H_d).abs().max().item()) / Hmax; rep_r = float((rho2 - rho_d).abs().max().item()) / rmax
+        del H2, rho2
+        # a pin that does not go through the oracle: V == 1 gives the overlap matrix, whose on-site blocks have a closed form
+        S = g.vlocal(torch.ones_like(V_d)).cpu().numpy()
+        g.close()
+        eS = 0.0
+        if E is not None:
+            eS = max(float(np.max(np.abs(S[off[k]:off[k + 1]].reshape(E.shape) - E))) for k in onsite)
+        else:       # several species: orthonormality of every on-site block (real harmonics, normalised radial functions of one l differ)
+            no = np.asarray(w.basis.norb)[w.atom_species]
+            for k in onsite[::37]:
+                blk = S[off[k]:off[k + 1]].reshape(no[A[k]], no[A[k]])
+                eS = max(eS, float(np.max(np.abs(np.diag(blk) - 1.0))), float(np.max(np.abs(blk - blk.T))))
+        del S
+        tag = f"cfg{cfg} flags={flags:#x} batch {st['batch_bx']}x{st['batch_by']}x{st['batch_bz']}"
+        assert abs(lhs - rhs) <= 1e-11 * abs(lhs), f"{tag} identity P4 {abs(lhs - rhs) / abs(lhs):.3e}"
+        assert rep_H <= 1e-13 and rep_r <= 1e-13, f"{tag} repeatability {rep_H:.3e} {rep_r:.3e}"
+        assert eS <= 1e-8, f"{tag} on-site overlap blocks against the closed form {eS:.3e}"
+        # keep only the sampled outputs on the host: the H blocks of `keys` and (below) rho at the union of the sampled points
+        runs.append((tag, st, [H_d[off[k]:off[k + 1]].cpu().numpy() for k in keys], rho_d.cpu().numpy(), Hmax, rmax))
+        del H_d, rho_d, V_d, D_d
+        torch.cuda.empty_cache()
+    pts = np.unique(np.concatenate(pts_parts)).astype(np.int64)
+    assert len(pts) >= n_pts // 2
     H_or = O.vlocal(w, V, plist, sel=keys)
     rho_or = O.rho(w, D, plist, sel=pts)
-    # the scale of the tolerance is the largest |H| (|rho|) of the whole result, as in north_star
-    Hmax, rmax = float(np.max(np.abs(H))), float(np.max(np.abs(rho)))
-    eH = max(float(np.max(np.abs(H[off[k]:off[k + 1]] - H_or[off[k]:off[k + 1]]))) for k in keys) / Hmax
-    er = float(np.max(np.abs(rho[pts] - rho_or[pts]))) / rmax
-    dV = abs(np.linalg.det(w.cell)) / w.n_points
-    lhs = float((V_d * rho_d).sum().item() * dV); rhs = float((D_d * H_d).sum().item())
-    # run-to-run: accumulation into H and rho is by floating-point atomics (order not fixed): equal to rounding, not bitwise
-    H2, rho2 = g.vlocal(V_d), g.rho(D_d)
-    rep_H = float((H2 - H_d).abs().max().item()) / Hmax; rep_r = float((rho2 - rho_d).abs().max().item()) / rmax
-    # a pin that does not go through the oracle: V == 1 gives the overlap matrix, whose on-site blocks have a closed form
-    S = g.vlocal(torch.ones_like(V_d)).cpu().numpy()
-    g.close()
-    eS = 0.0
-    if w.basis.n_species == 1:
-        E = _onsite_overlap_closed_form(w)
-        onsite = np.flatnonzero((A == B) & (np.abs(R).sum(1) == 0))
-        eS = max(float(np.max(np.abs(S[off[k]:off[k + 1]].reshape(E.shape) - E))) for k in onsite)
-    else:       # several species: orthonormality of every on-site block (real harmonics, normalised radial functions of one l differ)
-        no = np.asarray(w.basis.norb)[w.atom_species]
-        for k in np.flatnonzero((A == B) & (np.abs(R).sum(1) == 0))[::37]:
-            blk = S[off[k]:off[k + 1]].reshape(no[A[k]], no[A[k]])
-            eS = max(eS, float(np.max(np.abs(np.diag(blk) - 1.0))), float(np.max(np.abs(blk - blk.T))))
-    assert eH <= TOL, f"cfg{cfg} H parity on {len(keys)} sampled keys {eH:.3e}"
-    assert er <= TOL, f"cfg{cfg} rho parity on {len(pts)} sampled points {er:.3e}"
-    assert abs(lhs - rhs) <= 1e-11 * abs(lhs), f"cfg{cfg} identity P4 {abs(lhs - rhs) / abs(lhs):.3e}"
-    assert rep_H <= 1e-13 and rep_r <= 1e-13, f"cfg{cfg} repeatability {rep_H:.3e} {rep_r:.3e}"
-    assert eS <= 1e-8, f"cfg{cfg} on-site overlap blocks against the closed form {eS:.3e}"
+    for tag, st, Hk, rho, Hmax, rmax in runs:
+        # the scale of the tolerance is the largest |H| (|rho|) of the whole result, as in north_star
+        eH = max(float(np.max(np.abs(h - H_or[off[k]:off[k + 1]]))) for h, k in zip(Hk, keys)) / Hmax
+        er = float(np.max(np.abs(rho[pts] - rho_or[pts]))) / rmax
+        assert eH <= TOL, f"{tag} H parity on {len(keys)} sampled keys {eH:.3e}"
+        assert er <= TOL, f"{tag} rho parity on {len(pts)} sampled points {er:.3e}"
+    return [r[1] for r in runs]
 
 
 def _onsite_overlap_closed_form(w):
@@ -303,12 +320,25 @@ def test_cfg2_bulk_sampled(torch_cuda):
 
 
 def test_cfg3_tbg_sampled(torch_cuda):
-    _sampled_parity(torch_cuda, 3, 600, 50000)
+    """Default batch shape, and GINT_FLAG_TUNE as bench.py initialises (whatever shape the tuner then keeps)."""
+    from paper_2409_09399_b200.gint import FLAG_TUNE
+    _sampled_parity(torch_cuda, 3, 600, 50000, flag_sets=(0, FLAG_TUNE))
+
+
+def test_cfg3_tbg_sampled_nonsymmetric_D(torch_cuda):
+    """Full size with a D that has no mirror symmetry: Dh = D + mirror^T of k_sym_D must carry every ordered block (reading R9)."""
+    _sampled_parity(torch_cuda, 3, 300, 20000, seed_extra=13)
 
 
 def test_cfg4_tbg_headline_sampled(torch_cuda):
-    """The headline workload (10,444 atoms, 1.76e8 points) exactly as bench.py launches it."""
-    _sampled_parity(torch_cuda, 4, 1000, 100000)
+    """The headline workload (10,444 atoms, 1.76e8 points) in the launch configurations bench.py can time: initialised with
+    GINT_FLAG_TUNE exactly as bench.py does (the tuner keeps the default 8x8x16 unless another shape is clearly faster), and with
+    the 4x8x16 shape forced, the one the round-2 tuner picked and the committed ncu captures pin."""
+    from paper_2409_09399_b200.gint import FLAG_TUNE, batch_flag
+    sts = _sampled_parity(torch_cuda, 4, 1000, 100000, flag_sets=(FLAG_TUNE, batch_flag(4, 8, 16)))
+    assert (sts[0]["batch_bx"], sts[0]["batch_by"], sts[0]["batch_bz"]) in ((8, 8, 16), (8, 8, 8), (4, 8, 16), (4, 4, 16), (4, 4, 8))
+    assert sts[0]["n_pairs"] == 1246278                                         # SURVEY.md P9 (oracle_pairs == library list == this count)
+    assert sts[0]["tune_us"] > 0 and (sts[1]["batch_bx"], sts[1]["batch_by"], sts[1]["batch_bz"]) == (4, 8, 16)
 
 
 def test_cfg5_mixed_species_sampled(torch_cuda):
@@ -373,7 +403,7 @@ def test_many_orbitals_per_atom(torch_cuda):
 
 def test_batch_shape_tuner(torch_cuda):
     """GINT_FLAG_TUNE (the paper's online auto-tuning): gint_init times the candidate batch shapes on a slab of the
-    mesh, keeps the fastest, reports what it tried -- and the context it returns is exact."""
+    mesh, keeps the default unless another shape is clearly faster, reports what it tried -- and the context it returns is exact."""
     from paper_2409_09399_b200.gint import FLAG_TUNE
     st = _full_parity(torch_cuda, W.make_workload(1), flags=FLAG_TUNE)
     from paper_2409_09399_b200.gint import Gint
@@ -383,8 +413,14 @@ def test_batch_shape_tuner(torch_cuda):
     g.close()
     tried = [r for r in rep if r[3] > 0]
     assert len(rep) >= 3 and len(tried) >= 2 and 0 < st["tune_us"] < 2_000_000          # "no more than two seconds"
-    best = min(tried, key=lambda r: r[3])
-    assert (st["batch_bx"], st["batch_by"], st["batch_bz"]) == best[:3]
+    # the rule of include/gint.h: the default shape (first row) stays unless the fastest other shape is more than 2 % faster
+    chosen = (st["batch_bx"], st["batch_by"], st["batch_bz"])
+    others = [r for r in tried if r is not rep[0]]
+    fastest = min(others, key=lambda r: r[3])
+    if rep[0][3] > 0 and not fastest[3] < rep[0][3] * (1.0 - 0.02):
+        assert chosen == rep[0][:3]
+    else:
+        assert chosen == fastest[:3]
     # without the flag nothing is tuned
     g = Gint.from_workload(W.make_workload(0))
     assert g.tune_report() == [] and g.stats()["tune_us"] == 0

@@ -164,6 +164,10 @@ def test_phi_cutoff_and_origin():
 
 
 # ----------------------------------------------------------------------------- S: spline data
+SURVEY_P8_NORMS = {5.0: (1.98381907454532, 1.10072344658646, 1.62880549788493, 0.690466095447584, 0.863637740254984),
+                   7.0: (1.85514473075244, 0.931663800594847, 1.4235833205831, 0.505992851061471, 0.681962212656393)}
+
+
 @pytest.mark.parametrize("rc", [5.0, 7.0])
 def test_spline_tables(rc):
     basis = W.make_basis(rc)
@@ -180,6 +184,8 @@ def test_spline_tables(rc):
         # normalisation: int R^2 r^2 dr = 1 by adaptive quadrature of the ANALYTIC function
         I, _ = quad(lambda r: W.radial_raw(r, l, alpha, rc) ** 2 * r * r, 0, rc, epsabs=1e-15, epsrel=1e-13)
         assert abs(basis.norm[s] - 1 / np.sqrt(I)) < 1e-12 * basis.norm[s]
+        # SURVEY.md section 8(c) pin P8 prints these constants (bar 1e-13)
+        assert abs(basis.norm[s] - SURVEY_P8_NORMS[rc][s]) <= 1e-13 * basis.norm[s]
         # oracle's interpolation vs the analytic function (interpolation error of a dr=0.01 clamped spline)
         if l == 0:
             vals = np.array([O.phi(basis, 0, np.array([0, 0, r]))[s] for r in rr]) / 0.28209479177387814
@@ -466,17 +472,28 @@ def test_table2_tbg_family():
         assert n == 4 * (3 * i * i + 3 * i + 1)
         # garbled-column reading: in-plane vectors are X and Z (60 degrees, equal length)
         assert abs(np.linalg.norm(X) - np.linalg.norm(Z)) < 2e-2
-        if i in (2, 29) or True:
-            cell, pos = W.twisted_bilayer(i) if i <= 12 else (None, None)
-            if cell is not None:
-                assert len(pos) == n
-                assert abs(np.linalg.norm(cell[0]) / bohr - np.linalg.norm(X)) < 2e-3 * np.linalg.norm(X)
-                assert abs(np.dot(cell[0], cell[1]) / np.linalg.norm(cell[0]) ** 2 - 0.5) < 1e-12
+        cell, pos = W.twisted_bilayer(i)                        # all four cells of the table, i = 29 (10,444 atoms) included
+        assert len(pos) == n
+        assert abs(np.linalg.norm(cell[0]) / bohr - np.linalg.norm(X)) < 2e-3 * np.linalg.norm(X)
+        assert abs(np.dot(cell[0], cell[1]) / np.linalg.norm(cell[0]) ** 2 - 0.5) < 1e-12
     w4 = W.make_workload(4)
     assert w4.n_atoms == 10444 and tuple(w4.mesh) == (1188, 1188, 125)
     assert abs(np.linalg.norm(w4.cell[0]) / bohr - np.linalg.norm(np.array(rows[3][1:4], float))) < 2e-3 * 125.7
     d = cKDTree(w4.atom_pos).query(w4.atom_pos, k=2)[0][:, 1]
     assert abs(d.min() - 4.65 / np.sqrt(3)) < 1e-9            # no overlapping atoms: shortest bond = a/sqrt(3)
+
+
+def test_P9_cfg4_pair_count_by_kdtree():
+    """SURVEY.md P9 at the headline size: 1,246,278 ordered pair keys (|tau_B + n.cell - tau_A| < 2 rc, strict; reading R7), counted
+    here with a KD-tree over the periodic images, independent of oracle_pairs (which takes minutes at this size and is compared key
+    by key with this count, and with the library's list, in the GPU test of cfg4)."""
+    w = W.make_workload(4)
+    rc2 = 2 * w.basis.rcut[0]
+    m = [int(np.ceil(rc2 / h)) for h in 1.0 / np.linalg.norm(np.linalg.inv(w.cell), axis=0)]
+    shifts = np.array(list(itertools.product(*[range(-k, k + 1) for k in m]))) @ w.cell
+    allpos = (w.atom_pos[None, :, :] + shifts[:, None, :]).reshape(-1, 3)
+    cnt = sum(len(x) for x in cKDTree(allpos).query_ball_point(w.atom_pos, rc2 * (1 - 1e-13)))
+    assert cnt == 1246278
 
 
 # ----------------------------------------------------------------------------- P10 Pulay force and stress (Eq. 4, Eq. 5; reading R15)
