@@ -37,39 +37,52 @@ def alg_flops(st: dict) -> float:
     return float(st["alg_sum_n2"] + st["alg_sum_n"]) + float(st["alg_sum_n"]) + EVAL_FLOP_PER_INCIDENCE * st["alg_incidence"]
 
 
-TRAFFIC_CSV = os.path.join("profiles", "r2_traffic.csv")
+TRAFFIC_CSV = os.path.join("profiles", "r3_traffic.csv")
+FORCE_GRAD_FLOP_PER_INCIDENCE = 360.0                # value + gradient of the orbitals of one atom at one point (3x the value alone)
+
+
+def force_alg_flops(st: dict) -> float:
+    """Algorithmic flops of ONE gint_force_stress call: Psi needs every ORDERED pair of orbitals non-zero at a point
+    (2 n_g^2; the mirror halving of Eq. 2 / Eq. 3 does not apply), then three gradient components times Psi (6 n_g), plus the
+    evaluation of values and gradients."""
+    return 2.0 * st["alg_sum_n2"] + 6.0 * st["alg_sum_n"] + FORCE_GRAD_FLOP_PER_INCIDENCE * st["alg_incidence"]
 
 
 def csrc_digest() -> str:
-    """sha256 over the kernel sources: the committed ncu capture names the digest it was taken on."""
+    """sha256 over the sources of the timed gint_vlocal / gint_rho path (everything in csrc/ but the force kernels): the committed
+    ncu capture names the digest it was taken on."""
     import hashlib
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2409_09399_b200", "csrc")
     for name in sorted(os.listdir(d)):
+        if name == "gint_force.cu":
+            continue
         with open(os.path.join(d, name), "rb") as f:
             h.update(name.encode()); h.update(f.read())
     return h.hexdigest()[:16]
 
 
-def ncu_traffic(cfg: int, call: str):
+def ncu_traffic(cfg: int, batch, call: str):
     """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum, summed over the kernels of one `call` = "vlocal_main" or
-    "rho_main", all waves) from the committed ncu capture profiles/r2_traffic.csv, with a note.  The capture names the digest of
-    the kernel sources it was taken on: when csrc/ has changed since, the figure is STALE and is not reported."""
+    "rho_main", all waves) from the committed ncu capture profiles/r3_traffic.csv, with a note.  A row is keyed by the config AND
+    the grid-batch shape it was captured with (the launch the tuner chose may differ from run to run), and names the digest of the
+    kernel sources: no row for this shape, or sources changed since, and the figure is not reported."""
     path = os.path.join(ROOT, TRAFFIC_CSV)
+    shape = "x".join(str(int(b)) for b in batch)
     try:
         with open(path) as f:
             lines = [ln for ln in f.read().splitlines() if ln and not ln.startswith("#")]
         for ln in lines[1:]:
-            c, k, rd, wr, digest = [x.strip() for x in ln.split(",")[:5]]
-            if int(c) == cfg and k == call:
+            c, b, k, rd, wr, digest = [x.strip() for x in ln.split(",")[:6]]
+            if int(c) == cfg and b == shape and k == call:
                 if digest != csrc_digest():
                     print(f"bench.py: {TRAFFIC_CSV} was captured on csrc digest {digest}, the tree is at {csrc_digest()}: "
                           "roofline.traffic not reported (re-capture with ncu)", file=sys.stderr)
                     return None, f"stale capture (csrc digest {digest} != {csrc_digest()})"
-                return int(rd) + int(wr), f"{TRAFFIC_CSV}, csrc digest {digest}"
+                return int(rd) + int(wr), f"{TRAFFIC_CSV}, batch {shape}, csrc digest {digest}"
     except (OSError, ValueError):
         pass
-    return None, "no capture for this config"
+    return None, f"no capture for cfg {cfg} with batch {shape}"
 
 
 def cpu_model() -> str:
@@ -170,7 +183,8 @@ def oracle_sample(w, V, D, plist, budget_s: float = 20.0):
     t0 = time.perf_counter(); O.vlocal(w, V, plist, sel=np.arange(p0, p0 + np_s, dtype=np.int64)); t_v = time.perf_counter() - t0
     t0 = time.perf_counter(); O.rho(w, D, plist, sel=(np.arange(g0, g0 + ng_s, dtype=np.int64) % npts)); t_r = time.perf_counter() - t0
     t_step = t_v * npairs / np_s + t_r * npts / ng_s          # extrapolated full-mesh step
-    info = {"kind": "oracle", "cores": O.threads(), "cpu": cpu_model(),
+    info = {"kind": "oracle", "cores": O.threads(), "cpu": cpu_model(), "extrapolated": True,
+            "sample_fraction": {"vlocal_pair_keys": np_s / npairs, "rho_mesh_points": ng_s / npts},
             "sample": f"vlocal: {np_s} of {npairs} pair keys in {t_v:.2f} s; rho: {ng_s} of {npts} mesh points in {t_r:.2f} s; "
                       f"scaled to the full mesh (vlocal {t_v * npairs / np_s:.1f} s + rho {t_r * npts / ng_s:.1f} s per step)"}
     return npts / t_step, info
@@ -216,7 +230,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-force", action="store_true", help="skip the (separately reported) gint_force_stress timing")
     ap.add_argument("--batch", default="", help="override grid-batch shape, e.g. 8,8,8")
-    ap.add_argument("--csrc-digest", action="store_true", help="print the digest of the kernel sources (for profiles/r2_traffic.csv) and exit")
+    ap.add_argument("--csrc-digest", action="store_true", help="print the digest of the kernel sources (for profiles/r3_traffic.csv) and exit")
     args = ap.parse_args()
     if args.csrc_digest:
         print(csrc_digest())
@@ -304,11 +318,20 @@ def main():
     force = None
     if not args.no_force:
         g.force_stress(V_d, D_d); torch.cuda.synchronize()
+        fs = ClockSampler(local)
+        if rank == 0:
+            fs.start()
         tf = []
         for _ in range(2):
             g.force_stress(V_d, D_d); torch.cuda.synchronize(); tf.append(g.force_time())
-        force = {"ms": 1e3 * float(np.median(tf)), "points_per_s": npts / float(np.median(tf)),
-                 "what": "gint_force_stress: forces of all atoms and the 3x3 stress in one call (k_sym_full + k_force_batch)"}
+        t_f = float(np.median(tf))
+        F_force = force_alg_flops(st)
+        force = {"ms": 1e3 * t_f, "points_per_s": npts / t_f,
+                 "what": "gint_force_stress: forces of all atoms and the 3x3 stress in one call (k_sym_full + k_force_batch)",
+                 "roofline": {"bound": "alu", "achieved": F_force / t_f / 1e12, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                              "frac": F_force / t_f / 1e12 / FP64_PEAK_TFLOPS, "alg_flop_per_call": F_force,
+                              "flops": "2 sum n_g^2 (Psi, every ordered orbital pair) + 6 sum n_g (grad . Psi) + 360 per (point, atom) incidence"},
+                 "clocks": fs.stop() if rank == 0 else None}
 
     # ---- end to end through the host-buffer entry points (pinned host memory, H2D + D2H every step)
     e2e = None
@@ -317,13 +340,17 @@ def main():
         H_h = torch.empty(g.n_values, dtype=torch.float64).pin_memory(); rho_h = torch.empty(npts, dtype=torch.float64).pin_memory()
         g.vlocal_host(V_h, H_h); g.rho_host(D_h, rho_h)
         barrier()
-        n_e2e = max(1, min(args.steps, 3))
+        n_e2e = max(1, args.steps)
+        es = ClockSampler(local)
+        if rank == 0:
+            es.start()
         te0 = time.perf_counter()
         for _ in range(n_e2e):
             g.vlocal_host(V_h, H_h); g.rho_host(D_h, rho_h)      # each call synchronises its stream before returning
         barrier()
         t_e2e = (time.perf_counter() - te0) / n_e2e
-        e2e = {"t": t_e2e, "h2d": 8 * (npts + g.n_values), "d2h": 8 * (g.n_values + npts)}
+        e2e = {"t": t_e2e, "h2d": 8 * (npts + g.n_values), "d2h": 8 * (g.n_values + npts), "steps": n_e2e,
+               "clocks": es.stop() if rank == 0 else None}
         del V_h, D_h, H_h, rho_h
 
     t_step, t_e2e_max = max_over_ranks([t_step, e2e["t"] if e2e else 0.0], dev, world)
@@ -337,7 +364,7 @@ def main():
             cpu = {"value": val, "unit": "mesh points/s", **info}
         dom = "vlocal_main" if kt["vlocal_main"] >= kt["rho_main"] else "rho_main"
         achieved = F_alg / kt[dom] / 1e12
-        traffic, traffic_note = ncu_traffic(args.cfg, dom)
+        traffic, traffic_note = ncu_traffic(args.cfg, (st["batch_bx"], st["batch_by"], st["batch_bz"]), dom)
         # context: the same kernel against the HBM roofline (measured copy bandwidth of this pool's B200s, MEASURED_PEAKS.json;
         # 6650 GB/s is the profiling guide's fallback).  Algorithmic bytes: V + canonical H (vlocal) / canonical D + rho (rho).
         try:
@@ -380,7 +407,8 @@ def main():
         }
         if e2e:
             line["e2e"] = {"value": world * npts / e2e["t"], "unit": "mesh points/s", "h2d_bytes_per_step": e2e["h2d"],
-                           "d2h_bytes_per_step": e2e["d2h"], "ms_per_step": 1e3 * e2e["t"]}
+                           "d2h_bytes_per_step": e2e["d2h"], "ms_per_step": 1e3 * e2e["t"], "steps": e2e["steps"],
+                           "clocks": e2e["clocks"]}
         if force:
             line["force_stress"] = force
         if cpu:

@@ -57,6 +57,11 @@ typedef enum gint_status {
  * 16 GiB and a quarter of the device memory free at gint_init.  A smaller cap trades memory for more, shorter waves; a batch shape
  * whose single largest batch exceeds the cap counts as "does not fit" and the next smaller shape is tried. */
 #define GINT_FLAG_PHI_CAP_MB(mb) (((unsigned long long)(mb) & 0xfffffull) << 40)
+/* GINT_FLAG_FORCE: the context will be used for gint_force_stress as well.  The force kernel keeps the orbital values and the
+ * Psi rows of a whole batch in shared memory, so it can need more of it than the contraction kernels; with this flag the automatic
+ * choice of the batch shape (and the tuner) only accepts shapes that gint_force_stress supports too.  Without it gint_force_stress
+ * may return GINT_ERR_UNSUPPORTED on cells with many orbitals per batch although gint_vlocal / gint_rho work. */
+#define GINT_FLAG_FORCE (1ull << 33)
 #define GINT_FLAG_BATCH(bx, by, bz) ((unsigned long long)(bx) | ((unsigned long long)(by) << 8) | ((unsigned long long)(bz) << 16))
 
 /*
@@ -131,7 +136,9 @@ int gint_rho(gint_ctx* ctx, const double* D_dev, double* rho_dev, void* cuda_str
  *   sigma_dev device, 9 doubles [a][b], or NULL (stress not wanted)    -- OVERWRITTEN
  * Enqueued on `cuda_stream`, no synchronisation.  The first call allocates a context-owned copy of D in the pair-list layout
  * (8 * n_values bytes; GINT_ERR_OUT_OF_MEMORY if that fails).  GINT_ERR_UNSUPPORTED: more than 2^32 matrix elements, or a
- * grid batch whose orbitals do not fit the kernel's shared memory (about 800 orbitals per batch). */
+ * grid batch that does not fit the kernel's shared memory: about 8.6 KB + 4 n^2 + 192 n + 128 R bytes for the n atom images and R
+ * orbitals of the largest batch, against 227 KB per CTA (R <= about 1,300 at n = 96, 1,600 at n = 32).  GINT_FLAG_FORCE at
+ * gint_init picks a batch shape that fits. */
 int gint_force_stress(gint_ctx* ctx, const double* V_dev, const double* D_dev, double* F_dev, double* sigma_dev, void* cuda_stream);
 
 /*

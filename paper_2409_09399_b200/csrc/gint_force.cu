@@ -324,14 +324,17 @@ int gint_launch_force(gint_ctx* c, const double* V, const double* D, double* F, 
     if (c->n_batch == 0 || c->n_values == 0) return GINT_OK;
     if (c->n_values >= (1ll << 32)) GINT_FAIL(GINT_ERR_UNSUPPORTED, "gint_force_stress: more than 2^32 matrix elements");
     const size_t smem = gint_force_smem(c);
-    cudaDeviceProp prop;
-    GINT_CUDA(cudaGetDeviceProperties(&prop, c->device));
-    if (smem > prop.sharedMemPerBlockOptin) GINT_FAIL(GINT_ERR_UNSUPPORTED, "gint_force_stress: a batch of %d orbitals needs %zu bytes of shared memory", c->geom.max_cols, smem);
+    if (smem > c->smem_optin)
+        GINT_FAIL(GINT_ERR_UNSUPPORTED, "gint_force_stress: a batch of %d atom images and %d orbitals needs %zu bytes of shared memory (limit %zu); "
+                  "initialise with GINT_FLAG_FORCE, or a smaller GINT_FLAG_BATCH", c->geom.max_nb, c->geom.max_cols, smem, c->smem_optin);
     if (!c->d_dfull) {
         GINT_CUDA(cudaMalloc((void**)&c->d_dfull, sizeof(double) * (size_t)c->n_values));
         c->device_bytes += sizeof(double) * (size_t)c->n_values;
     }
-    GINT_CUDA(cudaFuncSetAttribute(k_force_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin));
+    if (!c->force_configured) {      // once per context, not per call
+        GINT_CUDA(cudaFuncSetAttribute(k_force_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_optin));
+        c->force_configured = true;
+    }
     GINT_CUDA(cudaEventRecord(c->ev_force[0], st));
     k_sym_full<<<(unsigned)((c->n_pairs + 7) / 8), 256, 0, st>>>(c->n_pairs, c->d_poff, c->d_pcanon, c->d_pflag, c->d_cpub, c->d_cmir, c->d_pnA, D, c->d_dfull);
     GINT_CUDA(cudaGetLastError());

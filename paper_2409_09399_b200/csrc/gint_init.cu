@@ -574,7 +574,8 @@ static int build_batches(gint_ctx* c, const int bs[3], size_t smem_limit, size_t
     int max_nb = 0, max_cols = 0;
     for (long long b = 0; b < nbt; b++) { max_nb = std::max(max_nb, count[b]); max_cols = std::max(max_cols, cols[b]); }
     g.max_nb = std::max(max_nb, 1); g.max_cols = std::max(max_cols, 1);
-    const bool ok = max_nb <= GINT_MAX_NB && gint_smem_needed(c, smem_limit) <= smem_limit;     // else: try a smaller batch shape
+    const bool ok = max_nb <= GINT_MAX_NB && gint_smem_needed(c, smem_limit) <= smem_limit &&     // else: try a smaller batch shape
+                    (!c->want_force || gint_force_smem(c) <= smem_limit);
     if (!ok) return GINT_OK;
     *fits = true;
 
@@ -676,6 +677,8 @@ static int gint_init_impl(gint_ctx** out, gint_ctx*& c, int n_species, const int
     if ((rc = build_pairs(c))) { return rc; }
 
     const size_t smem_limit = prop.sharedMemPerBlockOptin;
+    c->smem_optin = smem_limit;
+    c->want_force = (flags & GINT_FLAG_FORCE) != 0;
     // scratch for the orbital values of one wave of batches: at most 16 GiB and a quarter of the free device memory, or what the caller asks for
     size_t mem_free = 0, mem_total = 0;
     GINT_CUDA(cudaMemGetInfo(&mem_free, &mem_total));

@@ -234,6 +234,9 @@ struct gint_ctx {
     double* d_stage_in = nullptr; size_t stage_in_n = 0;
     double* d_stage_out = nullptr; size_t stage_out_n = 0;
     cudaStream_t copy_stream = nullptr;
+    size_t smem_optin = 0;           // cudaDevAttrMaxSharedMemoryPerBlockOptin of the device (set by gint_init)
+    bool want_force = false;         // GINT_FLAG_FORCE: the batch shape must also fit the force kernel's shared memory
+    bool force_configured = false;   // k_force_batch's shared-memory limit has been raised on this context's device
     int rho_planes = 0;              // > 0 (batch-shape tuner only): gint_rho clears just the first rho_planes mesh planes along a1
     // gint_force_stress: full-layout copy of D + mirror^T (allocated by the first call), events around its kernels
     double* d_dfull = nullptr;

@@ -69,6 +69,9 @@ def fp64_peak(device: int = 0) -> dict:
 FLAG_TUNE = 1 << 32       # gint_init times several grid-batch shapes; the default stays unless another is > 2 % faster
 
 
+FLAG_FORCE = 1 << 33      # the batch shape must also fit gint_force_stress's shared memory
+
+
 def batch_flag(bx: int, by: int, bz: int) -> int:
     return bx | (by << 8) | (bz << 16)
 
