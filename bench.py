@@ -183,7 +183,7 @@ def oracle_sample(w, V, D, plist, budget_s: float = 20.0):
     t0 = time.perf_counter(); O.vlocal(w, V, plist, sel=np.arange(p0, p0 + np_s, dtype=np.int64)); t_v = time.perf_counter() - t0
     t0 = time.perf_counter(); O.rho(w, D, plist, sel=(np.arange(g0, g0 + ng_s, dtype=np.int64) % npts)); t_r = time.perf_counter() - t0
     t_step = t_v * npairs / np_s + t_r * npts / ng_s          # extrapolated full-mesh step
-    info = {"kind": "oracle", "cores": O.threads(), "cpu": cpu_model(), "extrapolated": True,
+    info = {"kind": "oracle", "cores": O.threads(), "cpu": cpu_model(), "extrapolated": bool(np_s < npairs or ng_s < npts),
             "sample_fraction": {"vlocal_pair_keys": np_s / npairs, "rho_mesh_points": ng_s / npts},
             "sample": f"vlocal: {np_s} of {npairs} pair keys in {t_v:.2f} s; rho: {ng_s} of {npts} mesh points in {t_r:.2f} s; "
                       f"scaled to the full mesh (vlocal {t_v * npairs / np_s:.1f} s + rho {t_r * npts / ng_s:.1f} s per step)"}
